@@ -1,0 +1,153 @@
+/* west.h - C ABI of the B200-native chi0*dV hot path of arXiv 2203.05623 (Yu & Govoni).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines):
+ *   Eq. 10   (h - eps_i) P_c dpsi_i^j = -P_c v_j^pert psi_i,  P_c = 1 - P_v,
+ *                           solved "by a preconditioned conjugate gradient method";
+ *   Eq. 11   dn_j(r) = sum_sigma sum_i [psi_i^* dpsi_i^j + c.c.];
+ *   dual-space H application "kinetic operator and local potential are applied in the reciprocal or direct
+ *                           space ... at least two FFTs (one forward and one backward)";
+ *   sphere-truncated FFT    "retains only the Fourier components that correspond to a chosen kinetic energy
+ *                           cutoff".
+ * Readings of everything the paper leaves open (alpha*P_v, preconditioner, tolerance, i*omega, ordering of G,
+ * FFT sign and scale, synthetic pseudopotential) are listed in DESIGN.md section 3 and referenced here as (Rn).
+ *
+ * Conventions
+ *   Units: Rydberg atomic units, kinetic energy |G|^2 Ry, G = (2 pi / L) n, n integer triple, cubic cell of side L bohr.
+ *   Sphere (R2): S = { n : |n|^2 <= n2max }, stored in ascending lexicographic order of the signed triple
+ *     (n_x, n_y, n_z).  mode WEST_FULL stores all of S (n_g = |S|) and vectors are complex functions.
+ *     mode WEST_GAMMA stores the tail of that list starting at n = 0 (n_g = (|S|+1)/2: n = 0 and every triple whose
+ *     first non-zero component is positive) and every vector is a REAL function of r, c(-G) = conj c(G), c(0) real.
+ *   Coefficient blocks: row-major [vector][n_g], interleaved complex128 (re, im), G fastest.
+ *   Grids: [ix][iy][iz], z fastest, N^3 points, r = (L/N)(ix, iy, iz).  Real grids are f64, complex grids c128.
+ *   FFT (R10): G->r  f(r_j) = sum_G c(G) exp(+i G.r_j)          (unscaled)
+ *              r->G  c(G)   = (1/N^3) sum_j f(r_j) exp(-i G.r_j) (truncated to S)
+ *   Requires N even and N >= 4*floor(sqrt(n2max)) + 1 (products of two sphere-limited functions alias-free);
+ *     supported N: 24, 36, 48, 72, 144.
+ *
+ * Ownership and streams
+ *   Every pointer is a DEVICE pointer owned by the caller unless marked "host".  The library allocates device
+ *   memory only in west_create / west_set_* / the first call of an operation at a larger batch size (internal
+ *   workspace, grown lazily, never shrunk, freed by west_destroy).  All work is enqueued on the CUDA stream given to
+ *   west_create (a cudaStream_t passed as void*; NULL = the legacy default stream).  Calls are asynchronous with
+ *   respect to the host except where stated.  Pointers given to west_set_* are COPIED (the caller may free them after
+ *   the call returns; the copy is enqueued on the stream).  A context is not thread-safe.
+ *
+ * Errors
+ *   Every int-returning call returns 0 on success, a negative WEST_E* on a hard error (nothing useful written) or the
+ *   positive WEST_NOTCONVERGED (outputs written; stats say how many columns hit max_iter).  The message of the last
+ *   error is kept per context (west_last_error).  No exceptions cross the ABI, nothing calls exit().
+ *   There is no CPU fallback: without a CUDA device west_create fails with WEST_ECUDA.
+ */
+#ifndef WEST_H
+#define WEST_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WEST_OK            0
+#define WEST_NOTCONVERGED  1
+#define WEST_EINVAL       -1
+#define WEST_ECUDA        -2
+#define WEST_ESTATE       -3   /* a required west_set_* has not been called */
+#define WEST_ENOMEM       -4
+
+#define WEST_FULL   0
+#define WEST_GAMMA  1
+
+#define WEST_FP64   0   /* everything in FP64 */
+#define WEST_MIXED  1   /* FFT + real-space multiply inside H*psi in FP32; vectors, GEMMs, dots, dn in FP64 */
+
+typedef struct west_ctx west_ctx;
+
+typedef struct {
+    double  L;       /* cell side, bohr */
+    int32_t n2max;   /* integer sphere radius^2: floor(E_cut L^2 / 4 pi^2) (R2: the inclusion test is integer) */
+    int32_t N;       /* FFT grid points per axis */
+    int32_t mode;    /* WEST_FULL | WEST_GAMMA */
+} west_cell;
+
+typedef struct {
+    int32_t max_iter;   /* iteration cap per column (R5), e.g. 500 */
+    double  tol;        /* stop when ||r||_2 <= tol * ||b||_2 per column (R5) */
+    double  alpha_pv;   /* alpha of the alpha*P_v term (R3); the converged result does not depend on it */
+    int32_t precond;    /* 0: none; 1: M_v(G) = 1/max(1, |G|^2/(1.35 <psi_v|T|psi_v>)) (R4) */
+    int32_t check_every;/* host polls convergence every this many iterations (>=1) */
+} west_cg_opts;
+
+typedef struct {            /* host struct, filled when non-NULL (forces one stream synchronisation) */
+    int32_t iters;          /* iterations executed (max over columns) */
+    int32_t n_unconverged;  /* columns above tol at exit */
+    double  resid_max;      /* max over columns of ||r|| / ||b|| (recurrence residual) */
+    int64_t n_h_apply;      /* vectors pushed through H in this call (real functions in GAMMA mode) */
+    float   ms_rhs, ms_cg, ms_dn;   /* CUDA-event times of the three phases */
+} west_stats;
+
+/* Context. cuda_stream: cudaStream_t as void*. */
+int  west_create (west_ctx** ctx, const west_cell* cell, void* cuda_stream);
+int  west_destroy(west_ctx* ctx);
+const char* west_last_error(const west_ctx* ctx);   /* ctx may be NULL: last error of a failed west_create */
+
+/* Step a0 - the sphere S and its maps, computed on the HOST with integer arithmetic only.
+ * All output pointers are HOST pointers, any may be NULL.  miller [n_g][3]; fft_index[n_g] = ((n_x mod N) N + (n_y mod N)) N
+ * + (n_z mod N); fft_index_minus[n_g] = the same for -G; g2[n_g] = |G|^2 in Ry.  Order and n_g follow cell.mode. */
+int  west_gsphere(const west_ctx* ctx, int64_t* n_g, int32_t* miller, int32_t* fft_index, int32_t* fft_index_minus, double* g2);
+
+/* Operator data (device pointers, copied).  vloc [N^3] f64.  beta [n_proj][n_g] c128 in the storage of cell.mode
+ * (in GAMMA mode each projector must be a real function of r), dcoef [n_proj] f64 HOST: V_NL = sum_k |beta_k> D_k <beta_k|
+ * (Kleinman-Bylander, R12).  psi [n_occ][n_g] c128 orthonormal occupied orbitals (sum_G |c|^2 = 1 over the FULL sphere),
+ * eps [n_occ] f64 HOST eigenvalues in Ry: the inputs psi_i, eps_i of Eq. 10. n_proj = 0 removes V_NL. */
+int  west_set_vloc  (west_ctx* ctx, const double* vloc);
+int  west_set_kb    (west_ctx* ctx, int32_t n_proj, const void* beta, const double* dcoef_host);
+int  west_set_states(west_ctx* ctx, int32_t n_occ, const void* psi, const double* eps_host);
+
+/* Sphere-truncated 3D FFT (R10).
+ * dir = +1: in = coefficients [n_batch][n_g] c128, out = grids.   dir = -1: in = grids, out = coefficients.
+ * WEST_FULL:  grids are complex [n_batch][N^3] c128.
+ * WEST_GAMMA: vectors are real functions, grids are REAL [n_batch][N^3] f64 (two are packed per complex transform
+ *             internally; an odd trailing vector is padded).
+ * r->G of data that is not sphere-limited is the truncation to S of its DFT. */
+int  west_fft3d(west_ctx* ctx, int32_t dir, int32_t precision, int32_t n_batch, const void* in, void* out);
+
+/* y = H x = (T + V_loc + V_NL) x for n_vec vectors, x and y [n_vec][n_g] c128 (Eq. 1).
+ * x and y must not overlap.  Needs west_set_vloc; V_NL only if west_set_kb was called with n_proj > 0. */
+int  west_h_apply(west_ctx* ctx, int32_t precision, int32_t n_vec, const void* x, void* y);
+
+/* dn = chi0(i omega) dV for a block of perturbations (Eq. 10-11; R3-R9).
+ *   dV     [n_pert][N^3] f64 real perturbing potentials on the grid (Ry)
+ *   omega  [n_freq] HOST, imaginary frequencies in Ry, >= 0; omega = 0 runs real-symmetric PCG, omega > 0 runs COCG (R7)
+ *   dn     [n_freq][n_pert][N^3] f64: dn_i(r) = (4/Omega) Re sum_v conj(u_v(r)) du_iv(r)  (e/bohr^3, spin-unpolarised, R9/R11)
+ *   dpsi_opt  NULL, or the converged solutions:
+ *             WEST_FULL  [n_freq][n_pert][n_occ][n_g] c128
+ *             WEST_GAMMA [n_freq][n_pert][n_occ][2][n_g] c128 - real part and imaginary part of dpsi as two real functions
+ *   stats_opt NULL or HOST struct.
+ * For every (frequency w, perturbation i, occupied state v) it forms b = -P_c (dV_i psi_v), solves
+ * (H - eps_v - i omega_w + alpha P_v) dpsi = b by batched (one recurrence per column) preconditioned CG and accumulates dn. */
+int  west_chi0_apply(west_ctx* ctx, int32_t precision, int32_t n_pert, const double* dV,
+                     int32_t n_freq, const double* omega_host, const west_cg_opts* opts,
+                     double* dn, void* dpsi_opt, west_stats* stats_opt);
+
+/* Dense contraction building blocks (FP64 DMMA), exported for tests and the roofline bench.
+ * C[m][n] = sum_k A[m][k] B[n][k]          (west_gemm_tn: both operands K-contiguous, row-major [rows][ld])
+ * Y[n][k] += sum_m C[m][n] A[m][k]          (west_gemm_update)
+ * All f64, device pointers; ld* are leading dimensions in elements. */
+int  west_gemm_tn    (west_ctx* ctx, int32_t m, int32_t n, int64_t k, const double* A, int64_t lda,
+                      const double* B, int64_t ldb, double* C, int64_t ldc);
+int  west_gemm_update(west_ctx* ctx, int32_t m, int32_t n, int64_t k, const double* C, int64_t ldc,
+                      const double* A, int64_t lda, double* Y, int64_t ldy);
+
+/* Introspection for the bench: bytes of device memory the context currently holds, and the number of kernels it has
+ * launched since creation (the bench's gpu_launches claim). */
+int64_t west_device_bytes(const west_ctx* ctx);
+int64_t west_launch_count(const west_ctx* ctx);
+/* Tuning knob: how many FFT slots (complex transforms) are processed per internal chunk (0 = default).  The stick
+ * intermediate of a chunk is sized to stay L2-resident between the three FFT kernels. */
+int  west_set_fft_chunk(west_ctx* ctx, int32_t n_slots);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WEST_H */

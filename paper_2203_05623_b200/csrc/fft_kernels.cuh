@@ -1,0 +1,446 @@
+// Sphere-pruned batched 3D FFT for the dual-space H*psi, "sticks and planes" decomposition:
+//   K1  g2r_z   : sphere -> z sticks  (one 1D transform per non-empty (n_x,n_y) column)            -> W[slot][pz][col]
+//   K2  planes  : per (slot, z-plane): y inverse on the disc rows, x inverse line by line, real-space op
+//                 (x V_loc | store | dn accumulate | load product), x forward, y forward                -> W in place
+//   K3  r2g_z   : z sticks -> sphere, fused with 1/N^3, the kinetic diagonal and the (eps + i omega) shift
+// A 1D transform of length N = N1*N2 is two in-place register passes (strided DFT-N1 + twiddle, contiguous DFT-N2);
+// the inverse leaves real-space index j = k1 + N1 k2 at POSITION p = N2 k1 + k2 and the forward transform consumes
+// exactly that order, so no transposition or bit reversal is ever done.  All real-space arrays inside the library
+// ([pz][py][px], x fastest) live in this position order; west.cu converts at the API boundary.
+//
+// Every phase between two barriers is a function of (tid, nthreads) so that the same code can be stepped on the host.
+#pragma once
+#include "dft_small.cuh"
+
+struct WestGeom {
+    int N, n_max, nr, n_cols, n_units, gamma;
+    long long n_g;
+    const int* row_off;     // [nr+1]  first column of each n_x row of the disc (columns are lexicographic (n_x, n_y))
+    const int* unit_off;    // [n_units] offset in sphere storage of the stick's first stored coefficient
+    const int* unit_zmax;   // [n_units]
+    const cx<double>* tw;   // [N] exp(+2 pi i m / N)
+    const double* g2;       // [n_g] |G|^2 in storage order
+};
+
+// vector <-> slot mapping of K1/K3: FFT f (0 or 1) of slot s is vector s*vstride + f*voffb; vectors >= n_vec are zero padding.
+struct VecMap {
+    int vstride, voffb, n_vec;
+};
+
+template <typename T> WHD cx<T> cvt(cx<double> a) { return mk<T>((T)a.x, (T)a.y); }
+template <typename T> WHD cx<double> cvd(cx<T> a) { return mk<double>((double)a.x, (double)a.y); }
+WHD int wrap_signed(int n, int N) { return n < N / 2 ? n : n - N; }
+
+// ---------------------------------------------------------------------------------------------------------------- K1
+template <typename T, int N1, int N2, bool GAMMA, int CU>
+struct K1 {
+    static constexpr int N = N1 * N2, PITCH = N + 1, NF = GAMMA ? 2 : 1, NL = CU * NF;
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + N);
+
+    // phase A: strided DFT-N1 straight from the sphere coefficients, twiddle, store to the line buffer
+    static WHD void phaseA(int tid, int nthr, cx<T>* lines, const cx<T>* tw, const WestGeom& g, VecMap vm, int slot, int u0,
+                           const cx<double>* X) {
+        for (int it = tid; it < NL * N2; it += nthr) {
+            const int line = it / N2, n2 = it - line * N2;
+            const int u = u0 + line / NF, f = line % NF;
+            cx<T> v[N1];
+            const long long vec = (long long)slot * vm.vstride + (long long)f * vm.voffb;
+            if (u < g.n_units && vec < vm.n_vec) {
+                const int zmax = g.unit_zmax[u];
+                const cx<double>* src = X + vec * g.n_g + g.unit_off[u];
+                const bool half00 = GAMMA && u == 0;
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    const int nz = wrap_signed(N2 * n1 + n2, N);
+                    cx<T> val = mk<T>(0, 0);
+                    if (nz <= zmax && nz >= -zmax) {
+                        if (half00) {
+                            cx<double> c = src[nz >= 0 ? nz : -nz];
+                            val = mk<T>((T)c.x, (T)(nz >= 0 ? c.y : -c.y));
+                            if (nz == 0) val.y = 0;     // c(0) of a real function is real
+                        } else {
+                            val = cvt<T>(src[nz + zmax]);
+                        }
+                    }
+                    v[n1] = val;
+                }
+                Dft<T, N1, +1>::run(v);
+            } else {
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) v[n1] = mk<T>(0, 0);
+            }
+            cx<T>* dst = lines + line * PITCH + n2;
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
+        }
+    }
+    // phase B: contiguous DFT-N2
+    static WHD void phaseB(int tid, int nthr, cx<T>* lines) {
+        for (int it = tid; it < NL * N1; it += nthr) {
+            const int line = it / N1, k1 = it - line * N1;
+            cx<T>* p = lines + line * PITCH + N2 * k1;
+            cx<T> v[N2];
+#pragma unroll
+            for (int j = 0; j < N2; ++j) v[j] = p[j];
+            Dft<T, N2, +1>::run(v);
+#pragma unroll
+            for (int j = 0; j < N2; ++j) p[j] = v[j];
+        }
+    }
+    // phase C: write sticks, column index fastest.  GAMMA: S+ = A + iB to column cp, S- = conj(A) + i conj(B) to its mirror.
+    static WHD void phaseC(int tid, int nthr, const cx<T>* lines, const WestGeom& g, int slot, int u0, cx<T>* W) {
+        for (int it = tid; it < N * CU; it += nthr) {
+            const int pos = it / CU, ul = it - pos * CU, u = u0 + ul;
+            if (u >= g.n_units) continue;
+            cx<T>* dst = W + ((long long)slot * N + pos) * g.n_cols;
+            if (GAMMA) {
+                const cx<T> a = lines[(2 * ul) * PITCH + pos], b = lines[(2 * ul + 1) * PITCH + pos];
+                const int cp = u + (g.n_cols - g.n_units);
+                dst[cp] = mk<T>(a.x - b.y, a.y + b.x);
+                if (u != 0) dst[g.n_cols - 1 - cp] = mk<T>(a.x + b.y, b.x - a.y);
+            } else {
+                dst[u] = lines[ul * PITCH + pos];
+            }
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------------------- K3
+struct K3Epi {
+    double scale;           // 1/N^3
+    int kinetic;            // 1: y += (g2 - shift[vec]) * x
+    const double* shift;    // [n_vec] or NULL (0)
+    double omega;           // i*omega shift: FULL y -= i omega x ; GAMMA (pairs f=0: Re, f=1: Im)  y_a += omega x_b, y_b -= omega x_a
+    const cx<double>* X;    // input vectors (kinetic / shift terms), may be NULL when kinetic == 0
+};
+
+template <typename T, int N1, int N2, bool GAMMA, int CU>
+struct K3 {
+    static constexpr int N = N1 * N2, PITCH = N + 1, NF = GAMMA ? 2 : 1, NL = CU * NF;
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + N);
+
+    static WHD void phaseA(int tid, int nthr, cx<T>* lines, const WestGeom& g, int slot, int u0, const cx<T>* W) {
+        for (int it = tid; it < N * CU; it += nthr) {
+            const int pos = it / CU, ul = it - pos * CU, u = u0 + ul;
+            const cx<T>* src = W + ((long long)slot * N + pos) * g.n_cols;
+            if (GAMMA) {
+                cx<T> a = mk<T>(0, 0), b = mk<T>(0, 0);
+                if (u < g.n_units) {
+                    const int cp = u + (g.n_cols - g.n_units);
+                    const cx<T> sp = src[cp];
+                    const cx<T> sm = u == 0 ? sp : src[g.n_cols - 1 - cp];
+                    a = mk<T>((T)0.5 * (sp.x + sm.x), (T)0.5 * (sp.y - sm.y));      // (S+ + conj S-)/2
+                    b = mk<T>((T)0.5 * (sp.y + sm.y), (T)0.5 * (sm.x - sp.x));      // (S+ - conj S-)/(2i)
+                }
+                lines[(2 * ul) * PITCH + pos] = a;
+                lines[(2 * ul + 1) * PITCH + pos] = b;
+            } else {
+                lines[ul * PITCH + pos] = u < g.n_units ? src[u] : mk<T>(0, 0);
+            }
+        }
+    }
+    // phase B': contiguous DFT-N2 (sign -), twiddle
+    static WHD void phaseB(int tid, int nthr, cx<T>* lines, const cx<T>* tw) {
+        for (int it = tid; it < NL * N1; it += nthr) {
+            const int line = it / N1, k1 = it - line * N1;
+            cx<T>* p = lines + line * PITCH + N2 * k1;
+            cx<T> v[N2];
+#pragma unroll
+            for (int j = 0; j < N2; ++j) v[j] = p[j];
+            Dft<T, N2, -1>::run(v);
+#pragma unroll
+            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
+        }
+    }
+    // phase A': strided DFT-N1 (sign -), epilogue to the sphere
+    static WHD void phaseC(int tid, int nthr, const cx<T>* lines, const WestGeom& g, VecMap vm, int slot, int u0,
+                           K3Epi e, cx<double>* Y) {
+        for (int it = tid; it < NL * N2; it += nthr) {
+            const int line = it / N2, n2 = it - line * N2;
+            const int u = u0 + line / NF, f = line % NF;
+            const long long vec = (long long)slot * vm.vstride + (long long)f * vm.voffb;
+            if (u >= g.n_units || vec >= vm.n_vec) continue;
+            const cx<T>* p = lines + line * PITCH + n2;
+            cx<T> v[N1];
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
+            Dft<T, N1, -1>::run(v);
+            const int zmax = g.unit_zmax[u];
+            const bool half00 = GAMMA && u == 0;
+            const long long base = vec * g.n_g + g.unit_off[u];
+            const long long pbase = GAMMA ? ((long long)slot * vm.vstride + (long long)(1 - f) * vm.voffb) * g.n_g + g.unit_off[u] : 0;
+            const double sh = (e.kinetic && e.shift) ? e.shift[vec] : 0.0;
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int nz = wrap_signed(N2 * n1 + n2, N);
+                if (nz > zmax || nz < (half00 ? 0 : -zmax)) continue;
+                const long long o = half00 ? nz : nz + zmax;
+                cx<double> r = mk<double>(e.scale * (double)v[n1].x, e.scale * (double)v[n1].y);
+                if (e.kinetic) {
+                    const double d = g.g2[g.unit_off[u] + o] - sh;
+                    const cx<double> x = e.X[base + o];
+                    r.x += d * x.x; r.y += d * x.y;
+                    if (e.omega != 0.0) {
+                        if (GAMMA) {
+                            const cx<double> xp = e.X[pbase + o];
+                            const double w = f == 0 ? e.omega : -e.omega;
+                            r.x += w * xp.x; r.y += w * xp.y;
+                        } else {
+                            r.x += e.omega * x.y; r.y -= e.omega * x.x;
+                        }
+                    }
+                }
+                if (half00 && nz == 0) r.y = 0.0;
+                Y[base + o] = r;
+            }
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------------------- K2
+enum { K2_H = 0, K2_TOR = 1, K2_DN = 2, K2_FROMR = 3 };
+
+template <typename T>
+struct K2Args {
+    cx<T>* W;                   // [n_slots][N][n_cols] stick intermediate (in place)
+    const T* V;                 // K2_H: V_loc in position order [pz][py][px]
+    cx<double>* R;              // K2_TOR: out [n_slots][N^3] ; K2_FROMR with ucache == NULL: in
+    const cx<double>* ucache;   // K2_DN / K2_FROMR: occupied orbitals in real space [n_uslots][N^3] position order
+    const double* dV;           // K2_FROMR: [n_pert][N^3] position order (real)
+    double* dn;                 // K2_DN: [n_pert][N^3] position order, accumulated with atomics
+    int n_uslots;               // slot = ipert * n_uslots + uslot
+    double fac;                 // K2_DN: 4/Omega
+};
+
+template <typename T, int N1, int N2, int MODE, int LC>
+struct K2 {
+    static constexpr int N = N1 * N2, PITCH = N + 1;
+    static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + N); }
+
+    static WHD cx<T> load_disc(const cx<T>* Wp, const WestGeom& g, int row, int n) {
+        const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
+        const int ny = wrap_signed(n, N);
+        return (ny <= ymax && ny >= -ymax) ? Wp[c0 + ny + ymax] : mk<T>(0, 0);
+    }
+    // y inverse, pass A: rows of the disc straight from W
+    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp) {
+        for (int it = tid; it < g.nr * N2; it += nthr) {
+            const int row = it / N2, n2 = it - row * N2;
+            cx<T> v[N1];
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) v[n1] = load_disc(Wp, g, row, N2 * n1 + n2);
+            Dft<T, N1, +1>::run(v);
+            cx<T>* dst = S + row * PITCH + n2;
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
+        }
+    }
+    static WHD void yB(int tid, int nthr, cx<T>* S, const WestGeom& g) {
+        for (int it = tid; it < g.nr * N1; it += nthr) {
+            const int row = it / N1, k1 = it - row * N1;
+            cx<T>* p = S + row * PITCH + N2 * k1;
+            cx<T> v[N2];
+#pragma unroll
+            for (int j = 0; j < N2; ++j) v[j] = p[j];
+            Dft<T, N2, +1>::run(v);
+#pragma unroll
+            for (int j = 0; j < N2; ++j) p[j] = v[j];
+        }
+    }
+    // x inverse, pass A: gather the 2 n_max + 1 non-zero inputs of LC lines from S
+    static WHD void xA(int tid, int nthr, const cx<T>* S, cx<T>* X, const cx<T>* tw, const WestGeom& g, int py0) {
+        for (int it = tid; it < LC * N2; it += nthr) {
+            const int l = it / N2, n2 = it - l * N2;
+            const int py = py0 + l;
+            if (py >= N) continue;
+            cx<T> v[N1];
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int nx = wrap_signed(N2 * n1 + n2, N);
+                v[n1] = (nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + py] : mk<T>(0, 0);
+            }
+            Dft<T, N1, +1>::run(v);
+            cx<T>* dst = X + l * PITCH + n2;
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
+        }
+    }
+    // x inverse pass B, the real-space operation, x forward pass B' - all on the same N2 contiguous values
+    static WHD void xB(int tid, int nthr, cx<T>* X, const cx<T>* tw, const K2Args<T>& a, int slot, int pz, int py0) {
+        for (int it = tid; it < LC * N1; it += nthr) {
+            const int l = it / N1, k1 = it - l * N1;
+            const int py = py0 + l;
+            if (py >= N) continue;
+            cx<T>* p = X + l * PITCH + N2 * k1;
+            const long long r0 = ((long long)pz * N + py) * N + N2 * k1;      // position-order real-space index
+            const long long n3 = (long long)N * N * N;
+            cx<T> v[N2];
+            if (MODE != K2_FROMR) {
+#pragma unroll
+                for (int j = 0; j < N2; ++j) v[j] = p[j];
+                Dft<T, N2, +1>::run(v);
+            }
+            if (MODE == K2_H) {
+                const T* V = a.V + r0;
+#pragma unroll
+                for (int j = 0; j < N2; ++j) { const T w = V[j]; v[j].x *= w; v[j].y *= w; }
+            } else if (MODE == K2_TOR) {
+                cx<double>* R = a.R + (long long)slot * n3 + r0;
+#pragma unroll
+                for (int j = 0; j < N2; ++j) R[j] = cvd<T>(v[j]);
+                continue;
+            } else if (MODE == K2_DN) {
+                const int ip = slot / a.n_uslots, us = slot - ip * a.n_uslots;
+                const cx<double>* U = a.ucache + (long long)us * n3 + r0;
+                double* D = a.dn + (long long)ip * n3 + r0;
+#pragma unroll
+                for (int j = 0; j < N2; ++j) {
+                    const cx<double> u = U[j];
+                    const double val = a.fac * ((double)v[j].x * u.x + (double)v[j].y * u.y);
+#ifdef __CUDA_ARCH__
+                    atomicAdd(D + j, val);
+#else
+                    D[j] += val;
+#endif
+                }
+                continue;
+            } else {   // K2_FROMR
+                if (a.ucache) {
+                    const int ip = slot / a.n_uslots, us = slot - ip * a.n_uslots;
+                    const cx<double>* U = a.ucache + (long long)us * n3 + r0;
+                    const double* D = a.dV + (long long)ip * n3 + r0;
+#pragma unroll
+                    for (int j = 0; j < N2; ++j) { const double w = D[j]; const cx<double> u = U[j]; v[j] = mk<T>((T)(u.x * w), (T)(u.y * w)); }
+                } else {
+                    const cx<double>* R = a.R + (long long)slot * n3 + r0;
+#pragma unroll
+                    for (int j = 0; j < N2; ++j) v[j] = cvt<T>(R[j]);
+                }
+            }
+            Dft<T, N2, -1>::run(v);
+#pragma unroll
+            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
+        }
+    }
+    // x forward pass A': strided DFT-N1, keep |n_x| <= n_max, back into S
+    static WHD void xC(int tid, int nthr, cx<T>* S, const cx<T>* X, const WestGeom& g, int py0) {
+        for (int it = tid; it < LC * N2; it += nthr) {
+            const int l = it / N2, n2 = it - l * N2;
+            const int py = py0 + l;
+            if (py >= N) continue;
+            const cx<T>* p = X + l * PITCH + n2;
+            cx<T> v[N1];
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
+            Dft<T, N1, -1>::run(v);
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int nx = wrap_signed(N2 * n1 + n2, N);
+                if (nx <= g.n_max && nx >= -g.n_max) S[(nx + g.n_max) * PITCH + py] = v[n1];
+            }
+        }
+    }
+    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g) {
+        for (int it = tid; it < g.nr * N1; it += nthr) {
+            const int row = it / N1, k1 = it - row * N1;
+            cx<T>* p = S + row * PITCH + N2 * k1;
+            cx<T> v[N2];
+#pragma unroll
+            for (int j = 0; j < N2; ++j) v[j] = p[j];
+            Dft<T, N2, -1>::run(v);
+#pragma unroll
+            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
+        }
+    }
+    static WHD void yD(int tid, int nthr, const cx<T>* S, const WestGeom& g, cx<T>* Wp) {
+        for (int it = tid; it < g.nr * N2; it += nthr) {
+            const int row = it / N2, n2 = it - row * N2;
+            const cx<T>* p = S + row * PITCH + n2;
+            cx<T> v[N1];
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
+            Dft<T, N1, -1>::run(v);
+            const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
+#pragma unroll
+            for (int n1 = 0; n1 < N1; ++n1) {
+                const int ny = wrap_signed(N2 * n1 + n2, N);
+                if (ny <= ymax && ny >= -ymax) Wp[c0 + ny + ymax] = v[n1];
+            }
+        }
+    }
+};
+
+#ifdef __CUDACC__
+template <typename T, int N>
+__device__ __forceinline__ void load_tw(cx<T>* tw_s, const cx<double>* tw_g) {
+    for (int i = threadIdx.x; i < N; i += blockDim.x) tw_s[i] = cvt<T>(tw_g[i]);
+}
+
+template <typename T, int N1, int N2, bool GAMMA, int CU>
+__global__ void __launch_bounds__(256) k1_g2r_z(WestGeom g, VecMap vm, const cx<double>* X, cx<T>* W) {
+    using K = K1<T, N1, N2, GAMMA, CU>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* lines = reinterpret_cast<cx<T>*>(smem_raw);
+    cx<T>* tw = lines + K::NL * K::PITCH;
+    load_tw<T, K::N>(tw, g.tw);
+    __syncthreads();
+    const int slot = blockIdx.y, u0 = blockIdx.x * CU;
+    K::phaseA(threadIdx.x, blockDim.x, lines, tw, g, vm, slot, u0, X);
+    __syncthreads();
+    K::phaseB(threadIdx.x, blockDim.x, lines);
+    __syncthreads();
+    K::phaseC(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
+}
+
+template <typename T, int N1, int N2, bool GAMMA, int CU>
+__global__ void __launch_bounds__(256) k3_r2g_z(WestGeom g, VecMap vm, const cx<T>* W, K3Epi e, cx<double>* Y) {
+    using K = K3<T, N1, N2, GAMMA, CU>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* lines = reinterpret_cast<cx<T>*>(smem_raw);
+    cx<T>* tw = lines + K::NL * K::PITCH;
+    load_tw<T, K::N>(tw, g.tw);
+    const int slot = blockIdx.y, u0 = blockIdx.x * CU;
+    K::phaseA(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
+    __syncthreads();
+    K::phaseB(threadIdx.x, blockDim.x, lines, tw);
+    __syncthreads();
+    K::phaseC(threadIdx.x, blockDim.x, lines, g, vm, slot, u0, e, Y);
+}
+
+template <typename T, int N1, int N2, int MODE, int LC, int NT>
+__global__ void __launch_bounds__(NT) k2_planes(WestGeom g, K2Args<T> a) {
+    using K = K2<T, N1, N2, MODE, LC>;
+    constexpr int N = K::N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);
+    cx<T>* X = S + g.nr * K::PITCH;
+    cx<T>* tw = X + LC * K::PITCH;
+    load_tw<T, N>(tw, g.tw);
+    const int pz = blockIdx.x, slot = blockIdx.y;
+    cx<T>* Wp = a.W + ((long long)slot * N + pz) * g.n_cols;
+    __syncthreads();
+    if (MODE != K2_FROMR) {
+        K::yA(threadIdx.x, NT, S, tw, g, Wp);
+        __syncthreads();
+        K::yB(threadIdx.x, NT, S, g);
+        __syncthreads();
+    }
+    for (int py0 = 0; py0 < N; py0 += LC) {
+        if (MODE != K2_FROMR) {
+            K::xA(threadIdx.x, NT, S, X, tw, g, py0);
+            __syncthreads();
+        }
+        K::xB(threadIdx.x, NT, X, tw, a, slot, pz, py0);
+        if (MODE == K2_H || MODE == K2_FROMR) {
+            __syncthreads();
+            K::xC(threadIdx.x, NT, S, X, g, py0);
+        }
+        __syncthreads();
+    }
+    if (MODE == K2_H || MODE == K2_FROMR) {
+        K::yC(threadIdx.x, NT, S, tw, g);
+        __syncthreads();
+        K::yD(threadIdx.x, NT, S, g, Wp);
+    }
+}
+#endif
