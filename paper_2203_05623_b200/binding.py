@@ -1,0 +1,224 @@
+"""Thin ctypes binding of include/west.h: same names, argument marshalling only.
+
+Device buffers are torch CUDA tensors (PyTorch is the allocator and stream provider); their ``data_ptr()`` is what crosses
+the C ABI.  Host arrays are numpy.  Nothing here computes: every step of the path runs in libwest.so's kernels, and the
+import fails loudly if the library is missing (no CPU fallback).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libwest.so")
+
+WEST_OK, WEST_NOTCONVERGED = 0, 1
+WEST_EINVAL, WEST_ECUDA, WEST_ESTATE, WEST_ENOMEM = -1, -2, -3, -4
+WEST_FULL, WEST_GAMMA = 0, 1
+WEST_FP64, WEST_MIXED = 0, 1
+
+
+class west_cell(C.Structure):
+    _fields_ = [("L", C.c_double), ("n2max", C.c_int32), ("N", C.c_int32), ("mode", C.c_int32)]
+
+
+class west_cg_opts(C.Structure):
+    _fields_ = [("max_iter", C.c_int32), ("tol", C.c_double), ("alpha_pv", C.c_double), ("precond", C.c_int32),
+                ("check_every", C.c_int32)]
+
+
+class west_stats(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("n_unconverged", C.c_int32), ("resid_max", C.c_double), ("n_h_apply", C.c_int64),
+                ("ms_rhs", C.c_float), ("ms_cg", C.c_float), ("ms_dn", C.c_float)]
+
+
+EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states",
+           "west_fft3d", "west_h_apply", "west_chi0_apply", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
+           "west_launch_count", "west_set_fft_chunk"]
+
+
+def load_library():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("%s is missing: run `python -m paper_2203_05623_b200.build` (there is no CPU fallback)" % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    lib.west_create.argtypes = [C.POINTER(vp), C.POINTER(west_cell), vp]
+    lib.west_destroy.argtypes = [vp]
+    lib.west_last_error.argtypes = [vp]
+    lib.west_last_error.restype = C.c_char_p
+    lib.west_gsphere.argtypes = [vp, C.POINTER(i64), vp, vp, vp, vp]
+    lib.west_set_vloc.argtypes = [vp, vp]
+    lib.west_set_kb.argtypes = [vp, i32, vp, vp]
+    lib.west_set_states.argtypes = [vp, i32, vp, vp]
+    lib.west_fft3d.argtypes = [vp, i32, i32, i32, vp, vp]
+    lib.west_h_apply.argtypes = [vp, i32, i32, vp, vp]
+    lib.west_chi0_apply.argtypes = [vp, i32, i32, vp, i32, vp, C.POINTER(west_cg_opts), vp, vp, C.POINTER(west_stats)]
+    lib.west_gemm_tn.argtypes = [vp, i32, i32, i64, vp, i64, vp, i64, vp, i64]
+    lib.west_gemm_update.argtypes = [vp, i32, i32, i64, vp, i64, vp, i64, vp, i64]
+    lib.west_device_bytes.argtypes = [vp]
+    lib.west_device_bytes.restype = i64
+    lib.west_launch_count.argtypes = [vp]
+    lib.west_launch_count.restype = i64
+    lib.west_set_fft_chunk.argtypes = [vp, i32]
+    for name in EXPORTS:
+        getattr(lib, name)
+        if name not in ("west_last_error", "west_device_bytes", "west_launch_count"):
+            getattr(lib, name).restype = C.c_int
+    return lib
+
+
+class WestError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("west error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _dev(t, dtype=None):
+    """device pointer of a contiguous CUDA tensor"""
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("expected a CUDA torch tensor")
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return C.c_void_p(t.data_ptr())
+
+
+class West:
+    """One west_ctx.  Method names follow the C entry points (west_ prefix dropped)."""
+
+    def __init__(self, L, n2max, N, mode, stream=None):
+        import torch
+        self.lib = load_library()
+        self.cell = west_cell(float(L), int(n2max), int(N), int(mode))
+        self.ctx = C.c_void_p()
+        if stream is None:
+            stream = torch.cuda.current_stream()
+        self.stream = stream
+        rc = self.lib.west_create(C.byref(self.ctx), C.byref(self.cell), C.c_void_p(stream.cuda_stream))
+        if rc != 0:
+            raise WestError(rc, (self.lib.west_last_error(None) or b"").decode())
+        n_g = C.c_int64()
+        self._ck(self.lib.west_gsphere(self.ctx, C.byref(n_g), None, None, None, None))
+        self.n_g = int(n_g.value)
+        self.N, self.mode, self.L = int(N), int(mode), float(L)
+
+    def _ck(self, rc):
+        if rc < 0:
+            raise WestError(rc, (self.lib.west_last_error(self.ctx) or b"").decode())
+        return rc
+
+    def close(self):
+        if self.ctx:
+            self.lib.west_destroy(self.ctx)
+            self.ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def gsphere(self):
+        miller = np.empty((self.n_g, 3), dtype=np.int32)
+        idx = np.empty(self.n_g, dtype=np.int32)
+        idxm = np.empty(self.n_g, dtype=np.int32)
+        g2 = np.empty(self.n_g, dtype=np.float64)
+        n = C.c_int64()
+        self._ck(self.lib.west_gsphere(self.ctx, C.byref(n), miller.ctypes.data, idx.ctypes.data, idxm.ctypes.data, g2.ctypes.data))
+        return miller, idx, idxm, g2
+
+    def set_vloc(self, vloc):
+        import torch
+        assert vloc.numel() == self.N ** 3
+        self._ck(self.lib.west_set_vloc(self.ctx, _dev(vloc, torch.float64)))
+
+    def set_kb(self, beta, dcoef):
+        import torch
+        d = np.ascontiguousarray(dcoef, dtype=np.float64)
+        n_proj = 0 if beta is None else int(beta.shape[0])
+        if n_proj:
+            assert beta.shape[1] == self.n_g and len(d) == n_proj
+        self._ck(self.lib.west_set_kb(self.ctx, n_proj, _dev(beta, torch.complex128) if n_proj else None, d.ctypes.data if n_proj else None))
+
+    def set_states(self, psi, eps):
+        import torch
+        e = np.ascontiguousarray(eps, dtype=np.float64)
+        assert psi.shape[1] == self.n_g and len(e) == psi.shape[0]
+        self._ck(self.lib.west_set_states(self.ctx, int(psi.shape[0]), _dev(psi, torch.complex128), e.ctypes.data))
+
+    def fft3d(self, dir, x, out=None, precision=WEST_FP64):
+        import torch
+        N = self.N
+        n_batch = int(x.shape[0])
+        if dir == 1:
+            assert x.shape[1] == self.n_g
+            if out is None:
+                out = torch.empty((n_batch, N, N, N), dtype=torch.float64 if self.mode == WEST_GAMMA else torch.complex128, device=x.device)
+            self._ck(self.lib.west_fft3d(self.ctx, 1, precision, n_batch, _dev(x, torch.complex128), _dev(out)))
+        else:
+            if out is None:
+                out = torch.empty((n_batch, self.n_g), dtype=torch.complex128, device=x.device)
+            self._ck(self.lib.west_fft3d(self.ctx, -1, precision, n_batch, _dev(x, torch.float64 if self.mode == WEST_GAMMA else torch.complex128), _dev(out, torch.complex128)))
+        return out
+
+    def h_apply(self, x, out=None, precision=WEST_FP64):
+        import torch
+        assert x.shape[1] == self.n_g
+        if out is None:
+            out = torch.empty_like(x)
+        self._ck(self.lib.west_h_apply(self.ctx, precision, int(x.shape[0]), _dev(x, torch.complex128), _dev(out, torch.complex128)))
+        return out
+
+    def chi0_apply(self, dV, omegas, tol=1e-12, max_iter=500, alpha_pv=1.0, precond=1, check_every=4, precision=WEST_FP64,
+                   dn=None, want_dpsi=False, n_occ=None, want_stats=True):
+        import torch
+        N = self.N
+        n_pert = int(dV.shape[0])
+        om = np.ascontiguousarray(omegas, dtype=np.float64)
+        n_freq = len(om)
+        if dn is None:
+            dn = torch.empty((n_freq, n_pert, N, N, N), dtype=torch.float64, device=dV.device)
+        dpsi = None
+        if want_dpsi:
+            assert n_occ is not None
+            shape = (n_freq, n_pert, n_occ, 2, self.n_g) if self.mode == WEST_GAMMA else (n_freq, n_pert, n_occ, self.n_g)
+            dpsi = torch.empty(shape, dtype=torch.complex128, device=dV.device)
+        opts = west_cg_opts(int(max_iter), float(tol), float(alpha_pv), int(precond), int(check_every))
+        st = west_stats()
+        rc = self._ck(self.lib.west_chi0_apply(self.ctx, precision, n_pert, _dev(dV, torch.float64), n_freq, om.ctypes.data, C.byref(opts),
+                                               _dev(dn, torch.float64), _dev(dpsi) if dpsi is not None else None,
+                                               C.byref(st) if want_stats else None))
+        stats = {k: getattr(st, k) for k, _ in west_stats._fields_}
+        stats["rc"] = rc
+        return dn, dpsi, stats
+
+    def gemm_tn(self, A, B, out=None):
+        """C[m][n] = sum_k A[m][k] B[n][k], f64 row-major."""
+        import torch
+        m, k = A.shape
+        n = B.shape[0]
+        if out is None:
+            out = torch.empty((m, n), dtype=torch.float64, device=A.device)
+        self._ck(self.lib.west_gemm_tn(self.ctx, m, n, k, _dev(A, torch.float64), A.stride(0), _dev(B, torch.float64), B.stride(0),
+                                       _dev(out, torch.float64), out.stride(0)))
+        return out
+
+    def gemm_update(self, Cm, A, Y):
+        """Y[n][k] += sum_m C[m][n] A[m][k]."""
+        import torch
+        m, k = A.shape
+        n = Y.shape[0]
+        self._ck(self.lib.west_gemm_update(self.ctx, m, n, k, _dev(Cm, torch.float64), Cm.stride(0), _dev(A, torch.float64), A.stride(0),
+                                           _dev(Y, torch.float64), Y.stride(0)))
+        return Y
+
+    def device_bytes(self):
+        return int(self.lib.west_device_bytes(self.ctx))
+
+    def launch_count(self):
+        return int(self.lib.west_launch_count(self.ctx))
+
+    def set_fft_chunk(self, n):
+        self._ck(self.lib.west_set_fft_chunk(self.ctx, int(n)))

@@ -1,0 +1,72 @@
+"""Builds paper_2203_05623_b200/libwest.so (the C-ABI library of include/west.h) with nvcc for sm_100a, in-tree.
+
+    python -m paper_2203_05623_b200.build [--force]
+
+No torch involvement: the library links only against the CUDA runtime.
+"""
+import concurrent.futures as cf
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+ROOT = os.path.dirname(HERE)
+OBJ = os.path.join(ROOT, "build", "west_obj")
+LIB = os.path.join(HERE, "libwest.so")
+
+# (N1, N2, N, LC): N = N1*N2 grid size; LC = x lines per chunk in the plane kernel
+FFT_SIZES = [(4, 6, 24, 24), (6, 6, 36, 36), (6, 8, 48, 24), (8, 9, 72, 24), (12, 12, 144, 16)]
+NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
+
+
+def _nvcc():
+    for p in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
+        if p and (os.path.isabs(p) and os.path.exists(p) or not os.path.isabs(p)):
+            return p
+    raise RuntimeError("nvcc not found")
+
+
+def _sources():
+    out = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h", ".hpp"))]
+    out.append(os.path.join(ROOT, "include", "west.h"))
+    out.append(os.path.abspath(__file__))
+    return out
+
+
+def up_to_date():
+    if not os.path.exists(LIB):
+        return False
+    t = os.path.getmtime(LIB)
+    return all(os.path.getmtime(s) <= t for s in _sources())
+
+
+def _run(cmd):
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("command failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    return r
+
+
+def build(force=False, verbose=False):
+    if not force and up_to_date():
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
+    nvcc = _nvcc()
+    jobs = []
+    for n1, n2, n, lc in FFT_SIZES:
+        o = os.path.join(OBJ, "fft_%d.o" % n)
+        jobs.append((o, [nvcc] + NVCC_FLAGS + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_LC=%d" % lc,
+                                               "-c", os.path.join(CSRC, "fft_n.cu"), "-o", o]))
+    o = os.path.join(OBJ, "west.o")
+    jobs.append((o, [nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "west.cu"), "-o", o]))
+    with cf.ThreadPoolExecutor(max_workers=min(8, len(jobs))) as ex:
+        list(ex.map(lambda j: _run(j[1]), jobs))
+    _run([nvcc, "-shared", "-o", LIB] + [j[0] for j in jobs] + ["-gencode", "arch=compute_100a,code=sm_100a"])
+    if verbose:
+        print("built", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    build(force="--force" in sys.argv, verbose=True)

@@ -1,0 +1,241 @@
+// Batched preconditioned CG / COCG for Eq. 10: one recurrence per column (perturbation i, state v),
+// all columns advanced together, per-column scalars kept on the device.  Readings R3-R5, R7 of DESIGN.md.
+//   MODE 0  WEST_GAMMA, omega = 0 : real functions, <f,g> = 2 sum_reals f g - f(0) g(0)
+//   MODE 1  WEST_GAMMA, omega > 0 : column = (Re, Im) pair of real functions, COCG with the unconjugated bilinear form
+//                                   (x,y) = <xR,yR> - <xI,yI> + i(<xR,yI> + <xI,yR>)  = int x(r) y(r) dr
+//   MODE 2  WEST_FULL,  omega = 0 : complex vectors, Hermitian inner product
+// One CTA per column; vectors are [col][nvpc][n_g] complex128, nvpc = 2 in MODE 1 else 1.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace wcg {
+
+constexpr int NT = 256;
+
+struct Scalars {
+    double2* rz;      // (r, z)
+    double2* pAp;     // (p, A p)
+    double2* rznew;
+    double*  rr;      // Hermitian ||r||^2
+    double*  b2;      // ||b||^2
+    int*     active;  // 1 while ||r|| > tol ||b||
+    int*     counters;   // [0] number of active columns after the last p-update
+    double*  resid_max;  // [1] max ||r||/||b|| (as bits-ordered non-negative double, atomicMax on long long)
+};
+
+__device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
+    const double d = b.x * b.x + b.y * b.y;
+    return make_double2((a.x * b.x + a.y * b.y) / d, (a.y * b.x - a.x * b.y) / d);
+}
+__device__ __forceinline__ double2 cmul2(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
+// block reduction of up to 4 doubles
+template <int NV>
+__device__ __forceinline__ void block_reduce(double (&v)[NV], double* sh /* [NV*8] */) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0)
+#pragma unroll
+        for (int i = 0; i < NV; ++i) sh[i * 8 + warp] = v[i];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        double s = 0;
+#pragma unroll
+        for (int w = 0; w < NT / 32; ++w) s += sh[i * 8 + w];
+        v[i] = s;
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ double precond(double g2, double tk, int on) {
+    if (!on) return 1.0;
+    const double q = g2 / (1.35 * tk);
+    return 1.0 / fmax(1.0, q);
+}
+
+// accumulate the mode's inner products of (a, b) over this thread's elements.  out: [0]=re, [1]=im
+template <int MODE>
+__device__ __forceinline__ void dot_accum(const double2* a, const double2* b, long long n_g, int g, double w, double (&acc)[2]) {
+    // w: extra real weight on b (preconditioner), applied as a -> (a, w b)
+    if (MODE == 0) {
+        const double2 x = a[g], y = b[g];
+        acc[0] += (g == 0 ? x.x * y.x : 2.0 * (x.x * y.x + x.y * y.y)) * w;
+    } else if (MODE == 1) {
+        const double2 xr = a[g], xi = a[n_g + g], yr = b[g], yi = b[n_g + g];
+        const double f = g == 0 ? 1.0 : 2.0;
+        const double rr = g == 0 ? xr.x * yr.x : xr.x * yr.x + xr.y * yr.y;
+        const double ii = g == 0 ? xi.x * yi.x : xi.x * yi.x + xi.y * yi.y;
+        const double ri = g == 0 ? xr.x * yi.x : xr.x * yi.x + xr.y * yi.y;
+        const double ir = g == 0 ? xi.x * yr.x : xi.x * yr.x + xi.y * yr.y;
+        acc[0] += f * (rr - ii) * w;
+        acc[1] += f * (ri + ir) * w;
+    } else {
+        const double2 x = a[g], y = b[g];
+        acc[0] += (x.x * y.x + x.y * y.y) * w;
+        acc[1] += (x.x * y.y - x.y * y.x) * w;
+    }
+}
+template <int MODE>
+__device__ __forceinline__ double norm_accum(const double2* a, long long n_g, int g) {
+    if (MODE == 0) { const double2 x = a[g]; return g == 0 ? x.x * x.x : 2.0 * (x.x * x.x + x.y * x.y); }
+    if (MODE == 1) {
+        const double2 xr = a[g], xi = a[n_g + g];
+        return g == 0 ? xr.x * xr.x + xi.x * xi.x : 2.0 * (xr.x * xr.x + xr.y * xr.y + xi.x * xi.x + xi.y * xi.y);
+    }
+    const double2 x = a[g];
+    return x.x * x.x + x.y * x.y;
+}
+
+// r holds b on entry.  p = M r, rz = (r, M r), b2 = rr = ||r||^2, active = b2 > 0
+template <int MODE>
+__global__ void __launch_bounds__(NT) cg_init(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
+                                              const double2* R, double2* P, Scalars s) {
+    __shared__ double sh[32];
+    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    const double2* r = R + (long long)col * nvpc * n_g;
+    double2* p = P + (long long)col * nvpc * n_g;
+    const double tkv = tk[col % n_occ];
+    double acc[3] = {0, 0, 0};
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        const double m = precond(g2[g], tkv, precond_on);
+        double d[2] = {0, 0};
+        dot_accum<MODE>(r, r, n_g, g, m, d);
+        acc[0] += d[0]; acc[1] += d[1];
+        acc[2] += norm_accum<MODE>(r, n_g, g);
+#pragma unroll
+        for (int q = 0; q < nvpc; ++q) {
+            const double2 x = r[q * n_g + g];
+            p[q * n_g + g] = make_double2(m * x.x, m * x.y);
+        }
+    }
+    block_reduce<3>(acc, sh);
+    if (threadIdx.x == 0) {
+        s.rz[col] = make_double2(acc[0], MODE == 1 ? acc[1] : 0.0);
+        s.b2[col] = acc[2];
+        s.rr[col] = acc[2];
+        const int act = acc[2] > 0.0;
+        s.active[col] = act;
+        if (act) atomicAdd(s.counters, 1);
+    }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(NT) cg_dot_pAp(long long n_g, const double2* P, const double2* AP, Scalars s) {
+    __shared__ double sh[16];
+    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    if (!s.active[col]) return;
+    const double2* p = P + (long long)col * nvpc * n_g;
+    const double2* ap = AP + (long long)col * nvpc * n_g;
+    double acc[2] = {0, 0};
+    for (int g = threadIdx.x; g < n_g; g += NT) dot_accum<MODE>(p, ap, n_g, g, 1.0, acc);
+    block_reduce<2>(acc, sh);
+    if (threadIdx.x == 0) s.pAp[col] = make_double2(acc[0], MODE == 1 ? acc[1] : 0.0);
+}
+
+// x += a p ; r -= a Ap ; rznew = (r, M r) ; rr = ||r||^2
+template <int MODE>
+__global__ void __launch_bounds__(NT) cg_update_xr(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
+                                                   const double2* P, const double2* AP, double2* X, double2* R, Scalars s) {
+    __shared__ double sh[32];
+    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    if (!s.active[col]) return;
+    const long long o = (long long)col * nvpc * n_g;
+    const double2* p = P + o; const double2* ap = AP + o;
+    double2* x = X + o; double2* r = R + o;
+    const double2 a = cdiv(s.rz[col], s.pAp[col]);
+    const double tkv = tk[col % n_occ];
+    double acc[3] = {0, 0, 0};
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        if (MODE == 1) {
+            const double2 pr = p[g], pi = p[n_g + g], qr = ap[g], qi = ap[n_g + g];
+            double2 xr = x[g], xi = x[n_g + g], rr = r[g], ri = r[n_g + g];
+            xr.x += a.x * pr.x - a.y * pi.x; xr.y += a.x * pr.y - a.y * pi.y;
+            xi.x += a.x * pi.x + a.y * pr.x; xi.y += a.x * pi.y + a.y * pr.y;
+            rr.x -= a.x * qr.x - a.y * qi.x; rr.y -= a.x * qr.y - a.y * qi.y;
+            ri.x -= a.x * qi.x + a.y * qr.x; ri.y -= a.x * qi.y + a.y * qr.y;
+            x[g] = xr; x[n_g + g] = xi; r[g] = rr; r[n_g + g] = ri;
+        } else {
+            const double2 pp = p[g], q = ap[g];
+            double2 xx = x[g], rr = r[g];
+            xx.x += a.x * pp.x; xx.y += a.x * pp.y;
+            rr.x -= a.x * q.x;  rr.y -= a.x * q.y;
+            x[g] = xx; r[g] = rr;
+        }
+        const double m = precond(g2[g], tkv, precond_on);
+        double d[2] = {0, 0};
+        dot_accum<MODE>(r, r, n_g, g, m, d);      // re-reads this thread's own freshly written r
+        acc[0] += d[0]; acc[1] += d[1];
+        acc[2] += norm_accum<MODE>(r, n_g, g);
+    }
+    block_reduce<3>(acc, sh);
+    if (threadIdx.x == 0) {
+        s.rznew[col] = make_double2(acc[0], MODE == 1 ? acc[1] : 0.0);
+        s.rr[col] = acc[2];
+    }
+}
+
+// p = M r + beta p ; rz = rznew ; convergence bookkeeping
+template <int MODE>
+__global__ void __launch_bounds__(NT) cg_update_p(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
+                                                  double tol2, const double2* R, double2* P, Scalars s) {
+    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    if (!s.active[col]) return;
+    const long long o = (long long)col * nvpc * n_g;
+    const double2* r = R + o; double2* p = P + o;
+    const double rr = s.rr[col], b2 = s.b2[col];
+    const bool still = rr > tol2 * b2;
+    const double2 beta = cdiv(s.rznew[col], s.rz[col]);
+    const double tkv = tk[col % n_occ];
+    if (still) {
+        for (int g = threadIdx.x; g < n_g; g += NT) {
+            const double m = precond(g2[g], tkv, precond_on);
+            if (MODE == 1) {
+                const double2 zr = r[g], zi = r[n_g + g], pr = p[g], pi = p[n_g + g];
+                p[g] = make_double2(m * zr.x + beta.x * pr.x - beta.y * pi.x, m * zr.y + beta.x * pr.y - beta.y * pi.y);
+                p[n_g + g] = make_double2(m * zi.x + beta.x * pi.x + beta.y * pr.x, m * zi.y + beta.x * pi.y + beta.y * pr.y);
+            } else {
+                const double2 z = r[g], pp = p[g];
+                p[g] = make_double2(m * z.x + beta.x * pp.x, m * z.y + beta.x * pp.y);
+            }
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        s.rz[col] = s.rznew[col];
+        if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
+    }
+}
+
+// max over columns of sqrt(rr/b2), and count of columns above tol (final report)
+__global__ void cg_report(int n_col, double tol2, Scalars s, double* out /* [2]: resid_max, n_unconverged */) {
+    __shared__ double shm[NT]; __shared__ int shc[NT];
+    double m = 0; int c = 0;
+    for (int i = threadIdx.x; i < n_col; i += NT) {
+        const double b2 = s.b2[i];
+        if (b2 > 0) { const double q = s.rr[i] / b2; m = fmax(m, q); c += q > tol2; }
+    }
+    shm[threadIdx.x] = m; shc[threadIdx.x] = c;
+    __syncthreads();
+    for (int o = NT / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) { shm[threadIdx.x] = fmax(shm[threadIdx.x], shm[threadIdx.x + o]); shc[threadIdx.x] += shc[threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[0] = sqrt(shm[0]); out[1] = (double)shc[0]; }
+}
+
+// C[m][n] <- coef[m] * (gamma ? 2 C[m][n] - A[m][0] X[n][0] : C[m][n])      (A[m][0], X[n][0]: real part of G = 0)
+__global__ void lowrank_fix(int M, int Nn, long long ldc, double* C, const double* A, long long lda, const double* X, long long ldx,
+                            const double* coef, int gamma) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)M * Nn) return;
+    const int m = (int)(i / Nn), n = (int)(i - (long long)m * Nn);
+    double c = C[(long long)m * ldc + n];
+    if (gamma) c = 2.0 * c - A[(long long)m * lda] * X[(long long)n * ldx];
+    C[(long long)m * ldc + n] = coef[m] * c;
+}
+
+}  // namespace wcg

@@ -25,6 +25,7 @@ struct WestGeom {
 // vector <-> slot mapping of K1/K3: FFT f (0 or 1) of slot s is vector s*vstride + f*voffb; vectors >= n_vec are zero padding.
 struct VecMap {
     int vstride, voffb, n_vec;
+    int slot0;      // first slot of this launch (W is indexed by the launch-local slot, vectors by slot0 + slot)
 };
 
 template <typename T> WHD cx<T> cvt(cx<double> a) { return mk<T>((T)a.x, (T)a.y); }
@@ -44,7 +45,7 @@ struct K1 {
             const int line = it / N2, n2 = it - line * N2;
             const int u = u0 + line / NF, f = line % NF;
             cx<T> v[N1];
-            const long long vec = (long long)slot * vm.vstride + (long long)f * vm.voffb;
+            const long long vec = (long long)(vm.slot0 + slot) * vm.vstride + (long long)f * vm.voffb;
             if (u < g.n_units && vec < vm.n_vec) {
                 const int zmax = g.unit_zmax[u];
                 const cx<double>* src = X + vec * g.n_g + g.unit_off[u];
@@ -158,7 +159,7 @@ struct K3 {
         for (int it = tid; it < NL * N2; it += nthr) {
             const int line = it / N2, n2 = it - line * N2;
             const int u = u0 + line / NF, f = line % NF;
-            const long long vec = (long long)slot * vm.vstride + (long long)f * vm.voffb;
+            const long long vec = (long long)(vm.slot0 + slot) * vm.vstride + (long long)f * vm.voffb;
             if (u >= g.n_units || vec >= vm.n_vec) continue;
             const cx<T>* p = lines + line * PITCH + n2;
             cx<T> v[N1];
@@ -168,7 +169,7 @@ struct K3 {
             const int zmax = g.unit_zmax[u];
             const bool half00 = GAMMA && u == 0;
             const long long base = vec * g.n_g + g.unit_off[u];
-            const long long pbase = GAMMA ? ((long long)slot * vm.vstride + (long long)(1 - f) * vm.voffb) * g.n_g + g.unit_off[u] : 0;
+            const long long pbase = GAMMA ? ((long long)(vm.slot0 + slot) * vm.vstride + (long long)(1 - f) * vm.voffb) * g.n_g + g.unit_off[u] : 0;
             const double sh = (e.kinetic && e.shift) ? e.shift[vec] : 0.0;
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) {
@@ -208,7 +209,8 @@ struct K2Args {
     const cx<double>* ucache;   // K2_DN / K2_FROMR: occupied orbitals in real space [n_uslots][N^3] position order
     const double* dV;           // K2_FROMR: [n_pert][N^3] position order (real)
     double* dn;                 // K2_DN: [n_pert][N^3] position order, accumulated with atomics
-    int n_uslots;               // slot = ipert * n_uslots + uslot
+    int n_uslots;               // global slot = ipert * n_uslots + uslot
+    int slot0;                  // first global slot of this launch (W and R are indexed by the launch-local slot)
     double fac;                 // K2_DN: 4/Omega
 };
 
@@ -290,7 +292,7 @@ struct K2 {
                 for (int j = 0; j < N2; ++j) R[j] = cvd<T>(v[j]);
                 continue;
             } else if (MODE == K2_DN) {
-                const int ip = slot / a.n_uslots, us = slot - ip * a.n_uslots;
+                const int gs = a.slot0 + slot, ip = gs / a.n_uslots, us = gs - ip * a.n_uslots;
                 const cx<double>* U = a.ucache + (long long)us * n3 + r0;
                 double* D = a.dn + (long long)ip * n3 + r0;
 #pragma unroll
@@ -306,7 +308,7 @@ struct K2 {
                 continue;
             } else {   // K2_FROMR
                 if (a.ucache) {
-                    const int ip = slot / a.n_uslots, us = slot - ip * a.n_uslots;
+                    const int gs = a.slot0 + slot, ip = gs / a.n_uslots, us = gs - ip * a.n_uslots;
                     const cx<double>* U = a.ucache + (long long)us * n3 + r0;
                     const double* D = a.dV + (long long)ip * n3 + r0;
 #pragma unroll

@@ -1,0 +1,80 @@
+// Per-grid-size instantiation of the FFT kernels.  Compiled once per supported N with
+//   -DWEST_N1=.. -DWEST_N2=.. -DWEST_LC=..   (N = N1*N2; LC = x lines per chunk in K2)
+#include "fft_ops.h"
+
+#ifndef WEST_N1
+#error "compile with -DWEST_N1 -DWEST_N2 -DWEST_LC"
+#endif
+
+namespace {
+constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, LC = WEST_LC, CU = 16, NT2 = 256;
+
+template <typename KernelT>
+cudaError_t set_smem(KernelT k, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <typename T, bool GAMMA>
+cudaError_t k1_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const cx<double>* X, void* W) {
+    using K = K1<T, N1, N2, GAMMA, CU>;
+    auto kern = k1_g2r_z<T, N1, N2, GAMMA, CU>;
+    cudaError_t e = set_smem(kern, K::smem_bytes);
+    if (e != cudaSuccess) return e;
+    dim3 grid((g.n_units + CU - 1) / CU, n_slots);
+    kern<<<grid, 256, K::smem_bytes, st>>>(g, vm, X, reinterpret_cast<cx<T>*>(W));
+    return cudaGetLastError();
+}
+template <typename T, bool GAMMA>
+cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const void* W, K3Epi ep, cx<double>* Y) {
+    using K = K3<T, N1, N2, GAMMA, CU>;
+    auto kern = k3_r2g_z<T, N1, N2, GAMMA, CU>;
+    cudaError_t e = set_smem(kern, K::smem_bytes);
+    if (e != cudaSuccess) return e;
+    dim3 grid((g.n_units + CU - 1) / CU, n_slots);
+    kern<<<grid, 256, K::smem_bytes, st>>>(g, vm, reinterpret_cast<const cx<T>*>(W), ep, Y);
+    return cudaGetLastError();
+}
+template <typename T, int MODE>
+cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
+    using K = K2<T, N1, N2, MODE, LC>;
+    auto kern = k2_planes<T, N1, N2, MODE, LC, NT2>;
+    const size_t bytes = K::smem_bytes(g.nr);
+    cudaError_t e = set_smem(kern, bytes);
+    if (e != cudaSuccess) return e;
+    K2Args<T> t;
+    t.W = reinterpret_cast<cx<T>*>(a.W);
+    t.V = reinterpret_cast<const T*>(a.V);
+    t.R = a.R; t.ucache = a.ucache; t.dV = a.dV; t.dn = a.dn; t.n_uslots = a.n_uslots; t.slot0 = a.slot0; t.fac = a.fac;
+    dim3 grid(NN, n_slots);
+    kern<<<grid, NT2, bytes, st>>>(g, t);
+    return cudaGetLastError();
+}
+
+cudaError_t k1_entry(int f32, int gamma, int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const cx<double>* X, void* W) {
+    if (f32) return gamma ? k1_t<float, true>(n_slots, st, g, vm, X, W) : k1_t<float, false>(n_slots, st, g, vm, X, W);
+    return gamma ? k1_t<double, true>(n_slots, st, g, vm, X, W) : k1_t<double, false>(n_slots, st, g, vm, X, W);
+}
+cudaError_t k3_entry(int f32, int gamma, int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const void* W, K3Epi e, cx<double>* Y) {
+    if (f32) return gamma ? k3_t<float, true>(n_slots, st, g, vm, W, e, Y) : k3_t<float, false>(n_slots, st, g, vm, W, e, Y);
+    return gamma ? k3_t<double, true>(n_slots, st, g, vm, W, e, Y) : k3_t<double, false>(n_slots, st, g, vm, W, e, Y);
+}
+cudaError_t k2_entry(int f32, int mode, int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
+    if (f32) {
+        if (mode == K2_H) return k2_t<float, K2_H>(n_slots, st, g, a);
+        return cudaErrorInvalidValue;          // only the H*psi path has an FP32 variant
+    }
+    switch (mode) {
+        case K2_H: return k2_t<double, K2_H>(n_slots, st, g, a);
+        case K2_TOR: return k2_t<double, K2_TOR>(n_slots, st, g, a);
+        case K2_DN: return k2_t<double, K2_DN>(n_slots, st, g, a);
+        case K2_FROMR: return k2_t<double, K2_FROMR>(n_slots, st, g, a);
+    }
+    return cudaErrorInvalidValue;
+}
+const FftOps ops = {NN, N1, N2, CU, LC, k1_entry, k2_entry, k3_entry};
+}  // namespace
+
+#define WEST_CAT2(a, b) a##b
+#define WEST_CAT(a, b) WEST_CAT2(a, b)
+const FftOps* WEST_CAT(west_fft_ops_, WEST_NN)() { return &ops; }

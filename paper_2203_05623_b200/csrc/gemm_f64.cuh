@@ -1,0 +1,200 @@
+// FP64 tensor-core (DMMA, mma.sync m8n8k4) GEMMs for the dense contractions of the hot path: Kleinman-Bylander
+// projector overlaps, P_v / P_c projections ("cuBLAS", 291 "FP64 tensor cores").
+// There is no tcgen05 FP64 kind on sm_100a; DMMA.8x8x4 is the FP64 tensor instruction this chip has.
+//
+//   gemm_tn     C[m][n] (+)= sum_k A[m][k] B[n][k]      both operands K-contiguous; K is the long axis (2 n_g reals),
+//                                                        split over blockIdx.z, partial sums reduced with FP64 atomics
+//   gemm_update Y[n][k] += sum_m C[m][n] A[m][k]        rank-m update of the vector block
+// CTA tile 128 x 128, 8 warps as 2 x 4, warp tile 64 x 32 (64 accumulators / thread), k step 16 through a 4-stage
+// cp.async ring.  Shared-memory rows are padded to 20 doubles (tn) / 132 doubles (update) so every fragment load is
+// bank-conflict free.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wgemm {
+
+constexpr int BM = 128, BN = 128, BK = 16, STAGES = 4, NTHREADS = 256;
+constexpr int PITCH_TN = BK + 4;                  // doubles
+constexpr int PITCH_UP = 128 + 4;                 // doubles
+constexpr size_t SMEM_TN = (size_t)STAGES * (BM + BN) * PITCH_TN * sizeof(double);
+constexpr size_t SMEM_UP = (size_t)STAGES * 2 * BK * PITCH_UP * sizeof(double);
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int bytes = pred ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(bytes));
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int bytes = pred ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(gmem), "r"(bytes));
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// C[m][n] += sum_{k in this split} A[m][k] B[n][k].   lda, ldb even (16-byte aligned rows), A and B 16-byte aligned.
+__global__ void __launch_bounds__(NTHREADS) gemm_tn_kernel(int M, int Nn, long long K, const double* __restrict__ A, long long lda,
+                                                           const double* __restrict__ B, long long ldb, double* __restrict__ C,
+                                                           long long ldc, long long k_per_split, int use_atomic) {
+    extern __shared__ __align__(16) double smem[];
+    double* As = smem;                                   // [STAGES][BM][PITCH_TN]
+    double* Bs = smem + (size_t)STAGES * BM * PITCH_TN;  // [STAGES][BN][PITCH_TN]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 2, wn = warp & 3;             // 2 x 4 warps
+    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+    const long long kb = (long long)blockIdx.z * k_per_split;
+    long long ke = kb + k_per_split; if (ke > K) ke = K;
+    const int nk = (int)((ke - kb + BK - 1) / BK);
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    auto load_stage = [&](int stage, int kt) {
+        const long long k0 = kb + (long long)kt * BK;
+        // 128 rows x 8 chunks of 16 B per operand = 1024 chunks, 4 per thread per operand
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int c = tid + i * NTHREADS, row = c >> 3, ch = c & 7;
+            const long long k = k0 + ch * 2;
+            const bool pa = (m0 + row < M) && (k < ke);
+            const bool pb = (n0 + row < Nn) && (k < ke);
+            // k and ke are even whenever k_per_split and K are even, so a 16-byte chunk never straddles ke
+            cp_async16(As + ((size_t)stage * BM + row) * PITCH_TN + ch * 2, pa ? A + (long long)(m0 + row) * lda + k : A, pa);
+            cp_async16(Bs + ((size_t)stage * BN + row) * PITCH_TN + ch * 2, pb ? B + (long long)(n0 + row) * ldb + k : B, pb);
+        }
+    };
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nk) load_stage(s, s);
+        cp_commit();
+    }
+    for (int kt = 0; kt < nk; ++kt) {
+        cp_wait<STAGES - 2>();
+        __syncthreads();
+        if (kt + STAGES - 1 < nk) load_stage((kt + STAGES - 1) % STAGES, kt + STAGES - 1);
+        cp_commit();
+        const double* as = As + (size_t)(kt % STAGES) * BM * PITCH_TN + (wm * 64 + (lane >> 2)) * PITCH_TN + (lane & 3);
+        const double* bs = Bs + (size_t)(kt % STAGES) * BN * PITCH_TN + (wn * 32 + (lane >> 2)) * PITCH_TN + (lane & 3);
+#pragma unroll
+        for (int kk = 0; kk < BK; kk += 4) {
+            double a[8], b[4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = as[i * 8 * PITCH_TN + kk];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = bs[j * 8 * PITCH_TN + kk];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_wait<0>();
+    // C fragment: row = lane/4, cols 2*(lane%4), +1
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int m = m0 + wm * 64 + i * 8 + (lane >> 2);
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int n = n0 + wn * 32 + j * 8 + 2 * (lane & 3);
+            double* c = C + (long long)m * ldc + n;
+            if (use_atomic) {
+                if (n < Nn) atomicAdd(c, acc[i][j][0]);
+                if (n + 1 < Nn) atomicAdd(c + 1, acc[i][j][1]);
+            } else {
+                if (n < Nn) c[0] = acc[i][j][0];
+                if (n + 1 < Nn) c[1] = acc[i][j][1];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Y[n][k] += sum_m C[m][n] A[m][k].  Output tile: 128 vectors (n) x 128 reals (k).  MMA roles: rows = n, cols = k,
+// contraction = m.  A-operand element (n, m) = C[m][n] (n contiguous), B-operand element (m, k) = A[m][k] (k contiguous).
+__global__ void __launch_bounds__(NTHREADS) gemm_update_kernel(int M, int Nn, long long K, const double* __restrict__ C, long long ldc,
+                                                               const double* __restrict__ A, long long lda, double* __restrict__ Y,
+                                                               long long ldy) {
+    extern __shared__ __align__(16) double smem[];
+    double* Cs = smem;                                        // [STAGES][BK][PITCH_UP]  (m, n)
+    double* As = smem + (size_t)STAGES * BK * PITCH_UP;       // [STAGES][BK][PITCH_UP]  (m, k)
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 2, wn = warp & 3;
+    const int n0 = blockIdx.y * 128;
+    const long long k0 = (long long)blockIdx.x * 128;
+    const int nm = (M + BK - 1) / BK;
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    auto load_stage = [&](int stage, int mt) {
+        const int mb = mt * BK;
+        // 16 rows x 64 chunks of 16 B per operand = 1024 chunks
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int c = tid + i * NTHREADS, row = c >> 6, ch = c & 63;
+            const bool pm = mb + row < M;
+            const bool pc = pm && (n0 + ch * 2 < Nn);          // Nn, ldc even -> chunk never straddles
+            const bool pa = pm && (k0 + ch * 2 < K);           // K, lda even
+            cp_async16(Cs + ((size_t)stage * BK + row) * PITCH_UP + ch * 2, pc ? C + (long long)(mb + row) * ldc + n0 + ch * 2 : C, pc);
+            cp_async16(As + ((size_t)stage * BK + row) * PITCH_UP + ch * 2, pa ? A + (long long)(mb + row) * lda + k0 + ch * 2 : A, pa);
+        }
+    };
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nm) load_stage(s, s);
+        cp_commit();
+    }
+    for (int mt = 0; mt < nm; ++mt) {
+        cp_wait<STAGES - 2>();
+        __syncthreads();
+        if (mt + STAGES - 1 < nm) load_stage((mt + STAGES - 1) % STAGES, mt + STAGES - 1);
+        cp_commit();
+        // A-operand (row n = lane/4, contraction m = lane%4): Cs[m][n];  B-operand (m = lane%4, col k = lane/4): As[m][k]
+        const double* cs = Cs + (size_t)(mt % STAGES) * BK * PITCH_UP + (lane & 3) * PITCH_UP + wm * 64 + (lane >> 2);
+        const double* as = As + (size_t)(mt % STAGES) * BK * PITCH_UP + (lane & 3) * PITCH_UP + wn * 32 + (lane >> 2);
+#pragma unroll
+        for (int mm = 0; mm < BK; mm += 4) {
+            double a[8], b[4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = cs[mm * PITCH_UP + i * 8];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = as[mm * PITCH_UP + j * 8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_wait<0>();
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int n = n0 + wm * 64 + i * 8 + (lane >> 2);
+        if (n >= Nn) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const long long k = k0 + wn * 32 + j * 8 + 2 * (lane & 3);
+            if (k < K) {                                        // K even: k and k+1 are both valid
+                double2* y = reinterpret_cast<double2*>(Y + (long long)n * ldy + k);
+                double2 v = *y;
+                v.x += acc[i][j][0]; v.y += acc[i][j][1];
+                *y = v;
+            }
+        }
+    }
+}
+
+}  // namespace wgemm

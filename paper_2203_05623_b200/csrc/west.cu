@@ -1,0 +1,770 @@
+// C-ABI implementation (include/west.h): context, operator set-up, and the drivers that chain the hand-written kernels
+// of the chi0*dV hot path (Eq. 10-11).  Every step of the path runs in kernels of this library;
+// there is no CPU fallback.
+#include <cuda_runtime.h>
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/west.h"
+#include "cg_kernels.cuh"
+#include "fft_ops.h"
+#include "gemm_f64.cuh"
+#include "gsphere.hpp"
+
+namespace {
+
+std::string g_create_error;
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+}  // namespace
+
+struct west_ctx {
+    west_cell cell{};
+    cudaStream_t st = nullptr;
+    HostSphere hs;
+    const FftOps* ops = nullptr;
+    WestGeom geom{};
+    std::string err;
+    int64_t launches = 0;
+    int64_t dev_bytes = 0;
+    int fft_chunk = 0;
+    std::vector<void*> owned;          // every cudaMalloc of this context
+
+    // geometry tables
+    int *d_row_off = nullptr, *d_unit_off = nullptr, *d_unit_zmax = nullptr;
+    cx<double>* d_tw = nullptr;
+    double* d_g2 = nullptr;
+
+    // operator data
+    double* d_vpos = nullptr;          // V_loc, position order, f64
+    float* d_vpos_f = nullptr;         // same, f32 (WEST_MIXED)
+    bool have_vloc = false;
+    int n_proj = 0, n_occ = 0;
+    int rows_kb = 0, rows_psi = 0;     // rows of the stacked real operator matrix (x2 in WEST_FULL)
+    DevBuf A_kb, A_psi;                // [rows][2 n_g] f64 each (kept apart; concatenated lazily into A_all)
+    DevBuf A_all, coef_all;            // [rows_kb + rows_psi][2 n_g], coef [rows]
+    bool A_dirty = true;
+    std::vector<double> h_dcoef;       // per stacked KB row
+    std::vector<double> h_eps;
+    DevBuf tk;                         // [n_occ] <psi_v|T|psi_v>
+    DevBuf ucache;                     // [n_uslots][N^3] c128 position order
+    int n_uslots = 0;
+
+    // workspaces (grown lazily)
+    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc;
+    int* h_pinned = nullptr;           // pinned host scratch for convergence polling / reports
+};
+
+namespace {
+
+int fail(west_ctx* c, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf; else g_create_error = buf;
+    return code;
+}
+#define CK(call)                                                                                              \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess) return fail(c, WEST_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+int dev_alloc(west_ctx* c, void** p, size_t bytes) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, WEST_ENOMEM, "cudaMalloc of %zu bytes failed: %s", bytes, cudaGetErrorString(e));
+    }
+    c->owned.push_back(*p);
+    c->dev_bytes += (int64_t)bytes;
+    return WEST_OK;
+}
+// grow-only buffer
+int ensure(west_ctx* c, DevBuf& b, size_t bytes) {
+    if (b.bytes >= bytes && b.p) return WEST_OK;
+    if (b.p) {
+        cudaStreamSynchronize(c->st);
+        cudaFree(b.p);
+        c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), b.p), c->owned.end());
+        c->dev_bytes -= (int64_t)b.bytes;
+        b.p = nullptr; b.bytes = 0;
+    }
+    int rc = dev_alloc(c, &b.p, bytes);
+    if (rc == WEST_OK) b.bytes = bytes;
+    return rc;
+}
+
+inline long long n3_of(const west_ctx* c) { return (long long)c->cell.N * c->cell.N * c->cell.N; }
+inline bool is_gamma(const west_ctx* c) { return c->cell.mode == WEST_GAMMA; }
+
+// ------------------------------------------------------------------------------------------ boundary conversion kernels
+// position p of real-space index j along one axis: p = N2 (j mod N1) + j div N1 ;  j = p div N2 + N1 (p mod N2)
+__device__ __forceinline__ int j_of_p(int p, int N1, int N2) { return p / N2 + N1 * (p % N2); }
+
+// natural [b][ix][iy][iz] real f64 -> position order [b][pz][py][px] (T)
+template <typename T>
+__global__ void nat_to_pos_real(int N, int N1, int N2, long long total, const double* in, T* out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const long long n3 = (long long)N * N * N, b = i / n3;
+    long long r = i - b * n3;
+    const int px = (int)(r % N); r /= N;
+    const int py = (int)(r % N); const int pz = (int)(r / N);
+    const int ix = j_of_p(px, N1, N2), iy = j_of_p(py, N1, N2), iz = j_of_p(pz, N1, N2);
+    out[i] = (T)in[b * n3 + ((long long)ix * N + iy) * N + iz];
+}
+// position order real [b][pz][py][px] -> natural [b][ix][iy][iz]
+__global__ void pos_to_nat_real(int N, int N1, int N2, long long total, const double* in, double* out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const long long n3 = (long long)N * N * N, b = i / n3;
+    long long r = i - b * n3;
+    const int iz = (int)(r % N); r /= N;
+    const int iy = (int)(r % N); const int ix = (int)(r / N);
+    const int px = N2 * (ix % N1) + ix / N1, py = N2 * (iy % N1) + iy / N1, pz = N2 * (iz % N1) + iz / N1;
+    out[i] = in[b * n3 + ((long long)pz * N + py) * N + px];
+}
+// complex position-order slots [s][N^3] -> user grids.  gamma: real grids 2s (Re), 2s+1 (Im); full: complex grid s
+__global__ void pos_to_user(int N, int N1, int N2, int gamma, int slot0, int n_slots, int n_batch, const cx<double>* R, double* out) {
+    const long long n3 = (long long)N * N * N;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n3 * n_slots) return;
+    const long long s = i / n3;
+    long long r = i - s * n3;
+    const int iz = (int)(r % N); r /= N;
+    const int iy = (int)(r % N); const int ix = (int)(r / N);
+    const int px = N2 * (ix % N1) + ix / N1, py = N2 * (iy % N1) + iy / N1, pz = N2 * (iz % N1) + iz / N1;
+    const cx<double> v = R[s * n3 + ((long long)pz * N + py) * N + px];
+    const long long nat = ((long long)ix * N + iy) * N + iz;
+    const long long gs = slot0 + s;
+    if (gamma) {
+        if (2 * gs < n_batch) out[(2 * gs) * n3 + nat] = v.x;
+        if (2 * gs + 1 < n_batch) out[(2 * gs + 1) * n3 + nat] = v.y;
+    } else {
+        reinterpret_cast<cx<double>*>(out)[gs * n3 + nat] = v;
+    }
+}
+__global__ void user_to_pos(int N, int N1, int N2, int gamma, int slot0, int n_slots, int n_batch, const double* in, cx<double>* R) {
+    const long long n3 = (long long)N * N * N;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n3 * n_slots) return;
+    const long long s = i / n3;
+    long long r = i - s * n3;
+    const int px = (int)(r % N); r /= N;
+    const int py = (int)(r % N); const int pz = (int)(r / N);
+    const int ix = j_of_p(px, N1, N2), iy = j_of_p(py, N1, N2), iz = j_of_p(pz, N1, N2);
+    const long long nat = ((long long)ix * N + iy) * N + iz;
+    const long long gs = slot0 + s;
+    cx<double> v = mk<double>(0, 0);
+    if (gamma) {
+        if (2 * gs < n_batch) v.x = in[(2 * gs) * n3 + nat];
+        if (2 * gs + 1 < n_batch) v.y = in[(2 * gs + 1) * n3 + nat];
+    } else {
+        v = reinterpret_cast<const cx<double>*>(in)[gs * n3 + nat];
+    }
+    R[i] = v;
+}
+
+// stacked real operator rows from complex rows: FULL: row 2k = (re, im) as stored, row 2k+1 = i * row ; GAMMA: copy
+__global__ void stack_rows(long long n_g, int n_rows_in, int full, const cx<double>* in, double* out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_g * n_rows_in) return;
+    const long long k = i / n_g, g = i - k * n_g;
+    const cx<double> v = in[i];
+    if (full) {
+        double* r0 = out + (2 * k) * 2 * n_g + 2 * g;
+        double* r1 = out + (2 * k + 1) * 2 * n_g + 2 * g;
+        r0[0] = v.x; r0[1] = v.y;
+        r1[0] = -v.y; r1[1] = v.x;
+    } else {
+        double* r0 = out + k * 2 * n_g + 2 * g;
+        r0[0] = v.x; r0[1] = g == 0 ? 0.0 : v.y;     // c(0) of a real function is real
+    }
+}
+// tk[v] = <psi_v|T|psi_v> over the FULL sphere
+__global__ void kinetic_expect(long long n_g, int gamma, const double* g2, const cx<double>* psi, double* tk) {
+    __shared__ double sh[256];
+    const cx<double>* p = psi + (long long)blockIdx.x * n_g;
+    double a = 0;
+    for (long long g = threadIdx.x; g < n_g; g += blockDim.x) {
+        const cx<double> v = p[g];
+        a += g2[g] * (v.x * v.x + v.y * v.y) * ((gamma && g != 0) ? 2.0 : 1.0);
+    }
+    sh[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) tk[blockIdx.x] = sh[0];
+}
+__global__ void fill_shift(int n_vec, int nvpc, int n_occ, const double* eps, double* shift) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_vec) shift[i] = eps[(i / nvpc) % n_occ];
+}
+
+inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+}  // namespace
+
+// ===================================================================================================== internal drivers
+namespace {
+
+// slots per chunk: the stick intermediate W of one chunk is meant to stay L2-resident between K1, K2 and K3
+int chunk_slots(const west_ctx* c, int f32) {
+    if (c->fft_chunk > 0) return c->fft_chunk;
+    const size_t per_slot = (size_t)c->cell.N * c->hs.n_cols * (f32 ? 8 : 16);
+    long long n = (long long)((48ull << 20) / per_slot);
+    if (n < 4) n = 4;
+    if (n > 4096) n = 4096;
+    return (int)n;
+}
+int ensure_W(west_ctx* c, int n_slots, int f32) {
+    return ensure(c, c->W, (size_t)n_slots * c->cell.N * c->hs.n_cols * (f32 ? 8 : 16));
+}
+
+int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, long long lda, const double* B, long long ldb,
+                   double* C, long long ldc) {
+    using namespace wgemm;
+    if (M <= 0 || Nn <= 0) return WEST_OK;
+    static bool attr = false;
+    if (!attr) {
+        CK(cudaFuncSetAttribute(gemm_tn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TN));
+        CK(cudaFuncSetAttribute(gemm_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP));
+        attr = true;
+    }
+    const int tm = (M + BM - 1) / BM, tn = (Nn + BN - 1) / BN;
+    long long splits = (4 * 148 + (long long)tm * tn - 1) / ((long long)tm * tn);
+    const long long max_splits = std::max<long long>(1, K / (8 * BK));
+    splits = std::max<long long>(1, std::min(splits, max_splits));
+    long long kps = (K + splits - 1) / splits;
+    kps = (kps + BK - 1) / BK * BK;
+    splits = (K + kps - 1) / kps;
+    CK(cudaMemsetAsync(C, 0, (size_t)M * ldc * sizeof(double), c->st));
+    dim3 grid(tn, tm, (unsigned)splits);
+    gemm_tn_kernel<<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+int launch_gemm_update(west_ctx* c, int M, int Nn, long long K, const double* C, long long ldc, const double* A, long long lda,
+                       double* Y, long long ldy) {
+    using namespace wgemm;
+    if (M <= 0 || Nn <= 0) return WEST_OK;
+    static bool attr = false;
+    if (!attr) {
+        CK(cudaFuncSetAttribute(gemm_tn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TN));
+        CK(cudaFuncSetAttribute(gemm_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP));
+        attr = true;
+    }
+    dim3 grid((unsigned)((K + 127) / 128), (unsigned)((Nn + 127) / 128));
+    gemm_update_kernel<<<grid, NTHREADS, SMEM_UP, c->st>>>(M, Nn, K, C, ldc, A, lda, Y, ldy);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+
+// (re)build the concatenated operator matrix [KB rows ; psi rows] and its coefficient vector
+int ensure_opmatrix(west_ctx* c, double alpha) {
+    const long long K = 2 * c->hs.n_g;
+    const int rows = c->rows_kb + c->rows_psi;
+    if (rows == 0) return WEST_OK;
+    if (c->A_dirty) {
+        int rc = ensure(c, c->A_all, (size_t)rows * K * sizeof(double));
+        if (rc) return rc;
+        rc = ensure(c, c->coef_all, (size_t)rows * sizeof(double));
+        if (rc) return rc;
+        if (c->rows_kb) CK(cudaMemcpyAsync(c->A_all.p, c->A_kb.p, (size_t)c->rows_kb * K * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+        if (c->rows_psi)
+            CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)c->rows_kb * K, c->A_psi.p, (size_t)c->rows_psi * K * sizeof(double),
+                               cudaMemcpyDeviceToDevice, c->st));
+        c->A_dirty = false;
+    }
+    std::vector<double> coef(rows);
+    for (int i = 0; i < c->rows_kb; ++i) coef[i] = c->h_dcoef[i];
+    for (int i = 0; i < c->rows_psi; ++i) coef[c->rows_kb + i] = alpha;
+    // stream-ordered copy from a pageable vector is synchronous with respect to the host buffer: safe
+    CK(cudaMemcpyAsync(c->coef_all.p, coef.data(), rows * sizeof(double), cudaMemcpyHostToDevice, c->st));
+    return WEST_OK;
+}
+
+// Y += sum_{m in [r0, r0+nr)} coef_m A_m <A_m, X>   for n_vec real-function / complex vectors (as 2 n_g reals each).
+// coef_override: if non-NULL use this constant instead of the stored coefficients (RHS projection: -1).
+int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const double* coef_dev) {
+    if (nr <= 0 || n_vec <= 0) return WEST_OK;
+    const long long K = 2 * c->hs.n_g;
+    const long long ldc = (n_vec + 1) / 2 * 2;
+    int rc = ensure(c, c->Cbuf, (size_t)nr * ldc * sizeof(double));
+    if (rc) return rc;
+    const double* A = (const double*)c->A_all.p + (size_t)r0 * K;
+    double* C = (double*)c->Cbuf.p;
+    rc = launch_gemm_tn(c, nr, n_vec, K, A, K, X, K, C, ldc);
+    if (rc) return rc;
+    wcg::lowrank_fix<<<blocks_for((long long)nr * n_vec, 256), 256, 0, c->st>>>(nr, n_vec, ldc, C, A, K, X, K, coef_dev, is_gamma(c) ? 1 : 0);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return launch_gemm_update(c, nr, n_vec, K, C, ldc, A, K, Y, K);
+}
+
+// local part of (H - shift - i omega) on vectors: Y = T x + V_loc x - shift x -+ omega terms   (no KB, no P_v)
+int hloc_apply(west_ctx* c, int f32, VecMap vm, int n_slots, const cx<double>* X, cx<double>* Y, const double* shift, double omega) {
+    const int chunk = chunk_slots(c, f32);
+    int rc = ensure_W(c, std::min(chunk, n_slots), f32);
+    if (rc) return rc;
+    const int N = c->cell.N;
+    K3Epi e;
+    e.scale = 1.0 / ((double)N * N * N); e.kinetic = 1; e.shift = shift; e.omega = omega; e.X = X;
+    K2Any a{};
+    a.W = c->W.p; a.V = f32 ? (const void*)c->d_vpos_f : (const void*)c->d_vpos;
+    for (int s0 = 0; s0 < n_slots; s0 += chunk) {
+        const int ns = std::min(chunk, n_slots - s0);
+        vm.slot0 = s0;
+        CK(c->ops->k1(f32, is_gamma(c), ns, c->st, c->geom, vm, X, c->W.p));
+        CK(c->ops->k2(f32, K2_H, ns, c->st, c->geom, a));
+        CK(c->ops->k3(f32, is_gamma(c), ns, c->st, c->geom, vm, c->W.p, e, Y));
+        c->launches += 3;
+    }
+    return WEST_OK;
+}
+
+}  // namespace
+
+// ============================================================================================================ public API
+extern "C" {
+
+const char* west_last_error(const west_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+int64_t west_device_bytes(const west_ctx* c) { return c ? c->dev_bytes : 0; }
+int64_t west_launch_count(const west_ctx* c) { return c ? c->launches : 0; }
+int west_set_fft_chunk(west_ctx* c, int32_t n) {
+    if (!c || n < 0 || n > 65535) return WEST_EINVAL;
+    c->fft_chunk = n;
+    return WEST_OK;
+}
+
+int west_create(west_ctx** out, const west_cell* cell, void* stream) {
+    west_ctx* c = nullptr;
+    if (!out || !cell) return fail(c, WEST_EINVAL, "west_create: NULL argument");
+    *out = nullptr;
+    const FftOps* ops = nullptr;
+    switch (cell->N) {
+        case 24: ops = west_fft_ops_24(); break;
+        case 36: ops = west_fft_ops_36(); break;
+        case 48: ops = west_fft_ops_48(); break;
+        case 72: ops = west_fft_ops_72(); break;
+        case 144: ops = west_fft_ops_144(); break;
+        default: return fail(c, WEST_EINVAL, "west_create: unsupported N = %d (supported: 24, 36, 48, 72, 144)", cell->N);
+    }
+    if (cell->n2max < 0 || !(cell->L > 0) || (cell->mode != WEST_FULL && cell->mode != WEST_GAMMA))
+        return fail(c, WEST_EINVAL, "west_create: bad cell (L = %g, n2max = %d, mode = %d)", cell->L, cell->n2max, cell->mode);
+    if (cell->N < 4 * isqrt_floor(cell->n2max) + 1)
+        return fail(c, WEST_EINVAL, "west_create: N = %d < 4*floor(sqrt(n2max)) + 1 = %d", cell->N, 4 * isqrt_floor(cell->n2max) + 1);
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(c, WEST_ECUDA, "west_create: no CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+    }
+    west_ctx* ctx = new west_ctx();
+    ctx->cell = *cell;
+    ctx->st = (cudaStream_t)stream;
+    ctx->ops = ops;
+    ctx->hs = build_sphere(cell->n2max, cell->N, cell->mode == WEST_GAMMA, cell->L);
+    c = ctx;
+    auto bail = [&](int rc) { g_create_error = ctx->err; west_destroy(ctx); return rc; };
+    const HostSphere& s = ctx->hs;
+    int rc;
+    if ((rc = dev_alloc(c, (void**)&c->d_row_off, sizeof(int) * (s.nr + 1)))) return bail(rc);
+    if ((rc = dev_alloc(c, (void**)&c->d_unit_off, sizeof(int) * s.n_units))) return bail(rc);
+    if ((rc = dev_alloc(c, (void**)&c->d_unit_zmax, sizeof(int) * s.n_units))) return bail(rc);
+    if ((rc = dev_alloc(c, (void**)&c->d_tw, sizeof(cx<double>) * s.N))) return bail(rc);
+    if ((rc = dev_alloc(c, (void**)&c->d_g2, sizeof(double) * s.n_g))) return bail(rc);
+    std::vector<cx<double>> tw(s.N);
+    for (int i = 0; i < s.N; ++i) {
+        const double a = 2.0 * 3.14159265358979323846264338327950288 * (double)i / (double)s.N;
+        tw[i].x = std::cos(a); tw[i].y = std::sin(a);
+    }
+    // exact values on the axes
+    tw[0] = mk<double>(1, 0);
+    if (s.N % 4 == 0) { tw[s.N / 4] = mk<double>(0, 1); tw[3 * s.N / 4] = mk<double>(0, -1); }
+    if (s.N % 2 == 0) tw[s.N / 2] = mk<double>(-1, 0);
+    e = cudaMemcpy(c->d_row_off, s.row_off.data(), sizeof(int) * (s.nr + 1), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_unit_off, s.unit_off.data(), sizeof(int) * s.n_units, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_unit_zmax, s.unit_zmax.data(), sizeof(int) * s.n_units, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_tw, tw.data(), sizeof(cx<double>) * s.N, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_g2, s.g2.data(), sizeof(double) * s.n_g, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_pinned, 64);
+    if (e != cudaSuccess) { fail(c, WEST_ECUDA, "west_create: %s", cudaGetErrorString(e)); return bail(WEST_ECUDA); }
+    WestGeom& g = c->geom;
+    g.N = s.N; g.n_max = s.n_max; g.nr = s.nr; g.n_cols = s.n_cols; g.n_units = s.n_units; g.gamma = s.gamma; g.n_g = s.n_g;
+    g.row_off = c->d_row_off; g.unit_off = c->d_unit_off; g.unit_zmax = c->d_unit_zmax; g.tw = c->d_tw; g.g2 = c->d_g2;
+    *out = ctx;
+    return WEST_OK;
+}
+
+int west_destroy(west_ctx* c) {
+    if (!c) return WEST_OK;
+    cudaStreamSynchronize(c->st);
+    for (void* p : c->owned) cudaFree(p);
+    if (c->h_pinned) cudaFreeHost(c->h_pinned);
+    delete c;
+    return WEST_OK;
+}
+
+int west_gsphere(const west_ctx* cc, int64_t* n_g, int32_t* miller, int32_t* fft_index, int32_t* fft_index_minus, double* g2) {
+    west_ctx* c = const_cast<west_ctx*>(cc);
+    if (!c) return WEST_EINVAL;
+    const HostSphere& s = c->hs;
+    if (n_g) *n_g = s.n_g;
+    if (miller) std::memcpy(miller, s.miller.data(), sizeof(int32_t) * 3 * s.n_g);
+    if (g2) std::memcpy(g2, s.g2.data(), sizeof(double) * s.n_g);
+    const int N = s.N;
+    auto md = [N](int v) { int r = v % N; return r < 0 ? r + N : r; };
+    for (int64_t i = 0; i < s.n_g; ++i) {
+        const int a = s.miller[3 * i], b = s.miller[3 * i + 1], d = s.miller[3 * i + 2];
+        if (fft_index) fft_index[i] = (md(a) * N + md(b)) * N + md(d);
+        if (fft_index_minus) fft_index_minus[i] = (md(-a) * N + md(-b)) * N + md(-d);
+    }
+    return WEST_OK;
+}
+
+int west_set_vloc(west_ctx* c, const double* vloc) {
+    if (!c || !vloc) return fail(c, WEST_EINVAL, "west_set_vloc: NULL argument");
+    const long long n3 = n3_of(c);
+    int rc;
+    if (!c->d_vpos) {
+        if ((rc = dev_alloc(c, (void**)&c->d_vpos, sizeof(double) * n3))) return rc;
+        if ((rc = dev_alloc(c, (void**)&c->d_vpos_f, sizeof(float) * n3))) return rc;
+    }
+    nat_to_pos_real<double><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos);
+    nat_to_pos_real<float><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos_f);
+    CK(cudaGetLastError());
+    c->launches += 2;
+    c->have_vloc = true;
+    return WEST_OK;
+}
+
+int west_set_kb(west_ctx* c, int32_t n_proj, const void* beta, const double* dcoef_host) {
+    if (!c || n_proj < 0 || (n_proj > 0 && (!beta || !dcoef_host))) return fail(c, WEST_EINVAL, "west_set_kb: bad argument");
+    const int full = !is_gamma(c);
+    const long long n_g = c->hs.n_g;
+    c->n_proj = n_proj;
+    c->rows_kb = n_proj * (full ? 2 : 1);
+    c->A_dirty = true;
+    c->h_dcoef.resize(c->rows_kb);
+    for (int k = 0; k < n_proj; ++k) {
+        if (full) { c->h_dcoef[2 * k] = dcoef_host[k]; c->h_dcoef[2 * k + 1] = dcoef_host[k]; }
+        else c->h_dcoef[k] = dcoef_host[k];
+    }
+    if (n_proj == 0) return WEST_OK;
+    int rc = ensure(c, c->A_kb, (size_t)c->rows_kb * 2 * n_g * sizeof(double));
+    if (rc) return rc;
+    stack_rows<<<blocks_for(n_g * n_proj, 256), 256, 0, c->st>>>(n_g, n_proj, full, (const cx<double>*)beta, (double*)c->A_kb.p);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+
+int west_set_states(west_ctx* c, int32_t n_occ, const void* psi, const double* eps_host) {
+    if (!c || n_occ <= 0 || !psi || !eps_host) return fail(c, WEST_EINVAL, "west_set_states: bad argument");
+    const int full = !is_gamma(c);
+    const long long n_g = c->hs.n_g, n3 = n3_of(c);
+    c->n_occ = n_occ;
+    c->rows_psi = n_occ * (full ? 2 : 1);
+    c->A_dirty = true;
+    c->h_eps.assign(eps_host, eps_host + n_occ);
+    int rc = ensure(c, c->A_psi, (size_t)c->rows_psi * 2 * n_g * sizeof(double));
+    if (rc) return rc;
+    stack_rows<<<blocks_for(n_g * n_occ, 256), 256, 0, c->st>>>(n_g, n_occ, full, (const cx<double>*)psi, (double*)c->A_psi.p);
+    CK(cudaGetLastError());
+    if ((rc = ensure(c, c->tk, sizeof(double) * n_occ))) return rc;
+    kinetic_expect<<<n_occ, 256, 0, c->st>>>(n_g, is_gamma(c), c->d_g2, (const cx<double>*)psi, (double*)c->tk.p);
+    CK(cudaGetLastError());
+    c->launches += 2;
+    // u_v(r) cache in position order: GAMMA packs (v, v+1) as u_v + i u_{v+1}
+    c->n_uslots = full ? n_occ : (n_occ + 1) / 2;
+    if ((rc = ensure(c, c->ucache, sizeof(cx<double>) * n3 * c->n_uslots))) return rc;
+    const int chunk = std::max(1, std::min(c->n_uslots, chunk_slots(c, 0)));
+    if ((rc = ensure_W(c, chunk, 0))) return rc;
+    VecMap vm{full ? 1 : 2, full ? 0 : 1, n_occ, 0};
+    for (int s0 = 0; s0 < c->n_uslots; s0 += chunk) {
+        const int ns = std::min(chunk, c->n_uslots - s0);
+        vm.slot0 = s0;
+        K2Any a{};
+        a.W = c->W.p; a.R = (cx<double>*)c->ucache.p + (long long)s0 * n3;
+        CK(c->ops->k1(0, is_gamma(c), ns, c->st, c->geom, vm, (const cx<double>*)psi, c->W.p));
+        CK(c->ops->k2(0, K2_TOR, ns, c->st, c->geom, a));
+        c->launches += 2;
+    }
+    return WEST_OK;
+}
+
+int west_fft3d(west_ctx* c, int32_t dir, int32_t precision, int32_t n_batch, const void* in, void* out) {
+    if (!c || (dir != 1 && dir != -1) || n_batch < 0 || !in || !out) return fail(c, WEST_EINVAL, "west_fft3d: bad argument");
+    if (precision != WEST_FP64) return fail(c, WEST_EINVAL, "west_fft3d: only WEST_FP64 (the FP32 variant exists inside west_h_apply only)");
+    if (n_batch == 0) return WEST_OK;
+    const int gamma = is_gamma(c), N = c->cell.N;
+    const long long n3 = n3_of(c);
+    const int n_slots = gamma ? (n_batch + 1) / 2 : n_batch;
+    const int chunk = std::max(1, std::min(n_slots, std::min(chunk_slots(c, 0), 64)));
+    int rc;
+    if ((rc = ensure_W(c, chunk, 0))) return rc;
+    if ((rc = ensure(c, c->Rbuf, sizeof(cx<double>) * n3 * chunk))) return rc;
+    VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_batch, 0};
+    K2Any a{};
+    a.W = c->W.p; a.R = (cx<double>*)c->Rbuf.p;
+    for (int s0 = 0; s0 < n_slots; s0 += chunk) {
+        const int ns = std::min(chunk, n_slots - s0);
+        vm.slot0 = s0;
+        if (dir == 1) {
+            CK(c->ops->k1(0, gamma, ns, c->st, c->geom, vm, (const cx<double>*)in, c->W.p));
+            CK(c->ops->k2(0, K2_TOR, ns, c->st, c->geom, a));
+            pos_to_user<<<blocks_for(n3 * ns, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, gamma, s0, ns, n_batch, (const cx<double>*)c->Rbuf.p, (double*)out);
+        } else {
+            user_to_pos<<<blocks_for(n3 * ns, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, gamma, s0, ns, n_batch, (const double*)in, (cx<double>*)c->Rbuf.p);
+            CK(c->ops->k2(0, K2_FROMR, ns, c->st, c->geom, a));
+            K3Epi e{1.0 / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
+            CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, c->W.p, e, (cx<double>*)out));
+        }
+        CK(cudaGetLastError());
+        c->launches += 3;
+    }
+    return WEST_OK;
+}
+
+int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, void* y) {
+    if (!c || n_vec < 0 || !x || !y) return fail(c, WEST_EINVAL, "west_h_apply: bad argument");
+    if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_h_apply: bad precision %d", precision);
+    if (!c->have_vloc) return fail(c, WEST_ESTATE, "west_h_apply: west_set_vloc has not been called");
+    if (n_vec == 0) return WEST_OK;
+    const int gamma = is_gamma(c);
+    const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
+    VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
+    int rc = hloc_apply(c, precision == WEST_MIXED, vm, n_slots, (const cx<double>*)x, (cx<double>*)y, nullptr, 0.0);
+    if (rc) return rc;
+    if (c->rows_kb > 0) {
+        if ((rc = ensure_opmatrix(c, 0.0))) return rc;
+        rc = lowrank_apply(c, 0, c->rows_kb, n_vec, (const double*)x, (double*)y, (const double*)c->coef_all.p);
+    }
+    return rc;
+}
+
+int west_gemm_tn(west_ctx* c, int32_t m, int32_t n, int64_t k, const double* A, int64_t lda, const double* B, int64_t ldb, double* C, int64_t ldc) {
+    if (!c || !A || !B || !C || (k & 1) || (lda & 1) || (ldb & 1)) return fail(c, WEST_EINVAL, "west_gemm_tn: k, lda, ldb must be even");
+    return launch_gemm_tn(c, m, n, k, A, lda, B, ldb, C, ldc);
+}
+int west_gemm_update(west_ctx* c, int32_t m, int32_t n, int64_t k, const double* C, int64_t ldc, const double* A, int64_t lda, double* Y, int64_t ldy) {
+    if (!c || !A || !Y || !C || (k & 1) || (lda & 1) || (ldc & 1) || (ldy & 1)) return fail(c, WEST_EINVAL, "west_gemm_update: k, lda, ldc, ldy must be even");
+    return launch_gemm_update(c, m, n, k, C, ldc, A, lda, Y, ldy);
+}
+
+}  // extern "C"
+
+// ============================================================================================================ chi0 * dV
+namespace {
+
+template <int MODE>
+int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omega, cx<double>* X, cx<double>* R, cx<double>* P,
+             cx<double>* AP, const double* shift, wcg::Scalars s, int* iters_out) {
+    const long long n_g = c->hs.n_g;
+    const int nvpc = MODE == 1 ? 2 : 1, n_vec = n_col * nvpc, n_occ = c->n_occ;
+    const int gamma = is_gamma(c);
+    const double* g2 = c->d_g2;
+    const double* tk = (const double*)c->tk.p;
+    const double tol2 = o.tol * o.tol;
+    const int every = std::max(1, o.check_every);
+    CK(cudaMemsetAsync(s.counters, 0, 2 * sizeof(int), c->st));
+    CK(cudaMemsetAsync(X, 0, sizeof(cx<double>) * n_g * n_vec, c->st));
+    wcg::cg_init<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)R, (double2*)P, s);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    // slots of the H application: GAMMA pairs vectors (2s, 2s+1) - in MODE 1 these are (Re, Im) of one column
+    VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
+    const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
+    const int rows = c->rows_kb + c->rows_psi;
+    int it = 0;
+    for (; it < o.max_iter; ++it) {
+        int rc = hloc_apply(c, f32, vm, n_slots, P, AP, shift, omega);
+        if (rc) return rc;
+        rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, (const double*)c->coef_all.p);
+        if (rc) return rc;
+        wcg::cg_dot_pAp<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, (const double2*)P, (const double2*)AP, s);
+        wcg::cg_update_xr<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)P, (const double2*)AP,
+                                                              (double2*)X, (double2*)R, s);
+        wcg::cg_update_p<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (const double2*)R, (double2*)P, s);
+        CK(cudaGetLastError());
+        c->launches += 3;
+        if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
+            CK(cudaMemcpyAsync(c->h_pinned, s.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+            CK(cudaStreamSynchronize(c->st));
+            if (c->h_pinned[0] <= 0) { ++it; break; }
+        }
+    }
+    *iters_out = it;
+    return WEST_OK;
+}
+
+}  // namespace
+
+extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, const double* dV, int32_t n_freq,
+                               const double* omega_host, const west_cg_opts* opts, double* dn, void* dpsi_opt, west_stats* stats) {
+    if (!c || n_pert < 0 || n_freq < 0 || !dV || !omega_host || !opts || !dn) return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
+    if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
+    if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
+    if (opts->max_iter < 1 || !(opts->tol > 0)) return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
+    const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
+    if (gamma && (n_occ & 1)) return fail(c, WEST_EINVAL, "west_chi0_apply: WEST_GAMMA needs an even number of occupied states (two per FFT)");
+    for (int w = 0; w < n_freq; ++w) {
+        if (omega_host[w] < 0) return fail(c, WEST_EINVAL, "west_chi0_apply: omega must be >= 0");
+        if (omega_host[w] > 0 && !gamma) return fail(c, WEST_EINVAL, "west_chi0_apply: omega > 0 needs WEST_GAMMA (COCG needs real orbitals, R7)");
+    }
+    if (stats) std::memset(stats, 0, sizeof *stats);
+    if (n_pert == 0 || n_freq == 0) return WEST_OK;
+    const int f32 = precision == WEST_MIXED;
+    const long long n_g = c->hs.n_g, n3 = n3_of(c);
+    const int n_col = n_pert * n_occ;
+    const double vol = c->cell.L * c->cell.L * c->cell.L;
+    bool any_omega = false;
+    for (int w = 0; w < n_freq; ++w) any_omega |= omega_host[w] > 0;
+    const int nvpc_max = any_omega ? 2 : 1;
+    int rc;
+    if ((rc = ensure_opmatrix(c, opts->alpha_pv))) return rc;
+    for (int i = 0; i < 4; ++i)
+        if ((rc = ensure(c, c->vecs[i], sizeof(cx<double>) * n_g * n_col * nvpc_max))) return rc;
+    if ((rc = ensure(c, c->shift, sizeof(double) * ((size_t)n_col * nvpc_max + n_occ)))) return rc;
+    if ((rc = ensure(c, c->dVpos, sizeof(double) * n3 * n_pert))) return rc;
+    if ((rc = ensure(c, c->dnpos, sizeof(double) * n3 * n_pert))) return rc;
+    if ((rc = ensure(c, c->scal, (size_t)n_col * (3 * sizeof(double2) + 2 * sizeof(double) + sizeof(int)) + 64))) return rc;
+    wcg::Scalars s;
+    {
+        char* p = (char*)c->scal.p;
+        s.rz = (double2*)p; p += sizeof(double2) * n_col;
+        s.pAp = (double2*)p; p += sizeof(double2) * n_col;
+        s.rznew = (double2*)p; p += sizeof(double2) * n_col;
+        s.rr = (double*)p; p += sizeof(double) * n_col;
+        s.b2 = (double*)p; p += sizeof(double) * n_col;
+        s.active = (int*)p; p += sizeof(int) * n_col;
+        p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
+        s.counters = (int*)p; p += 16;
+        s.resid_max = (double*)p;
+    }
+    cx<double>* X = (cx<double>*)c->vecs[0].p; cx<double>* R = (cx<double>*)c->vecs[1].p;
+    cx<double>* P = (cx<double>*)c->vecs[2].p; cx<double>* AP = (cx<double>*)c->vecs[3].p;
+    double* d_eps = (double*)c->shift.p + (size_t)n_col * nvpc_max;
+    CK(cudaMemcpyAsync(d_eps, c->h_eps.data(), sizeof(double) * n_occ, cudaMemcpyHostToDevice, c->st));
+    nat_to_pos_real<double><<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, dV, (double*)c->dVpos.p);
+    CK(cudaGetLastError());
+    c->launches += 1;
+
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    if (stats) for (auto& e : ev) CK(cudaEventCreate(&e));
+    int ret = WEST_OK;
+    const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
+    const int chunk = std::max(1, chunk_slots(c, 0));
+    if ((rc = ensure_W(c, std::min(chunk, std::max(n_rslots, 1)), 0))) return rc;
+
+    for (int w = 0; w < n_freq; ++w) {
+        const double omega = omega_host[w];
+        const int mode = gamma ? (omega > 0 ? 1 : 0) : 2;
+        const int nvpc = mode == 1 ? 2 : 1, n_vec = n_col * nvpc;
+        fill_shift<<<blocks_for(n_vec, 256), 256, 0, c->st>>>(n_vec, nvpc, n_occ, d_eps, (double*)c->shift.p);
+        CK(cudaGetLastError());
+        if (stats) CK(cudaEventRecord(ev[0], c->st));
+        // ---- a1: b = -P_c (dV_i psi_v), written into R.   slot (i, us) -> columns i*n_occ + 2us (+1)  [GAMMA] or i*n_occ + us
+        if (mode == 1) CK(cudaMemsetAsync(R, 0, sizeof(cx<double>) * n_g * n_vec, c->st));
+        {
+            VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
+            K2Any a{};
+            a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dV = (const double*)c->dVpos.p; a.n_uslots = n_uslots;
+            K3Epi e{-1.0 / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
+            for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
+                const int ns = std::min(chunk, n_rslots - s0);
+                vm.slot0 = s0; a.slot0 = s0;
+                CK(c->ops->k2(0, K2_FROMR, ns, c->st, c->geom, a));
+                CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, c->W.p, e, R));
+                c->launches += 2;
+            }
+            // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows
+            if ((rc = ensure(c, c->misc, sizeof(double) * c->rows_psi))) return rc;
+            std::vector<double> m1(c->rows_psi, -1.0);
+            CK(cudaMemcpyAsync(c->misc.p, m1.data(), sizeof(double) * c->rows_psi, cudaMemcpyHostToDevice, c->st));
+            CK(cudaStreamSynchronize(c->st));     // m1 is a stack-lifetime pageable buffer
+            if ((rc = lowrank_apply(c, c->rows_kb, c->rows_psi, n_vec, (const double*)R, (double*)R, (const double*)c->misc.p))) return rc;
+        }
+        if (stats) CK(cudaEventRecord(ev[1], c->st));
+        // ---- a2-a9: batched PCG / COCG
+        int iters = 0;
+        if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (const double*)c->shift.p, s, &iters);
+        else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (const double*)c->shift.p, s, &iters);
+        else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (const double*)c->shift.p, s, &iters);
+        if (rc) return rc;
+        if (stats) CK(cudaEventRecord(ev[2], c->st));
+        // ---- a10: dn_i(r) = (4/Omega) Re sum_v conj(u_v) du_iv
+        CK(cudaMemsetAsync(c->dnpos.p, 0, sizeof(double) * n3 * n_pert, c->st));
+        {
+            VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
+            K2Any a{};
+            a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dn = (double*)c->dnpos.p; a.n_uslots = n_uslots; a.fac = 4.0 / vol;
+            for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
+                const int ns = std::min(chunk, n_rslots - s0);
+                vm.slot0 = s0; a.slot0 = s0;
+                CK(c->ops->k1(0, gamma, ns, c->st, c->geom, vm, X, c->W.p));
+                CK(c->ops->k2(0, K2_DN, ns, c->st, c->geom, a));
+                c->launches += 2;
+            }
+            pos_to_nat_real<<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, (const double*)c->dnpos.p,
+                                                                           dn + (long long)w * n_pert * n3);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        if (dpsi_opt) {
+            // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 the imaginary part is zero
+            const long long per = n_g * n_col * (gamma ? 2 : 1);
+            cx<double>* dst = (cx<double>*)dpsi_opt + (long long)w * per;
+            if (gamma && mode == 0) {
+                CK(cudaMemsetAsync(dst, 0, sizeof(cx<double>) * per, c->st));
+                CK(cudaMemcpy2DAsync(dst, sizeof(cx<double>) * 2 * n_g, X, sizeof(cx<double>) * n_g, sizeof(cx<double>) * n_g, n_col,
+                                     cudaMemcpyDeviceToDevice, c->st));
+            } else {
+                CK(cudaMemcpyAsync(dst, X, sizeof(cx<double>) * per, cudaMemcpyDeviceToDevice, c->st));
+            }
+        }
+        if (stats) {
+            CK(cudaEventRecord(ev[3], c->st));
+            double* rep = (double*)c->misc.p;     // misc holds >= rows_psi doubles >= 2
+            if ((rc = ensure(c, c->misc, 64))) return rc;
+            rep = (double*)c->misc.p;
+            wcg::cg_report<<<1, wcg::NT, 0, c->st>>>(n_col, opts->tol * opts->tol, s, rep);
+            double h[2];
+            CK(cudaMemcpyAsync(h, rep, sizeof h, cudaMemcpyDeviceToHost, c->st));
+            CK(cudaStreamSynchronize(c->st));
+            float t;
+            cudaEventElapsedTime(&t, ev[0], ev[1]); stats->ms_rhs += t;
+            cudaEventElapsedTime(&t, ev[1], ev[2]); stats->ms_cg += t;
+            cudaEventElapsedTime(&t, ev[2], ev[3]); stats->ms_dn += t;
+            stats->iters = std::max(stats->iters, iters);
+            stats->n_unconverged += (int)h[1];
+            stats->resid_max = std::max(stats->resid_max, h[0]);
+            stats->n_h_apply += (int64_t)iters * n_vec;
+            if (h[1] > 0) ret = WEST_NOTCONVERGED;
+        } else {
+            // convergence status without stats: the last polled counter
+            if (c->h_pinned[0] > 0) ret = WEST_NOTCONVERGED;
+        }
+    }
+    if (stats) for (auto& e : ev) cudaEventDestroy(e);
+    return ret;
+}

@@ -1,0 +1,101 @@
+"""GPU parity, part 1: G-sphere maps (bit-exact), west_fft3d, west_h_apply, the DMMA GEMMs - all through the C ABI."""
+import numpy as np
+import pytest
+
+import synth
+from oracle import gsphere as ogs
+from oracle import hamiltonian as oham
+import oracle_problem
+from gpu_common import make_west, random_vectors, relmax
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-9    # north_star: relative max-norm 1e-9 for FP64
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mini2", "mini48", "cfg2", "cfg5"])
+def test_gsphere_bit_exact(name):
+    import paper_2203_05623_b200 as wb
+    cfg = synth.get_config(name)
+    m = ogs.enumerate_sphere(cfg["n2max"])
+    for mode in (wb.WEST_FULL, wb.WEST_GAMMA):
+        w = wb.West(cfg["L"], cfg["n2max"], cfg["N"], mode)
+        miller, idx, idxm, g2 = w.gsphere()
+        ref = m if mode == wb.WEST_FULL else m[ogs.half_sphere_mask(m)]
+        assert miller.dtype == np.int32 and np.array_equal(miller, ref)
+        assert np.array_equal(idx, ogs.fft_index(ref, cfg["N"]))
+        assert np.array_equal(idxm, ogs.fft_index(-ref, cfg["N"]))
+        assert np.array_equal(g2, ogs.g2_of(ref, cfg["L"]))      # same expression order -> same bits
+        w.close()
+
+
+@pytest.mark.parametrize("name,n_vec", [("cfg1", 5), ("mini2", 5), ("mini48", 3), ("cfg2", 7), ("cfg5", 3)])
+def test_fft3d_vs_library_fft(name, n_vec):
+    import torch
+    p = oracle_problem.build(name, dense=False)
+    w, sel = make_west(p, with_states=False, with_kb=False)
+    c, cfull = random_vectors(p, n_vec, 99)
+    x = torch.from_numpy(c).cuda()
+    r = w.fft3d(+1, x)
+    ref = oham.to_real_space(cfull, p.fft_idx, p.N)
+    if p.gamma:
+        assert np.max(np.abs(ref.imag)) < 1e-9 * np.max(np.abs(ref.real))
+        ref = ref.real
+    assert relmax(r.cpu().numpy(), ref) < TOL
+    # r -> G of a function that is NOT sphere-limited (product of two): truncation of its DFT
+    f = ref * ref[::-1].copy()
+    back = w.fft3d(-1, torch.from_numpy(np.ascontiguousarray(f)).cuda())
+    refc = oham.to_g_space(f, p.fft_idx)[:, sel]
+    assert relmax(back.cpu().numpy(), refc) < TOL
+    # round trip identity on sphere-limited data
+    rt = w.fft3d(-1, r)
+    assert relmax(rt.cpu().numpy(), c) < TOL
+    w.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mini2", "mini48"])
+def test_h_apply_vs_dense(name):
+    import torch
+    p = oracle_problem.build(name)
+    w, sel = make_west(p, with_states=False)
+    c, cfull = random_vectors(p, 7, 98)
+    y = w.h_apply(torch.from_numpy(c).cuda()).cpu().numpy()
+    ref = (p.H @ cfull.T).T[:, sel]
+    assert relmax(y, ref) < TOL
+    w.close()
+
+
+@pytest.mark.parametrize("name,n_vec", [("cfg2", 9), ("cfg5", 4)])
+def test_h_apply_vs_matrix_free(name, n_vec):
+    import torch
+    p = oracle_problem.build(name, dense=False)
+    w, sel = make_west(p, with_states=False)
+    c, cfull = random_vectors(p, n_vec, 97)
+    y = w.h_apply(torch.from_numpy(c).cuda()).cpu().numpy()
+    ref = oham.apply_h(cfull, p.miller, p.L, p.N, p.vloc, p.beta, p.dcoef)[:, sel]
+    assert relmax(y, ref) < TOL
+    # mixed precision: FP32 FFT path, tolerance 1e-4 (config 4)
+    import paper_2203_05623_b200 as wb
+    ym = w.h_apply(torch.from_numpy(c).cuda(), precision=wb.WEST_MIXED).cpu().numpy()
+    assert relmax(ym, ref) < 1e-4
+    assert relmax(ym, ref) > 1e-12      # it really ran in FP32
+    w.close()
+
+
+@pytest.mark.parametrize("m,n,k", [(10, 32, 1030), (384, 1000, 18278), (130, 257, 4098)])
+def test_gemm_tn_and_update(m, n, k):
+    import torch
+    import paper_2203_05623_b200 as wb
+    w = wb.West(10.0, 25, 24, wb.WEST_FULL)
+    rng = np.random.Generator(np.random.PCG64(5))
+    A = rng.standard_normal((m, k))
+    B = rng.standard_normal((n, k))
+    Cg = w.gemm_tn(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()).cpu().numpy()
+    assert relmax(Cg, A @ B.T) < 1e-12
+    ldc = (n + 1) // 2 * 2
+    Cm = np.zeros((m, ldc))
+    Cm[:, :n] = rng.standard_normal((m, n))
+    Y0 = rng.standard_normal((n, k))
+    Y = torch.from_numpy(Y0.copy()).cuda()
+    w.gemm_update(torch.from_numpy(Cm).cuda(), torch.from_numpy(A).cuda(), Y)
+    assert relmax(Y.cpu().numpy(), Y0 + Cm[:, :n].T @ A) < 1e-12
+    w.close()
