@@ -1,0 +1,82 @@
+"""GPU parity, part 2: west_chi0_apply against the sum-over-states oracle (Eq. 10-11)."""
+import numpy as np
+import pytest
+
+import oracle_problem
+from gpu_common import make_west, relmax
+from oracle import chi0 as ochi0
+from oracle import gsphere as ogs
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-9
+
+
+def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1):
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build(name)
+    w, sel = make_west(p)
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
+    prec = wb.WEST_FP64 if precision is None else precision
+    dn, dpsi, st = w.chi0_apply(dV, p.omegas, tol=tol_cg, max_iter=500, alpha_pv=p.alpha if alpha is None else alpha,
+                                precond=precond, precision=prec, want_dpsi=True, n_occ=p.n_occ)
+    ref_dn, ref_dpsi = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, p.dV, p.omegas, p.miller, p.L, p.N, return_dpsi=True)
+    w.close()
+    return p, sel, dn.cpu().numpy(), dpsi.cpu().numpy(), st, ref_dn, ref_dpsi
+
+
+def _check_dpsi(p, sel, dpsi, ref_dpsi, tol):
+    if p.gamma:
+        # [w][i][v][2][n_g]: Re and Im parts of dpsi(r) as two real functions -> dpsi(G) = R(G) + i I(G) on the full sphere
+        full = ogs.expand_half_to_full(dpsi[..., 0, :], p.miller) + 1j * ogs.expand_half_to_full(dpsi[..., 1, :], p.miller)
+        assert relmax(full, ref_dpsi) < tol
+    else:
+        assert relmax(dpsi, ref_dpsi) < tol
+
+
+def test_chi0_cfg1_full_complex():
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("cfg1")
+    assert st["rc"] == 0 and st["n_unconverged"] == 0 and st["resid_max"] <= 1e-12
+    assert relmax(dn, ref_dn) < TOL
+    _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+
+
+def test_chi0_mini2_gamma():
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini2")
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    assert relmax(dn, ref_dn) < TOL
+    _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+    assert np.max(np.abs(dpsi[..., 1, :])) == 0.0          # omega = 0: dpsi is a real function
+
+
+def test_chi0_mini3_imaginary_frequencies():
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini3")
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    for w in range(len(p.omegas)):
+        assert relmax(dn[w], ref_dn[w]) < TOL
+    _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+
+
+def test_chi0_mini4_mixed_precision():
+    import paper_2203_05623_b200 as wb
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini4", precision=wb.WEST_MIXED, tol_cg=1e-6)
+    assert relmax(dn, ref_dn) < 1e-4                        # north_star: 1e-4 for the mixed path
+    assert relmax(dn, ref_dn) > 1e-11
+
+
+def test_chi0_alpha_and_preconditioner_do_not_change_the_result():
+    p, sel, dn0, _, st0, ref_dn, _ = _run("mini2")
+    _, _, dn1, _, st1, _, _ = _run("mini2", alpha=3.0 * p.alpha, precond=0)
+    assert relmax(dn1, ref_dn) < TOL and relmax(dn1, dn0) < TOL
+    assert st1["iters"] >= st0["iters"]                    # the preconditioner only changes the iteration count
+
+
+def test_chi0_not_converged_status():
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build("cfg1")
+    w, _ = make_west(p)
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
+    dn, _, st = w.chi0_apply(dV, [0.0], tol=1e-14, max_iter=3, alpha_pv=p.alpha)
+    assert st["rc"] == wb.WEST_NOTCONVERGED and st["n_unconverged"] > 0 and st["iters"] == 3
+    w.close()
