@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the chi0*dV hot path (Eq. 10-11 of arXiv 2203.05623) on B200, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
+
+A step = one west_chi0_apply over the workload's perturbation block: RHS (a1), batched PCG to the stated tolerance with
+the dual-space H*psi, KB / P_v GEMMs and fused vector updates (a2-a9), and the dn accumulation (a10).
+metric  = chi0*dV perturbations/s (whole job, all ranks); the line also carries H*psi applications/s.
+N > 1   = weak scaling: every rank holds the full orbitals and its own block of perturbations, no collective on the
+          data path ("images"); value = all ranks' perturbations / max-over-ranks time.
+--impl reference = the CPU oracle (oracle/) timed on a bounded sample of the same workload.
+Inputs are seeded and synthetic (synth/), the occupied orbitals come from the library's own GPU eigensolver (set-up,
+untimed).  Nothing here reads /root/reference.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+TOL = 1e-8          # CG stopping tolerance of the throughput runs (reading R5)
+MAX_ITER = 300
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--chunk", type=int, default=0, help="FFT slots per chunk (0 = library default)")
+    ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.stop_flag = threading.Event()
+        self.rows = []
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self.stop_flag.wait(0.2)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def build_inputs(cfg):
+    """Seeded synthetic cell (synth/): potentials, projectors on the library's own sphere, perturbations."""
+    import synth
+    atoms = synth.atoms_for(cfg)
+    vloc = synth.vloc_for(cfg, atoms)
+    return atoms, vloc
+
+
+def setup_gpu(cfg, n_pert, chunk, verbose):
+    import torch
+    import synth
+    import paper_2203_05623_b200 as wb
+    from paper_2203_05623_b200 import eigs
+    mode = wb.WEST_GAMMA if cfg["mode"] == "gamma" else wb.WEST_FULL
+    w = wb.West(cfg["L"], cfg["n2max"], cfg["N"], mode)
+    if chunk:
+        w.set_fft_chunk(chunk)
+    miller, _, _, g2 = w.gsphere()
+    atoms, vloc = build_inputs(cfg)
+    beta, dcoef = synth.kb_projectors(miller, cfg["L"], atoms, 0.8, cfg["projectors"])
+    if mode == wb.WEST_GAMMA:
+        # synth normalises over the rows it is given (the half sphere); rescale to sum over the FULL sphere = 1
+        nrm = np.sqrt(2.0 * np.sum(np.abs(beta) ** 2, axis=1) - np.abs(beta[:, 0]) ** 2)
+        beta = beta / nrm[:, None]
+    dev = torch.device("cuda")
+    w.set_vloc(torch.from_numpy(vloc).to(dev))
+    w.set_kb(torch.from_numpy(np.ascontiguousarray(beta)).to(dev), dcoef)
+    t0 = time.time()
+    eps, psi, res = eigs.lowest_states(w, cfg["n_occ"], tol=1e-10, verbose=False)
+    gap = float(eps[cfg["n_occ"]] - eps[cfg["n_occ"] - 1])
+    if verbose:
+        print("# eigensolver: %.1f s, residual %.2e, gap %.4f Ry" % (time.time() - t0, res, gap), file=sys.stderr)
+    w.set_states(psi, eps[:cfg["n_occ"]])
+    alpha = max(2.0 * float(eps[cfg["n_occ"] - 1] - eps[0]), 0.01)
+    dV = synth.perturbations(cfg, n_pert=n_pert)
+    return w, dV, alpha, dict(eps=eps, psi=psi, gap=gap, res=res, miller=miller, vloc=vloc, beta=beta, dcoef=dcoef)
+
+
+def cpu_baseline(cfg, aux, dV0, alpha, budget_s=20.0):
+    """The oracle's own PCG route (oracle/iterative.py) on a bounded sample of (perturbation 0, state v) columns.
+
+    The orbitals handed to it are the bench's GPU-computed ones; the oracle first re-checks them as eigenvectors with its
+    own matrix-free H (no parity claim rests on this leg - it is a timing baseline)."""
+    from oracle import gsphere as ogs
+    from oracle import hamiltonian as oham
+    from oracle import iterative as oit
+    from oracle import chi0 as ochi0
+    L, N = cfg["L"], cfg["N"]
+    m = ogs.enumerate_sphere(cfg["n2max"])
+    idx = ogs.fft_index(m, N)
+    g2 = ogs.g2_of(m, L)
+    gamma = cfg["mode"] == "gamma"
+    sel = np.nonzero(ogs.half_sphere_mask(m))[0] if gamma else np.arange(len(m))
+    psi = aux["psi"].cpu().numpy()
+    U = (ogs.expand_half_to_full(psi, m) if gamma else psi).T.copy()          # [n_g_full, n_occ]
+    beta = ogs.expand_half_to_full(aux["beta"], m) if gamma else aux["beta"]
+    eps = aux["eps"]
+    apply_H = lambda y: oham.apply_h(y, m, L, N, aux["vloc"], beta, aux["dcoef"])
+    r = apply_H(U[:, 0]) - eps[0] * U[:, 0]
+    assert np.linalg.norm(r) < 1e-6, "orbitals are not eigenvectors of the oracle's H"
+    b = ochi0.rhs_vectors(U, dV0[None], idx, N)[0]                             # [n_occ, n_g]
+    cores = len(os.sched_getaffinity(0))
+    t0 = time.time()
+    n_done, iters = 0, 0
+    for v in range(cfg["n_occ"]):
+        x, it, rel = oit.pcg_sternheimer(apply_H, U, eps[v], v, b[v], g2, alpha, tol=TOL, max_iter=MAX_ITER)
+        n_done += 1
+        iters += it
+        if time.time() - t0 > budget_s:
+            break
+    dt = time.time() - t0
+    return {"value": n_done / cfg["n_occ"] / dt, "unit": "perturbations/s", "cores": cores, "kind": "oracle",
+            "sample": "oracle.iterative.pcg_sternheimer on %d of %d (i=0, v) columns of %s, tol %.0e, %d H*psi, %.1f s"
+                      % (n_done, cfg["n_occ"], cfg["name"], TOL, iters, dt),
+            "h_apply_per_s": iters / dt}
+
+
+def main():
+    a = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    import synth
+    cfg = synth.get_config(a.workload)
+    n_pert = a.n_pert or cfg.get("pert_batch", cfg["n_pert"])
+    omegas = [0.0] if a.workload != "cfg3" else list(cfg["omegas"])
+
+    if a.impl == "reference":
+        if rank != 0:
+            return
+        run_reference(a, cfg, n_pert)
+        return
+
+    import torch
+    import torch.distributed as dist
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2203_05623_b200 as wb
+    precision = wb.WEST_MIXED if cfg["precision"] == "mixed" else wb.WEST_FP64
+    # every rank: same cell and orbitals, its own block of perturbations (seeded stream offset by rank)
+    w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0))
+    if world > 1:
+        dV_np = synth.perturbations(cfg, n_pert=n_pert, first=rank * n_pert)
+    dev = torch.device("cuda")
+    dV = torch.from_numpy(dV_np).to(dev)
+    N = cfg["N"]
+    dn = torch.empty((len(omegas), n_pert, N, N, N), dtype=torch.float64, device=dev)
+    kw = dict(tol=TOL, max_iter=MAX_ITER, alpha_pv=alpha, precond=1, check_every=4, precision=precision, dn=dn)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stats = None
+    for _ in range(a.warmup):
+        _, _, stats = w.chi0_apply(dV, omegas, **kw)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    w.set_profile(True)
+    launches0 = w.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    n_h = 0
+    for _ in range(a.steps):
+        _, _, stats = w.chi0_apply(dV, omegas, **kw)
+        n_h += stats["n_h_apply"]
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    prof = w.get_profile()
+    w.set_profile(False)
+    launches = w.launch_count() - launches0
+    sampler.stop_flag.set()
+    sampler.join()
+
+    # ---- end to end: pinned host dV -> device, chi0_apply, dn -> pinned host, all inside the timed region
+    h_dV = torch.from_numpy(dV_np).pin_memory()
+    h_dn = torch.empty(dn.shape, dtype=torch.float64).pin_memory()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        dV.copy_(h_dV, non_blocking=True)
+        w.chi0_apply(dV, omegas, **kw)
+        h_dn.copy_(dn, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    units = n_pert * len(omegas) * world
+    value = units * a.steps / (ms * 1e-3)
+    hbm_peak, peak_src = peaks()
+    # ---- roofline of the dominant kernel class
+    top = max(prof, key=lambda k: prof[k]["ms"])
+    n_cols = aux_ncols(cfg)
+    roof = roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, precision == wb.WEST_MIXED, w)
+    line = {
+        "metric": "chi0*dV perturbations/s (batched Sternheimer PCG to tol %.0e)" % TOL,
+        "value": value, "unit": "perturbations/s", "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if precision == wb.WEST_FP64 else "f32 FFT / f64 vectors",
+        "data": "synthetic (seeded Si-like cell, GPU-computed orbitals)",
+        "config": {"workload": a.workload, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": len(omegas),
+                   "n_proj": cfg["n_proj"], "tol": TOL, "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
+                   "gap_ry": aux["gap"], "l2": "inputs per step (4 vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
+        "h_apply_per_s": n_h * world / (ms * 1e-3),
+        "e2e": {"value": units * a.steps / (e2e_ms * 1e-3), "unit": "perturbations/s",
+                "h2d_bytes_per_step": int(dV.numel() * 8), "d2h_bytes_per_step": int(dn.numel() * 8)},
+        "gpu_launches": int(launches),
+        "clocks": sampler.summary(),
+        "roofline": roof,
+        "kernel_ms_per_step": {k: round(v["ms"] / a.steps, 3) for k, v in prof.items() if v["spans"]},
+        "phase_ms_last_step": {"rhs": stats["ms_rhs"], "cg": stats["ms_cg"], "dn": stats["ms_dn"]},
+        "device_gb": w.device_bytes() / 1e9,
+    }
+    if world == 1 and not a.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(cfg, aux, dV_np[0], alpha)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def aux_ncols(cfg):
+    m = cfg["n_max"]
+    return sum(1 for x in range(-m, m + 1) for y in range(-m, m + 1) if x * x + y * y <= cfg["n2max"])
+
+
+def roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, mixed, w):
+    """Roofline entry for the kernel class that took the most time (DESIGN.md section 6 states the per-unit figures)."""
+    N = cfg["N"]
+    gamma = cfg["mode"] == "gamma"
+    slots = n_h / (2 if gamma else 1)                       # FFT slots pushed through H*psi in the timed region
+    csz = 8 if mixed else 16
+    t = prof[top]["ms"] * 1e-3
+    spans = max(1, prof[top]["spans"])
+    out = {"kernel": top, "avg_launch_ms": prof[top]["ms"] / spans, "peak_source": peak_src, "traffic": None}
+    if top in ("k1_g2r_z", "k2_planes", "k3_r2g_z"):
+        stick = N * n_cols * csz
+        sphere = (2 if gamma else 1) * w.n_g * 16
+        per_slot = {"k1_g2r_z": sphere + stick, "k2_planes": 2 * stick, "k3_r2g_z": stick + 2 * sphere}[top]
+        ach = per_slot * slots / t / 1e9
+        # the planes kernel is bound by FP64 arithmetic: report its flop rate against the DFMA peak as well
+        fl = 0.0
+        if top == "k2_planes":
+            nr = 2 * cfg["n_max"] + 1
+            fl = slots * N * (2 * (nr + N) * 5.0 * N * np.log2(N) + 2 * N * N) / t / 1e12
+        out.update({"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                    "algorithmic_bytes_per_slot": per_slot, "fft_tflops_nominal_5NlogN": fl})
+    elif top in ("gemm_tn", "gemm_update"):
+        rows = cfg["n_proj"] + cfg["n_occ"]
+        if not gamma:
+            rows *= 2
+        flops = 2.0 * rows * (2 * w.n_g) * n_h
+        ach = flops / t / 1e12
+        peak = 148 * 64 * 2 * 1.965e9 / 1e12
+        out.update({"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                    "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DMMA has the same rate on B200)"})
+    else:
+        per_col = 10 * 16 * w.n_g
+        ach = per_col * n_h / t / 1e9
+        out.update({"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak})
+    return out
+
+
+def run_reference(a, cfg, n_pert):
+    """--impl reference: the oracle on the host cores, same metric/unit; needs the GPU only to produce the orbitals."""
+    import torch
+    w, dV_np, alpha, aux = setup_gpu(cfg, 1, 0, verbose=True)
+    res = []
+    for _ in range(a.warmup + a.steps):
+        res.append(cpu_baseline(cfg, aux, dV_np[0], alpha, budget_s=10.0))
+    res = res[a.warmup:]
+    v = float(np.mean([r["value"] for r in res]))
+    line = {"impl": "reference", "metric": "chi0*dV perturbations/s (batched Sternheimer PCG to tol %.0e)" % TOL, "value": v,
+            "unit": "perturbations/s", "n_gpus": a.gpus, "steps": a.steps, "warmup": a.warmup, "ms_per_step": 1e3 / v if v else None,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": a.workload}, "cpu_baseline": dict(res[-1], value=v),
+            "e2e": {"value": v, "unit": "perturbations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

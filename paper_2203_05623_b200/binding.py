@@ -34,7 +34,7 @@ class west_stats(C.Structure):
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states",
            "west_fft3d", "west_h_apply", "west_chi0_apply", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
-           "west_launch_count", "west_set_fft_chunk"]
+           "west_launch_count", "west_set_fft_chunk", "west_set_profile", "west_get_profile"]
 
 
 def load_library():
@@ -60,6 +60,8 @@ def load_library():
     lib.west_launch_count.argtypes = [vp]
     lib.west_launch_count.restype = i64
     lib.west_set_fft_chunk.argtypes = [vp, i32]
+    lib.west_set_profile.argtypes = [vp, i32]
+    lib.west_get_profile.argtypes = [vp, vp, vp]
     for name in EXPORTS:
         getattr(lib, name)
         if name not in ("west_last_error", "west_device_bytes", "west_launch_count"):
@@ -222,3 +224,14 @@ class West:
 
     def set_fft_chunk(self, n):
         self._ck(self.lib.west_set_fft_chunk(self.ctx, int(n)))
+
+    PROFILE_CLASSES = ("k1_g2r_z", "k2_planes", "k3_r2g_z", "gemm_tn", "gemm_update", "cg_vec", "fft_rhs_dn", "misc")
+
+    def set_profile(self, on):
+        self._ck(self.lib.west_set_profile(self.ctx, 1 if on else 0))
+
+    def get_profile(self):
+        ms = np.zeros(8, dtype=np.float64)
+        cnt = np.zeros(8, dtype=np.int64)
+        self._ck(self.lib.west_get_profile(self.ctx, ms.ctypes.data, cnt.ctypes.data))
+        return {k: {"ms": float(ms[i]), "spans": int(cnt[i])} for i, k in enumerate(self.PROFILE_CLASSES)}

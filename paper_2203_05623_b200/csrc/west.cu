@@ -62,6 +62,13 @@ struct west_ctx {
     // workspaces (grown lazily)
     DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc;
     int* h_pinned = nullptr;           // pinned host scratch for convergence polling / reports
+
+    // optional per-kernel-class timing (west_set_profile): CUDA events on the context's stream around every launch
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    struct Span { size_t e0, e1; int cls; };
+    std::vector<Span> spans;
 };
 
 namespace {
@@ -107,6 +114,22 @@ int ensure(west_ctx* c, DevBuf& b, size_t bytes) {
     if (rc == WEST_OK) b.bytes = bytes;
     return rc;
 }
+
+// profiling classes
+enum { PC_K1 = 0, PC_K2 = 1, PC_K3 = 2, PC_GEMM_TN = 3, PC_GEMM_UP = 4, PC_CGVEC = 5, PC_FFT_OTHER = 6, PC_MISC = 7, PC_N = 8 };
+struct Prof {
+    west_ctx* c; int cls; size_t e0 = 0; bool on;
+    static size_t grab(west_ctx* c) {
+        if (c->ev_used == c->ev_pool.size()) { cudaEvent_t e; cudaEventCreate(&e); c->ev_pool.push_back(e); }
+        return c->ev_used++;
+    }
+    Prof(west_ctx* c_, int cls_) : c(c_), cls(cls_), on(c_->profile) {
+        if (on) { e0 = grab(c); cudaEventRecord(c->ev_pool[e0], c->st); }
+    }
+    ~Prof() {
+        if (on) { size_t e1 = grab(c); cudaEventRecord(c->ev_pool[e1], c->st); c->spans.push_back({e0, e1, cls}); }
+    }
+};
 
 inline long long n3_of(const west_ctx* c) { return (long long)c->cell.N * c->cell.N * c->cell.N; }
 inline bool is_gamma(const west_ctx* c) { return c->cell.mode == WEST_GAMMA; }
@@ -256,6 +279,7 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
     splits = (K + kps - 1) / kps;
     CK(cudaMemsetAsync(C, 0, (size_t)M * ldc * sizeof(double), c->st));
     dim3 grid(tn, tm, (unsigned)splits);
+    Prof prof_(c, PC_GEMM_TN);
     gemm_tn_kernel<<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1);
     CK(cudaGetLastError());
     c->launches += 1;
@@ -272,6 +296,7 @@ int launch_gemm_update(west_ctx* c, int M, int Nn, long long K, const double* C,
         attr = true;
     }
     dim3 grid((unsigned)((K + 127) / 128), (unsigned)((Nn + 127) / 128));
+    Prof prof_(c, PC_GEMM_UP);
     gemm_update_kernel<<<grid, NTHREADS, SMEM_UP, c->st>>>(M, Nn, K, C, ldc, A, lda, Y, ldy);
     CK(cudaGetLastError());
     c->launches += 1;
@@ -333,9 +358,9 @@ int hloc_apply(west_ctx* c, int f32, VecMap vm, int n_slots, const cx<double>* X
     for (int s0 = 0; s0 < n_slots; s0 += chunk) {
         const int ns = std::min(chunk, n_slots - s0);
         vm.slot0 = s0;
-        CK(c->ops->k1(f32, is_gamma(c), ns, c->st, c->geom, vm, X, c->W.p));
-        CK(c->ops->k2(f32, K2_H, ns, c->st, c->geom, a));
-        CK(c->ops->k3(f32, is_gamma(c), ns, c->st, c->geom, vm, c->W.p, e, Y));
+        { Prof p_(c, PC_K1); CK(c->ops->k1(f32, is_gamma(c), ns, c->st, c->geom, vm, X, c->W.p)); }
+        { Prof p_(c, PC_K2); CK(c->ops->k2(f32, K2_H, ns, c->st, c->geom, a)); }
+        { Prof p_(c, PC_K3); CK(c->ops->k3(f32, is_gamma(c), ns, c->st, c->geom, vm, c->W.p, e, Y)); }
         c->launches += 3;
     }
     return WEST_OK;
@@ -349,6 +374,24 @@ extern "C" {
 const char* west_last_error(const west_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 int64_t west_device_bytes(const west_ctx* c) { return c ? c->dev_bytes : 0; }
 int64_t west_launch_count(const west_ctx* c) { return c ? c->launches : 0; }
+int west_set_profile(west_ctx* c, int32_t on) {
+    if (!c) return WEST_EINVAL;
+    c->profile = on != 0;
+    return WEST_OK;
+}
+int west_get_profile(west_ctx* c, double* ms, int64_t* count) {
+    if (!c || !ms || !count) return WEST_EINVAL;
+    cudaStreamSynchronize(c->st);
+    for (int i = 0; i < PC_N; ++i) { ms[i] = 0; count[i] = 0; }
+    for (const auto& sp : c->spans) {
+        float t = 0;
+        cudaEventElapsedTime(&t, c->ev_pool[sp.e0], c->ev_pool[sp.e1]);
+        ms[sp.cls] += t; count[sp.cls] += 1;
+    }
+    c->spans.clear();
+    c->ev_used = 0;
+    return WEST_OK;
+}
 int west_set_fft_chunk(west_ctx* c, int32_t n) {
     if (!c || n < 0 || n > 65535) return WEST_EINVAL;
     c->fft_chunk = n;
@@ -419,6 +462,7 @@ int west_destroy(west_ctx* c) {
     if (!c) return WEST_OK;
     cudaStreamSynchronize(c->st);
     for (void* p : c->owned) cudaFree(p);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     delete c;
     return WEST_OK;
@@ -601,12 +645,15 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
         if (rc) return rc;
         rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, (const double*)c->coef_all.p);
         if (rc) return rc;
+        {
+        Prof p_(c, PC_CGVEC);
         wcg::cg_dot_pAp<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, (const double2*)P, (const double2*)AP, s);
         wcg::cg_update_xr<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)P, (const double2*)AP,
                                                               (double2*)X, (double2*)R, s);
         wcg::cg_update_p<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (const double2*)R, (double2*)P, s);
         CK(cudaGetLastError());
         c->launches += 3;
+        }
         if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
             CK(cudaMemcpyAsync(c->h_pinned, s.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
             CK(cudaStreamSynchronize(c->st));
@@ -693,6 +740,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
                 const int ns = std::min(chunk, n_rslots - s0);
                 vm.slot0 = s0; a.slot0 = s0;
+                Prof p_(c, PC_FFT_OTHER);
                 CK(c->ops->k2(0, K2_FROMR, ns, c->st, c->geom, a));
                 CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, c->W.p, e, R));
                 c->launches += 2;
@@ -721,6 +769,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
                 const int ns = std::min(chunk, n_rslots - s0);
                 vm.slot0 = s0; a.slot0 = s0;
+                Prof p_(c, PC_FFT_OTHER);
                 CK(c->ops->k1(0, gamma, ns, c->st, c->geom, vm, X, c->W.p));
                 CK(c->ops->k2(0, K2_DN, ns, c->st, c->geom, a));
                 c->launches += 2;
