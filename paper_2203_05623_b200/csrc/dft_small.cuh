@@ -7,7 +7,7 @@
 #endif
 
 template <typename T>
-struct cx {
+struct alignas(2 * sizeof(T)) cx {      // 16-byte (f64) / 8-byte (f32) aligned: one LDS.128 / LDG.128 per element
     T x, y;
 };
 template <typename T> WHD cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }

@@ -409,8 +409,8 @@ __global__ void __launch_bounds__(256) k3_r2g_z(WestGeom g, VecMap vm, const cx<
     K::phaseC(threadIdx.x, blockDim.x, lines, g, vm, slot, u0, e, Y);
 }
 
-template <typename T, int N1, int N2, int MODE, int LC, int NT>
-__global__ void __launch_bounds__(NT) k2_planes(WestGeom g, K2Args<T> a) {
+template <typename T, int N1, int N2, int MODE, int LC, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) k2_planes(WestGeom g, K2Args<T> a) {
     using K = K2<T, N1, N2, MODE, LC>;
     constexpr int N = K::N;
     extern __shared__ __align__(16) unsigned char smem_raw[];

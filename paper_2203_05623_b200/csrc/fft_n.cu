@@ -5,6 +5,9 @@
 #ifndef WEST_N1
 #error "compile with -DWEST_N1 -DWEST_N2 -DWEST_LC"
 #endif
+#ifndef WEST_MINB
+#define WEST_MINB 1
+#endif
 
 namespace {
 constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, LC = WEST_LC, CU = 16, NT2 = 256;
@@ -38,7 +41,7 @@ cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
 template <typename T, int MODE>
 cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
     using K = K2<T, N1, N2, MODE, LC>;
-    auto kern = k2_planes<T, N1, N2, MODE, LC, NT2>;
+    auto kern = k2_planes<T, N1, N2, MODE, LC, NT2, WEST_MINB>;
     const size_t bytes = K::smem_bytes(g.nr);
     cudaError_t e = set_smem(kern, bytes);
     if (e != cudaSuccess) return e;
