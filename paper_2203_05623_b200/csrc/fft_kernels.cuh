@@ -225,9 +225,9 @@ struct K2 {
         return (ny <= ymax && ny >= -ymax) ? Wp[c0 + ny + ymax] : mk<T>(0, 0);
     }
     // y inverse, pass A: rows of the disc straight from W
-    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp) {
-        for (int it = tid; it < g.nr * N2; it += nthr) {
-            const int row = it / N2, n2 = it - row * N2;
+    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp, int row0, int nrow) {
+        for (int it = tid; it < nrow * N2; it += nthr) {
+            const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
             cx<T> v[N1];
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) v[n1] = load_disc(Wp, g, row, N2 * n1 + n2);
@@ -237,9 +237,9 @@ struct K2 {
             for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
         }
     }
-    static WHD void yB(int tid, int nthr, cx<T>* S, const WestGeom& g) {
-        for (int it = tid; it < g.nr * N1; it += nthr) {
-            const int row = it / N1, k1 = it - row * N1;
+    static WHD void yB(int tid, int nthr, cx<T>* S, const WestGeom& g, int row0, int nrow) {
+        for (int it = tid; it < nrow * N1; it += nthr) {
+            const int rl = it / N1, k1 = it - rl * N1, row = row0 + rl;
             cx<T>* p = S + row * PITCH + N2 * k1;
             cx<T> v[N2];
 #pragma unroll
@@ -342,9 +342,9 @@ struct K2 {
             }
         }
     }
-    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g) {
-        for (int it = tid; it < g.nr * N1; it += nthr) {
-            const int row = it / N1, k1 = it - row * N1;
+    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, int row0, int nrow) {
+        for (int it = tid; it < nrow * N1; it += nthr) {
+            const int rl = it / N1, k1 = it - rl * N1, row = row0 + rl;
             cx<T>* p = S + row * PITCH + N2 * k1;
             cx<T> v[N2];
 #pragma unroll
@@ -354,9 +354,9 @@ struct K2 {
             for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
         }
     }
-    static WHD void yD(int tid, int nthr, const cx<T>* S, const WestGeom& g, cx<T>* Wp) {
-        for (int it = tid; it < g.nr * N2; it += nthr) {
-            const int row = it / N2, n2 = it - row * N2;
+    static WHD void yD(int tid, int nthr, const cx<T>* S, const WestGeom& g, cx<T>* Wp, int row0, int nrow) {
+        for (int it = tid; it < nrow * N2; it += nthr) {
+            const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
             const cx<T>* p = S + row * PITCH + n2;
             cx<T> v[N1];
 #pragma unroll
@@ -409,40 +409,54 @@ __global__ void __launch_bounds__(256) k3_r2g_z(WestGeom g, VecMap vm, const cx<
     K::phaseC(threadIdx.x, blockDim.x, lines, g, vm, slot, u0, e, Y);
 }
 
-template <typename T, int N1, int N2, int MODE, int LC, int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) k2_planes(WestGeom g, K2Args<T> a) {
-    using K = K2<T, N1, N2, MODE, LC>;
+// Plane kernel.  NW warps per CTA; each warp owns LPW = 32 / max(N1, N2) lines at a time and runs the three passes of
+// "its" lines with warp-level barriers only, so the CTA synchronises just twice (after y inverse, before y forward).
+template <int N1, int N2> struct K2Cfg { static constexpr int LPW = 32 / (N1 > N2 ? N1 : N2); };
+
+template <typename T, int N1, int N2, int MODE, int NW, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T> a) {
+    constexpr int LPW = K2Cfg<N1, N2>::LPW;
+    using K = K2<T, N1, N2, MODE, LPW>;
     constexpr int N = K::N;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);
     cx<T>* X = S + g.nr * K::PITCH;
-    cx<T>* tw = X + LC * K::PITCH;
+    cx<T>* tw = X + NW * LPW * K::PITCH;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    cx<T>* Xw = X + warp * LPW * K::PITCH;
     load_tw<T, N>(tw, g.tw);
     const int pz = blockIdx.x, slot = blockIdx.y;
     cx<T>* Wp = a.W + ((long long)slot * N + pz) * g.n_cols;
     __syncthreads();
     if (MODE != K2_FROMR) {
-        K::yA(threadIdx.x, NT, S, tw, g, Wp);
-        __syncthreads();
-        K::yB(threadIdx.x, NT, S, g);
+        for (int r0 = warp * LPW; r0 < g.nr; r0 += NW * LPW) {
+            const int nrow = g.nr - r0 < LPW ? g.nr - r0 : LPW;
+            K::yA(lane, 32, S, tw, g, Wp, r0, nrow);
+            __syncwarp();
+            K::yB(lane, 32, S, g, r0, nrow);
+        }
         __syncthreads();
     }
-    for (int py0 = 0; py0 < N; py0 += LC) {
+    for (int py0 = warp * LPW; py0 < N; py0 += NW * LPW) {
         if (MODE != K2_FROMR) {
-            K::xA(threadIdx.x, NT, S, X, tw, g, py0);
-            __syncthreads();
+            K::xA(lane, 32, S, Xw, tw, g, py0);
+            __syncwarp();
         }
-        K::xB(threadIdx.x, NT, X, tw, a, slot, pz, py0);
+        K::xB(lane, 32, Xw, tw, a, slot, pz, py0);
         if (MODE == K2_H || MODE == K2_FROMR) {
-            __syncthreads();
-            K::xC(threadIdx.x, NT, S, X, g, py0);
+            __syncwarp();
+            K::xC(lane, 32, S, Xw, g, py0);
         }
-        __syncthreads();
+        __syncwarp();
     }
     if (MODE == K2_H || MODE == K2_FROMR) {
-        K::yC(threadIdx.x, NT, S, tw, g);
         __syncthreads();
-        K::yD(threadIdx.x, NT, S, g, Wp);
+        for (int r0 = warp * LPW; r0 < g.nr; r0 += NW * LPW) {
+            const int nrow = g.nr - r0 < LPW ? g.nr - r0 : LPW;
+            K::yC(lane, 32, S, tw, g, r0, nrow);
+            __syncwarp();
+            K::yD(lane, 32, S, g, Wp, r0, nrow);
+        }
     }
 }
 #endif

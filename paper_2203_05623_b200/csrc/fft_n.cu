@@ -1,16 +1,19 @@
 // Per-grid-size instantiation of the FFT kernels.  Compiled once per supported N with
-//   -DWEST_N1=.. -DWEST_N2=.. -DWEST_LC=..   (N = N1*N2; LC = x lines per chunk in K2)
+//   -DWEST_N1=.. -DWEST_N2=.. -DWEST_NN=.. -DWEST_NW=.. -DWEST_MINB=.. -DWEST_CU=..
+//   (N = N1*N2; NW = warps per CTA of the plane kernel, MINB = its resident CTAs per SM; CU = stick units per CTA in K1/K3)
 #include "fft_ops.h"
 
 #ifndef WEST_N1
-#error "compile with -DWEST_N1 -DWEST_N2 -DWEST_LC"
+#error "compile with -DWEST_N1 -DWEST_N2 -DWEST_NN -DWEST_NW -DWEST_MINB -DWEST_CU"
 #endif
 #ifndef WEST_MINB
 #define WEST_MINB 1
 #endif
 
 namespace {
-constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, LC = WEST_LC, CU = 16, NT2 = 256;
+constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, NW = WEST_NW, LPW = K2Cfg<N1, N2>::LPW;
+// stick units per CTA: GAMMA runs two transforms per unit, so FULL takes twice as many units for the same 256 threads
+template <bool GAMMA> struct CUof { static constexpr int v = GAMMA ? WEST_CU : 2 * WEST_CU; };
 
 template <typename KernelT>
 cudaError_t set_smem(KernelT k, size_t bytes) {
@@ -20,6 +23,7 @@ cudaError_t set_smem(KernelT k, size_t bytes) {
 
 template <typename T, bool GAMMA>
 cudaError_t k1_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const cx<double>* X, void* W) {
+    constexpr int CU = CUof<GAMMA>::v;
     using K = K1<T, N1, N2, GAMMA, CU>;
     auto kern = k1_g2r_z<T, N1, N2, GAMMA, CU>;
     cudaError_t e = set_smem(kern, K::smem_bytes);
@@ -30,6 +34,7 @@ cudaError_t k1_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
 }
 template <typename T, bool GAMMA>
 cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const void* W, K3Epi ep, cx<double>* Y) {
+    constexpr int CU = CUof<GAMMA>::v;
     using K = K3<T, N1, N2, GAMMA, CU>;
     auto kern = k3_r2g_z<T, N1, N2, GAMMA, CU>;
     cudaError_t e = set_smem(kern, K::smem_bytes);
@@ -40,9 +45,9 @@ cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
 }
 template <typename T, int MODE>
 cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
-    using K = K2<T, N1, N2, MODE, LC>;
-    auto kern = k2_planes<T, N1, N2, MODE, LC, NT2, WEST_MINB>;
-    const size_t bytes = K::smem_bytes(g.nr);
+    using K = K2<T, N1, N2, MODE, LPW>;
+    auto kern = k2_planes<T, N1, N2, MODE, NW, WEST_MINB>;
+    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + NW * LPW) * K::PITCH + NN);
     cudaError_t e = set_smem(kern, bytes);
     if (e != cudaSuccess) return e;
     K2Args<T> t;
@@ -50,7 +55,7 @@ cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a
     t.V = reinterpret_cast<const T*>(a.V);
     t.R = a.R; t.ucache = a.ucache; t.dV = a.dV; t.dn = a.dn; t.n_uslots = a.n_uslots; t.slot0 = a.slot0; t.fac = a.fac;
     dim3 grid(NN, n_slots);
-    kern<<<grid, NT2, bytes, st>>>(g, t);
+    kern<<<grid, NW * 32, bytes, st>>>(g, t);
     return cudaGetLastError();
 }
 
@@ -75,7 +80,7 @@ cudaError_t k2_entry(int f32, int mode, int n_slots, cudaStream_t st, const West
     }
     return cudaErrorInvalidValue;
 }
-const FftOps ops = {NN, N1, N2, CU, LC, k1_entry, k2_entry, k3_entry};
+const FftOps ops = {NN, N1, N2, WEST_CU, LPW, k1_entry, k2_entry, k3_entry};
 }  // namespace
 
 #define WEST_CAT2(a, b) a##b
