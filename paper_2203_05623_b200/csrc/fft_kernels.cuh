@@ -31,12 +31,19 @@ struct VecMap {
 template <typename T> WHD cx<T> cvt(cx<double> a) { return mk<T>((T)a.x, (T)a.y); }
 template <typename T> WHD cx<double> cvd(cx<T> a) { return mk<double>((double)a.x, (double)a.y); }
 WHD int wrap_signed(int n, int N) { return n < N / 2 ? n : n - N; }
+// Alias-free grids have N >= 4 n_max + 1, so every non-zero frequency satisfies |n| <= (N-1)/4.  For the strided pass
+// (n = N2 n1 + n2) this tells at COMPILE time which n1 can hold a non-zero input / a needed output at all.
+template <int N1, int N2> WHD constexpr bool keep_n1(int n1) {
+    constexpr int N = N1 * N2, LIM = (N - 1) / 4;
+    // the run n = N2 n1 .. N2 n1 + N2 - 1 meets [0, LIM] or [N - LIM, N - 1]
+    return (N2 * n1 <= LIM) || (N2 * n1 + N2 - 1 >= N - LIM);
+}
 
 // ---------------------------------------------------------------------------------------------------------------- K1
 template <typename T, int N1, int N2, bool GAMMA, int CU>
 struct K1 {
     static constexpr int N = N1 * N2, PITCH = N + 1, NF = GAMMA ? 2 : 1, NL = CU * NF;
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + N);
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + 2 * N);
 
     // phase A: strided DFT-N1 straight from the sphere coefficients, twiddle, store to the line buffer
     static WHD void phaseA(int tid, int nthr, cx<T>* lines, const cx<T>* tw, const WestGeom& g, VecMap vm, int slot, int u0,
@@ -54,7 +61,7 @@ struct K1 {
                 for (int n1 = 0; n1 < N1; ++n1) {
                     const int nz = wrap_signed(N2 * n1 + n2, N);
                     cx<T> val = mk<T>(0, 0);
-                    if (nz <= zmax && nz >= -zmax) {
+                    if (keep_n1<N1, N2>(n1) && nz <= zmax && nz >= -zmax) {
                         if (half00) {
                             cx<double> c = src[nz >= 0 ? nz : -nz];
                             val = mk<T>((T)c.x, (T)(nz >= 0 ? c.y : -c.y));
@@ -72,7 +79,7 @@ struct K1 {
             }
             cx<T>* dst = lines + line * PITCH + n2;
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
+            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
         }
     }
     // phase B: contiguous DFT-N2
@@ -118,7 +125,7 @@ struct K3Epi {
 template <typename T, int N1, int N2, bool GAMMA, int CU>
 struct K3 {
     static constexpr int N = N1 * N2, PITCH = N + 1, NF = GAMMA ? 2 : 1, NL = CU * NF;
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + N);
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + 2 * N);
 
     static WHD void phaseA(int tid, int nthr, cx<T>* lines, const WestGeom& g, int slot, int u0, const cx<T>* W) {
         for (int it = tid; it < N * CU; it += nthr) {
@@ -150,7 +157,7 @@ struct K3 {
             for (int j = 0; j < N2; ++j) v[j] = p[j];
             Dft<T, N2, -1>::run(v);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
+            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
         }
     }
     // phase A': strided DFT-N1 (sign -), epilogue to the sphere
@@ -173,6 +180,7 @@ struct K3 {
             const double sh = (e.kinetic && e.shift) ? e.shift[vec] : 0.0;
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) {
+                if (!keep_n1<N1, N2>(n1)) continue;
                 const int nz = wrap_signed(N2 * n1 + n2, N);
                 if (nz > zmax || nz < (half00 ? 0 : -zmax)) continue;
                 const long long o = half00 ? nz : nz + zmax;
@@ -217,7 +225,7 @@ struct K2Args {
 template <typename T, int N1, int N2, int MODE, int LC>
 struct K2 {
     static constexpr int N = N1 * N2, PITCH = N + 1;
-    static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + N); }
+    static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + 2 * N); }
 
     static WHD cx<T> load_disc(const cx<T>* Wp, const WestGeom& g, int row, int n) {
         const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
@@ -230,11 +238,11 @@ struct K2 {
             const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
             cx<T> v[N1];
 #pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) v[n1] = load_disc(Wp, g, row, N2 * n1 + n2);
+            for (int n1 = 0; n1 < N1; ++n1) v[n1] = keep_n1<N1, N2>(n1) ? load_disc(Wp, g, row, N2 * n1 + n2) : mk<T>(0, 0);
             Dft<T, N1, +1>::run(v);
             cx<T>* dst = S + row * PITCH + n2;
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
+            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
         }
     }
     static WHD void yB(int tid, int nthr, cx<T>* S, const WestGeom& g, int row0, int nrow) {
@@ -259,12 +267,12 @@ struct K2 {
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) {
                 const int nx = wrap_signed(N2 * n1 + n2, N);
-                v[n1] = (nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + py] : mk<T>(0, 0);
+                v[n1] = (keep_n1<N1, N2>(n1) && nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + py] : mk<T>(0, 0);
             }
             Dft<T, N1, +1>::run(v);
             cx<T>* dst = X + l * PITCH + n2;
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[n2 * k1]);
+            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
         }
     }
     // x inverse pass B, the real-space operation, x forward pass B' - all on the same N2 contiguous values
@@ -321,7 +329,7 @@ struct K2 {
             }
             Dft<T, N2, -1>::run(v);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
+            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
         }
     }
     // x forward pass A': strided DFT-N1, keep |n_x| <= n_max, back into S
@@ -337,6 +345,7 @@ struct K2 {
             Dft<T, N1, -1>::run(v);
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) {
+                if (!keep_n1<N1, N2>(n1)) continue;
                 const int nx = wrap_signed(N2 * n1 + n2, N);
                 if (nx <= g.n_max && nx >= -g.n_max) S[(nx + g.n_max) * PITCH + py] = v[n1];
             }
@@ -351,7 +360,7 @@ struct K2 {
             for (int j = 0; j < N2; ++j) v[j] = p[j];
             Dft<T, N2, -1>::run(v);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[k1 * j]);
+            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
         }
     }
     static WHD void yD(int tid, int nthr, const cx<T>* S, const WestGeom& g, cx<T>* Wp, int row0, int nrow) {
@@ -365,6 +374,7 @@ struct K2 {
             const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) {
+                if (!keep_n1<N1, N2>(n1)) continue;
                 const int ny = wrap_signed(N2 * n1 + n2, N);
                 if (ny <= ymax && ny >= -ymax) Wp[c0 + ny + ymax] = v[n1];
             }
@@ -373,9 +383,17 @@ struct K2 {
 };
 
 #ifdef __CUDACC__
-template <typename T, int N>
+template <typename T, int N1, int N2>
 __device__ __forceinline__ void load_tw(cx<T>* tw_s, const cx<double>* tw_g) {
-    for (int i = threadIdx.x; i < N; i += blockDim.x) tw_s[i] = cvt<T>(tw_g[i]);
+    // level twiddles in the two orders the passes read them, so that the lanes of a warp hit consecutive entries:
+    // tw_s[k1 * N2 + n2] = w^(n2 k1) (strided pass, lanes run over n2); tw_s[N + j * N1 + k1] = w^(k1 j) (contiguous pass, lanes over k1)
+    constexpr int N = N1 * N2;
+    for (int i = threadIdx.x; i < N; i += blockDim.x) {
+        const int k1 = i / N2, n2 = i - k1 * N2;
+        tw_s[i] = cvt<T>(tw_g[n2 * k1]);
+        const int j = i / N1, k1b = i - j * N1;
+        tw_s[N + i] = cvt<T>(tw_g[k1b * j]);
+    }
 }
 
 template <typename T, int N1, int N2, bool GAMMA, int CU>
@@ -384,7 +402,7 @@ __global__ void __launch_bounds__(256) k1_g2r_z(WestGeom g, VecMap vm, const cx<
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* lines = reinterpret_cast<cx<T>*>(smem_raw);
     cx<T>* tw = lines + K::NL * K::PITCH;
-    load_tw<T, K::N>(tw, g.tw);
+    load_tw<T, N1, N2>(tw, g.tw);
     __syncthreads();
     const int slot = blockIdx.y, u0 = blockIdx.x * CU;
     K::phaseA(threadIdx.x, blockDim.x, lines, tw, g, vm, slot, u0, X);
@@ -400,7 +418,7 @@ __global__ void __launch_bounds__(256) k3_r2g_z(WestGeom g, VecMap vm, const cx<
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* lines = reinterpret_cast<cx<T>*>(smem_raw);
     cx<T>* tw = lines + K::NL * K::PITCH;
-    load_tw<T, K::N>(tw, g.tw);
+    load_tw<T, N1, N2>(tw, g.tw);
     const int slot = blockIdx.y, u0 = blockIdx.x * CU;
     K::phaseA(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
     __syncthreads();
@@ -424,7 +442,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T>
     cx<T>* tw = X + NW * LPW * K::PITCH;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     cx<T>* Xw = X + warp * LPW * K::PITCH;
-    load_tw<T, N>(tw, g.tw);
+    load_tw<T, N1, N2>(tw, g.tw);
     const int pz = blockIdx.x, slot = blockIdx.y;
     cx<T>* Wp = a.W + ((long long)slot * N + pz) * g.n_cols;
     __syncthreads();

@@ -47,7 +47,7 @@ template <typename T, int MODE>
 cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
     using K = K2<T, N1, N2, MODE, LPW>;
     auto kern = k2_planes<T, N1, N2, MODE, NW, WEST_MINB>;
-    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + NW * LPW) * K::PITCH + NN);
+    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + NW * LPW) * K::PITCH + 2 * NN);
     cudaError_t e = set_smem(kern, bytes);
     if (e != cudaSuccess) return e;
     K2Args<T> t;
