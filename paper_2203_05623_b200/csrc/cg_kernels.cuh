@@ -93,9 +93,10 @@ __device__ __forceinline__ double norm_accum(const double2* a, long long n_g, in
 // r holds b on entry.  p = M r, rz = (r, M r), b2 = rr = ||r||^2, active = b2 > 0
 template <int MODE>
 __global__ void __launch_bounds__(NT) cg_init(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
-                                              const double2* R, double2* P, Scalars s) {
+                                              const double2* R, double2* P, Scalars s, int* colmap) {
     __shared__ double sh[32];
     const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    if (threadIdx.x == 0) colmap[col] = col;
     const double2* r = R + (long long)col * nvpc * n_g;
     double2* p = P + (long long)col * nvpc * n_g;
     const double tkv = tk[col % n_occ];
@@ -124,12 +125,12 @@ __global__ void __launch_bounds__(NT) cg_init(long long n_g, int n_occ, const do
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(NT) cg_dot_pAp(long long n_g, const double2* P, const double2* AP, Scalars s) {
+__global__ void __launch_bounds__(NT) cg_dot_pAp(long long n_g, const double2* P, const double2* AP, Scalars s, const int* colmap) {
     __shared__ double sh[16];
-    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
     if (!s.active[col]) return;
-    const double2* p = P + (long long)col * nvpc * n_g;
-    const double2* ap = AP + (long long)col * nvpc * n_g;
+    const double2* p = P + (long long)k * nvpc * n_g;
+    const double2* ap = AP + (long long)k * nvpc * n_g;
     double acc[2] = {0, 0};
     for (int g = threadIdx.x; g < n_g; g += NT) dot_accum<MODE>(p, ap, n_g, g, 1.0, acc);
     block_reduce<2>(acc, sh);
@@ -139,13 +140,14 @@ __global__ void __launch_bounds__(NT) cg_dot_pAp(long long n_g, const double2* P
 // x += a p ; r -= a Ap ; rznew = (r, M r) ; rr = ||r||^2
 template <int MODE>
 __global__ void __launch_bounds__(NT) cg_update_xr(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
-                                                   const double2* P, const double2* AP, double2* X, double2* R, Scalars s) {
+                                                   const double2* P, const double2* AP, double2* X, double2* R, Scalars s,
+                                                   const int* colmap) {
     __shared__ double sh[32];
-    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+    const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
     if (!s.active[col]) return;
-    const long long o = (long long)col * nvpc * n_g;
+    const long long o = (long long)k * nvpc * n_g;          // r, p, Ap live in compacted order; x in original column order
     const double2* p = P + o; const double2* ap = AP + o;
-    double2* x = X + o; double2* r = R + o;
+    double2* x = X + (long long)col * nvpc * n_g; double2* r = R + o;
     const double2 a = cdiv(s.rz[col], s.pAp[col]);
     const double tkv = tk[col % n_occ];
     double acc[3] = {0, 0, 0};
@@ -181,10 +183,10 @@ __global__ void __launch_bounds__(NT) cg_update_xr(long long n_g, int n_occ, con
 // p = M r + beta p ; rz = rznew ; convergence bookkeeping
 template <int MODE>
 __global__ void __launch_bounds__(NT) cg_update_p(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
-                                                  double tol2, const double2* R, double2* P, Scalars s) {
-    const int col = blockIdx.x, nvpc = MODE == 1 ? 2 : 1;
+                                                  double tol2, const double2* R, double2* P, Scalars s, const int* colmap) {
+    const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
     if (!s.active[col]) return;
-    const long long o = (long long)col * nvpc * n_g;
+    const long long o = (long long)k * nvpc * n_g;
     const double2* r = R + o; double2* p = P + o;
     const double rr = s.rr[col], b2 = s.b2[col];
     const bool still = rr > tol2 * b2;
@@ -225,6 +227,43 @@ __global__ void cg_report(int n_col, double tol2, Scalars s, double* out /* [2]:
         __syncthreads();
     }
     if (threadIdx.x == 0) { out[0] = sqrt(shm[0]); out[1] = (double)shc[0]; }
+}
+
+// Compaction of the active columns (order preserving).  One CTA: new_map[j] = original column of the j-th still-active
+// entry of old_map[0..n_old), src[j] = its old compacted position.
+__global__ void __launch_bounds__(1024) cg_compact_map(int n_old, const int* old_map, const int* active, int* new_map, int* src) {
+    __shared__ int warp_sums[32];
+    __shared__ int base;
+    if (threadIdx.x == 0) base = 0;
+    __syncthreads();
+    for (int start = 0; start < n_old; start += 1024) {
+        const int i = start + threadIdx.x;
+        const int col = i < n_old ? old_map[i] : -1;
+        const int flag = (col >= 0 && active[col]) ? 1 : 0;
+        int v = flag;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, v, o); if ((threadIdx.x & 31) >= o) v += t; }
+        if ((threadIdx.x & 31) == 31) warp_sums[threadIdx.x >> 5] = v;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            int w = warp_sums[threadIdx.x];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, w, o); if (threadIdx.x >= o) w += t; }
+            warp_sums[threadIdx.x] = w;
+        }
+        __syncthreads();
+        const int before = base + v - flag + ((threadIdx.x >> 5) ? warp_sums[(threadIdx.x >> 5) - 1] : 0);
+        if (flag) { new_map[before] = col; src[before] = i; }
+        __syncthreads();
+        if (threadIdx.x == 0) base += warp_sums[31];
+        __syncthreads();
+    }
+}
+// dst[j] = src_vec[src[j]] for whole columns (nvpc * n_g complex each)
+__global__ void __launch_bounds__(NT) cg_gather_cols(long long len, const int* src, const double2* in, double2* out) {
+    const double2* a = in + (long long)src[blockIdx.x] * len;
+    double2* b = out + (long long)blockIdx.x * len;
+    for (long long g = threadIdx.x; g < len; g += NT) b[g] = a[g];
 }
 
 // C[m][n] <- coef[m] * (gamma ? 2 C[m][n] - A[m][0] X[n][0] : C[m][n])      (A[m][0], X[n][0]: real part of G = 0)

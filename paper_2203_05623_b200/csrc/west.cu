@@ -60,7 +60,7 @@ struct west_ctx {
     int n_uslots = 0;
 
     // workspaces (grown lazily)
-    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc;
+    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps;
     int* h_pinned = nullptr;           // pinned host scratch for convergence polling / reports
 
     // optional per-kernel-class timing (west_set_profile): CUDA events on the context's stream around every launch
@@ -235,9 +235,9 @@ __global__ void kinetic_expect(long long n_g, int gamma, const double* g2, const
     }
     if (threadIdx.x == 0) tk[blockIdx.x] = sh[0];
 }
-__global__ void fill_shift(int n_vec, int nvpc, int n_occ, const double* eps, double* shift) {
+__global__ void fill_shift(int n_vec, int nvpc, int n_occ, const double* eps, double* shift, const int* colmap) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_vec) shift[i] = eps[(i / nvpc) % n_occ];
+    if (i < n_vec) shift[i] = eps[(colmap ? colmap[i / nvpc] : i / nvpc) % n_occ];
 }
 
 inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
@@ -621,46 +621,71 @@ int west_gemm_update(west_ctx* c, int32_t m, int32_t n, int64_t k, const double*
 namespace {
 
 template <int MODE>
-int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omega, cx<double>* X, cx<double>* R, cx<double>* P,
-             cx<double>* AP, const double* shift, wcg::Scalars s, int* iters_out) {
+int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omega, cx<double>* X, cx<double>*& R, cx<double>*& P,
+             cx<double>*& AP, double* shift, const double* d_eps, wcg::Scalars s, int* maps /* [3][n_col] */, int* iters_out,
+             int64_t* n_h_out) {
     const long long n_g = c->hs.n_g;
-    const int nvpc = MODE == 1 ? 2 : 1, n_vec = n_col * nvpc, n_occ = c->n_occ;
+    const int nvpc = MODE == 1 ? 2 : 1, n_occ = c->n_occ;
+    const long long len = (long long)nvpc * n_g;
     const int gamma = is_gamma(c);
     const double* g2 = c->d_g2;
     const double* tk = (const double*)c->tk.p;
     const double tol2 = o.tol * o.tol;
     const int every = std::max(1, o.check_every);
+    int* colmap = maps; int* newmap = maps + n_col; int* src = maps + 2 * (size_t)n_col;
     CK(cudaMemsetAsync(s.counters, 0, 2 * sizeof(int), c->st));
-    CK(cudaMemsetAsync(X, 0, sizeof(cx<double>) * n_g * n_vec, c->st));
-    wcg::cg_init<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)R, (double2*)P, s);
+    CK(cudaMemsetAsync(X, 0, sizeof(cx<double>) * len * n_col, c->st));
+    wcg::cg_init<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)R, (double2*)P, s, colmap);
     CK(cudaGetLastError());
     c->launches += 1;
-    // slots of the H application: GAMMA pairs vectors (2s, 2s+1) - in MODE 1 these are (Re, Im) of one column
-    VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
-    const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
     const int rows = c->rows_kb + c->rows_psi;
+    int n_act = n_col;          // columns currently held (compacted) in R, P, AP
     int it = 0;
+    int64_t n_h = 0;
     for (; it < o.max_iter; ++it) {
+        // slots of the H application: GAMMA pairs vectors (2s, 2s+1) - in MODE 1 these are (Re, Im) of one column
+        const int n_vec = n_act * nvpc;
+        VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
+        const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
         int rc = hloc_apply(c, f32, vm, n_slots, P, AP, shift, omega);
         if (rc) return rc;
         rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, (const double*)c->coef_all.p);
         if (rc) return rc;
+        n_h += n_vec;
         {
-        Prof p_(c, PC_CGVEC);
-        wcg::cg_dot_pAp<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, (const double2*)P, (const double2*)AP, s);
-        wcg::cg_update_xr<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)P, (const double2*)AP,
-                                                              (double2*)X, (double2*)R, s);
-        wcg::cg_update_p<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (const double2*)R, (double2*)P, s);
-        CK(cudaGetLastError());
-        c->launches += 3;
+            Prof p_(c, PC_CGVEC);
+            wcg::cg_dot_pAp<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, (const double2*)P, (const double2*)AP, s, colmap);
+            wcg::cg_update_xr<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)P, (const double2*)AP,
+                                                                  (double2*)X, (double2*)R, s, colmap);
+            wcg::cg_update_p<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (const double2*)R, (double2*)P, s, colmap);
+            CK(cudaGetLastError());
+            c->launches += 3;
         }
         if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
             CK(cudaMemcpyAsync(c->h_pinned, s.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
             CK(cudaStreamSynchronize(c->st));
-            if (c->h_pinned[0] <= 0) { ++it; break; }
+            const int live = c->h_pinned[0];
+            if (live <= 0) { ++it; break; }
+            // drop converged columns from the working set when that removes at least ~6 % of it (a1-a9 then run on fewer vectors)
+            if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
+                Prof p_(c, PC_CGVEC);
+                wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, colmap, s.active, newmap, src);
+                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(len, src, (const double2*)R, (double2*)AP);
+                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(len, src, (const double2*)P, (double2*)R);
+                CK(cudaGetLastError());
+                c->launches += 3;
+                cx<double>* oldR = R; cx<double>* oldP = P;
+                R = AP; P = oldR; AP = oldP;           // rotate: AP (scratch) now holds r, the old r buffer holds p
+                std::swap(colmap, newmap);
+                n_act = live;
+                fill_shift<<<blocks_for(n_act * nvpc, 256), 256, 0, c->st>>>(n_act * nvpc, nvpc, n_occ, d_eps, shift, colmap);
+                CK(cudaGetLastError());
+                c->launches += 1;
+            }
         }
     }
     *iters_out = it;
+    *n_h_out = n_h;
     return WEST_OK;
 }
 
@@ -695,6 +720,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     if ((rc = ensure(c, c->dVpos, sizeof(double) * n3 * n_pert))) return rc;
     if ((rc = ensure(c, c->dnpos, sizeof(double) * n3 * n_pert))) return rc;
     if ((rc = ensure(c, c->scal, (size_t)n_col * (3 * sizeof(double2) + 2 * sizeof(double) + sizeof(int)) + 64))) return rc;
+    if ((rc = ensure(c, c->maps, sizeof(int) * 3 * (size_t)n_col))) return rc;
     wcg::Scalars s;
     {
         char* p = (char*)c->scal.p;
@@ -727,7 +753,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         const double omega = omega_host[w];
         const int mode = gamma ? (omega > 0 ? 1 : 0) : 2;
         const int nvpc = mode == 1 ? 2 : 1, n_vec = n_col * nvpc;
-        fill_shift<<<blocks_for(n_vec, 256), 256, 0, c->st>>>(n_vec, nvpc, n_occ, d_eps, (double*)c->shift.p);
+        fill_shift<<<blocks_for(n_vec, 256), 256, 0, c->st>>>(n_vec, nvpc, n_occ, d_eps, (double*)c->shift.p, nullptr);
         CK(cudaGetLastError());
         if (stats) CK(cudaEventRecord(ev[0], c->st));
         // ---- a1: b = -P_c (dV_i psi_v), written into R.   slot (i, us) -> columns i*n_occ + 2us (+1)  [GAMMA] or i*n_occ + us
@@ -755,9 +781,10 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         if (stats) CK(cudaEventRecord(ev[1], c->st));
         // ---- a2-a9: batched PCG / COCG
         int iters = 0;
-        if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (const double*)c->shift.p, s, &iters);
-        else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (const double*)c->shift.p, s, &iters);
-        else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (const double*)c->shift.p, s, &iters);
+        int64_t n_h = 0;
+        if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
+        else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
+        else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
         if (rc) return rc;
         if (stats) CK(cudaEventRecord(ev[2], c->st));
         // ---- a10: dn_i(r) = (4/Omega) Re sum_v conj(u_v) du_iv
@@ -807,7 +834,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             stats->iters = std::max(stats->iters, iters);
             stats->n_unconverged += (int)h[1];
             stats->resid_max = std::max(stats->resid_max, h[0]);
-            stats->n_h_apply += (int64_t)iters * n_vec;
+            stats->n_h_apply += n_h;
             if (h[1] > 0) ret = WEST_NOTCONVERGED;
         } else {
             // convergence status without stats: the last polled counter
