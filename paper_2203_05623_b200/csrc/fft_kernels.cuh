@@ -128,22 +128,39 @@ struct K3 {
     static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + 2 * N);
 
     static WHD void phaseA(int tid, int nthr, cx<T>* lines, const WestGeom& g, int slot, int u0, const cx<T>* W) {
-        for (int it = tid; it < N * CU; it += nthr) {
-            const int pos = it / CU, ul = it - pos * CU, u = u0 + ul;
-            const cx<T>* src = W + ((long long)slot * N + pos) * g.n_cols;
-            if (GAMMA) {
-                cx<T> a = mk<T>(0, 0), b = mk<T>(0, 0);
-                if (u < g.n_units) {
-                    const int cp = u + (g.n_cols - g.n_units);
-                    const cx<T> sp = src[cp];
-                    const cx<T> sm = u == 0 ? sp : src[g.n_cols - 1 - cp];
-                    a = mk<T>((T)0.5 * (sp.x + sm.x), (T)0.5 * (sp.y - sm.y));      // (S+ + conj S-)/2
-                    b = mk<T>((T)0.5 * (sp.y + sm.y), (T)0.5 * (sm.x - sp.x));      // (S+ - conj S-)/(2i)
+        // loads of UNR items are issued before any shared-memory store so that several global loads are in flight per thread
+        constexpr int UNR = 4;
+        for (int it0 = tid; it0 < N * CU; it0 += nthr * UNR) {
+            cx<T> sp[UNR], sm[UNR];
+#pragma unroll
+            for (int q = 0; q < UNR; ++q) {
+                const int it = it0 + q * nthr;
+                sp[q] = mk<T>(0, 0); sm[q] = mk<T>(0, 0);
+                if (it < N * CU) {
+                    const int pos = it / CU, ul = it - pos * CU, u = u0 + ul;
+                    const cx<T>* src = W + ((long long)slot * N + pos) * g.n_cols;
+                    if (u < g.n_units) {
+                        if (GAMMA) {
+                            const int cp = u + (g.n_cols - g.n_units);
+                            sp[q] = src[cp];
+                            sm[q] = u == 0 ? sp[q] : src[g.n_cols - 1 - cp];
+                        } else {
+                            sp[q] = src[u];
+                        }
+                    }
                 }
-                lines[(2 * ul) * PITCH + pos] = a;
-                lines[(2 * ul + 1) * PITCH + pos] = b;
-            } else {
-                lines[ul * PITCH + pos] = u < g.n_units ? src[u] : mk<T>(0, 0);
+            }
+#pragma unroll
+            for (int q = 0; q < UNR; ++q) {
+                const int it = it0 + q * nthr;
+                if (it >= N * CU) continue;
+                const int pos = it / CU, ul = it - pos * CU;
+                if (GAMMA) {
+                    lines[(2 * ul) * PITCH + pos] = mk<T>((T)0.5 * (sp[q].x + sm[q].x), (T)0.5 * (sp[q].y - sm[q].y));      // (S+ + conj S-)/2
+                    lines[(2 * ul + 1) * PITCH + pos] = mk<T>((T)0.5 * (sp[q].y + sm[q].y), (T)0.5 * (sm[q].x - sp[q].x));  // (S+ - conj S-)/(2i)
+                } else {
+                    lines[ul * PITCH + pos] = sp[q];
+                }
             }
         }
     }
@@ -168,16 +185,16 @@ struct K3 {
             const int u = u0 + line / NF, f = line % NF;
             const long long vec = (long long)(vm.slot0 + slot) * vm.vstride + (long long)f * vm.voffb;
             if (u >= g.n_units || vec >= vm.n_vec) continue;
-            const cx<T>* p = lines + line * PITCH + n2;
-            cx<T> v[N1];
-#pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
-            Dft<T, N1, -1>::run(v);
             const int zmax = g.unit_zmax[u];
             const bool half00 = GAMMA && u == 0;
             const long long base = vec * g.n_g + g.unit_off[u];
             const long long pbase = GAMMA ? ((long long)(vm.slot0 + slot) * vm.vstride + (long long)(1 - f) * vm.voffb) * g.n_g + g.unit_off[u] : 0;
             const double sh = (e.kinetic && e.shift) ? e.shift[vec] : 0.0;
+            const cx<T>* p = lines + line * PITCH + n2;
+            cx<T> v[N1];
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
+            Dft<T, N1, -1>::run(v);
 #pragma unroll
             for (int n1 = 0; n1 < N1; ++n1) {
                 if (!keep_n1<N1, N2>(n1)) continue;

@@ -271,9 +271,17 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
         attr = true;
     }
     const int tm = (M + BM - 1) / BM, tn = (Nn + BN - 1) / BN;
-    long long splits = (4 * 148 + (long long)tm * tn - 1) / ((long long)tm * tn);
-    const long long max_splits = std::max<long long>(1, K / (8 * BK));
-    splits = std::max<long long>(1, std::min(splits, max_splits));
+    // split K so that the CTA count fills whole waves of the 148 SMs (one 164 KB CTA per SM): pick the split count with
+    // the best wave efficiency, each split keeping at least 32 k-steps
+    const long long tiles = (long long)tm * tn;
+    const long long max_splits = std::max<long long>(1, std::min<long long>(16, K / (32 * BK)));
+    long long splits = 1;
+    double best = -1.0;
+    for (long long sp = 1; sp <= max_splits; ++sp) {
+        const double waves = (double)(tiles * sp) / 148.0;
+        const double eff = waves / std::ceil(waves) - 0.004 * (double)sp;     // mild preference for fewer splits (atomic traffic)
+        if (eff > best) { best = eff; splits = sp; }
+    }
     long long kps = (K + splits - 1) / splits;
     kps = (kps + BK - 1) / BK * BK;
     splits = (K + kps - 1) / kps;
