@@ -247,13 +247,15 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
 // ===================================================================================================== internal drivers
 namespace {
 
-// slots per chunk: the stick intermediate W of one chunk is meant to stay L2-resident between K1, K2 and K3
+// slots per chunk.  Measured on B200 (profiles/r01_chunk_sweep.md): keeping a chunk's stick intermediate W inside the L2
+// (48 MB chunks) is SLOWER than large chunks - the three kernels are bound by FP64 issue and shared memory, not by HBM,
+// and small chunks pay wave-quantisation tails on every launch.  Default: up to 2 GB of W per chunk.
 int chunk_slots(const west_ctx* c, int f32) {
     if (c->fft_chunk > 0) return c->fft_chunk;
     const size_t per_slot = (size_t)c->cell.N * c->hs.n_cols * (f32 ? 8 : 16);
-    long long n = (long long)((48ull << 20) / per_slot);
+    long long n = (long long)((2048ull << 20) / per_slot);
     if (n < 4) n = 4;
-    if (n > 4096) n = 4096;
+    if (n > 32768) n = 32768;
     return (int)n;
 }
 int ensure_W(west_ctx* c, int n_slots, int f32) {
