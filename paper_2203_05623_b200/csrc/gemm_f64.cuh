@@ -5,20 +5,24 @@
 //   gemm_tn     C[m][n] (+)= sum_k A[m][k] B[n][k]      both operands K-contiguous; K is the long axis (2 n_g reals),
 //                                                        split over blockIdx.z, partial sums reduced with FP64 atomics
 //   gemm_update Y[n][k] += sum_m C[m][n] A[m][k]        rank-m update of the vector block
-// CTA tile 128 x 128, 8 warps as 2 x 4, warp tile 64 x 32 (64 accumulators / thread), k step 16 through a 4-stage
-// cp.async ring.  Shared-memory rows are padded to 20 doubles (tn) / 132 doubles (update) so every fragment load is
-// bank-conflict free.
+// Warp tile 64 x 32 (64 accumulators / thread), k step 16 through a cp.async ring.  Shared-memory rows are padded by 4
+// doubles so every fragment load is bank-conflict free.  Yardstick on the same box: cuBLAS DGEMM 35-36 TFLOP/s on these shapes.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace wgemm {
 
-constexpr int BM = 128, BN = 128, BK = 16, STAGES = 4, NTHREADS = 256;
+// CTA tile BM x BN with BM = 128 and BN = 32 * WN (WN = warps along n).  The shipped configuration is WN = 2: 128 x 64
+// tiles, 4 warps (2 x 2, warp tile 64 x 32), 3 stages, TWO CTAs per SM so that one CTA's barrier / prologue / epilogue
+// bubbles are covered by the other's DMMA stream.
+constexpr int BM = 128, BK = 16;
+constexpr int WN = 2, BN = 32 * WN, STAGES = 3, NTHREADS = 2 * WN * 32, MINB = 2;
 constexpr int PITCH_TN = BK + 4;                  // doubles
-constexpr int PITCH_UP = 128 + 4;                 // doubles
+constexpr int PITCH_UPC = BM + 4;                 // doubles, C^T panel (n contiguous)
+constexpr int PITCH_UPA = BN + 4;                 // doubles, A panel (k contiguous)
 constexpr size_t SMEM_TN = (size_t)STAGES * (BM + BN) * PITCH_TN * sizeof(double);
-constexpr size_t SMEM_UP = (size_t)STAGES * 2 * BK * PITCH_UP * sizeof(double);
+constexpr size_t SMEM_UP = (size_t)STAGES * BK * (PITCH_UPC + PITCH_UPA) * sizeof(double);
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool pred) {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -40,14 +44,14 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 
 // ---------------------------------------------------------------------------------------------------------------------
 // C[m][n] += sum_{k in this split} A[m][k] B[n][k].   lda, ldb even (16-byte aligned rows), A and B 16-byte aligned.
-__global__ void __launch_bounds__(NTHREADS) gemm_tn_kernel(int M, int Nn, long long K, const double* __restrict__ A, long long lda,
+__global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, long long K, const double* __restrict__ A, long long lda,
                                                            const double* __restrict__ B, long long ldb, double* __restrict__ C,
                                                            long long ldc, long long k_per_split, int use_atomic) {
     extern __shared__ __align__(16) double smem[];
     double* As = smem;                                   // [STAGES][BM][PITCH_TN]
     double* Bs = smem + (size_t)STAGES * BM * PITCH_TN;  // [STAGES][BN][PITCH_TN]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp >> 2, wn = warp & 3;             // 2 x 4 warps
+    const int wm = warp / WN, wn = warp % WN;            // 2 x WN warps
     const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
     const long long kb = (long long)blockIdx.z * k_per_split;
     long long ke = kb + k_per_split; if (ke > K) ke = K;
@@ -61,15 +65,19 @@ __global__ void __launch_bounds__(NTHREADS) gemm_tn_kernel(int M, int Nn, long l
 
     auto load_stage = [&](int stage, int kt) {
         const long long k0 = kb + (long long)kt * BK;
-        // 128 rows x 8 chunks of 16 B per operand = 1024 chunks, 4 per thread per operand
+        // rows x 8 chunks of 16 B.  k and ke are even whenever k_per_split and K are even, so a chunk never straddles ke
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < BM * 8 / NTHREADS; ++i) {
             const int c = tid + i * NTHREADS, row = c >> 3, ch = c & 7;
             const long long k = k0 + ch * 2;
             const bool pa = (m0 + row < M) && (k < ke);
-            const bool pb = (n0 + row < Nn) && (k < ke);
-            // k and ke are even whenever k_per_split and K are even, so a 16-byte chunk never straddles ke
             cp_async16(As + ((size_t)stage * BM + row) * PITCH_TN + ch * 2, pa ? A + (long long)(m0 + row) * lda + k : A, pa);
+        }
+#pragma unroll
+        for (int i = 0; i < BN * 8 / NTHREADS; ++i) {
+            const int c = tid + i * NTHREADS, row = c >> 3, ch = c & 7;
+            const long long k = k0 + ch * 2;
+            const bool pb = (n0 + row < Nn) && (k < ke);
             cp_async16(Bs + ((size_t)stage * BN + row) * PITCH_TN + ch * 2, pb ? B + (long long)(n0 + row) * ldb + k : B, pb);
         }
     };
@@ -122,16 +130,16 @@ __global__ void __launch_bounds__(NTHREADS) gemm_tn_kernel(int M, int Nn, long l
 // ---------------------------------------------------------------------------------------------------------------------
 // Y[n][k] += sum_m C[m][n] A[m][k].  Output tile: 128 vectors (n) x 128 reals (k).  MMA roles: rows = n, cols = k,
 // contraction = m.  A-operand element (n, m) = C[m][n] (n contiguous), B-operand element (m, k) = A[m][k] (k contiguous).
-__global__ void __launch_bounds__(NTHREADS) gemm_update_kernel(int M, int Nn, long long K, const double* __restrict__ C, long long ldc,
+__global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int Nn, long long K, const double* __restrict__ C, long long ldc,
                                                                const double* __restrict__ A, long long lda, double* __restrict__ Y,
                                                                long long ldy) {
     extern __shared__ __align__(16) double smem[];
-    double* Cs = smem;                                        // [STAGES][BK][PITCH_UP]  (m, n)
-    double* As = smem + (size_t)STAGES * BK * PITCH_UP;       // [STAGES][BK][PITCH_UP]  (m, k)
+    double* Cs = smem;                                        // [STAGES][BK][PITCH_UPC]  (m, n)
+    double* As = smem + (size_t)STAGES * BK * PITCH_UPC;      // [STAGES][BK][PITCH_UPA]  (m, k)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp >> 2, wn = warp & 3;
-    const int n0 = blockIdx.y * 128;
-    const long long k0 = (long long)blockIdx.x * 128;
+    const int wm = warp / WN, wn = warp % WN;
+    const int n0 = blockIdx.y * BM;
+    const long long k0 = (long long)blockIdx.x * BN;
     const int nm = (M + BK - 1) / BK;
 
     double acc[8][4][2];
@@ -142,15 +150,18 @@ __global__ void __launch_bounds__(NTHREADS) gemm_update_kernel(int M, int Nn, lo
 
     auto load_stage = [&](int stage, int mt) {
         const int mb = mt * BK;
-        // 16 rows x 64 chunks of 16 B per operand = 1024 chunks
+        // 16 rows x (BM/2 | BN/2) chunks of 16 B
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int c = tid + i * NTHREADS, row = c >> 6, ch = c & 63;
-            const bool pm = mb + row < M;
-            const bool pc = pm && (n0 + ch * 2 < Nn);          // Nn, ldc even -> chunk never straddles
-            const bool pa = pm && (k0 + ch * 2 < K);           // K, lda even
-            cp_async16(Cs + ((size_t)stage * BK + row) * PITCH_UP + ch * 2, pc ? C + (long long)(mb + row) * ldc + n0 + ch * 2 : C, pc);
-            cp_async16(As + ((size_t)stage * BK + row) * PITCH_UP + ch * 2, pa ? A + (long long)(mb + row) * lda + k0 + ch * 2 : A, pa);
+        for (int i = 0; i < BK * (BM / 2) / NTHREADS; ++i) {
+            const int c = tid + i * NTHREADS, row = c / (BM / 2), ch = c % (BM / 2);
+            const bool pc = (mb + row < M) && (n0 + ch * 2 < Nn);          // Nn, ldc even -> chunk never straddles
+            cp_async16(Cs + ((size_t)stage * BK + row) * PITCH_UPC + ch * 2, pc ? C + (long long)(mb + row) * ldc + n0 + ch * 2 : C, pc);
+        }
+#pragma unroll
+        for (int i = 0; i < BK * (BN / 2) / NTHREADS; ++i) {
+            const int c = tid + i * NTHREADS, row = c / (BN / 2), ch = c % (BN / 2);
+            const bool pa = (mb + row < M) && (k0 + ch * 2 < K);           // K, lda even
+            cp_async16(As + ((size_t)stage * BK + row) * PITCH_UPA + ch * 2, pa ? A + (long long)(mb + row) * lda + k0 + ch * 2 : A, pa);
         }
     };
 #pragma unroll
@@ -164,15 +175,15 @@ __global__ void __launch_bounds__(NTHREADS) gemm_update_kernel(int M, int Nn, lo
         if (mt + STAGES - 1 < nm) load_stage((mt + STAGES - 1) % STAGES, mt + STAGES - 1);
         cp_commit();
         // A-operand (row n = lane/4, contraction m = lane%4): Cs[m][n];  B-operand (m = lane%4, col k = lane/4): As[m][k]
-        const double* cs = Cs + (size_t)(mt % STAGES) * BK * PITCH_UP + (lane & 3) * PITCH_UP + wm * 64 + (lane >> 2);
-        const double* as = As + (size_t)(mt % STAGES) * BK * PITCH_UP + (lane & 3) * PITCH_UP + wn * 32 + (lane >> 2);
+        const double* cs = Cs + (size_t)(mt % STAGES) * BK * PITCH_UPC + (lane & 3) * PITCH_UPC + wm * 64 + (lane >> 2);
+        const double* as = As + (size_t)(mt % STAGES) * BK * PITCH_UPA + (lane & 3) * PITCH_UPA + wn * 32 + (lane >> 2);
 #pragma unroll
         for (int mm = 0; mm < BK; mm += 4) {
             double a[8], b[4];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = cs[mm * PITCH_UP + i * 8];
+            for (int i = 0; i < 8; ++i) a[i] = cs[mm * PITCH_UPC + i * 8];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = as[mm * PITCH_UP + j * 8];
+            for (int j = 0; j < 4; ++j) b[j] = as[mm * PITCH_UPA + j * 8];
 #pragma unroll
             for (int i = 0; i < 8; ++i)
 #pragma unroll

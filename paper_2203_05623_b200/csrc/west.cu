@@ -273,14 +273,14 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
         attr = true;
     }
     const int tm = (M + BM - 1) / BM, tn = (Nn + BN - 1) / BN;
-    // split K so that the CTA count fills whole waves of the 148 SMs (one 164 KB CTA per SM): pick the split count with
+    // split K so that the CTA count fills whole waves of the 148 SMs (MINB CTAs per SM): pick the split count with
     // the best wave efficiency, each split keeping at least 32 k-steps
     const long long tiles = (long long)tm * tn;
     const long long max_splits = std::max<long long>(1, std::min<long long>(16, K / (32 * BK)));
     long long splits = 1;
     double best = -1.0;
     for (long long sp = 1; sp <= max_splits; ++sp) {
-        const double waves = (double)(tiles * sp) / 148.0;
+        const double waves = (double)(tiles * sp) / (148.0 * MINB);
         const double eff = waves / std::ceil(waves) - 0.004 * (double)sp;     // mild preference for fewer splits (atomic traffic)
         if (eff > best) { best = eff; splits = sp; }
     }
@@ -305,7 +305,7 @@ int launch_gemm_update(west_ctx* c, int M, int Nn, long long K, const double* C,
         CK(cudaFuncSetAttribute(gemm_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP));
         attr = true;
     }
-    dim3 grid((unsigned)((K + 127) / 128), (unsigned)((Nn + 127) / 128));
+    dim3 grid((unsigned)((K + BN - 1) / BN), (unsigned)((Nn + BM - 1) / BM));
     Prof prof_(c, PC_GEMM_UP);
     gemm_update_kernel<<<grid, NTHREADS, SMEM_UP, c->st>>>(M, Nn, K, C, ldc, A, lda, Y, ldy);
     CK(cudaGetLastError());
