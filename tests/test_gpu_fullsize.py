@@ -24,7 +24,8 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.fixture(scope="module")
-def big():
+def states():
+    """Config 2/3/4 cell with the ORACLE's orbitals, loaded into one library context (shared by the tests below)."""
     import torch
     import paper_2203_05623_b200 as wb
     p = oracle_problem.build("cfg2", dense=False)
@@ -36,12 +37,18 @@ def big():
     w.set_vloc(torch.from_numpy(np.ascontiguousarray(p.vloc)).to(dev))
     w.set_kb(torch.from_numpy(np.ascontiguousarray(p.beta[:, p.half])).to(dev), p.dcoef)
     w.set_states(torch.from_numpy(np.ascontiguousarray(U.T[:, p.half])).to(dev), eps)
+    yield dict(p=p, eps=eps, U=U, alpha=alpha, w=w, dev=dev)
+    w.close()
+
+
+@pytest.fixture(scope="module")
+def big(states):
+    import torch
+    p, eps, U, alpha, w, dev = (states[k] for k in ("p", "eps", "U", "alpha", "w", "dev"))
     dV = torch.from_numpy(np.ascontiguousarray(p.dV)).to(dev)           # all 64 perturbations
     dn, dpsi, st = w.chi0_apply(dV, [0.0], tol=1e-12, max_iter=500, alpha_pv=alpha, want_dpsi=True, n_occ=p.n_occ)
     assert st["rc"] == 0 and st["n_unconverged"] == 0
-    out = dict(p=p, eps=eps, U=U, alpha=alpha, dn=dn.cpu().numpy()[0], dpsi=dpsi.cpu().numpy()[0], st=st)
-    w.close()
-    return out
+    return dict(p=p, eps=eps, U=U, alpha=alpha, dn=dn.cpu().numpy()[0], dpsi=dpsi.cpu().numpy()[0], st=st)
 
 
 def _full(p, c_half):
@@ -89,3 +96,51 @@ def test_invariants_on_the_full_batch(big):
     x = _full(p, big["dpsi"][5, :, 0])                                                           # [n_occ][n_g]
     ov = U.conj().T @ x.T
     assert np.max(np.abs(ov)) < 1e-9 * np.max(np.abs(x)) * np.sqrt(x.shape[1])
+
+
+def test_cfg3_imaginary_frequencies_sampled_columns(states):
+    """Config 3: complex-shifted Sternheimer at the lowest and highest of its 8 frequencies, against the oracle's COCG."""
+    import torch
+    p, eps, U, alpha, w, dev = (states[k] for k in ("p", "eps", "U", "alpha", "w", "dev"))
+    import synth
+    omegas = [synth.get_config("cfg3")["omegas"][0], synth.get_config("cfg3")["omegas"][-1]]
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV[:2])).to(dev)
+    dn, dpsi, st = w.chi0_apply(dV, omegas, tol=1e-12, max_iter=500, alpha_pv=alpha, want_dpsi=True, n_occ=p.n_occ)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    dpsi = dpsi.cpu().numpy()
+    apply_H = lambda y: oham.apply_h(y, p.miller, p.L, p.N, p.vloc, p.beta, p.dcoef)
+    for wi, om in enumerate(omegas):
+        for i, v in ((0, 3), (1, p.n_occ - 1)):
+            b = ochi0.rhs_vectors(U[:, v:v + 1], p.dV[i:i + 1], p.fft_idx, p.N)[0, 0]
+            x, it, rel = oit.cocg_sternheimer(apply_H, U, eps[v], v, b, p.g2, p.minus, alpha, om, tol=1e-12, max_iter=500)
+            assert rel <= 1e-12
+            got = _full(p, dpsi[wi, i, v, 0]) + 1j * _full(p, dpsi[wi, i, v, 1])
+            assert relmax(got, x) < 1e-9
+        # Eq. 11 from the returned dpsi, and monotone decay of the response with omega
+        full = _full(p, dpsi[wi, 0, :, 0]) + 1j * _full(p, dpsi[wi, 0, :, 1])
+        assert relmax(dn[wi, 0].cpu().numpy(), ochi0.dn_from_dpsi(U, full, p.miller, p.L, p.N)) < 1e-12
+    dnn = dn.cpu().numpy()
+    m_lo = ochi0.response_matrix(p.dV[:2], dnn[0], p.L)
+    m_hi = ochi0.response_matrix(p.dV[:2], dnn[1], p.L)
+    assert m_lo[0, 0] < m_hi[0, 0] < 0.0 and m_lo[1, 1] < m_hi[1, 1] < 0.0
+
+
+def test_cfg4_mixed_precision_sampled_columns(states):
+    """Config 4: FP32 FFT / real-space multiply inside H*psi, FP64 vectors, dots and dn; tolerance 1e-4 (north_star)."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p, eps, U, alpha, w, dev = (states[k] for k in ("p", "eps", "U", "alpha", "w", "dev"))
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV[:2])).to(dev)
+    dn, dpsi, st = w.chi0_apply(dV, [0.0], tol=1e-6, max_iter=500, alpha_pv=alpha, want_dpsi=True, n_occ=p.n_occ,
+                                precision=wb.WEST_MIXED)
+    dn64, _, _ = w.chi0_apply(dV, [0.0], tol=1e-12, max_iter=500, alpha_pv=alpha)
+    dpsi = dpsi.cpu().numpy()[0]
+    apply_H = lambda y: oham.apply_h(y, p.miller, p.L, p.N, p.vloc, p.beta, p.dcoef)
+    for i, v in ((0, 0), (1, 77), (1, p.n_occ - 1)):
+        b = ochi0.rhs_vectors(U[:, v:v + 1], p.dV[i:i + 1], p.fft_idx, p.N)[0, 0]
+        x, it, rel = oit.pcg_sternheimer(apply_H, U, eps[v], v, b, p.g2, alpha, tol=1e-12, max_iter=500)
+        err = relmax(_full(p, dpsi[i, v, 0]), x)
+        assert 1e-12 < err < 1e-4, err
+    # dn of the mixed path against the FP64 path of the same library (itself pinned to the oracle above) and Eq. 11 by the oracle
+    assert relmax(dn.cpu().numpy(), dn64.cpu().numpy()) < 1e-4
+    assert relmax(dn[0, 0].cpu().numpy(), ochi0.dn_from_dpsi(U, _full(p, dpsi[0, :, 0]), p.miller, p.L, p.N)) < 1e-12
