@@ -247,7 +247,11 @@ def main():
     # ---- roofline of the dominant kernel class
     top = max(prof, key=lambda k: prof[k]["ms"])
     n_cols = aux_ncols(cfg)
-    roof = roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, precision == wb.WEST_MIXED, w)
+    fp64_peak = measure_fp64_peak()
+    roof = roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, precision == wb.WEST_MIXED, w, fp64_peak)
+    rows = (cfg["n_proj"] + cfg["n_occ"]) * (1 if cfg["mode"] == "gamma" else 2)
+    t_gemm = (prof["gemm_tn"]["ms"] + prof["gemm_update"]["ms"]) * 1e-3
+    gemm_tf = 2 * 2.0 * rows * (2 * w.n_g) * n_h / t_gemm / 1e12 if t_gemm > 0 else None
     line = {
         "metric": "chi0*dV perturbations/s (batched Sternheimer PCG to tol %.0e)" % TOL,
         "value": value, "unit": "perturbations/s", "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
@@ -263,6 +267,8 @@ def main():
         "gpu_launches": int(launches),
         "clocks": sampler.summary(),
         "roofline": roof,
+        "gemm": {"achieved_tflops": gemm_tf, "peak_tflops": fp64_peak, "frac": (gemm_tf / fp64_peak) if gemm_tf else None,
+                 "note": "KB + P_v DMMA GEMMs of the CG loop (RHS projection excluded from the flop count)"},
         "kernel_ms_per_step": {k: round(v["ms"] / a.steps, 3) for k, v in prof.items() if v["spans"]},
         "phase_ms_last_step": {"rhs": stats["ms_rhs"], "cg": stats["ms_cg"], "dn": stats["ms_dn"]},
         "device_gb": w.device_bytes() / 1e9,
@@ -279,7 +285,30 @@ def aux_ncols(cfg):
     return sum(1 for x in range(-m, m + 1) for y in range(-m, m + 1) if x * x + y * y <= cfg["n2max"])
 
 
-def roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, mixed, w):
+# dram__bytes_read.sum + dram__bytes_write.sum of one k2_planes<double,8,9,K2_H> launch of 51 slots under
+# `ncu --set full` (profiles/r01_k2_planes_full_details_v6.txt): 52.66 MB + 0.84 MB -> bytes per slot
+NCU_K2_DRAM_BYTES_PER_SLOT_CFG2 = (52.657920e6 + 0.844032e6) / 51.0
+
+
+def measure_fp64_peak():
+    """The box's own FP64 yardstick: cuBLAS DGEMM 8192^3 through torch, best of 5, TFLOP/s."""
+    import torch
+    n = 8192
+    a = torch.randn((n, n), dtype=torch.float64, device="cuda")
+    b = torch.randn((n, n), dtype=torch.float64, device="cuda")
+    best = 1e9
+    for _ in range(6):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    del a, b
+    return 2.0 * n ** 3 / (best * 1e-3) / 1e12
+
+
+def roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, mixed, w, fp64_peak):
     """Roofline entry for the kernel class that took the most time (DESIGN.md section 6 states the per-unit figures)."""
     N = cfg["N"]
     gamma = cfg["mode"] == "gamma"
@@ -287,32 +316,42 @@ def roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, mixed, w):
     csz = 8 if mixed else 16
     t = prof[top]["ms"] * 1e-3
     spans = max(1, prof[top]["spans"])
-    out = {"kernel": top, "avg_launch_ms": prof[top]["ms"] / spans, "peak_source": peak_src, "traffic": None}
+    fp64_src = "measured in this run: cuBLAS DGEMM 8192^3 FP64 (DMMA and the FP64 FMA pipe have the same nominal rate on B200, 37.2 TFLOP/s)"
+    out = {"kernel": top, "avg_launch_ms": prof[top]["ms"] / spans, "traffic": None}
     if top in ("k1_g2r_z", "k2_planes", "k3_r2g_z"):
         stick = N * n_cols * csz
         sphere = (2 if gamma else 1) * w.n_g * 16
         per_slot = {"k1_g2r_z": sphere + stick, "k2_planes": 2 * stick, "k3_r2g_z": stick + 2 * sphere}[top]
-        ach = per_slot * slots / t / 1e9
-        # the planes kernel is bound by FP64 arithmetic: report its flop rate against the DFMA peak as well
-        fl = 0.0
+        gbs = per_slot * slots / t / 1e9
         if top == "k2_planes":
+            # the plane kernel is bound by FP64 issue / shared memory, not by HBM: nominal 5 N log2 N flops
+            # per 1D transform, 2 (nr + N) transforms per plane, plus the V_loc multiply
             nr = 2 * cfg["n_max"] + 1
-            fl = slots * N * (2 * (nr + N) * 5.0 * N * np.log2(N) + 2 * N * N) / t / 1e12
-        out.update({"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
-                    "algorithmic_bytes_per_slot": per_slot, "fft_tflops_nominal_5NlogN": fl})
+            fl_slot = N * (2 * (nr + N) * 5.0 * N * np.log2(N) + 2 * N * N)
+            ach = fl_slot * slots / t / 1e12
+            peak = fp64_peak * (2.0 if mixed else 1.0)
+            out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                        "peak_source": fp64_src + ("; x2 for the FP32 path" if mixed else ""),
+                        "algorithmic_flops_per_slot": fl_slot, "algorithmic_bytes_per_slot": per_slot,
+                        "hbm_view": {"achieved_gbs": gbs, "peak_gbs": hbm_peak, "frac": gbs / hbm_peak, "peak_source": peak_src}})
+            if N == 72 and not mixed:
+                out["traffic"] = NCU_K2_DRAM_BYTES_PER_SLOT_CFG2 * slots / spans
+                out["traffic_note"] = "ncu dram bytes per slot (51-slot capture, cold L2) x slots per launch; algorithmic = %.3e B/slot" % per_slot
+        else:
+            out.update({"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                        "peak_source": peak_src, "algorithmic_bytes_per_slot": per_slot})
     elif top in ("gemm_tn", "gemm_update"):
         rows = cfg["n_proj"] + cfg["n_occ"]
         if not gamma:
             rows *= 2
         flops = 2.0 * rows * (2 * w.n_g) * n_h
         ach = flops / t / 1e12
-        peak = 148 * 64 * 2 * 1.965e9 / 1e12
-        out.update({"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                    "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DMMA has the same rate on B200)"})
+        out.update({"bound": "tensor", "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach / fp64_peak,
+                    "peak_source": fp64_src})
     else:
         per_col = 10 * 16 * w.n_g
         ach = per_col * n_h / t / 1e9
-        out.update({"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak})
+        out.update({"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": peak_src})
     return out
 
 
