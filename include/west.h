@@ -147,7 +147,7 @@ int64_t west_launch_count(const west_ctx* ctx);
  * events on the context's stream.  west_get_profile synchronises the stream, writes the summed milliseconds and span
  * counts of the 8 classes into the HOST arrays ms[8], count[8] and resets the record.  Classes: 0 K1 (sphere -> z sticks,
  * H*psi), 1 K2 (planes: y/x inverse, x V_loc, x/y forward), 2 K3 (z sticks -> sphere + kinetic), 3 gemm_tn, 4 gemm_update,
- * 5 CG vector kernels (three launches per span), 6 FFT kernels of the RHS / dn stages (two launches per span), 7 unused. */
+ * 5 CG vector kernel (fused step; compaction launches included), 6 FFT kernels of the RHS / dn stages (two launches per span), 7 unused. */
 int  west_set_profile(west_ctx* ctx, int32_t on);
 int  west_get_profile(west_ctx* ctx, double* ms, int64_t* count);
 /* Tuning knob: how many FFT slots (complex transforms) are processed per internal chunk (0 = default).  The stick

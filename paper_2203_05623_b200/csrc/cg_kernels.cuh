@@ -124,34 +124,31 @@ __global__ void __launch_bounds__(NT) cg_init(long long n_g, int n_occ, const do
     }
 }
 
+// One CG iteration's vector work for one column, fused (steps a8 + a9):
+//   (p, Ap) -> a = rz / (p, Ap) ; x += a p ; r -= a Ap ; rznew = (r, M r), rr = ||r||^2 ; b = rznew / rz ; p = M r + b p
+// One CTA per live column; the two reductions are CTA-wide, so no grid-wide dependency separates the three phases.  r, p,
+// Ap are in compacted order (index k), x and the scalars in original column order (colmap[k]).  p and Ap are read twice and
+// r is re-read after its update; the second touches hit L1/L2 (a column is 146 KB), so HBM sees 4 reads + 3 writes.
 template <int MODE>
-__global__ void __launch_bounds__(NT) cg_dot_pAp(long long n_g, const double2* P, const double2* AP, Scalars s, const int* colmap) {
-    __shared__ double sh[16];
-    const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
-    if (!s.active[col]) return;
-    const double2* p = P + (long long)k * nvpc * n_g;
-    const double2* ap = AP + (long long)k * nvpc * n_g;
-    double acc[2] = {0, 0};
-    for (int g = threadIdx.x; g < n_g; g += NT) dot_accum<MODE>(p, ap, n_g, g, 1.0, acc);
-    block_reduce<2>(acc, sh);
-    if (threadIdx.x == 0) s.pAp[col] = make_double2(acc[0], MODE == 1 ? acc[1] : 0.0);
-}
-
-// x += a p ; r -= a Ap ; rznew = (r, M r) ; rr = ||r||^2
-template <int MODE>
-__global__ void __launch_bounds__(NT) cg_update_xr(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
-                                                   const double2* P, const double2* AP, double2* X, double2* R, Scalars s,
-                                                   const int* colmap) {
+__global__ void __launch_bounds__(NT) cg_step(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on, double tol2,
+                                              double2* P, const double2* AP, double2* X, double2* R, Scalars s, const int* colmap) {
     __shared__ double sh[32];
     const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
     if (!s.active[col]) return;
-    const long long o = (long long)k * nvpc * n_g;          // r, p, Ap live in compacted order; x in original column order
-    const double2* p = P + o; const double2* ap = AP + o;
+    const long long o = (long long)k * nvpc * n_g;
+    double2* p = P + o; const double2* ap = AP + o;
     double2* x = X + (long long)col * nvpc * n_g; double2* r = R + o;
-    const double2 a = cdiv(s.rz[col], s.pAp[col]);
     const double tkv = tk[col % n_occ];
+    // ---- (p, Ap)
+    double d2[2] = {0, 0};
+    for (int g = threadIdx.x; g < n_g; g += NT) dot_accum<MODE>(p, ap, n_g, g, 1.0, d2);
+    block_reduce<2>(d2, sh);
+    const double2 rz = s.rz[col];
+    const double2 a = cdiv(rz, make_double2(d2[0], MODE == 1 ? d2[1] : 0.0));
+    // ---- x, r, and the new inner products
     double acc[3] = {0, 0, 0};
     for (int g = threadIdx.x; g < n_g; g += NT) {
+        const double m = precond(g2[g], tkv, precond_on);
         if (MODE == 1) {
             const double2 pr = p[g], pi = p[n_g + g], qr = ap[g], qi = ap[n_g + g];
             double2 xr = x[g], xi = x[n_g + g], rr = r[g], ri = r[n_g + g];
@@ -160,39 +157,27 @@ __global__ void __launch_bounds__(NT) cg_update_xr(long long n_g, int n_occ, con
             rr.x -= a.x * qr.x - a.y * qi.x; rr.y -= a.x * qr.y - a.y * qi.y;
             ri.x -= a.x * qi.x + a.y * qr.x; ri.y -= a.x * qi.y + a.y * qr.y;
             x[g] = xr; x[n_g + g] = xi; r[g] = rr; r[n_g + g] = ri;
+            const double f = g == 0 ? 1.0 : 2.0;
+            const double srr = g == 0 ? rr.x * rr.x : rr.x * rr.x + rr.y * rr.y;
+            const double sii = g == 0 ? ri.x * ri.x : ri.x * ri.x + ri.y * ri.y;
+            const double sri = g == 0 ? rr.x * ri.x : rr.x * ri.x + rr.y * ri.y;
+            acc[0] += f * (srr - sii) * m; acc[1] += f * (2.0 * sri) * m; acc[2] += f * (srr + sii);
         } else {
             const double2 pp = p[g], q = ap[g];
             double2 xx = x[g], rr = r[g];
             xx.x += a.x * pp.x; xx.y += a.x * pp.y;
             rr.x -= a.x * q.x;  rr.y -= a.x * q.y;
             x[g] = xx; r[g] = rr;
+            const double n2 = (MODE == 0) ? (g == 0 ? rr.x * rr.x : 2.0 * (rr.x * rr.x + rr.y * rr.y)) : rr.x * rr.x + rr.y * rr.y;
+            acc[0] += n2 * m; acc[2] += n2;
         }
-        const double m = precond(g2[g], tkv, precond_on);
-        double d[2] = {0, 0};
-        dot_accum<MODE>(r, r, n_g, g, m, d);      // re-reads this thread's own freshly written r
-        acc[0] += d[0]; acc[1] += d[1];
-        acc[2] += norm_accum<MODE>(r, n_g, g);
     }
     block_reduce<3>(acc, sh);
-    if (threadIdx.x == 0) {
-        s.rznew[col] = make_double2(acc[0], MODE == 1 ? acc[1] : 0.0);
-        s.rr[col] = acc[2];
-    }
-}
-
-// p = M r + beta p ; rz = rznew ; convergence bookkeeping
-template <int MODE>
-__global__ void __launch_bounds__(NT) cg_update_p(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on,
-                                                  double tol2, const double2* R, double2* P, Scalars s, const int* colmap) {
-    const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
-    if (!s.active[col]) return;
-    const long long o = (long long)k * nvpc * n_g;
-    const double2* r = R + o; double2* p = P + o;
-    const double rr = s.rr[col], b2 = s.b2[col];
-    const bool still = rr > tol2 * b2;
-    const double2 beta = cdiv(s.rznew[col], s.rz[col]);
-    const double tkv = tk[col % n_occ];
+    const double2 rznew = make_double2(acc[0], MODE == 1 ? acc[1] : 0.0);
+    const bool still = acc[2] > tol2 * s.b2[col];
+    // ---- p = M r + beta p (each thread re-reads the r elements it wrote itself)
     if (still) {
+        const double2 beta = cdiv(rznew, rz);
         for (int g = threadIdx.x; g < n_g; g += NT) {
             const double m = precond(g2[g], tkv, precond_on);
             if (MODE == 1) {
@@ -205,9 +190,9 @@ __global__ void __launch_bounds__(NT) cg_update_p(long long n_g, int n_occ, cons
             }
         }
     }
-    __syncthreads();
     if (threadIdx.x == 0) {
-        s.rz[col] = s.rznew[col];
+        s.rz[col] = rznew;
+        s.rr[col] = acc[2];
         if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
     }
 }

@@ -664,12 +664,10 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
         n_h += n_vec;
         {
             Prof p_(c, PC_CGVEC);
-            wcg::cg_dot_pAp<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, (const double2*)P, (const double2*)AP, s, colmap);
-            wcg::cg_update_xr<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)P, (const double2*)AP,
-                                                                  (double2*)X, (double2*)R, s, colmap);
-            wcg::cg_update_p<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (const double2*)R, (double2*)P, s, colmap);
+            wcg::cg_step<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (double2*)P, (const double2*)AP,
+                                                             (double2*)X, (double2*)R, s, colmap);
             CK(cudaGetLastError());
-            c->launches += 3;
+            c->launches += 1;
         }
         if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
             CK(cudaMemcpyAsync(c->h_pinned, s.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
