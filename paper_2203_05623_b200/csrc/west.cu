@@ -567,7 +567,7 @@ int west_set_states(west_ctx* c, int32_t n_occ, const void* psi, const double* e
 }
 
 int west_fft3d(west_ctx* c, int32_t dir, int32_t precision, int32_t n_batch, const void* in, void* out) {
-    if (!c || (dir != 1 && dir != -1) || n_batch < 0 || !in || !out) return fail(c, WEST_EINVAL, "west_fft3d: bad argument");
+    if (!c || (dir != 1 && dir != -1) || n_batch < 0 || (n_batch > 0 && (!in || !out))) return fail(c, WEST_EINVAL, "west_fft3d: bad argument");
     if (precision != WEST_FP64) return fail(c, WEST_EINVAL, "west_fft3d: only WEST_FP64 (the FP32 variant exists inside west_h_apply only)");
     if (n_batch == 0) return WEST_OK;
     const int gamma = is_gamma(c), N = c->cell.N;
@@ -600,7 +600,7 @@ int west_fft3d(west_ctx* c, int32_t dir, int32_t precision, int32_t n_batch, con
 }
 
 int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, void* y) {
-    if (!c || n_vec < 0 || !x || !y) return fail(c, WEST_EINVAL, "west_h_apply: bad argument");
+    if (!c || n_vec < 0 || (n_vec > 0 && (!x || !y))) return fail(c, WEST_EINVAL, "west_h_apply: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_h_apply: bad precision %d", precision);
     if (!c->have_vloc) return fail(c, WEST_ESTATE, "west_h_apply: west_set_vloc has not been called");
     if (n_vec == 0) return WEST_OK;
@@ -701,7 +701,8 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
 
 extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, const double* dV, int32_t n_freq,
                                const double* omega_host, const west_cg_opts* opts, double* dn, void* dpsi_opt, west_stats* stats) {
-    if (!c || n_pert < 0 || n_freq < 0 || !dV || !omega_host || !opts || !dn) return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
+    if (!c || n_pert < 0 || n_freq < 0 || !opts || (n_freq > 0 && !omega_host) || (n_pert > 0 && n_freq > 0 && (!dV || !dn)))
+        return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
     if (opts->max_iter < 1 || !(opts->tol > 0)) return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
