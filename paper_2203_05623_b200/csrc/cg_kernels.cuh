@@ -14,20 +14,16 @@ constexpr int NT = 256;
 
 struct Scalars {
     double2* rz;      // (r, z)
-    double2* pAp;     // (p, A p)
-    double2* rznew;
     double*  rr;      // Hermitian ||r||^2
     double*  b2;      // ||b||^2
     int*     active;  // 1 while ||r|| > tol ||b||
     int*     counters;   // [0] number of active columns after the last p-update
-    double*  resid_max;  // [1] max ||r||/||b|| (as bits-ordered non-negative double, atomicMax on long long)
 };
 
 __device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
     const double d = b.x * b.x + b.y * b.y;
     return make_double2((a.x * b.x + a.y * b.y) / d, (a.y * b.x - a.x * b.y) / d);
 }
-__device__ __forceinline__ double2 cmul2(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
 // block reduction of up to 4 doubles
 template <int NV>

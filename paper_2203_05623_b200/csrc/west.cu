@@ -734,14 +734,11 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     {
         char* p = (char*)c->scal.p;
         s.rz = (double2*)p; p += sizeof(double2) * n_col;
-        s.pAp = (double2*)p; p += sizeof(double2) * n_col;
-        s.rznew = (double2*)p; p += sizeof(double2) * n_col;
         s.rr = (double*)p; p += sizeof(double) * n_col;
         s.b2 = (double*)p; p += sizeof(double) * n_col;
         s.active = (int*)p; p += sizeof(int) * n_col;
         p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
-        s.counters = (int*)p; p += 16;
-        s.resid_max = (double*)p;
+        s.counters = (int*)p;
     }
     cx<double>* X = (cx<double>*)c->vecs[0].p; cx<double>* R = (cx<double>*)c->vecs[1].p;
     cx<double>* P = (cx<double>*)c->vecs[2].p; cx<double>* AP = (cx<double>*)c->vecs[3].p;
