@@ -39,6 +39,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunk", type=int, default=0, help="FFT slots per chunk (0 = library default)")
     ap.add_argument("--check-every", type=int, default=1, help="CG convergence poll / compaction period")
+    ap.add_argument("--precond", type=int, default=1, help="0 none, 1 R4 default, 2 Teter-Payne-Allan")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
     return ap.parse_args()
 
@@ -190,7 +191,7 @@ def main():
     dV = torch.from_numpy(dV_np).to(dev)
     N = cfg["N"]
     dn = torch.empty((len(omegas), n_pert, N, N, N), dtype=torch.float64, device=dev)
-    kw = dict(tol=TOL, max_iter=MAX_ITER, alpha_pv=alpha, precond=1, check_every=a.check_every, precision=precision, dn=dn)
+    kw = dict(tol=TOL, max_iter=MAX_ITER, alpha_pv=alpha, precond=a.precond, check_every=a.check_every, precision=precision, dn=dn)
 
     def barrier():
         if world > 1:

@@ -74,7 +74,7 @@ typedef struct {
     int32_t max_iter;   /* iteration cap per column (R5), e.g. 500 */
     double  tol;        /* stop when ||r||_2 <= tol * ||b||_2 per column (R5) */
     double  alpha_pv;   /* alpha of the alpha*P_v term (R3); the converged result does not depend on it */
-    int32_t precond;    /* 0: none; 1: M_v(G) = 1/max(1, |G|^2/(1.35 <psi_v|T|psi_v>)) (R4) */
+    int32_t precond;    /* 0: none; 1: M_v(G) = 1/max(1, |G|^2/(1.35 <psi_v|T|psi_v>)) (R4); 2: Teter-Payne-Allan polynomial form */
     int32_t check_every;/* host polls convergence every this many iterations (>=1) */
 } west_cg_opts;
 

@@ -47,8 +47,16 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* sh /* [NV*
     __syncthreads();
 }
 
+// Diagonal preconditioners M_v(G) (reading R4; they change iteration counts only, never the converged result):
+//   1: 1 / max(1, |G|^2 / (1.35 <psi_v|T|psi_v>))                      (the reading's default, also what the oracle's PCG uses)
+//   2: Teter-Payne-Allan: (27 + 18x + 12x^2 + 8x^3) / (27 + 18x + 12x^2 + 8x^3 + 16x^4), x = |G|^2 / (1.5 <psi_v|T|psi_v>)
 __device__ __forceinline__ double precond(double g2, double tk, int on) {
-    if (!on) return 1.0;
+    if (on == 0) return 1.0;
+    if (on == 2) {
+        const double x = g2 / (1.5 * tk);
+        const double num = 27.0 + x * (18.0 + x * (12.0 + 8.0 * x));
+        return num / (num + 16.0 * x * x * x * x);
+    }
     const double q = g2 / (1.35 * tk);
     return 1.0 / fmax(1.0, q);
 }
