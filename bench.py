@@ -40,6 +40,7 @@ def parse():
     ap.add_argument("--chunk", type=int, default=0, help="FFT slots per chunk (0 = library default)")
     ap.add_argument("--check-every", type=int, default=1, help="CG convergence poll / compaction period")
     ap.add_argument("--precond", type=int, default=1, help="0 none, 1 R4 default, 2 Teter-Payne-Allan")
+    ap.add_argument("--solver", type=int, default=-1, help="0 per-frequency PCG/COCG, 1 multi-shift CG; -1 = 1 for cfg3, else 0")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
     return ap.parse_args()
 
@@ -191,7 +192,8 @@ def main():
     dV = torch.from_numpy(dV_np).to(dev)
     N = cfg["N"]
     dn = torch.empty((len(omegas), n_pert, N, N, N), dtype=torch.float64, device=dev)
-    kw = dict(tol=TOL, max_iter=MAX_ITER, alpha_pv=alpha, precond=a.precond, check_every=a.check_every, precision=precision, dn=dn)
+    solver = a.solver if a.solver >= 0 else (1 if a.workload == "cfg3" else 0)
+    kw = dict(solver=solver, tol=TOL, max_iter=MAX_ITER if solver == 0 else 2000, alpha_pv=alpha, precond=a.precond, check_every=a.check_every, precision=precision, dn=dn)
 
     def barrier():
         if world > 1:
@@ -260,7 +262,7 @@ def main():
         "dtype": "f64" if precision == wb.WEST_FP64 else "f32 FFT / f64 vectors",
         "data": "synthetic (seeded Si-like cell, GPU-computed orbitals)",
         "config": {"workload": a.workload, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": len(omegas),
-                   "n_proj": cfg["n_proj"], "tol": TOL, "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
+                   "n_proj": cfg["n_proj"], "tol": TOL, "solver": "multi-shift CG" if solver == 1 else "PCG/COCG per frequency", "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
                    "gap_ry": aux["gap"], "l2": "inputs per step (4 vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
         "h_apply_per_s": n_h * world / (ms * 1e-3),
         "e2e": {"value": units * a.steps / (e2e_ms * 1e-3), "unit": "perturbations/s",

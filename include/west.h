@@ -76,6 +76,9 @@ typedef struct {
     double  alpha_pv;   /* alpha of the alpha*P_v term (R3); the converged result does not depend on it */
     int32_t precond;    /* 0: none; 1: M_v(G) = 1/max(1, |G|^2/(1.35 <psi_v|T|psi_v>)) (R4); 2: Teter-Payne-Allan polynomial form */
     int32_t check_every;/* host polls convergence every this many iterations (>=1) */
+    int32_t solver;     /* 0: one preconditioned PCG (omega = 0) / COCG (omega > 0) solve per frequency (R7);
+                           1: multi-shift CG (WEST_GAMMA only, <= 16 frequencies): all frequencies from ONE unpreconditioned Krylov
+                              sequence of the real seed operator H - eps_v + alpha P_v, one H*psi per iteration for every omega */
 } west_cg_opts;
 
 typedef struct {            /* host struct, filled when non-NULL (forces one stream synchronisation) */

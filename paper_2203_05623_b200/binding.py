@@ -24,7 +24,7 @@ class west_cell(C.Structure):
 
 class west_cg_opts(C.Structure):
     _fields_ = [("max_iter", C.c_int32), ("tol", C.c_double), ("alpha_pv", C.c_double), ("precond", C.c_int32),
-                ("check_every", C.c_int32)]
+                ("check_every", C.c_int32), ("solver", C.c_int32)]
 
 
 class west_stats(C.Structure):
@@ -173,7 +173,7 @@ class West:
         self._ck(self.lib.west_h_apply(self.ctx, precision, int(x.shape[0]), _dev(x, torch.complex128), _dev(out, torch.complex128)))
         return out
 
-    def chi0_apply(self, dV, omegas, tol=1e-12, max_iter=500, alpha_pv=1.0, precond=1, check_every=4, precision=WEST_FP64,
+    def chi0_apply(self, dV, omegas, tol=1e-12, max_iter=500, alpha_pv=1.0, precond=1, check_every=4, precision=WEST_FP64, solver=0,
                    dn=None, want_dpsi=False, n_occ=None, want_stats=True):
         import torch
         N = self.N
@@ -187,7 +187,7 @@ class West:
             assert n_occ is not None
             shape = (n_freq, n_pert, n_occ, 2, self.n_g) if self.mode == WEST_GAMMA else (n_freq, n_pert, n_occ, self.n_g)
             dpsi = torch.empty(shape, dtype=torch.complex128, device=dV.device)
-        opts = west_cg_opts(int(max_iter), float(tol), float(alpha_pv), int(precond), int(check_every))
+        opts = west_cg_opts(int(max_iter), float(tol), float(alpha_pv), int(precond), int(check_every), int(solver))
         st = west_stats()
         rc = self._ck(self.lib.west_chi0_apply(self.ctx, precision, n_pert, _dev(dV, torch.float64), n_freq, om.ctypes.data, C.byref(opts),
                                                _dev(dn, torch.float64), _dev(dpsi) if dpsi is not None else None,

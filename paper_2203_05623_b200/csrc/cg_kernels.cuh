@@ -25,6 +25,8 @@ __device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
     return make_double2((a.x * b.x + a.y * b.y) / d, (a.y * b.x - a.x * b.y) / d);
 }
 
+__device__ __forceinline__ double2 cmul2(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
 // block reduction of up to 4 doubles
 template <int NV>
 __device__ __forceinline__ void block_reduce(double (&v)[NV], double* sh /* [NV*8] */) {
@@ -199,6 +201,164 @@ __global__ void __launch_bounds__(NT) cg_step(long long n_g, int n_occ, const do
         s.rr[col] = acc[2];
         if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
     }
+}
+
+// ------------------------------------------------------------------------------------------------- multi-shift CG
+// All imaginary frequencies from ONE Krylov sequence (Frommer's shifted CG): the seed system is the
+// real symmetric A = H - eps_v + alpha P_v (WEST_GAMMA, unpreconditioned), the shifted systems are (A + sigma_s) x_s = b with
+// sigma_s = -i omega_s.  Shifted residuals stay collinear with the seed residual, r_s = zeta_s r, so one H*psi per iteration
+// serves every frequency:
+//   zeta_{k+1} = zeta_k zeta_{k-1} a_{k-1} / [ a_k b_{k-1} (zeta_{k-1} - zeta_k) + zeta_{k-1} a_{k-1} (1 + sigma a_k) ]
+//   a_s = a_k zeta_{k+1} / zeta_k ;  b_s = b_k (zeta_{k+1} / zeta_k)^2 ;  x_s += a_s p_s ;  p_s = zeta_{k+1} r_{k+1} + b_s p_s
+// Vectors: r, p, Ap real functions in compacted order; XS, PS [shift][col][2][n_g] (Re and Im part as two real functions)
+// in original column order.
+constexpr int MS_MAX_SHIFTS = 16;
+
+struct MsState {
+    double*  a_prev;     // [n_col]
+    double*  b_prev;     // [n_col]
+    double*  rr;         // [n_col] <r_k, r_k>
+    double*  b2;         // [n_col] <b, b>
+    double2* zeta;       // [n_shift][n_col]
+    double2* zeta_prev;  // [n_shift][n_col]
+    double*  res2;       // [n_shift][n_col] |zeta|^2 rr / b2 at the moment the shift was frozen (or now)
+    int*     active;     // [n_col]
+    int*     sactive;    // [n_shift][n_col]
+    int*     counters;   // [0] live columns
+};
+struct MsShifts { int n; double omega[MS_MAX_SHIFTS]; };
+
+__device__ __forceinline__ double rdot_gamma(const double2 x, const double2 y, int g) {
+    return g == 0 ? x.x * y.x : 2.0 * (x.x * y.x + x.y * y.y);
+}
+
+// r holds b.  p = r, x_s = 0 (memset by the host), p_s = (b, 0)
+__global__ void __launch_bounds__(NT) ms_init(long long n_g, int n_col, MsShifts sh, const double2* R, double2* P, double2* PS, MsState st,
+                                              int* colmap) {
+    __shared__ double red[32];
+    const int col = blockIdx.x;
+    const double2* r = R + (long long)col * n_g;
+    double2* p = P + (long long)col * n_g;
+    double acc[1] = {0};
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        const double2 v = r[g];
+        acc[0] += rdot_gamma(v, v, g);
+        p[g] = v;
+        for (int s = 0; s < sh.n; ++s) {
+            double2* ps = PS + ((long long)s * n_col + col) * 2 * n_g;
+            ps[g] = v;
+            ps[n_g + g] = make_double2(0.0, 0.0);
+        }
+    }
+    block_reduce<1>(acc, red);
+    if (threadIdx.x == 0) {
+        colmap[col] = col;
+        st.rr[col] = acc[0]; st.b2[col] = acc[0]; st.a_prev[col] = 1.0; st.b_prev[col] = 0.0;
+        const int act = acc[0] > 0.0;
+        st.active[col] = act;
+        if (act) atomicAdd(st.counters, 1);
+        for (int s = 0; s < sh.n; ++s) {
+            const long long i = (long long)s * n_col + col;
+            st.zeta[i] = make_double2(1.0, 0.0); st.zeta_prev[i] = make_double2(1.0, 0.0);
+            st.sactive[i] = act; st.res2[i] = act ? 1.0 : 0.0;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts sh, double tol2, double2* P, const double2* AP, double2* R,
+                                              double2* XS, double2* PS, MsState st, const int* colmap) {
+    __shared__ double red[32];
+    __shared__ double2 s_zn[MS_MAX_SHIFTS], s_as[MS_MAX_SHIFTS], s_bs[MS_MAX_SHIFTS];
+    __shared__ int s_on[MS_MAX_SHIFTS];
+    const int k = blockIdx.x, col = colmap[k];
+    if (!st.active[col]) return;
+    double2* p = P + (long long)k * n_g; const double2* ap = AP + (long long)k * n_g; double2* r = R + (long long)k * n_g;
+    // ---- a_k
+    double acc[1] = {0};
+    for (int g = threadIdx.x; g < n_g; g += NT) acc[0] += rdot_gamma(p[g], ap[g], g);
+    block_reduce<1>(acc, red);
+    const double rr = st.rr[col], a = rr / acc[0];
+    // ---- r_{k+1}, b_k
+    acc[0] = 0;
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        double2 v = r[g]; const double2 q = ap[g];
+        v.x -= a * q.x; v.y -= a * q.y;
+        r[g] = v;
+        acc[0] += rdot_gamma(v, v, g);
+    }
+    block_reduce<1>(acc, red);
+    const double rrn = acc[0], b = rrn / rr;
+    // ---- shifted scalars
+    if (threadIdx.x < sh.n) {
+        const int s = threadIdx.x;
+        const long long i = (long long)s * n_col + col;
+        int on = st.sactive[i];
+        if (on) {
+            const double2 z = st.zeta[i], zp = st.zeta_prev[i];
+            const double ap_ = st.a_prev[col], bp_ = st.b_prev[col];
+            const double2 sigma = make_double2(0.0, -sh.omega[s]);
+            // den = a b_{k-1} (zp - z) + zp a_{k-1} (1 + sigma a)
+            const double2 t1 = make_double2(a * bp_ * (zp.x - z.x), a * bp_ * (zp.y - z.y));
+            const double2 one_sa = make_double2(1.0 + sigma.x * a, sigma.y * a);
+            const double2 t2 = cmul2(make_double2(zp.x * ap_, zp.y * ap_), one_sa);
+            const double2 num = cmul2(z, make_double2(zp.x * ap_, zp.y * ap_));
+            const double2 zn = cdiv(num, make_double2(t1.x + t2.x, t1.y + t2.y));
+            const double2 ratio = cdiv(zn, z);
+            s_zn[s] = zn;
+            s_as[s] = make_double2(a * ratio.x, a * ratio.y);
+            const double2 r2 = cmul2(ratio, ratio);
+            s_bs[s] = make_double2(b * r2.x, b * r2.y);
+            st.zeta_prev[i] = z; st.zeta[i] = zn;
+            const double res2 = (zn.x * zn.x + zn.y * zn.y) * rrn / st.b2[col];
+            st.res2[i] = res2;
+            if (!(res2 > tol2)) st.sactive[i] = 0;       // x_s still takes this iteration's update below, then freezes
+        }
+        s_on[s] = on;
+    }
+    __syncthreads();
+    // ---- vector updates
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        const double2 rn = r[g];
+        for (int s = 0; s < sh.n; ++s) {
+            if (!s_on[s]) continue;
+            double2* xs = XS + ((long long)s * n_col + col) * 2 * n_g;
+            double2* ps = PS + ((long long)s * n_col + col) * 2 * n_g;
+            const double2 as = s_as[s], bs = s_bs[s], zn = s_zn[s];
+            const double2 pr = ps[g], pi = ps[n_g + g];
+            double2 xr = xs[g], xi = xs[n_g + g];
+            xr.x += as.x * pr.x - as.y * pi.x; xr.y += as.x * pr.y - as.y * pi.y;
+            xi.x += as.x * pi.x + as.y * pr.x; xi.y += as.x * pi.y + as.y * pr.y;
+            xs[g] = xr; xs[n_g + g] = xi;
+            ps[g] = make_double2(zn.x * rn.x + bs.x * pr.x - bs.y * pi.x, zn.x * rn.y + bs.x * pr.y - bs.y * pi.y);
+            ps[n_g + g] = make_double2(zn.y * rn.x + bs.x * pi.x + bs.y * pr.x, zn.y * rn.y + bs.x * pi.y + bs.y * pr.y);
+        }
+        const double2 pp = p[g];
+        p[g] = make_double2(rn.x + b * pp.x, rn.y + b * pp.y);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        st.a_prev[col] = a; st.b_prev[col] = b; st.rr[col] = rrn;
+        int any = 0;
+        for (int s = 0; s < sh.n; ++s) any |= st.sactive[(long long)s * n_col + col];
+        if (!any) { st.active[col] = 0; atomicSub(st.counters, 1); }
+    }
+}
+
+// per-frequency report of the multi-shift solve: out[0] = max relative residual, out[1] = number of unconverged (col, shift)
+__global__ void ms_report(int n_col, int n_shift, double tol2, MsState st, double* out) {
+    __shared__ double shm[NT]; __shared__ int shc[NT];
+    double m = 0; int c = 0;
+    for (long long i = threadIdx.x; i < (long long)n_col * n_shift; i += NT) {
+        const double q = st.res2[i];
+        m = fmax(m, q); c += q > tol2;
+    }
+    shm[threadIdx.x] = m; shc[threadIdx.x] = c;
+    __syncthreads();
+    for (int o = NT / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) { shm[threadIdx.x] = fmax(shm[threadIdx.x], shm[threadIdx.x + o]); shc[threadIdx.x] += shc[threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[0] = sqrt(shm[0]); out[1] = (double)shc[0]; }
 }
 
 // max over columns of sqrt(rr/b2), and count of columns above tol (final report)

@@ -60,7 +60,7 @@ struct west_ctx {
     int n_uslots = 0;
 
     // workspaces (grown lazily)
-    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps;
+    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst;
     int* h_pinned = nullptr;           // pinned host scratch for convergence polling / reports
 
     // optional per-kernel-class timing (west_set_profile): CUDA events on the context's stream around every launch
@@ -697,6 +697,120 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
     return WEST_OK;
 }
 
+// a1: b = -P_c (dV_i psi_v) written into R ([n_col][nvpc][n_g]; the imaginary-part vectors of nvpc = 2 stay zero)
+int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R) {
+    const int gamma = is_gamma(c), N = c->cell.N, n_col = n_pert * c->n_occ, n_vec = n_col * nvpc;
+    const long long n_g = c->hs.n_g;
+    const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
+    const int chunk = std::max(1, chunk_slots(c, 0));
+    int rc = ensure_W(c, std::min(chunk, std::max(n_rslots, 1)), 0);
+    if (rc) return rc;
+    if (nvpc == 2) CK(cudaMemsetAsync(R, 0, sizeof(cx<double>) * n_g * n_vec, c->st));
+    // slot (i, us) -> columns i*n_occ + 2us (+1)  [GAMMA] or i*n_occ + us
+    VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
+    K2Any a{};
+    a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dV = (const double*)c->dVpos.p; a.n_uslots = n_uslots;
+    K3Epi e{-1.0 / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
+    for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
+        const int ns = std::min(chunk, n_rslots - s0);
+        vm.slot0 = s0; a.slot0 = s0;
+        Prof p_(c, PC_FFT_OTHER);
+        CK(c->ops->k2(0, K2_FROMR, ns, c->st, c->geom, a));
+        CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, c->W.p, e, R));
+        c->launches += 2;
+    }
+    // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows
+    if ((rc = ensure(c, c->misc, sizeof(double) * std::max(c->rows_psi, 8)))) return rc;
+    std::vector<double> m1(c->rows_psi, -1.0);
+    CK(cudaMemcpyAsync(c->misc.p, m1.data(), sizeof(double) * c->rows_psi, cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));     // m1 is a stack-lifetime pageable buffer
+    return lowrank_apply(c, c->rows_kb, c->rows_psi, n_vec, (const double*)R, (double*)R, (const double*)c->misc.p);
+}
+
+// a10: dn_i(r) = (4/Omega) Re sum_v conj(u_v) du_iv from X ([n_col][nvpc][n_g]) into dn_out ([n_pert][N^3], natural order)
+int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_out) {
+    const int gamma = is_gamma(c), N = c->cell.N, n_col = n_pert * c->n_occ, n_vec = n_col * nvpc;
+    const long long n3 = n3_of(c);
+    const double vol = c->cell.L * c->cell.L * c->cell.L;
+    const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
+    const int chunk = std::max(1, chunk_slots(c, 0));
+    int rc = ensure_W(c, std::min(chunk, std::max(n_rslots, 1)), 0);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(c->dnpos.p, 0, sizeof(double) * n3 * n_pert, c->st));
+    VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
+    K2Any a{};
+    a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dn = (double*)c->dnpos.p; a.n_uslots = n_uslots; a.fac = 4.0 / vol;
+    for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
+        const int ns = std::min(chunk, n_rslots - s0);
+        vm.slot0 = s0; a.slot0 = s0;
+        Prof p_(c, PC_FFT_OTHER);
+        CK(c->ops->k1(0, gamma, ns, c->st, c->geom, vm, X, c->W.p));
+        CK(c->ops->k2(0, K2_DN, ns, c->st, c->geom, a));
+        c->launches += 2;
+    }
+    pos_to_nat_real<<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, (const double*)c->dnpos.p, dn_out);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+
+// multi-shift CG (WEST_GAMMA): all frequencies from one unpreconditioned Krylov sequence of the real seed operator
+int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::MsShifts& sh, cx<double>*& R, cx<double>*& P, cx<double>*& AP,
+             cx<double>* XS, cx<double>* PS, double* shift, const double* d_eps, wcg::MsState st, int* maps, int* iters_out, int64_t* n_h_out) {
+    const long long n_g = c->hs.n_g;
+    const int n_occ = c->n_occ;
+    const double tol2 = o.tol * o.tol;
+    const int every = std::max(1, o.check_every);
+    int* colmap = maps; int* newmap = maps + n_col; int* src = maps + 2 * (size_t)n_col;
+    CK(cudaMemsetAsync(st.counters, 0, 2 * sizeof(int), c->st));
+    CK(cudaMemsetAsync(XS, 0, sizeof(cx<double>) * 2 * n_g * n_col * sh.n, c->st));
+    wcg::ms_init<<<n_col, wcg::NT, 0, c->st>>>(n_g, n_col, sh, (const double2*)R, (double2*)P, (double2*)PS, st, colmap);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    const int rows = c->rows_kb + c->rows_psi;
+    int n_act = n_col, it = 0;
+    int64_t n_h = 0;
+    for (; it < o.max_iter; ++it) {
+        VecMap vm{2, 1, n_act, 0};
+        int rc = hloc_apply(c, f32, vm, (n_act + 1) / 2, P, AP, shift, 0.0);
+        if (rc) return rc;
+        rc = lowrank_apply(c, 0, rows, n_act, (const double*)P, (double*)AP, (const double*)c->coef_all.p);
+        if (rc) return rc;
+        n_h += n_act;
+        {
+            Prof p_(c, PC_CGVEC);
+            wcg::ms_step<<<n_act, wcg::NT, 0, c->st>>>(n_g, n_col, sh, tol2, (double2*)P, (const double2*)AP, (double2*)R, (double2*)XS,
+                                                       (double2*)PS, st, colmap);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
+            CK(cudaMemcpyAsync(c->h_pinned, st.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+            CK(cudaStreamSynchronize(c->st));
+            const int live = c->h_pinned[0];
+            if (live <= 0) { ++it; break; }
+            if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
+                Prof p_(c, PC_CGVEC);
+                wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, colmap, st.active, newmap, src);
+                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(n_g, src, (const double2*)R, (double2*)AP);
+                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(n_g, src, (const double2*)P, (double2*)R);
+                CK(cudaGetLastError());
+                c->launches += 3;
+                cx<double>* oldR = R; cx<double>* oldP = P;
+                R = AP; P = oldR; AP = oldP;
+                std::swap(colmap, newmap);
+                n_act = live;
+                fill_shift<<<blocks_for(n_act, 256), 256, 0, c->st>>>(n_act, 1, n_occ, d_eps, shift, colmap);
+                CK(cudaGetLastError());
+                c->launches += 1;
+            }
+        }
+    }
+    *iters_out = it;
+    *n_h_out = n_h;
+    return WEST_OK;
+}
+
 }  // namespace
 
 extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, const double* dV, int32_t n_freq,
@@ -705,7 +819,9 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
-    if (opts->max_iter < 1 || !(opts->tol > 0)) return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
+    if (opts->max_iter < 1 || !(opts->tol > 0) || (opts->solver != 0 && opts->solver != 1)) return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
+    if (opts->solver == 1 && (c->cell.mode != WEST_GAMMA || n_freq > wcg::MS_MAX_SHIFTS))
+        return fail(c, WEST_EINVAL, "west_chi0_apply: the multi-shift solver needs WEST_GAMMA and at most %d frequencies", wcg::MS_MAX_SHIFTS);
     const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
     if (gamma && (n_occ & 1)) return fail(c, WEST_EINVAL, "west_chi0_apply: WEST_GAMMA needs an even number of occupied states (two per FFT)");
     for (int w = 0; w < n_freq; ++w) {
@@ -751,9 +867,82 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     if (stats) for (auto& e : ev) CK(cudaEventCreate(&e));
     int ret = WEST_OK;
-    const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
-    const int chunk = std::max(1, chunk_slots(c, 0));
-    if ((rc = ensure_W(c, std::min(chunk, std::max(n_rslots, 1)), 0))) return rc;
+    auto copy_dpsi = [&](int w, int mode, const cx<double>* Xw) -> int {
+        // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 (per-frequency solver) the imaginary part is zero
+        const long long per = n_g * n_col * (gamma ? 2 : 1);
+        cx<double>* dst = (cx<double>*)dpsi_opt + (long long)w * per;
+        if (gamma && mode == 0) {
+            CK(cudaMemsetAsync(dst, 0, sizeof(cx<double>) * per, c->st));
+            CK(cudaMemcpy2DAsync(dst, sizeof(cx<double>) * 2 * n_g, Xw, sizeof(cx<double>) * n_g, sizeof(cx<double>) * n_g, n_col,
+                                 cudaMemcpyDeviceToDevice, c->st));
+        } else {
+            CK(cudaMemcpyAsync(dst, Xw, sizeof(cx<double>) * per, cudaMemcpyDeviceToDevice, c->st));
+        }
+        return WEST_OK;
+    };
+    auto add_times = [&]() {
+        float t;
+        cudaEventElapsedTime(&t, ev[0], ev[1]); stats->ms_rhs += t;
+        cudaEventElapsedTime(&t, ev[1], ev[2]); stats->ms_cg += t;
+        cudaEventElapsedTime(&t, ev[2], ev[3]); stats->ms_dn += t;
+    };
+
+    if (opts->solver == 1) {
+        // ------------------------------------------------------------ multi-shift CG: every frequency from one Krylov sequence
+        wcg::MsShifts sh;
+        sh.n = n_freq;
+        for (int w = 0; w < n_freq; ++w) sh.omega[w] = omega_host[w];
+        const size_t per = (size_t)n_g * n_col * 2;                       // complex-valued solution of one frequency
+        if ((rc = ensure(c, c->xs, sizeof(cx<double>) * per * n_freq))) return rc;
+        if ((rc = ensure(c, c->ps, sizeof(cx<double>) * per * n_freq))) return rc;
+        const size_t ncs = (size_t)n_col * n_freq;
+        if ((rc = ensure(c, c->msst, sizeof(double) * 4 * n_col + sizeof(double2) * 2 * ncs + sizeof(double) * ncs + sizeof(int) * (n_col + ncs) + 64)))
+            return rc;
+        wcg::MsState st;
+        {
+            char* p = (char*)c->msst.p;
+            st.zeta = (double2*)p; p += sizeof(double2) * ncs;
+            st.zeta_prev = (double2*)p; p += sizeof(double2) * ncs;
+            st.a_prev = (double*)p; p += sizeof(double) * n_col;
+            st.b_prev = (double*)p; p += sizeof(double) * n_col;
+            st.rr = (double*)p; p += sizeof(double) * n_col;
+            st.b2 = (double*)p; p += sizeof(double) * n_col;
+            st.res2 = (double*)p; p += sizeof(double) * ncs;
+            st.active = (int*)p; p += sizeof(int) * n_col;
+            st.sactive = (int*)p; p += sizeof(int) * ncs;
+            p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
+            st.counters = (int*)p;
+        }
+        fill_shift<<<blocks_for(n_col, 256), 256, 0, c->st>>>(n_col, 1, n_occ, d_eps, (double*)c->shift.p, nullptr);
+        CK(cudaGetLastError());
+        if (stats) CK(cudaEventRecord(ev[0], c->st));
+        if ((rc = chi0_rhs(c, n_pert, 1, R))) return rc;
+        if (stats) CK(cudaEventRecord(ev[1], c->st));
+        int iters = 0;
+        int64_t n_h = 0;
+        if ((rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, (double*)c->shift.p, d_eps, st,
+                           (int*)c->maps.p, &iters, &n_h)))
+            return rc;
+        if (stats) CK(cudaEventRecord(ev[2], c->st));
+        for (int w = 0; w < n_freq; ++w) {
+            const cx<double>* Xw = (const cx<double>*)c->xs.p + (size_t)w * per;
+            if ((rc = chi0_dn(c, n_pert, 2, Xw, dn + (long long)w * n_pert * n3))) return rc;
+            if (dpsi_opt && (rc = copy_dpsi(w, 1, Xw))) return rc;
+        }
+        if ((rc = ensure(c, c->misc, 64))) return rc;
+        wcg::ms_report<<<1, wcg::NT, 0, c->st>>>(n_col, n_freq, opts->tol * opts->tol, st, (double*)c->misc.p);
+        double h[2];
+        if (stats) CK(cudaEventRecord(ev[3], c->st));
+        CK(cudaMemcpyAsync(h, c->misc.p, sizeof h, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+        if (h[1] > 0) ret = WEST_NOTCONVERGED;
+        if (stats) {
+            add_times();
+            stats->iters = iters; stats->n_unconverged = (int)h[1]; stats->resid_max = h[0]; stats->n_h_apply = n_h;
+        }
+        if (stats) for (auto& e : ev) cudaEventDestroy(e);
+        return ret;
+    }
 
     for (int w = 0; w < n_freq; ++w) {
         const double omega = omega_host[w];
@@ -762,28 +951,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         fill_shift<<<blocks_for(n_vec, 256), 256, 0, c->st>>>(n_vec, nvpc, n_occ, d_eps, (double*)c->shift.p, nullptr);
         CK(cudaGetLastError());
         if (stats) CK(cudaEventRecord(ev[0], c->st));
-        // ---- a1: b = -P_c (dV_i psi_v), written into R.   slot (i, us) -> columns i*n_occ + 2us (+1)  [GAMMA] or i*n_occ + us
-        if (mode == 1) CK(cudaMemsetAsync(R, 0, sizeof(cx<double>) * n_g * n_vec, c->st));
-        {
-            VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
-            K2Any a{};
-            a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dV = (const double*)c->dVpos.p; a.n_uslots = n_uslots;
-            K3Epi e{-1.0 / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
-            for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
-                const int ns = std::min(chunk, n_rslots - s0);
-                vm.slot0 = s0; a.slot0 = s0;
-                Prof p_(c, PC_FFT_OTHER);
-                CK(c->ops->k2(0, K2_FROMR, ns, c->st, c->geom, a));
-                CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, c->W.p, e, R));
-                c->launches += 2;
-            }
-            // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows
-            if ((rc = ensure(c, c->misc, sizeof(double) * c->rows_psi))) return rc;
-            std::vector<double> m1(c->rows_psi, -1.0);
-            CK(cudaMemcpyAsync(c->misc.p, m1.data(), sizeof(double) * c->rows_psi, cudaMemcpyHostToDevice, c->st));
-            CK(cudaStreamSynchronize(c->st));     // m1 is a stack-lifetime pageable buffer
-            if ((rc = lowrank_apply(c, c->rows_kb, c->rows_psi, n_vec, (const double*)R, (double*)R, (const double*)c->misc.p))) return rc;
-        }
+        if ((rc = chi0_rhs(c, n_pert, nvpc, R))) return rc;
         if (stats) CK(cudaEventRecord(ev[1], c->st));
         // ---- a2-a9: batched PCG / COCG
         int iters = 0;
@@ -793,50 +961,17 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
         if (rc) return rc;
         if (stats) CK(cudaEventRecord(ev[2], c->st));
-        // ---- a10: dn_i(r) = (4/Omega) Re sum_v conj(u_v) du_iv
-        CK(cudaMemsetAsync(c->dnpos.p, 0, sizeof(double) * n3 * n_pert, c->st));
-        {
-            VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
-            K2Any a{};
-            a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dn = (double*)c->dnpos.p; a.n_uslots = n_uslots; a.fac = 4.0 / vol;
-            for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
-                const int ns = std::min(chunk, n_rslots - s0);
-                vm.slot0 = s0; a.slot0 = s0;
-                Prof p_(c, PC_FFT_OTHER);
-                CK(c->ops->k1(0, gamma, ns, c->st, c->geom, vm, X, c->W.p));
-                CK(c->ops->k2(0, K2_DN, ns, c->st, c->geom, a));
-                c->launches += 2;
-            }
-            pos_to_nat_real<<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, (const double*)c->dnpos.p,
-                                                                           dn + (long long)w * n_pert * n3);
-            CK(cudaGetLastError());
-            c->launches += 1;
-        }
-        if (dpsi_opt) {
-            // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 the imaginary part is zero
-            const long long per = n_g * n_col * (gamma ? 2 : 1);
-            cx<double>* dst = (cx<double>*)dpsi_opt + (long long)w * per;
-            if (gamma && mode == 0) {
-                CK(cudaMemsetAsync(dst, 0, sizeof(cx<double>) * per, c->st));
-                CK(cudaMemcpy2DAsync(dst, sizeof(cx<double>) * 2 * n_g, X, sizeof(cx<double>) * n_g, sizeof(cx<double>) * n_g, n_col,
-                                     cudaMemcpyDeviceToDevice, c->st));
-            } else {
-                CK(cudaMemcpyAsync(dst, X, sizeof(cx<double>) * per, cudaMemcpyDeviceToDevice, c->st));
-            }
-        }
+        if ((rc = chi0_dn(c, n_pert, nvpc, X, dn + (long long)w * n_pert * n3))) return rc;
+        if (dpsi_opt && (rc = copy_dpsi(w, mode, X))) return rc;
         if (stats) {
             CK(cudaEventRecord(ev[3], c->st));
-            double* rep = (double*)c->misc.p;     // misc holds >= rows_psi doubles >= 2
             if ((rc = ensure(c, c->misc, 64))) return rc;
-            rep = (double*)c->misc.p;
+            double* rep = (double*)c->misc.p;
             wcg::cg_report<<<1, wcg::NT, 0, c->st>>>(n_col, opts->tol * opts->tol, s, rep);
             double h[2];
             CK(cudaMemcpyAsync(h, rep, sizeof h, cudaMemcpyDeviceToHost, c->st));
             CK(cudaStreamSynchronize(c->st));
-            float t;
-            cudaEventElapsedTime(&t, ev[0], ev[1]); stats->ms_rhs += t;
-            cudaEventElapsedTime(&t, ev[1], ev[2]); stats->ms_cg += t;
-            cudaEventElapsedTime(&t, ev[2], ev[3]); stats->ms_dn += t;
+            add_times();
             stats->iters = std::max(stats->iters, iters);
             stats->n_unconverged += (int)h[1];
             stats->resid_max = std::max(stats->resid_max, h[0]);

@@ -11,16 +11,17 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-9
 
 
-def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1):
+def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500):
     import torch
     import paper_2203_05623_b200 as wb
     p = oracle_problem.build(name)
     w, sel = make_west(p)
     dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
     prec = wb.WEST_FP64 if precision is None else precision
-    dn, dpsi, st = w.chi0_apply(dV, p.omegas, tol=tol_cg, max_iter=500, alpha_pv=p.alpha if alpha is None else alpha,
-                                precond=precond, precision=prec, want_dpsi=True, n_occ=p.n_occ)
-    ref_dn, ref_dpsi = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, p.dV, p.omegas, p.miller, p.L, p.N, return_dpsi=True)
+    om = p.omegas if omegas is None else omegas
+    dn, dpsi, st = w.chi0_apply(dV, om, tol=tol_cg, max_iter=max_iter, alpha_pv=p.alpha if alpha is None else alpha,
+                                precond=precond, precision=prec, want_dpsi=True, n_occ=p.n_occ, solver=solver)
+    ref_dn, ref_dpsi = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, p.dV, om, p.miller, p.L, p.N, return_dpsi=True)
     w.close()
     return p, sel, dn.cpu().numpy(), dpsi.cpu().numpy(), st, ref_dn, ref_dpsi
 
@@ -80,3 +81,15 @@ def test_chi0_not_converged_status():
     dn, _, st = w.chi0_apply(dV, [0.0], tol=1e-14, max_iter=3, alpha_pv=p.alpha)
     assert st["rc"] == wb.WEST_NOTCONVERGED and st["n_unconverged"] > 0 and st["iters"] == 3
     w.close()
+
+
+def test_chi0_multishift_all_frequencies_from_one_krylov_sequence():
+    """solver = 1: omega = 0 and three imaginary frequencies from one unpreconditioned CG sequence."""
+    omegas = [0.0, 0.05, 0.6947, 5.0]
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini3", solver=1, omegas=omegas, max_iter=2000)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    for w in range(len(omegas)):
+        assert relmax(dn[w], ref_dn[w]) < TOL
+    _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+    # one H*psi per column and iteration serves all four frequencies
+    assert st["n_h_apply"] <= st["iters"] * p.n_occ * len(p.dV)

@@ -98,14 +98,16 @@ def test_invariants_on_the_full_batch(big):
     assert np.max(np.abs(ov)) < 1e-9 * np.max(np.abs(x)) * np.sqrt(x.shape[1])
 
 
-def test_cfg3_imaginary_frequencies_sampled_columns(states):
-    """Config 3: complex-shifted Sternheimer at the lowest and highest of its 8 frequencies, against the oracle's COCG."""
+@pytest.mark.parametrize("solver", [0, 1])
+def test_cfg3_imaginary_frequencies_sampled_columns(states, solver):
+    """Config 3: complex-shifted Sternheimer at the lowest and highest of its 8 frequencies, against the oracle's COCG;
+    solver 0 = one preconditioned COCG solve per frequency, solver 1 = multi-shift CG (both frequencies from one sequence)."""
     import torch
     p, eps, U, alpha, w, dev = (states[k] for k in ("p", "eps", "U", "alpha", "w", "dev"))
     import synth
     omegas = [synth.get_config("cfg3")["omegas"][0], synth.get_config("cfg3")["omegas"][-1]]
     dV = torch.from_numpy(np.ascontiguousarray(p.dV[:2])).to(dev)
-    dn, dpsi, st = w.chi0_apply(dV, omegas, tol=1e-12, max_iter=500, alpha_pv=alpha, want_dpsi=True, n_occ=p.n_occ)
+    dn, dpsi, st = w.chi0_apply(dV, omegas, tol=1e-12, max_iter=2000, alpha_pv=alpha, want_dpsi=True, n_occ=p.n_occ, solver=solver)
     assert st["rc"] == 0 and st["n_unconverged"] == 0
     dpsi = dpsi.cpu().numpy()
     apply_H = lambda y: oham.apply_h(y, p.miller, p.L, p.N, p.vloc, p.beta, p.dcoef)
