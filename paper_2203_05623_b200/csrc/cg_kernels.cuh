@@ -265,8 +265,8 @@ __global__ void __launch_bounds__(NT) ms_init(long long n_g, int n_col, MsShifts
     }
 }
 
-__global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts sh, double tol2, double2* P, const double2* AP, double2* R,
-                                              double2* XS, double2* PS, MsState st, const int* colmap) {
+__global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts sh, double tol2, int want_imag, double2* P, const double2* AP,
+                                              double2* R, double2* XS, double2* PS, MsState st, const int* colmap) {
     __shared__ double red[32];
     __shared__ double2 s_zn[MS_MAX_SHIFTS], s_as[MS_MAX_SHIFTS], s_bs[MS_MAX_SHIFTS];
     __shared__ int s_on[MS_MAX_SHIFTS];
@@ -325,10 +325,14 @@ __global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts
             double2* ps = PS + ((long long)s * n_col + col) * 2 * n_g;
             const double2 as = s_as[s], bs = s_bs[s], zn = s_zn[s];
             const double2 pr = ps[g], pi = ps[n_g + g];
-            double2 xr = xs[g], xi = xs[n_g + g];
+            double2 xr = xs[g];
             xr.x += as.x * pr.x - as.y * pi.x; xr.y += as.x * pr.y - as.y * pi.y;
-            xi.x += as.x * pi.x + as.y * pr.x; xi.y += as.x * pi.y + as.y * pr.y;
-            xs[g] = xr; xs[n_g + g] = xi;
+            xs[g] = xr;
+            if (want_imag) {        // Im x_s is only needed when the caller asked for dpsi: dn uses Re x_s alone (real orbitals)
+                double2 xi = xs[n_g + g];
+                xi.x += as.x * pi.x + as.y * pr.x; xi.y += as.x * pi.y + as.y * pr.y;
+                xs[n_g + g] = xi;
+            }
             ps[g] = make_double2(zn.x * rn.x + bs.x * pr.x - bs.y * pi.x, zn.x * rn.y + bs.x * pr.y - bs.y * pi.y);
             ps[n_g + g] = make_double2(zn.y * rn.x + bs.x * pi.x + bs.y * pr.x, zn.y * rn.y + bs.x * pi.y + bs.y * pr.y);
         }

@@ -756,7 +756,8 @@ int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_o
 
 // multi-shift CG (WEST_GAMMA): all frequencies from one unpreconditioned Krylov sequence of the real seed operator
 int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::MsShifts& sh, cx<double>*& R, cx<double>*& P, cx<double>*& AP,
-             cx<double>* XS, cx<double>* PS, double* shift, const double* d_eps, wcg::MsState st, int* maps, int* iters_out, int64_t* n_h_out) {
+             cx<double>* XS, cx<double>* PS, int want_imag, double* shift, const double* d_eps, wcg::MsState st, int* maps, int* iters_out,
+             int64_t* n_h_out) {
     const long long n_g = c->hs.n_g;
     const int n_occ = c->n_occ;
     const double tol2 = o.tol * o.tol;
@@ -779,7 +780,7 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
         n_h += n_act;
         {
             Prof p_(c, PC_CGVEC);
-            wcg::ms_step<<<n_act, wcg::NT, 0, c->st>>>(n_g, n_col, sh, tol2, (double2*)P, (const double2*)AP, (double2*)R, (double2*)XS,
+            wcg::ms_step<<<n_act, wcg::NT, 0, c->st>>>(n_g, n_col, sh, tol2, want_imag, (double2*)P, (const double2*)AP, (double2*)R, (double2*)XS,
                                                        (double2*)PS, st, colmap);
             CK(cudaGetLastError());
             c->launches += 1;
@@ -920,7 +921,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         if (stats) CK(cudaEventRecord(ev[1], c->st));
         int iters = 0;
         int64_t n_h = 0;
-        if ((rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, (double*)c->shift.p, d_eps, st,
+        if ((rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, dpsi_opt != nullptr, (double*)c->shift.p, d_eps, st,
                            (int*)c->maps.p, &iters, &n_h)))
             return rc;
         if (stats) CK(cudaEventRecord(ev[2], c->st));
