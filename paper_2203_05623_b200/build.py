@@ -15,11 +15,13 @@ ROOT = os.path.dirname(HERE)
 OBJ = os.path.join(ROOT, "build", "west_obj")
 LIB = os.path.join(HERE, "libwest.so")
 
-# (N1, N2, N, NW, MINB, CU, ZMINB): N = N1*N2 grid size; LC = x lines per chunk in the plane kernel
+# (N1, N2, N, NW, MINB, CU, ZMINB, ZNT): N = N1*N2 grid size; LC = x lines per chunk in the plane kernel
 # NW = warps per CTA of the plane kernel, MINB = resident CTAs per SM it is compiled for (register cap),
 # CU = stick units per CTA of the z kernels (2 * CU * max(N1, N2) <= 256 threads)
 # ZMINB = resident CTAs per SM the z-stick kernels are compiled for
-FFT_SIZES = [(4, 6, 24, 4, 4, 20, 4), (6, 6, 36, 4, 4, 20, 4), (6, 8, 48, 6, 3, 16, 4), (8, 9, 72, 12, 2, 14, 4), (12, 12, 144, 16, 1, 10, 2)]
+# ZNT = threads per CTA of the z-stick kernels (2 * CU * max(N1, N2) <= ZNT)
+FFT_SIZES = [(4, 6, 24, 4, 4, 20, 4, 256), (6, 6, 36, 4, 4, 20, 4, 256), (6, 8, 48, 6, 3, 16, 4, 256), (8, 9, 72, 12, 2, 14, 4, 256),
+             (12, 12, 144, 16, 1, 10, 2, 256)]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
@@ -57,9 +59,9 @@ def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
     jobs = []
-    for n1, n2, n, nw, minb, cu, zminb in FFT_SIZES:
+    for n1, n2, n, nw, minb, cu, zminb, znt in FFT_SIZES:
         o = os.path.join(OBJ, "fft_%d.o" % n)
-        jobs.append((o, [nvcc] + NVCC_FLAGS + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_NW=%d" % nw, "-DWEST_MINB=%d" % minb, "-DWEST_CU=%d" % cu, "-DWEST_ZMINB=%d" % zminb,
+        jobs.append((o, [nvcc] + NVCC_FLAGS + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_NW=%d" % nw, "-DWEST_MINB=%d" % minb, "-DWEST_CU=%d" % cu, "-DWEST_ZMINB=%d" % zminb, "-DWEST_ZNT=%d" % znt,
                                                "-c", os.path.join(CSRC, "fft_n.cu"), "-o", o]))
     o = os.path.join(OBJ, "west.o")
     jobs.append((o, [nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "west.cu"), "-o", o]))

@@ -403,6 +403,9 @@ struct K2 {
 #ifndef WEST_ZMINB
 #define WEST_ZMINB 1      // resident CTAs per SM the z-stick kernels are compiled for (register cap)
 #endif
+#ifndef WEST_ZNT
+#define WEST_ZNT 256       // threads per CTA of the z-stick kernels
+#endif
 template <typename T, int N1, int N2>
 __device__ __forceinline__ void load_tw(cx<T>* tw_s, const cx<double>* tw_g) {
     // level twiddles in the two orders the passes read them, so that the lanes of a warp hit consecutive entries:
@@ -417,7 +420,7 @@ __device__ __forceinline__ void load_tw(cx<T>* tw_s, const cx<double>* tw_g) {
 }
 
 template <typename T, int N1, int N2, bool GAMMA, int CU>
-__global__ void __launch_bounds__(256, WEST_ZMINB) k1_g2r_z(WestGeom g, VecMap vm, const cx<double>* X, cx<T>* W) {
+__global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k1_g2r_z(WestGeom g, VecMap vm, const cx<double>* X, cx<T>* W) {
     using K = K1<T, N1, N2, GAMMA, CU>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* lines = reinterpret_cast<cx<T>*>(smem_raw);
@@ -433,7 +436,7 @@ __global__ void __launch_bounds__(256, WEST_ZMINB) k1_g2r_z(WestGeom g, VecMap v
 }
 
 template <typename T, int N1, int N2, bool GAMMA, int CU>
-__global__ void __launch_bounds__(256, WEST_ZMINB) k3_r2g_z(WestGeom g, VecMap vm, const cx<T>* W, K3Epi e, cx<double>* Y) {
+__global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k3_r2g_z(WestGeom g, VecMap vm, const cx<T>* W, K3Epi e, cx<double>* Y) {
     using K = K3<T, N1, N2, GAMMA, CU>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* lines = reinterpret_cast<cx<T>*>(smem_raw);

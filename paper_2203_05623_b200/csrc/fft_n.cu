@@ -9,6 +9,9 @@
 #ifndef WEST_MINB
 #define WEST_MINB 1
 #endif
+#ifndef WEST_ZNT
+#define WEST_ZNT 256
+#endif
 
 namespace {
 constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, NW = WEST_NW, LPW = K2Cfg<N1, N2>::LPW;
@@ -29,7 +32,7 @@ cudaError_t k1_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
     cudaError_t e = set_smem(kern, K::smem_bytes);
     if (e != cudaSuccess) return e;
     dim3 grid((g.n_units + CU - 1) / CU, n_slots);
-    kern<<<grid, 256, K::smem_bytes, st>>>(g, vm, X, reinterpret_cast<cx<T>*>(W));
+    kern<<<grid, WEST_ZNT, K::smem_bytes, st>>>(g, vm, X, reinterpret_cast<cx<T>*>(W));
     return cudaGetLastError();
 }
 template <typename T, bool GAMMA>
@@ -40,7 +43,7 @@ cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
     cudaError_t e = set_smem(kern, K::smem_bytes);
     if (e != cudaSuccess) return e;
     dim3 grid((g.n_units + CU - 1) / CU, n_slots);
-    kern<<<grid, 256, K::smem_bytes, st>>>(g, vm, reinterpret_cast<const cx<T>*>(W), ep, Y);
+    kern<<<grid, WEST_ZNT, K::smem_bytes, st>>>(g, vm, reinterpret_cast<const cx<T>*>(W), ep, Y);
     return cudaGetLastError();
 }
 template <typename T, int MODE>
