@@ -133,6 +133,19 @@ int  west_chi0_apply(west_ctx* ctx, int32_t precision, int32_t n_pert, const dou
                      int32_t n_freq, const double* omega_host, const west_cg_opts* opts,
                      double* dn, void* dpsi_opt, west_stats* stats_opt);
 
+/* Lanczos chains of the frequency-dependent step (Eq. 15-18; widening row SURVEY 8(f)-2).  For every function
+ * phi_m and occupied orbital psi_i: q^1 = psi_i phi_m / ||psi_i phi_m|| (Eq. 16; the norm is returned, reading R16),
+ * alpha^l = <q^l|H|q^l>, beta^{l+1} = ||(H - alpha^l) q^l - beta^l q^{l-1}||, q^{l+1} = that vector / beta^{l+1}; no
+ * re-orthogonalisation.  H = T + V_loc + V_NL as in west_h_apply.
+ *   phi    [n_pert][N^3] f64 real functions on the grid
+ *   alpha  [n_pert][n_occ][n_steps] f64 (device), alpha[..][l] = alpha^{l+1}
+ *   beta   [n_pert][n_occ][n_steps] f64 (device), beta[..][l]  = beta^{l+2} (the norm computed in step l)
+ *   norm   [n_pert][n_occ] f64 (device), ||psi_i phi_m|| in the plane-wave 2-norm
+ *   braket_opt NULL or [n_occ][n_steps][n_pert][n_pert] f64 (device, WEST_GAMMA only): <q^1_{n i} | q^{l+1}_{m i}>, the
+ *          matrix product of Eq. 19 / Fig. 4 as n_occ batched DMMA Gram blocks per step. */
+int  west_lanczos(west_ctx* ctx, int32_t precision, int32_t n_pert, const double* phi, int32_t n_steps, double* alpha, double* beta,
+                  double* norm, double* braket_opt);
+
 /* Dense contraction building blocks (FP64 DMMA), exported for tests and the roofline bench.
  * C[m][n] = sum_k A[m][k] B[n][k]          (west_gemm_tn: both operands K-contiguous, row-major [rows][ld])
  * Y[n][k] += sum_m C[m][n] A[m][k]          (west_gemm_update)

@@ -33,7 +33,7 @@ class west_stats(C.Structure):
 
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states",
-           "west_fft3d", "west_h_apply", "west_chi0_apply", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
+           "west_fft3d", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
            "west_launch_count", "west_set_fft_chunk", "west_set_profile", "west_get_profile"]
 
 
@@ -53,6 +53,7 @@ def load_library():
     lib.west_fft3d.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.west_h_apply.argtypes = [vp, i32, i32, vp, vp]
     lib.west_chi0_apply.argtypes = [vp, i32, i32, vp, i32, vp, C.POINTER(west_cg_opts), vp, vp, C.POINTER(west_stats)]
+    lib.west_lanczos.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp, vp]
     lib.west_gemm_tn.argtypes = [vp, i32, i32, i64, vp, i64, vp, i64, vp, i64]
     lib.west_gemm_update.argtypes = [vp, i32, i32, i64, vp, i64, vp, i64, vp, i64]
     lib.west_device_bytes.argtypes = [vp]
@@ -195,6 +196,19 @@ class West:
         stats = {k: getattr(st, k) for k, _ in west_stats._fields_}
         stats["rc"] = rc
         return dn, dpsi, stats
+
+    def lanczos(self, phi, n_steps, n_occ, want_brakets=False, precision=WEST_FP64):
+        """alpha, beta [n_pert][n_occ][n_steps], norm [n_pert][n_occ], brakets [n_occ][n_steps][n_pert][n_pert] or None."""
+        import torch
+        n_pert = int(phi.shape[0])
+        dev = phi.device
+        alpha = torch.empty((n_pert, n_occ, n_steps), dtype=torch.float64, device=dev)
+        beta = torch.empty_like(alpha)
+        norm = torch.empty((n_pert, n_occ), dtype=torch.float64, device=dev)
+        br = torch.empty((n_occ, n_steps, n_pert, n_pert), dtype=torch.float64, device=dev) if want_brakets else None
+        self._ck(self.lib.west_lanczos(self.ctx, precision, n_pert, _dev(phi, torch.float64), int(n_steps), _dev(alpha), _dev(beta),
+                                       _dev(norm), _dev(br) if br is not None else None))
+        return alpha, beta, norm, br
 
     def gemm_tn(self, A, B, out=None):
         """C[m][n] = sum_k A[m][k] B[n][k], f64 row-major."""

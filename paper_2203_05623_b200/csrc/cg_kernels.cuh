@@ -50,7 +50,7 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* sh /* [NV*
 }
 
 // Diagonal preconditioners M_v(G) (reading R4; they change iteration counts only, never the converged result):
-//   1: 1 / max(1, |G|^2 / (1.35 <psi_v|T|psi_v>))                      (the reading's default, also what the oracle's PCG uses)
+//   1: 1 / max(1, |G|^2 / (1.35 <psi_v|T|psi_v>))                      (the reading's default)
 //   2: Teter-Payne-Allan: (27 + 18x + 12x^2 + 8x^3) / (27 + 18x + 12x^2 + 8x^3 + 16x^4), x = |G|^2 / (1.5 <psi_v|T|psi_v>)
 __device__ __forceinline__ double precond(double g2, double tk, int on) {
     if (on == 0) return 1.0;

@@ -41,14 +41,18 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 // C[m][n] += sum_{k in this split} A[m][k] B[n][k].   lda, ldb even (16-byte aligned rows), A and B 16-byte aligned.
 __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, long long K, const double* __restrict__ A, long long lda,
                                                            const double* __restrict__ B, long long ldb, double* __restrict__ C,
-                                                           long long ldc, long long k_per_split, int use_atomic) {
+                                                           long long ldc, long long k_per_split, int use_atomic, int splits,
+                                                           long long sA, long long sB, long long sC) {
     extern __shared__ __align__(16) double smem[];
     double* As = smem;                                   // [STAGES][BM][PITCH_TN]
     double* Bs = smem + (size_t)STAGES * BM * PITCH_TN;  // [STAGES][BN][PITCH_TN]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp / WN, wn = warp % WN;            // 2 x WN warps
     const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
-    const long long kb = (long long)blockIdx.z * k_per_split;
+    // blockIdx.z = batch * splits + split; the batch strides shift all three matrices
+    const int batch = blockIdx.z / splits;
+    A += (long long)batch * sA; B += (long long)batch * sB; C += (long long)batch * sC;
+    const long long kb = (long long)(blockIdx.z - batch * splits) * k_per_split;
     long long ke = kb + k_per_split; if (ke > K) ke = K;
     const int nk = (int)((ke - kb + BK - 1) / BK);
 

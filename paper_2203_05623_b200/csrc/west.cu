@@ -15,6 +15,7 @@
 #include "fft_ops.h"
 #include "gemm_f64.cuh"
 #include "gsphere.hpp"
+#include "lanczos_kernels.cuh"
 
 namespace {
 
@@ -263,7 +264,7 @@ int ensure_W(west_ctx* c, int n_slots, int f32) {
 }
 
 int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, long long lda, const double* B, long long ldb,
-                   double* C, long long ldc) {
+                   double* C, long long ldc, int n_batch = 1, long long sA = 0, long long sB = 0, long long sC = 0, bool zero_c = true) {
     using namespace wgemm;
     if (M <= 0 || Nn <= 0) return WEST_OK;
     static bool attr = false;
@@ -275,7 +276,7 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
     const int tm = (M + BM - 1) / BM, tn = (Nn + BN - 1) / BN;
     // split K so that the CTA count fills whole waves of the 148 SMs (MINB CTAs per SM): pick the split count with
     // the best wave efficiency, each split keeping at least 32 k-steps
-    const long long tiles = (long long)tm * tn;
+    const long long tiles = (long long)tm * tn * n_batch;
     const long long max_splits = std::max<long long>(1, std::min<long long>(16, K / (32 * BK)));
     long long splits = 1;
     double best = -1.0;
@@ -287,10 +288,10 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
     long long kps = (K + splits - 1) / splits;
     kps = (kps + BK - 1) / BK * BK;
     splits = (K + kps - 1) / kps;
-    CK(cudaMemsetAsync(C, 0, (size_t)M * ldc * sizeof(double), c->st));
-    dim3 grid(tn, tm, (unsigned)splits);
+    if (zero_c) CK(cudaMemsetAsync(C, 0, (size_t)M * ldc * sizeof(double), c->st));     // batched callers zero their own output
+    dim3 grid(tn, tm, (unsigned)(splits * n_batch));
     Prof prof_(c, PC_GEMM_TN);
-    gemm_tn_kernel<<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1);
+    gemm_tn_kernel<<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1, (int)splits, sA, sB, sC);
     CK(cudaGetLastError());
     c->launches += 1;
     return WEST_OK;
@@ -698,7 +699,7 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
 }
 
 // a1: b = -P_c (dV_i psi_v) written into R ([n_col][nvpc][n_g]; the imaginary-part vectors of nvpc = 2 stay zero)
-int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R) {
+int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R, double sign = -1.0, bool project = true) {
     const int gamma = is_gamma(c), N = c->cell.N, n_col = n_pert * c->n_occ, n_vec = n_col * nvpc;
     const long long n_g = c->hs.n_g;
     const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
@@ -710,7 +711,7 @@ int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R) {
     VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
     K2Any a{};
     a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dV = (const double*)c->dVpos.p; a.n_uslots = n_uslots;
-    K3Epi e{-1.0 / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
+    K3Epi e{sign / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
     for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
         const int ns = std::min(chunk, n_rslots - s0);
         vm.slot0 = s0; a.slot0 = s0;
@@ -719,6 +720,7 @@ int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R) {
         CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, c->W.p, e, R));
         c->launches += 2;
     }
+    if (!project) return WEST_OK;
     // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows
     if ((rc = ensure(c, c->misc, sizeof(double) * std::max(c->rows_psi, 8)))) return rc;
     std::vector<double> m1(c->rows_psi, -1.0);
@@ -985,4 +987,66 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     }
     if (stats) for (auto& e : ev) cudaEventDestroy(e);
     return ret;
+}
+
+// ============================================================================================================ Lanczos chains
+extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, const double* phi, int32_t n_steps, double* alpha, double* beta,
+                            double* norm, double* braket_opt) {
+    if (!c || n_pert < 0 || n_steps < 1 || (n_pert > 0 && (!phi || !alpha || !beta || !norm))) return fail(c, WEST_EINVAL, "west_lanczos: bad argument");
+    if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_lanczos: bad precision %d", precision);
+    if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_lanczos: west_set_vloc and west_set_states are required");
+    const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
+    if (gamma && (n_occ & 1)) return fail(c, WEST_EINVAL, "west_lanczos: WEST_GAMMA needs an even number of occupied states");
+    if (braket_opt && !gamma) return fail(c, WEST_EINVAL, "west_lanczos: brakets are implemented for WEST_GAMMA only");
+    if (n_pert == 0) return WEST_OK;
+    const long long n_g = c->hs.n_g, n3 = n3_of(c), K = 2 * n_g;
+    const int n_col = n_pert * n_occ;
+    int rc;
+    if (c->rows_kb > 0 && (rc = ensure_opmatrix(c, 0.0))) return rc;
+    for (int i = 0; i < 4; ++i)
+        if ((rc = ensure(c, c->vecs[i], sizeof(cx<double>) * n_g * n_col))) return rc;
+    if ((rc = ensure(c, c->dVpos, sizeof(double) * n3 * n_pert))) return rc;
+    if ((rc = ensure(c, c->scal, sizeof(double) * n_col + 64))) return rc;
+    cx<double>* Q = (cx<double>*)c->vecs[0].p; cx<double>* QP = (cx<double>*)c->vecs[1].p;
+    cx<double>* HQ = (cx<double>*)c->vecs[2].p; cx<double>* Q1 = (cx<double>*)c->vecs[3].p;
+    double* beta_prev = (double*)c->scal.p;
+    nat_to_pos_real<double><<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, phi, (double*)c->dVpos.p);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    // q^1 = psi_i phi_m (Eq. 16), normalised (R16)
+    if ((rc = chi0_rhs(c, n_pert, 1, Q, +1.0, false))) return rc;
+    CK(cudaMemsetAsync(QP, 0, sizeof(cx<double>) * n_g * n_col, c->st));
+    if (gamma) wlz::lz_normalize<true><<<n_col, wcg::NT, 0, c->st>>>(n_g, (double2*)Q, braket_opt ? (double2*)Q1 : nullptr, norm, beta_prev);
+    else wlz::lz_normalize<false><<<n_col, wcg::NT, 0, c->st>>>(n_g, (double2*)Q, nullptr, norm, beta_prev);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    if (braket_opt) CK(cudaMemsetAsync(braket_opt, 0, sizeof(double) * (size_t)n_occ * n_steps * n_pert * n_pert, c->st));
+    const int f32 = precision == WEST_MIXED;
+    VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_col, 0};
+    const int n_slots = gamma ? (n_col + 1) / 2 : n_col;
+    for (int l = 0; l < n_steps; ++l) {
+        if (braket_opt) {
+            // <q^1_{n i} | q^l_{m i}> for every orbital i: n_occ Gram blocks, rows of one block n_occ vectors apart (Fig. 4)
+            double* C = braket_opt + (size_t)l * n_pert * n_pert;
+            const long long sC = (long long)n_steps * n_pert * n_pert;
+            if ((rc = launch_gemm_tn(c, n_pert, n_pert, K, (const double*)Q1, (long long)n_occ * K, (const double*)Q, (long long)n_occ * K, C,
+                                     n_pert, n_occ, K, K, sC, false)))
+                return rc;
+            wlz::braket_fix<<<blocks_for((long long)n_occ * n_pert * n_pert, 256), 256, 0, c->st>>>(n_occ, n_pert, sC, C, (const double*)Q1,
+                                                                                                  (const double*)Q, (long long)n_occ * K, K);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        if ((rc = hloc_apply(c, f32, vm, n_slots, Q, HQ, nullptr, 0.0))) return rc;
+        if (c->rows_kb > 0 && (rc = lowrank_apply(c, 0, c->rows_kb, n_col, (const double*)Q, (double*)HQ, (const double*)c->coef_all.p))) return rc;
+        {
+            Prof p_(c, PC_CGVEC);
+            if (gamma) wlz::lz_step<true><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_steps, l, (const double2*)Q, (const double2*)HQ, (double2*)QP, alpha, beta, beta_prev);
+            else wlz::lz_step<false><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_steps, l, (const double2*)Q, (const double2*)HQ, (double2*)QP, alpha, beta, beta_prev);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        std::swap(Q, QP);          // QP now holds q^l (the next q^{l-1}), Q holds q^{l+1}
+    }
+    return WEST_OK;
 }
