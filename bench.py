@@ -41,6 +41,7 @@ def parse():
     ap.add_argument("--check-every", type=int, default=1, help="CG convergence poll / compaction period")
     ap.add_argument("--precond", type=int, default=1, help="0 none, 1 R4 default, 2 Teter-Payne-Allan")
     ap.add_argument("--solver", type=int, default=-1, help="0 per-frequency PCG/COCG, 1 multi-shift CG; -1 = 1 for cfg3, else 0")
+    ap.add_argument("--op", default="chi0", choices=["chi0", "lanczos"], help="chi0 = the hot path (default); lanczos = Eq. 15-19 chains (widening row)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
     return ap.parse_args()
 
@@ -200,6 +201,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if a.op == "lanczos":
+        return bench_lanczos(a, cfg, w, dV, n_pert, rank, world, barrier)
     stats = None
     for _ in range(a.warmup):
         _, _, stats = w.chi0_apply(dV, omegas, **kw)
@@ -281,6 +284,34 @@ def main():
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def bench_lanczos(a, cfg, w, phi, n_pert, rank, world, barrier, n_steps=30):
+    """Widening row SURVEY 8(f)-2: N_Lanczos = 30 chains for every (perturbation, orbital), brakets included."""
+    import torch
+    for _ in range(a.warmup):
+        w.lanczos(phi, n_steps, cfg["n_occ"], want_brakets=True)
+    barrier()
+    w.set_profile(True)
+    l0 = w.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(a.steps):
+        w.lanczos(phi, n_steps, cfg["n_occ"], want_brakets=True)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    prof = w.get_profile()
+    w.set_profile(False)
+    if rank != 0:
+        return
+    chains = n_pert * cfg["n_occ"] * world
+    print(json.dumps({"metric": "Lanczos chains/s (N_Lanczos = %d, brakets included)" % n_steps, "value": chains * a.steps / (ms * 1e-3),
+                      "unit": "chains/s", "n_gpus": world, "steps": a.steps, "warmup": a.warmup, "ms_per_step": ms / a.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": a.workload, "op": "lanczos", "n_pert_per_gpu": n_pert, "n_occ": cfg["n_occ"], "n_steps": n_steps},
+                      "h_apply_per_s": chains * n_steps * a.steps / (ms * 1e-3), "gpu_launches": int(w.launch_count() - l0),
+                      "kernel_ms_per_step": {k: round(v["ms"] / a.steps, 3) for k, v in prof.items() if v["spans"]}}))
 
 
 def aux_ncols(cfg):
