@@ -99,3 +99,27 @@ def test_gemm_tn_and_update(m, n, k):
     w.gemm_update(torch.from_numpy(Cm).cuda(), torch.from_numpy(A).cuda(), Y)
     assert relmax(Y.cpu().numpy(), Y0 + Cm[:, :n].T @ A) < 1e-12
     w.close()
+
+
+@pytest.mark.parametrize("name,with_kb", [("cfg2", True), ("cfg5", False)])
+def test_full_sphere_mode_on_the_large_grids(name, with_kb):
+    """WEST_FULL (complex vectors, one transform per vector) on the 72^3 and 144^3 grids, which the configs themselves only use
+    in WEST_GAMMA mode: fft3d and h_apply against the library FFT / the oracle's matrix-free H."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build(name, dense=False)
+    w = wb.West(p.L, p.n2max, p.N, wb.WEST_FULL)
+    assert w.n_g == p.n_full
+    w.set_vloc(torch.from_numpy(np.ascontiguousarray(p.vloc)).cuda())
+    if with_kb:
+        w.set_kb(torch.from_numpy(np.ascontiguousarray(p.beta)).cuda(), p.dcoef)
+    rng = np.random.Generator(np.random.PCG64(96))
+    c = rng.standard_normal((3, p.n_full)) + 1j * rng.standard_normal((3, p.n_full))
+    x = torch.from_numpy(c).cuda()
+    r = w.fft3d(+1, x)
+    assert relmax(r.cpu().numpy(), oham.to_real_space(c, p.fft_idx, p.N)) < TOL
+    assert relmax(w.fft3d(-1, r).cpu().numpy(), c) < TOL
+    y = w.h_apply(x).cpu().numpy()
+    ref = oham.apply_h(c, p.miller, p.L, p.N, p.vloc, p.beta if with_kb else None, p.dcoef if with_kb else None)
+    assert relmax(y, ref) < TOL
+    w.close()
