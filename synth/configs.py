@@ -17,6 +17,9 @@ CONFIGS = {
     # BASELINE.json configs[0]
     "cfg1": dict(cfg=1, L=10.0, ecut=10.0, n2max=25, N=24, mode="full", lattice="random", n_atoms=2,
                  projectors="s", n_occ=8, n_pert=4, omegas=[0.0], vloc="random", precision="fp64"),
+    # config-1 cell with real orbitals (Gamma storage): small enough for a dense chi0 matrix in the PDEP oracle
+    "tinyg": dict(cfg=11, L=10.0, ecut=10.0, n2max=25, N=24, mode="gamma", lattice="random", n_atoms=2,
+                  projectors="s", n_occ=8, n_pert=4, omegas=[0.0], vloc="random", precision="fp64"),
     # reduced Si-like cell: one diamond cell, everything else as configs 2-4
     "mini2": dict(cfg=12, L=10.25, ecut=25.0, n2max=66, N=36, mode="gamma", lattice="diamond", ncell=1,
                   n_atoms=8, projectors="sp", n_occ=16, n_pert=6, omegas=[0.0], vloc="epm", precision="fp64"),
