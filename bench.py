@@ -41,7 +41,8 @@ def parse():
     ap.add_argument("--check-every", type=int, default=1, help="CG convergence poll / compaction period")
     ap.add_argument("--precond", type=int, default=1, help="0 none, 1 R4 default, 2 Teter-Payne-Allan")
     ap.add_argument("--solver", type=int, default=-1, help="0 per-frequency PCG/COCG, 1 multi-shift CG; -1 = 1 for cfg3, else 0")
-    ap.add_argument("--op", default="chi0", choices=["chi0", "lanczos"], help="chi0 = the hot path (default); lanczos = Eq. 15-19 chains (widening row)")
+    ap.add_argument("--op", default="chi0", choices=["chi0", "lanczos", "pdep"],
+                    help="chi0 = the hot path (default); lanczos = Eq. 15-19 chains; pdep = Davidson shell for chi0bar (widening rows)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
     return ap.parse_args()
 
@@ -203,6 +204,8 @@ def main():
 
     if a.op == "lanczos":
         return bench_lanczos(a, cfg, w, dV, n_pert, rank, world, barrier)
+    if a.op == "pdep":
+        return bench_pdep(a, cfg, w, alpha, n_pert, rank, world, barrier)
     stats = None
     for _ in range(a.warmup):
         _, _, stats = w.chi0_apply(dV, omegas, **kw)
@@ -312,6 +315,30 @@ def bench_lanczos(a, cfg, w, phi, n_pert, rank, world, barrier, n_steps=30):
                       "config": {"workload": a.workload, "op": "lanczos", "n_pert_per_gpu": n_pert, "n_occ": cfg["n_occ"], "n_steps": n_steps},
                       "h_apply_per_s": chains * n_steps * a.steps / (ms * 1e-3), "gpu_launches": int(w.launch_count() - l0),
                       "kernel_ms_per_step": {k: round(v["ms"] / a.steps, 3) for k, v in prof.items() if v["spans"]}}))
+
+
+def bench_pdep(a, cfg, w, alpha, n_pdep, rank, world, barrier):
+    """Widening row SURVEY 8(f)-3: wstat-like run, N_PDEP leading eigenpotentials of chi0bar by Davidson (residual 1e-4, CG tol 1e-8)."""
+    import torch
+    from paper_2203_05623_b200 import pdep as gp
+    out = None
+    for _ in range(a.warmup):
+        out = gp.pdep(w, n_pdep, cfg["n_occ"], alpha, tol=1e-4, tol_cg=TOL)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        out = gp.pdep(w, n_pdep, cfg["n_occ"], alpha, tol=1e-4, tol_cg=TOL)
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / a.steps
+    if rank != 0:
+        return
+    lam, _, res, n_app = out
+    print(json.dumps({"metric": "PDEP Davidson time (N_PDEP = %d, residual 1e-4)" % n_pdep, "value": dt, "unit": "s", "n_gpus": world,
+                      "steps": a.steps, "warmup": a.warmup, "ms_per_step": dt * 1e3, "higher_is_better": False, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": a.workload, "op": "pdep", "n_pdep": n_pdep, "chi0_applications": int(n_app),
+                                 "lambda_min": float(lam[0]), "lambda_max_kept": float(lam[-1]), "max_residual": float(res.max())},
+                      "chi0_applications_per_s": n_app / dt}))
 
 
 def aux_ncols(cfg):
