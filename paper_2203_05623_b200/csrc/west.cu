@@ -867,8 +867,12 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     CK(cudaGetLastError());
     c->launches += 1;
 
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
-    if (stats) for (auto& e : ev) CK(cudaEventCreate(&e));
+    struct Events {                      // destroyed on every return path
+        cudaEvent_t e[4] = {nullptr, nullptr, nullptr, nullptr};
+        ~Events() { for (auto x : e) if (x) cudaEventDestroy(x); }
+        cudaEvent_t& operator[](int i) { return e[i]; }
+    } ev;
+    if (stats) for (auto& e : ev.e) CK(cudaEventCreate(&e));
     int ret = WEST_OK;
     auto copy_dpsi = [&](int w, int mode, const cx<double>* Xw) -> int {
         // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 (per-frequency solver) the imaginary part is zero
@@ -943,7 +947,6 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             add_times();
             stats->iters = iters; stats->n_unconverged = (int)h[1]; stats->resid_max = h[0]; stats->n_h_apply = n_h;
         }
-        if (stats) for (auto& e : ev) cudaEventDestroy(e);
         return ret;
     }
 
@@ -985,7 +988,6 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             if (c->h_pinned[0] > 0) ret = WEST_NOTCONVERGED;
         }
     }
-    if (stats) for (auto& e : ev) cudaEventDestroy(e);
     return ret;
 }
 
