@@ -12,6 +12,10 @@
 #ifndef WEST_ZNT
 #define WEST_ZNT 256
 #endif
+#ifndef WEST_NW_H
+#define WEST_NW_H WEST_NW
+#define WEST_MINB_H WEST_MINB
+#endif
 
 namespace {
 constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, NW = WEST_NW, LPW = K2Cfg<N1, N2>::LPW;
@@ -49,8 +53,11 @@ cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
 template <typename T, int MODE>
 cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
     using K = K2<T, N1, N2, MODE, LPW>;
-    auto kern = k2_planes<T, N1, N2, MODE, NW, WEST_MINB>;
-    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + NW * LPW) * K::PITCH + 2 * NN);
+    // the H*psi variant may use a different CTA shape from the one-way variants (store / dn / load)
+    constexpr int NWm = MODE == K2_H ? WEST_NW_H : NW;
+    constexpr int MBm = MODE == K2_H ? WEST_MINB_H : WEST_MINB;
+    auto kern = k2_planes<T, N1, N2, MODE, NWm, MBm>;
+    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + NWm * LPW) * K::PITCH + 2 * NN);
     cudaError_t e = set_smem(kern, bytes);
     if (e != cudaSuccess) return e;
     K2Args<T> t;
@@ -58,7 +65,7 @@ cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a
     t.V = reinterpret_cast<const T*>(a.V);
     t.R = a.R; t.ucache = a.ucache; t.dV = a.dV; t.dn = a.dn; t.n_uslots = a.n_uslots; t.slot0 = a.slot0; t.fac = a.fac;
     dim3 grid(NN, n_slots);
-    kern<<<grid, NW * 32, bytes, st>>>(g, t);
+    kern<<<grid, NWm * 32, bytes, st>>>(g, t);
     return cudaGetLastError();
 }
 
