@@ -308,9 +308,11 @@ struct K2 {
                 Dft<T, N2, +1>::run(v);
             }
             if (MODE == K2_H) {
-                const T* V = a.V + r0;
+                // V_loc is stored with the x position transposed inside each line ([pz][py][k2][k1] instead of [k1][k2]) so that for
+                // a fixed j the lanes of a line (k1 = 0..N1-1) read consecutive words: whole sectors instead of one word per sector
+                const T* V = a.V + ((long long)pz * N + py) * N + k1;
 #pragma unroll
-                for (int j = 0; j < N2; ++j) { const T w = V[j]; v[j].x *= w; v[j].y *= w; }
+                for (int j = 0; j < N2; ++j) { const T w = V[j * N1]; v[j].x *= w; v[j].y *= w; }
             } else if (MODE == K2_TOR) {
                 cx<double>* R = a.R + (long long)slot * n3 + r0;
 #pragma unroll
@@ -450,53 +452,62 @@ __global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k3_r2g_z(WestGeom g, Vec
     K::phaseC(threadIdx.x, blockDim.x, lines, g, vm, slot, u0, e, Y);
 }
 
-// Plane kernel.  NW warps per CTA; each warp owns LPW = 32 / max(N1, N2) lines at a time and runs the three passes of
-// "its" lines with warp-level barriers only, so the CTA synchronises just twice (after y inverse, before y forward).
-template <int N1, int N2> struct K2Cfg { static constexpr int LPW = 32 / (N1 > N2 ? N1 : N2); };
+// Plane kernel.  NW warps per CTA in groups of GW warps (GW = 1 or 2); each group owns LPG = 32 GW / max(N1, N2) lines at a
+// time and runs the three passes of "its" lines with group-level barriers only (__syncwarp, or a named barrier for a warp
+// pair), so the CTA synchronises just twice (after y inverse, before y forward).  Warp pairs raise the lane utilisation of the
+// passes: at N = 72 a warp holds 3 lines (27 / 24 of 32 lanes busy), a pair holds 7 (63 / 56 of 64).
+template <int N1, int N2, int GW = 1> struct K2Cfg { static constexpr int LPW = 32 * GW / (N1 > N2 ? N1 : N2); };
 
-template <typename T, int N1, int N2, int MODE, int NW, int MINB>
+template <int GW>
+__device__ __forceinline__ void group_sync(int group) {
+    if (GW == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(GW * 32) : "memory");
+}
+
+template <typename T, int N1, int N2, int MODE, int NW, int MINB, int GW = 1>
 __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T> a) {
-    constexpr int LPW = K2Cfg<N1, N2>::LPW;
-    using K = K2<T, N1, N2, MODE, LPW>;
+    constexpr int LPG = K2Cfg<N1, N2, GW>::LPW, GT = GW * 32, NG = NW / GW;
+    static_assert(NW % GW == 0 && (GW == 1 || NG <= 15), "warp-pair groups use named barriers 1..15");
+    using K = K2<T, N1, N2, MODE, LPG>;
     constexpr int N = K::N;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);
     cx<T>* X = S + g.nr * K::PITCH;
-    cx<T>* tw = X + NW * LPW * K::PITCH;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    cx<T>* Xw = X + warp * LPW * K::PITCH;
+    cx<T>* tw = X + NG * LPG * K::PITCH;
+    const int group = threadIdx.x / GT, gt = threadIdx.x - group * GT;
+    cx<T>* Xw = X + group * LPG * K::PITCH;
     load_tw<T, N1, N2>(tw, g.tw);
     const int pz = blockIdx.x, slot = blockIdx.y;
     cx<T>* Wp = a.W + ((long long)slot * N + pz) * g.n_cols;
     __syncthreads();
     if (MODE != K2_FROMR) {
-        for (int r0 = warp * LPW; r0 < g.nr; r0 += NW * LPW) {
-            const int nrow = g.nr - r0 < LPW ? g.nr - r0 : LPW;
-            K::yA(lane, 32, S, tw, g, Wp, r0, nrow);
-            __syncwarp();
-            K::yB(lane, 32, S, g, r0, nrow);
+        for (int r0 = group * LPG; r0 < g.nr; r0 += NG * LPG) {
+            const int nrow = g.nr - r0 < LPG ? g.nr - r0 : LPG;
+            K::yA(gt, GT, S, tw, g, Wp, r0, nrow);
+            group_sync<GW>(group);
+            K::yB(gt, GT, S, g, r0, nrow);
         }
         __syncthreads();
     }
-    for (int py0 = warp * LPW; py0 < N; py0 += NW * LPW) {
+    for (int py0 = group * LPG; py0 < N; py0 += NG * LPG) {
         if (MODE != K2_FROMR) {
-            K::xA(lane, 32, S, Xw, tw, g, py0);
-            __syncwarp();
+            K::xA(gt, GT, S, Xw, tw, g, py0);
+            group_sync<GW>(group);
         }
-        K::xB(lane, 32, Xw, tw, a, slot, pz, py0);
+        K::xB(gt, GT, Xw, tw, a, slot, pz, py0);
         if (MODE == K2_H || MODE == K2_FROMR) {
-            __syncwarp();
-            K::xC(lane, 32, S, Xw, g, py0);
+            group_sync<GW>(group);
+            K::xC(gt, GT, S, Xw, g, py0);
         }
-        __syncwarp();
+        group_sync<GW>(group);
     }
     if (MODE == K2_H || MODE == K2_FROMR) {
         __syncthreads();
-        for (int r0 = warp * LPW; r0 < g.nr; r0 += NW * LPW) {
-            const int nrow = g.nr - r0 < LPW ? g.nr - r0 : LPW;
-            K::yC(lane, 32, S, tw, g, r0, nrow);
-            __syncwarp();
-            K::yD(lane, 32, S, g, Wp, r0, nrow);
+        for (int r0 = group * LPG; r0 < g.nr; r0 += NG * LPG) {
+            const int nrow = g.nr - r0 < LPG ? g.nr - r0 : LPG;
+            K::yC(gt, GT, S, tw, g, r0, nrow);
+            group_sync<GW>(group);
+            K::yD(gt, GT, S, g, Wp, r0, nrow);
         }
     }
 }

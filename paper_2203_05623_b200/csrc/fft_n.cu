@@ -16,6 +16,9 @@
 #define WEST_NW_H WEST_NW
 #define WEST_MINB_H WEST_MINB
 #endif
+#ifndef WEST_GW_H
+#define WEST_GW_H 1         // warps per line group of the H*psi plane kernel (2 = warp pairs)
+#endif
 
 namespace {
 constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, NW = WEST_NW, LPW = K2Cfg<N1, N2>::LPW;
@@ -52,12 +55,14 @@ cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
 }
 template <typename T, int MODE>
 cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
-    using K = K2<T, N1, N2, MODE, LPW>;
     // the H*psi variant may use a different CTA shape from the one-way variants (store / dn / load)
     constexpr int NWm = MODE == K2_H ? WEST_NW_H : NW;
     constexpr int MBm = MODE == K2_H ? WEST_MINB_H : WEST_MINB;
-    auto kern = k2_planes<T, N1, N2, MODE, NWm, MBm>;
-    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + NWm * LPW) * K::PITCH + 2 * NN);
+    constexpr int GWm = MODE == K2_H ? WEST_GW_H : 1;
+    constexpr int LPG = K2Cfg<N1, N2, GWm>::LPW;
+    using K = K2<T, N1, N2, MODE, LPG>;
+    auto kern = k2_planes<T, N1, N2, MODE, NWm, MBm, GWm>;
+    const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + (NWm / GWm) * LPG) * K::PITCH + 2 * NN);
     cudaError_t e = set_smem(kern, bytes);
     if (e != cudaSuccess) return e;
     K2Args<T> t;

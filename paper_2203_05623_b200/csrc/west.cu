@@ -140,13 +140,15 @@ inline bool is_gamma(const west_ctx* c) { return c->cell.mode == WEST_GAMMA; }
 __device__ __forceinline__ int j_of_p(int p, int N1, int N2) { return p / N2 + N1 * (p % N2); }
 
 // natural [b][ix][iy][iz] real f64 -> position order [b][pz][py][px] (T)
+// xt != 0: the x position inside each line is stored transposed (index k2 N1 + k1 for position N2 k1 + k2): the V_loc layout
 template <typename T>
-__global__ void nat_to_pos_real(int N, int N1, int N2, long long total, const double* in, T* out) {
+__global__ void nat_to_pos_real(int N, int N1, int N2, long long total, const double* in, T* out, int xt = 0) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
     const long long n3 = (long long)N * N * N, b = i / n3;
     long long r = i - b * n3;
-    const int px = (int)(r % N); r /= N;
+    int px = (int)(r % N); r /= N;
+    if (xt) px = N2 * (px % N1) + px / N1;
     const int py = (int)(r % N); const int pz = (int)(r / N);
     const int ix = j_of_p(px, N1, N2), iy = j_of_p(py, N1, N2), iz = j_of_p(pz, N1, N2);
     out[i] = (T)in[b * n3 + ((long long)ix * N + iy) * N + iz];
@@ -504,8 +506,8 @@ int west_set_vloc(west_ctx* c, const double* vloc) {
         if ((rc = dev_alloc(c, (void**)&c->d_vpos, sizeof(double) * n3))) return rc;
         if ((rc = dev_alloc(c, (void**)&c->d_vpos_f, sizeof(float) * n3))) return rc;
     }
-    nat_to_pos_real<double><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos);
-    nat_to_pos_real<float><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos_f);
+    nat_to_pos_real<double><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos, 1);
+    nat_to_pos_real<float><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos_f, 1);
     CK(cudaGetLastError());
     c->launches += 2;
     c->have_vloc = true;

@@ -29,7 +29,7 @@ void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V
     std::vector<T> Vp((size_t)N * N * N);
     auto jof = [&](int p) { return p / N2 + N1 * (p % N2); };
     for (int pz = 0; pz < N; pz++) for (int py = 0; py < N; py++) for (int px = 0; px < N; px++)
-        Vp[((size_t)pz * N + py) * N + px] = (T)V[((size_t)jof(px) * N + jof(py)) * N + jof(pz)];
+        Vp[((size_t)pz * N + py) * N + (px % N2) * N1 + px / N2] = (T)V[((size_t)jof(px) * N + jof(py)) * N + jof(pz)];   // x transposed in-line
     using KA = K1<T, N1, N2, GAMMA, CU>; using KC = K3<T, N1, N2, GAMMA, CU>; using KB = K2<T, N1, N2, K2_H, LC>;
     std::vector<cx<T>> lines(KA::NL * KA::PITCH);
     for (int slot = 0; slot < nslots; slot++) for (int u0 = 0; u0 < s.n_units; u0 += CU) {
