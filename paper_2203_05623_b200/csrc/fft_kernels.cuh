@@ -12,6 +12,10 @@
 #pragma once
 #include "dft_small.cuh"
 
+#ifndef WEST_PAD
+#define WEST_PAD 1        // row padding (complex elements) of every shared-memory line buffer
+#endif
+
 struct WestGeom {
     int N, n_max, nr, n_cols, n_units, gamma;
     long long n_g;
@@ -42,7 +46,7 @@ template <int N1, int N2> WHD constexpr bool keep_n1(int n1) {
 // ---------------------------------------------------------------------------------------------------------------- K1
 template <typename T, int N1, int N2, bool GAMMA, int CU>
 struct K1 {
-    static constexpr int N = N1 * N2, PITCH = N + 1, NF = GAMMA ? 2 : 1, NL = CU * NF;
+    static constexpr int N = N1 * N2, PITCH = N + WEST_PAD, NF = GAMMA ? 2 : 1, NL = CU * NF;
     static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + 2 * N);
 
     // phase A: strided DFT-N1 straight from the sphere coefficients, twiddle, store to the line buffer
@@ -124,7 +128,7 @@ struct K3Epi {
 
 template <typename T, int N1, int N2, bool GAMMA, int CU>
 struct K3 {
-    static constexpr int N = N1 * N2, PITCH = N + 1, NF = GAMMA ? 2 : 1, NL = CU * NF;
+    static constexpr int N = N1 * N2, PITCH = N + WEST_PAD, NF = GAMMA ? 2 : 1, NL = CU * NF;
     static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + 2 * N);
 
     static WHD void phaseA(int tid, int nthr, cx<T>* lines, const WestGeom& g, int slot, int u0, const cx<T>* W) {
@@ -241,7 +245,7 @@ struct K2Args {
 
 template <typename T, int N1, int N2, int MODE, int LC>
 struct K2 {
-    static constexpr int N = N1 * N2, PITCH = N + 1;
+    static constexpr int N = N1 * N2, PITCH = N + WEST_PAD;
     static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + 2 * N); }
 
     static WHD cx<T> load_disc(const cx<T>* Wp, const WestGeom& g, int row, int n) {
