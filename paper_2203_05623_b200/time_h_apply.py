@@ -1,0 +1,28 @@
+"""Times the kernel classes of west_h_apply on the cfg-2 cell with random vectors (no KB): `python -m paper_2203_05623_b200.time_h_apply`.
+A small fixed workload for ncu captures of the FFT kernels (8192 real vectors = 4096 transform slots, chunks of 2048 slots)."""
+import torch
+
+import synth
+
+from . import WEST_GAMMA, West
+
+
+def main(n_vec=8192, reps=5):
+    cfg = synth.get_config("cfg2")
+    w = West(cfg["L"], cfg["n2max"], cfg["N"], WEST_GAMMA)
+    g = torch.Generator(device="cuda").manual_seed(1)
+    w.set_vloc(torch.randn((cfg["N"],) * 3, dtype=torch.float64, device="cuda", generator=g))
+    x = torch.randn((n_vec, w.n_g), dtype=torch.float64, device="cuda", generator=g) + 0j
+    y = torch.empty_like(x)
+    for _ in range(2):
+        w.h_apply(x, y)
+    w.set_profile(True)
+    for _ in range(reps):
+        w.h_apply(x, y)
+    p = w.get_profile()
+    print({k: round(v["ms"] / reps, 3) for k, v in p.items() if v["spans"]})
+    w.close()
+
+
+if __name__ == "__main__":
+    main()
