@@ -35,6 +35,17 @@ struct VecMap {
 template <typename T> WHD cx<T> cvt(cx<double> a) { return mk<T>((T)a.x, (T)a.y); }
 template <typename T> WHD cx<double> cvd(cx<T> a) { return mk<double>((double)a.x, (double)a.y); }
 WHD int wrap_signed(int n, int N) { return n < N / 2 ? n : n - N; }
+
+#ifndef WEST_TW_POW
+#define WEST_TW_POW 1     // 1: level twiddles w^(m k) as powers of ONE table entry per thread (FP64 work traded for L1TEX wavefronts)
+#endif
+// zp[m] = z^m for m = 1 .. R-1 by binary splitting (dependency depth log2 R)
+template <typename T, int R> WHD void tw_powers(cx<T> z, cx<T> (&zp)[R]) {
+    zp[0] = mk<T>(1, 0);
+    if (R > 1) zp[1] = z;
+#pragma unroll
+    for (int m = 2; m < R; ++m) zp[m] = cmul(zp[m / 2], zp[m - m / 2]);
+}
 // Alias-free grids have N >= 4 n_max + 1, so every non-zero frequency satisfies |n| <= (N-1)/4.  For the strided pass
 // (n = N2 n1 + n2) this tells at COMPILE time which n1 can hold a non-zero input / a needed output at all.
 template <int N1, int N2> WHD constexpr bool keep_n1(int n1) {
@@ -82,8 +93,15 @@ struct K1 {
                 for (int n1 = 0; n1 < N1; ++n1) v[n1] = mk<T>(0, 0);
             }
             cx<T>* dst = lines + line * PITCH + n2;
+if (WEST_TW_POW) {
+                cx<T> zp[N1];
+                tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
+            } else {
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+            }
         }
     }
     // phase B: contiguous DFT-N2
@@ -177,8 +195,15 @@ struct K3 {
 #pragma unroll
             for (int j = 0; j < N2; ++j) v[j] = p[j];
             Dft<T, N2, -1>::run(v);
+if (WEST_TW_POW) {
+                cx<T> zp[N2];
+                tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+            }
         }
     }
     // phase A': strided DFT-N1 (sign -), epilogue to the sphere
@@ -262,8 +287,15 @@ struct K2 {
             for (int n1 = 0; n1 < N1; ++n1) v[n1] = keep_n1<N1, N2>(n1) ? load_disc(Wp, g, row, N2 * n1 + n2) : mk<T>(0, 0);
             Dft<T, N1, +1>::run(v);
             cx<T>* dst = S + row * PITCH + n2;
+if (WEST_TW_POW) {
+                cx<T> zp[N1];
+                tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
+            } else {
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+            }
         }
     }
     static WHD void yB(int tid, int nthr, cx<T>* S, const WestGeom& g, int row0, int nrow) {
@@ -292,8 +324,15 @@ struct K2 {
             }
             Dft<T, N1, +1>::run(v);
             cx<T>* dst = X + l * PITCH + n2;
+if (WEST_TW_POW) {
+                cx<T> zp[N1];
+                tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
+            } else {
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+            }
         }
     }
     // x inverse pass B, the real-space operation, x forward pass B' - all on the same N2 contiguous values
@@ -351,8 +390,15 @@ struct K2 {
                 }
             }
             Dft<T, N2, -1>::run(v);
+if (WEST_TW_POW) {
+                cx<T> zp[N2];
+                tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+            }
         }
     }
     // x forward pass A': strided DFT-N1, keep |n_x| <= n_max, back into S
@@ -382,8 +428,15 @@ struct K2 {
 #pragma unroll
             for (int j = 0; j < N2; ++j) v[j] = p[j];
             Dft<T, N2, -1>::run(v);
+if (WEST_TW_POW) {
+                cx<T> zp[N2];
+                tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+            }
         }
     }
     static WHD void yD(int tid, int nthr, const cx<T>* S, const WestGeom& g, cx<T>* Wp, int row0, int nrow) {
