@@ -7,8 +7,8 @@ import synth
 from . import WEST_GAMMA, West
 
 
-def main(n_vec=8192, reps=5):
-    cfg = synth.get_config("cfg2")
+def main(n_vec=8192, reps=5, workload="cfg2"):
+    cfg = synth.get_config(workload)
     w = West(cfg["L"], cfg["n2max"], cfg["N"], WEST_GAMMA)
     g = torch.Generator(device="cuda").manual_seed(1)
     w.set_vloc(torch.randn((cfg["N"],) * 3, dtype=torch.float64, device="cuda", generator=g))
@@ -25,4 +25,8 @@ def main(n_vec=8192, reps=5):
 
 
 if __name__ == "__main__":
-    main()
+    import sys
+    if len(sys.argv) > 1 and sys.argv[1] == "cfg5":
+        main(n_vec=1024, reps=3, workload="cfg5")
+    else:
+        main()
