@@ -502,6 +502,16 @@ __global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k3_r2g_z(WestGeom g, Vec
     cx<T>* tw = lines + K::NL * K::PITCH;
     load_tw<T, N1, N2>(tw, g.tw);
     const int slot = blockIdx.y, u0 = blockIdx.x * CU;
+    if (e.kinetic) {
+        // the epilogue reads x(G) of this CTA's sticks at the very end: pull those lines towards L2 now (128 B per request)
+        for (int it = threadIdx.x; it < K::NL * 5; it += blockDim.x) {
+            const int line = it / 5, seg = it - line * 5;
+            const int u = u0 + line / K::NF, f = line % K::NF;
+            const long long vec = (long long)(vm.slot0 + slot) * vm.vstride + (long long)f * vm.voffb;
+            if (u < g.n_units && vec < vm.n_vec && seg * 8 <= 2 * g.unit_zmax[u])
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(e.X + vec * g.n_g + g.unit_off[u] + seg * 8));
+        }
+    }
     K::phaseA(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
     __syncthreads();
     K::phaseB(threadIdx.x, blockDim.x, lines, tw);
