@@ -43,6 +43,7 @@ def parse():
     ap.add_argument("--solver", type=int, default=-1, help="0 per-frequency PCG/COCG, 1 multi-shift CG; -1 = 1 for cfg3, else 0")
     ap.add_argument("--op", default="chi0", choices=["chi0", "lanczos", "pdep"],
                     help="chi0 = the hot path (default); lanczos = Eq. 15-19 chains; pdep = Davidson shell for chi0bar (widening rows)")
+    ap.add_argument("--deflate", type=int, default=0, help="number of conduction eigenstates handed to west_set_deflation (0 = off)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
     return ap.parse_args()
 
@@ -94,7 +95,7 @@ def build_inputs(cfg):
     return atoms, vloc
 
 
-def setup_gpu(cfg, n_pert, chunk, verbose):
+def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0):
     import torch
     import synth
     import paper_2203_05623_b200 as wb
@@ -114,8 +115,12 @@ def setup_gpu(cfg, n_pert, chunk, verbose):
     w.set_vloc(torch.from_numpy(vloc).to(dev))
     w.set_kb(torch.from_numpy(np.ascontiguousarray(beta)).to(dev), dcoef)
     t0 = time.time()
-    eps, psi, res = eigs.lowest_states(w, cfg["n_occ"], tol=1e-10, verbose=False)
-    gap = float(eps[cfg["n_occ"]] - eps[cfg["n_occ"] - 1])
+    n_occ = cfg["n_occ"]
+    eps, psi, res = eigs.lowest_states(w, n_occ + n_defl, tol=1e-10, verbose=False)
+    gap = float(eps[n_occ] - eps[n_occ - 1])
+    if n_defl:
+        w.set_deflation(psi[n_occ:n_occ + n_defl].contiguous(), eps[n_occ:n_occ + n_defl])
+        psi = psi[:n_occ].contiguous()
     if verbose:
         print("# eigensolver: %.1f s, residual %.2e, gap %.4f Ry" % (time.time() - t0, res, gap), file=sys.stderr)
     w.set_states(psi, eps[:cfg["n_occ"]])
@@ -187,7 +192,7 @@ def main():
     import paper_2203_05623_b200 as wb
     precision = wb.WEST_MIXED if cfg["precision"] == "mixed" else wb.WEST_FP64
     # every rank: same cell and orbitals, its own block of perturbations (seeded stream offset by rank)
-    w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0))
+    w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0), n_defl=a.deflate)
     if world > 1:
         dV_np = synth.perturbations(cfg, n_pert=n_pert, first=rank * n_pert)
     dev = torch.device("cuda")
@@ -268,7 +273,7 @@ def main():
         "dtype": "f64" if precision == wb.WEST_FP64 else "f32 FFT / f64 vectors",
         "data": "synthetic (seeded Si-like cell, GPU-computed orbitals)",
         "config": {"workload": a.workload, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": len(omegas),
-                   "n_proj": cfg["n_proj"], "tol": TOL, "solver": "multi-shift CG" if solver == 1 else "PCG/COCG per frequency", "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
+                   "n_proj": cfg["n_proj"], "n_deflated": a.deflate, "tol": TOL, "solver": "multi-shift CG" if solver == 1 else "PCG/COCG per frequency", "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
                    "gap_ry": aux["gap"], "l2": "inputs per step (4 vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
         "h_apply_per_s": n_h * world / (ms * 1e-3),
         "e2e": {"value": units * a.steps / (e2e_ms * 1e-3), "unit": "perturbations/s",

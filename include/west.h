@@ -107,6 +107,14 @@ int  west_set_vloc  (west_ctx* ctx, const double* vloc);
 int  west_set_kb    (west_ctx* ctx, int32_t n_proj, const void* beta, const double* dcoef_host);
 int  west_set_states(west_ctx* ctx, int32_t n_occ, const void* psi, const double* eps_host);
 
+/* Optional deflation for west_chi0_apply (not in the paper; exact, not a truncation): n_defl eigenstates of H directly ABOVE the
+ * occupied ones (psi_c [n_defl][n_g] c128 orthonormal, device; eps_c [n_defl] HOST), e.g. the guard states an eigensolver returns
+ * anyway.  Their part of every solution is added in closed form, dpsi_low = - sum_c psi_c <psi_c|dV psi_v> / (eps_c - eps_v - i omega),
+ * and the CG runs on the complement (the states join P_v in the alpha-projector and the right-hand side is projected off them), so
+ * the smallest eigenvalue of the Sternheimer operator rises from the gap to eps_(first state not given) - eps_v and the iteration
+ * count drops.  Costs n_defl more rows in the projector GEMMs.  n_defl = 0 switches it off.  The result is unchanged (tested). */
+int  west_set_deflation(west_ctx* ctx, int32_t n_defl, const void* psi_c, const double* eps_c_host);
+
 /* Sphere-truncated 3D FFT (R10).
  * dir = +1: in = coefficients [n_batch][n_g] c128, out = grids.   dir = -1: in = grids, out = coefficients.
  * WEST_FULL:  grids are complex [n_batch][N^3] c128.

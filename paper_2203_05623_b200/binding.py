@@ -32,7 +32,7 @@ class west_stats(C.Structure):
                 ("ms_rhs", C.c_float), ("ms_cg", C.c_float), ("ms_dn", C.c_float)]
 
 
-EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states",
+EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
            "west_fft3d", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
            "west_launch_count", "west_set_fft_chunk", "west_set_profile", "west_get_profile"]
 
@@ -50,6 +50,7 @@ def load_library():
     lib.west_set_vloc.argtypes = [vp, vp]
     lib.west_set_kb.argtypes = [vp, i32, vp, vp]
     lib.west_set_states.argtypes = [vp, i32, vp, vp]
+    lib.west_set_deflation.argtypes = [vp, i32, vp, vp]
     lib.west_fft3d.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.west_h_apply.argtypes = [vp, i32, i32, vp, vp]
     lib.west_chi0_apply.argtypes = [vp, i32, i32, vp, i32, vp, C.POINTER(west_cg_opts), vp, vp, C.POINTER(west_stats)]
@@ -150,6 +151,13 @@ class West:
         e = np.ascontiguousarray(eps, dtype=np.float64)
         assert psi.shape[1] == self.n_g and len(e) == psi.shape[0]
         self._ck(self.lib.west_set_states(self.ctx, int(psi.shape[0]), _dev(psi, torch.complex128), e.ctypes.data))
+
+    def set_deflation(self, psi_c, eps_c):
+        """n_defl eigenstates directly above the occupied ones (or None / empty to switch deflation off)."""
+        import torch
+        n = 0 if psi_c is None else int(psi_c.shape[0])
+        e = np.ascontiguousarray(eps_c if n else [], dtype=np.float64)
+        self._ck(self.lib.west_set_deflation(self.ctx, n, _dev(psi_c, torch.complex128) if n else None, e.ctypes.data if n else None))
 
     def fft3d(self, dir, x, out=None, precision=WEST_FP64):
         import torch

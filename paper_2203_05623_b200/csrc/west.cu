@@ -51,6 +51,10 @@ struct west_ctx {
     bool have_vloc = false;
     int n_proj = 0, n_occ = 0;
     int rows_kb = 0, rows_psi = 0;     // rows of the stacked real operator matrix (x2 in WEST_FULL)
+    int n_defl = 0, rows_defl = 0;     // optional deflation states (lowest conduction orbitals), stacked after the psi rows
+    DevBuf A_defl, eps_defl, craw, dcoef_defl;
+    long long craw_ld = 0;
+    std::vector<double> h_eps_defl;
     DevBuf A_kb, A_psi;                // [rows][2 n_g] f64 each (kept apart; concatenated lazily into A_all)
     DevBuf A_all, coef_all;            // [rows_kb + rows_psi][2 n_g], coef [rows]
     bool A_dirty = true;
@@ -319,7 +323,7 @@ int launch_gemm_update(west_ctx* c, int M, int Nn, long long K, const double* C,
 // (re)build the concatenated operator matrix [KB rows ; psi rows] and its coefficient vector
 int ensure_opmatrix(west_ctx* c, double alpha) {
     const long long K = 2 * c->hs.n_g;
-    const int rows = c->rows_kb + c->rows_psi;
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     if (rows == 0) return WEST_OK;
     if (c->A_dirty) {
         int rc = ensure(c, c->A_all, (size_t)rows * K * sizeof(double));
@@ -330,11 +334,14 @@ int ensure_opmatrix(west_ctx* c, double alpha) {
         if (c->rows_psi)
             CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)c->rows_kb * K, c->A_psi.p, (size_t)c->rows_psi * K * sizeof(double),
                                cudaMemcpyDeviceToDevice, c->st));
+        if (c->rows_defl)
+            CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)(c->rows_kb + c->rows_psi) * K, c->A_defl.p,
+                               (size_t)c->rows_defl * K * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
         c->A_dirty = false;
     }
     std::vector<double> coef(rows);
     for (int i = 0; i < c->rows_kb; ++i) coef[i] = c->h_dcoef[i];
-    for (int i = 0; i < c->rows_psi; ++i) coef[c->rows_kb + i] = alpha;
+    for (int i = 0; i < c->rows_psi + c->rows_defl; ++i) coef[c->rows_kb + i] = alpha;     // alpha (P_v + P_deflated)
     // stream-ordered copy from a pageable vector is synchronous with respect to the host buffer: safe
     CK(cudaMemcpyAsync(c->coef_all.p, coef.data(), rows * sizeof(double), cudaMemcpyHostToDevice, c->st));
     return WEST_OK;
@@ -569,6 +576,25 @@ int west_set_states(west_ctx* c, int32_t n_occ, const void* psi, const double* e
     return WEST_OK;
 }
 
+int west_set_deflation(west_ctx* c, int32_t n_defl, const void* psi_c, const double* eps_host) {
+    if (!c || n_defl < 0 || (n_defl > 0 && (!psi_c || !eps_host))) return fail(c, WEST_EINVAL, "west_set_deflation: bad argument");
+    const int full = !is_gamma(c);
+    const long long n_g = c->hs.n_g;
+    c->n_defl = n_defl;
+    c->rows_defl = n_defl * (full ? 2 : 1);
+    c->A_dirty = true;
+    if (n_defl == 0) return WEST_OK;
+    c->h_eps_defl.assign(eps_host, eps_host + n_defl);
+    int rc = ensure(c, c->A_defl, (size_t)c->rows_defl * 2 * n_g * sizeof(double));
+    if (rc) return rc;
+    if ((rc = ensure(c, c->eps_defl, sizeof(double) * n_defl))) return rc;
+    CK(cudaMemcpyAsync(c->eps_defl.p, c->h_eps_defl.data(), sizeof(double) * n_defl, cudaMemcpyHostToDevice, c->st));
+    stack_rows<<<blocks_for(n_g * n_defl, 256), 256, 0, c->st>>>(n_g, n_defl, full, (const cx<double>*)psi_c, (double*)c->A_defl.p);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+
 int west_fft3d(west_ctx* c, int32_t dir, int32_t precision, int32_t n_batch, const void* in, void* out) {
     if (!c || (dir != 1 && dir != -1) || n_batch < 0 || (n_batch > 0 && (!in || !out))) return fail(c, WEST_EINVAL, "west_fft3d: bad argument");
     if (precision != WEST_FP64) return fail(c, WEST_EINVAL, "west_fft3d: only WEST_FP64 (the FP32 variant exists inside west_h_apply only)");
@@ -651,7 +677,7 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
     wcg::cg_init<MODE><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, (const double2*)R, (double2*)P, s, colmap);
     CK(cudaGetLastError());
     c->launches += 1;
-    const int rows = c->rows_kb + c->rows_psi;
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     int n_act = n_col;          // columns currently held (compacted) in R, P, AP
     int it = 0;
     int64_t n_h = 0;
@@ -724,11 +750,57 @@ int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R, double sign = -1.
     }
     if (!project) return WEST_OK;
     // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows
-    if ((rc = ensure(c, c->misc, sizeof(double) * std::max(c->rows_psi, 8)))) return rc;
-    std::vector<double> m1(c->rows_psi, -1.0);
-    CK(cudaMemcpyAsync(c->misc.p, m1.data(), sizeof(double) * c->rows_psi, cudaMemcpyHostToDevice, c->st));
+    const int rows_p = c->rows_psi + c->rows_defl;        // P_v and, if set, the deflated conduction states
+    if ((rc = ensure(c, c->misc, sizeof(double) * std::max(rows_p, 8)))) return rc;
+    std::vector<double> m1(rows_p, -1.0);
+    CK(cudaMemcpyAsync(c->misc.p, m1.data(), sizeof(double) * rows_p, cudaMemcpyHostToDevice, c->st));
     CK(cudaStreamSynchronize(c->st));     // m1 is a stack-lifetime pageable buffer
-    return lowrank_apply(c, c->rows_kb, c->rows_psi, n_vec, (const double*)R, (double*)R, (const double*)c->misc.p);
+    if ((rc = lowrank_apply(c, c->rows_kb, rows_p, n_vec, (const double*)R, (double*)R, (const double*)c->misc.p))) return rc;
+    if (c->rows_defl > 0) {
+        // Cbuf now holds <psi_m | dV psi_v> for every projector row: keep the deflation rows for the closed-form part of the solution
+        const long long ldc = (n_vec + 1) / 2 * 2;
+        if ((rc = ensure(c, c->craw, sizeof(double) * (size_t)c->rows_defl * ldc))) return rc;
+        c->craw_ld = ldc;
+        CK(cudaMemcpyAsync(c->craw.p, (const double*)c->Cbuf.p + (size_t)c->rows_psi * ldc, sizeof(double) * (size_t)c->rows_defl * ldc,
+                           cudaMemcpyDeviceToDevice, c->st));
+    }
+    return WEST_OK;
+}
+
+// Deflation (optional, west_set_deflation): the components of the solution along the given conduction eigenstates are known in
+// closed form, dpsi_low = - sum_c psi_c <psi_c|dV psi_v> / (eps_c - eps_v - i omega); the CG runs on the complement (those states sit
+// in the alpha-projector next to P_v, the right-hand side is projected off them), which raises the smallest eigenvalue of the
+// operator from the gap to eps_(first state not deflated) - eps_v and cuts the iteration count.  Exact, not a truncation.
+__global__ void defl_coef(int rows, int mult, int n_col, int in_nvpc, int out_nvpc, int n_occ, long long ld_in, const double* Craw,
+                          long long ld_out, double* D, const double* eps_c, const double* eps_v, double omega) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int n_out = n_col * out_nvpc;
+    if (i >= (long long)rows * n_out) return;
+    const int m = (int)(i / n_out), n = (int)(i - (long long)m * n_out);
+    const int col = n / out_nvpc, part = n - col * out_nvpc;
+    const double delta = eps_c[m / mult] - eps_v[col % n_occ];
+    const double cr = Craw[(long long)m * ld_in + (long long)col * in_nvpc];
+    double d;
+    if (out_nvpc == 1) d = -cr / delta;
+    else { const double den = delta * delta + omega * omega; d = part == 0 ? -cr * delta / den : -cr * omega / den; }
+    D[(long long)m * ld_out + n] = d;
+}
+
+int add_deflated(west_ctx* c, int n_col, int in_nvpc, int out_nvpc, double omega, const double* d_eps, cx<double>* X) {
+    if (c->rows_defl == 0) return WEST_OK;
+    const long long K = 2 * c->hs.n_g;
+    const int n_out = n_col * out_nvpc;
+    const long long ldo = (n_out + 1) / 2 * 2;
+    int rc = ensure(c, c->dcoef_defl, sizeof(double) * (size_t)c->rows_defl * ldo);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(c->dcoef_defl.p, 0, sizeof(double) * (size_t)c->rows_defl * ldo, c->st));
+    defl_coef<<<blocks_for((long long)c->rows_defl * n_out, 256), 256, 0, c->st>>>(
+        c->rows_defl, is_gamma(c) ? 1 : 2, n_col, in_nvpc, out_nvpc, c->n_occ, c->craw_ld, (const double*)c->craw.p, ldo,
+        (double*)c->dcoef_defl.p, (const double*)c->eps_defl.p, d_eps, omega);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    const double* A = (const double*)c->A_all.p + (size_t)(c->rows_kb + c->rows_psi) * K;
+    return launch_gemm_update(c, c->rows_defl, n_out, K, (const double*)c->dcoef_defl.p, ldo, A, K, (double*)X, K);
 }
 
 // a10: dn_i(r) = (4/Omega) Re sum_v conj(u_v) du_iv from X ([n_col][nvpc][n_g]) into dn_out ([n_pert][N^3], natural order)
@@ -772,7 +844,7 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
     wcg::ms_init<<<n_col, wcg::NT, 0, c->st>>>(n_g, n_col, sh, (const double2*)R, (double2*)P, (double2*)PS, st, colmap);
     CK(cudaGetLastError());
     c->launches += 1;
-    const int rows = c->rows_kb + c->rows_psi;
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     int n_act = n_col, it = 0;
     int64_t n_h = 0;
     for (; it < o.max_iter; ++it) {
@@ -934,7 +1006,8 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             return rc;
         if (stats) CK(cudaEventRecord(ev[2], c->st));
         for (int w = 0; w < n_freq; ++w) {
-            const cx<double>* Xw = (const cx<double>*)c->xs.p + (size_t)w * per;
+            cx<double>* Xw = (cx<double>*)c->xs.p + (size_t)w * per;
+            if ((rc = add_deflated(c, n_col, 1, 2, omega_host[w], d_eps, Xw))) return rc;
             if ((rc = chi0_dn(c, n_pert, 2, Xw, dn + (long long)w * n_pert * n3))) return rc;
             if (dpsi_opt && (rc = copy_dpsi(w, 1, Xw))) return rc;
         }
@@ -968,6 +1041,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
         else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
         if (rc) return rc;
+        if ((rc = add_deflated(c, n_col, nvpc, nvpc, omega, d_eps, X))) return rc;
         if (stats) CK(cudaEventRecord(ev[2], c->st));
         if ((rc = chi0_dn(c, n_pert, nvpc, X, dn + (long long)w * n_pert * n3))) return rc;
         if (dpsi_opt && (rc = copy_dpsi(w, mode, X))) return rc;

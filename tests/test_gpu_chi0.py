@@ -11,11 +11,13 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-9
 
 
-def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500):
+def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500, n_defl=0):
     import torch
     import paper_2203_05623_b200 as wb
     p = oracle_problem.build(name)
     w, sel = make_west(p)
+    if n_defl:
+        w.set_deflation(torch.from_numpy(np.ascontiguousarray(p.U[:, p.n_occ:p.n_occ + n_defl].T[:, sel])).cuda(), p.eps[p.n_occ:p.n_occ + n_defl])
     dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
     prec = wb.WEST_FP64 if precision is None else precision
     om = p.omegas if omegas is None else omegas
@@ -93,3 +95,15 @@ def test_chi0_multishift_all_frequencies_from_one_krylov_sequence():
     _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
     # one H*psi per column and iteration serves all four frequencies
     assert st["n_h_apply"] <= st["iters"] * p.n_occ * len(p.dV)
+
+
+@pytest.mark.parametrize("name,solver,omegas", [("cfg1", 0, None), ("mini2", 0, None), ("mini3", 0, None), ("mini3", 1, [0.0, 0.05, 5.0])])
+def test_chi0_with_deflated_conduction_states(name, solver, omegas):
+    """west_set_deflation: same result as without (parity against the sum over states), fewer iterations."""
+    p, sel, dn0, _, st0, ref_dn, ref_dpsi = _run(name, solver=solver, omegas=omegas, max_iter=2000)
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run(name, solver=solver, omegas=omegas, max_iter=2000, n_defl=12)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    assert relmax(dn, ref_dn) < TOL
+    _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+    # at omega = 0 the smallest eigenvalue of the operator is the gap and deflation must help; large omega already lifts the spectrum
+    assert st["iters"] <= st0["iters"] and (omegas is not None or name == "mini3" or st["iters"] < st0["iters"])
