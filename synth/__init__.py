@@ -18,4 +18,5 @@ from .fields import (  # noqa: F401
     perturbations,
     vloc_for,
     atoms_for,
+    dense_grid,
 )

@@ -132,3 +132,11 @@ def perturbations(cfg, n_pert=None, first=0):
     for i in range(n_pert):
         out[i] = smooth_field(cfg["N"], cfg["L"], 1.0, 0.1, make_rng(cfg["cfg"], 2 + first + i))
     return out
+
+
+def dense_grid(n, n_batch=1, seed=7000):
+    """Complex standard-normal data on an n^3 grid, [n_batch][n][n][n] complex128: the input of the dense FFT benchmark
+    (Fig. 3: the paper times transforms of wavefunction-like data whose values do not matter for the timing)."""
+    rng = np.random.Generator(np.random.PCG64(seed + n))
+    x = rng.standard_normal((n_batch, n, n, n)) + 1j * rng.standard_normal((n_batch, n, n, n))
+    return np.ascontiguousarray(x)
