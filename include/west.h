@@ -60,6 +60,7 @@ extern "C" {
 
 #define WEST_FP64   0   /* everything in FP64 */
 #define WEST_MIXED  1   /* FFT + real-space multiply inside H*psi in FP32; vectors, GEMMs, dots, dn in FP64 */
+#define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
 typedef struct west_ctx west_ctx;
 
@@ -122,6 +123,16 @@ int  west_set_deflation(west_ctx* ctx, int32_t n_defl, const void* psi_c, const 
  *             internally; an odd trailing vector is padded).
  * r->G of data that is not sphere-limited is the truncation to S of its DFT. */
 int  west_fft3d(west_ctx* ctx, int32_t dir, int32_t precision, int32_t n_batch, const void* in, void* out);
+
+/* Dense complex-to-complex 3D FFT on an n^3 cubic grid: the operation timed in Fig. 3 (one FP64 or FP32 C2C
+ * transform of a 128^3 or 256^3 grid, data resident on the device).  Independent of the context's cell: ctx supplies the stream,
+ * the error string and the launch counter only.
+ *   out[b][k_x][k_y][k_z] = sum_r in[b][r_x][r_y][r_z] exp(sign 2 pi i k.r / n),  sign = +1 or -1, no scaling (reading R17)
+ * in, out: DEVICE pointers, [n_batch][n][n][n], z fastest, complex128 (precision = WEST_FP64) or complex64 (WEST_FP32), 16-byte
+ * (8-byte) aligned; in == out (in place) is allowed, partial overlap is not.  n must be 64, 128 or 256; n_batch <= 65535.
+ * Three launches (z, y, x passes) on the context's stream; no workspace.  Errors: WEST_EINVAL (NULL, unsupported n / precision / sign),
+ * WEST_ECUDA. */
+int  west_fft3d_dense(west_ctx* ctx, int32_t n, int32_t sign, int32_t precision, int32_t n_batch, const void* in, void* out);
 
 /* y = H x = (T + V_loc + V_NL) x for n_vec vectors, x and y [n_vec][n_g] c128 (Eq. 1).
  * x and y must not overlap.  Needs west_set_vloc; V_NL only if west_set_kb was called with n_proj > 0. */

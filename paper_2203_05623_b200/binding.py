@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(HERE, "libwest.so")
 WEST_OK, WEST_NOTCONVERGED = 0, 1
 WEST_EINVAL, WEST_ECUDA, WEST_ESTATE, WEST_ENOMEM = -1, -2, -3, -4
 WEST_FULL, WEST_GAMMA = 0, 1
-WEST_FP64, WEST_MIXED = 0, 1
+WEST_FP64, WEST_MIXED, WEST_FP32 = 0, 1, 2
 
 
 class west_cell(C.Structure):
@@ -33,7 +33,7 @@ class west_stats(C.Structure):
 
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
-           "west_fft3d", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
+           "west_fft3d", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
            "west_launch_count", "west_set_fft_chunk", "west_set_profile", "west_get_profile"]
 
 
@@ -52,6 +52,7 @@ def load_library():
     lib.west_set_states.argtypes = [vp, i32, vp, vp]
     lib.west_set_deflation.argtypes = [vp, i32, vp, vp]
     lib.west_fft3d.argtypes = [vp, i32, i32, i32, vp, vp]
+    lib.west_fft3d_dense.argtypes = [vp, i32, i32, i32, i32, vp, vp]
     lib.west_h_apply.argtypes = [vp, i32, i32, vp, vp]
     lib.west_chi0_apply.argtypes = [vp, i32, i32, vp, i32, vp, C.POINTER(west_cg_opts), vp, vp, C.POINTER(west_stats)]
     lib.west_lanczos.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp, vp]
@@ -172,6 +173,16 @@ class West:
             if out is None:
                 out = torch.empty((n_batch, self.n_g), dtype=torch.complex128, device=x.device)
             self._ck(self.lib.west_fft3d(self.ctx, -1, precision, n_batch, _dev(x, torch.float64 if self.mode == WEST_GAMMA else torch.complex128), _dev(out, torch.complex128)))
+        return out
+
+    def fft3d_dense(self, x, sign, out=None):
+        """Dense C2C FFT of x [n_batch][n][n][n] (complex128 -> WEST_FP64, complex64 -> WEST_FP32); out=x runs in place."""
+        import torch
+        assert x.dim() == 4 and x.shape[1] == x.shape[2] == x.shape[3] and x.dtype in (torch.complex128, torch.complex64)
+        if out is None:
+            out = torch.empty_like(x)
+        prec = WEST_FP64 if x.dtype == torch.complex128 else WEST_FP32
+        self._ck(self.lib.west_fft3d_dense(self.ctx, int(x.shape[1]), int(sign), prec, int(x.shape[0]), _dev(x, x.dtype), _dev(out, x.dtype)))
         return out
 
     def h_apply(self, x, out=None, precision=WEST_FP64):

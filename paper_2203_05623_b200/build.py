@@ -64,6 +64,8 @@ def build(force=False, verbose=False):
         extra = ["-DWEST_NW_H=6", "-DWEST_MINB_H=3", "-DWEST_GW_H=2"] if n == 72 else []      # measured: 6 warps x 3 CTAs is 3 % faster for the H*psi planes at N = 72 (16-24 resident warps all give 215-217 ms: pipe-bound)
         jobs.append((o, [nvcc] + NVCC_FLAGS + extra + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_NW=%d" % nw, "-DWEST_MINB=%d" % minb, "-DWEST_CU=%d" % cu, "-DWEST_ZMINB=%d" % zminb, "-DWEST_ZNT=%d" % znt,
                                                "-c", os.path.join(CSRC, "fft_n.cu"), "-o", o]))
+    o = os.path.join(OBJ, "fft_dense.o")
+    jobs.append((o, [nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "fft_dense.cu"), "-o", o]))
     o = os.path.join(OBJ, "west.o")
     jobs.append((o, [nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "west.cu"), "-o", o]))
     with cf.ThreadPoolExecutor(max_workers=min(8, len(jobs))) as ex:

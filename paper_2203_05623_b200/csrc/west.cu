@@ -8,11 +8,13 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <map>
 #include <vector>
 
 #include "../../include/west.h"
 #include "cg_kernels.cuh"
 #include "fft_ops.h"
+#include "fft_dense.h"
 #include "gemm_f64.cuh"
 #include "gsphere.hpp"
 #include "lanczos_kernels.cuh"
@@ -63,6 +65,7 @@ struct west_ctx {
     DevBuf tk;                         // [n_occ] <psi_v|T|psi_v>
     DevBuf ucache;                     // [n_uslots][N^3] c128 position order
     int n_uslots = 0;
+    std::map<int, void*> dense_tw;     // twiddle tables of west_fft3d_dense, one per grid size used
 
     // workspaces (grown lazily)
     DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst;
@@ -625,6 +628,32 @@ int west_fft3d(west_ctx* c, int32_t dir, int32_t precision, int32_t n_batch, con
         CK(cudaGetLastError());
         c->launches += 3;
     }
+    return WEST_OK;
+}
+
+int west_fft3d_dense(west_ctx* c, int32_t n, int32_t sign, int32_t precision, int32_t n_batch, const void* in, void* out) {
+    if (!c || (sign != 1 && sign != -1) || n_batch < 0 || n_batch > 65535 || (n_batch > 0 && (!in || !out)))
+        return fail(c, WEST_EINVAL, "west_fft3d_dense: bad argument");
+    if (precision != WEST_FP64 && precision != WEST_FP32) return fail(c, WEST_EINVAL, "west_fft3d_dense: precision must be WEST_FP64 or WEST_FP32");
+    if (!west_dense_fft_supported(n)) return fail(c, WEST_EINVAL, "west_fft3d_dense: n = %d is not built (64, 128, 256)", n);
+    if (n_batch == 0) return WEST_OK;
+    auto it = c->dense_tw.find(n);
+    if (it == c->dense_tw.end()) {
+        std::vector<cx<double>> tw(n);
+        for (int i = 0; i < n; ++i) {
+            const double a = 2.0 * 3.14159265358979323846264338327950288 * (double)i / (double)n;
+            tw[i].x = std::cos(a); tw[i].y = std::sin(a);
+        }
+        tw[0] = mk<double>(1, 0); tw[n / 4] = mk<double>(0, 1); tw[n / 2] = mk<double>(-1, 0); tw[3 * n / 4] = mk<double>(0, -1);
+        void* d = nullptr;
+        int rc = dev_alloc(c, &d, sizeof(cx<double>) * n);
+        if (rc) return rc;
+        CK(cudaMemcpy(d, tw.data(), sizeof(cx<double>) * n, cudaMemcpyHostToDevice));
+        it = c->dense_tw.emplace(n, d).first;
+    }
+    Prof pf(c, PC_FFT_OTHER);
+    CK(west_dense_fft3d(n, precision == WEST_FP32, sign, n_batch, c->st, in, out, it->second));
+    c->launches += 3;
     return WEST_OK;
 }
 
