@@ -24,8 +24,10 @@ def rhs_vectors(U_occ, dV, fft_idx, N):
     return np.stack([ham.to_g_space(dV[i][None] * u, fft_idx) for i in range(len(dV))])
 
 
-def chi0_sum_over_states(eps, U, n_occ, dV, omegas, miller, L, N, return_dpsi=False):
-    """dn[w, i, N, N, N] (real, e/bohr^3) for every frequency omega_w >= 0 (imaginary axis) and perturbation i."""
+def chi0_sum_over_states(eps, U, n_occ, dV, omegas, miller, L, N, return_dpsi=False, occupation=2.0):
+    """dn[w, i, N, N, N] (real, e/bohr^3) for every frequency omega_w >= 0 (imaginary axis) and perturbation i.
+    occupation: electrons per orbital, 2 for a spin-unpolarised system, 1 for ONE channel of a spin-polarised one (the sum over
+    sigma of Eq. 11); the prefactor is occupation x 2 (c.c.) / Omega."""
     idx = gsphere.fft_index(miller, N)
     vol = float(L) ** 3
     Uo, Uc = U[:, :n_occ], U[:, n_occ:]
@@ -43,7 +45,7 @@ def chi0_sum_over_states(eps, U, n_occ, dV, omegas, miller, L, N, return_dpsi=Fa
             dpsi_all[w] = dpsi
         for i in range(len(dV)):
             du = ham.to_real_space(dpsi[i], idx, N)
-            dn[w, i] = (4.0 / vol) * np.real(np.sum(np.conj(u_occ) * du, axis=0))
+            dn[w, i] = (2.0 * occupation / vol) * np.real(np.sum(np.conj(u_occ) * du, axis=0))
     return (dn, dpsi_all) if return_dpsi else dn
 
 
@@ -52,7 +54,7 @@ def default_alpha(eps, n_occ):
     return max(2.0 * float(eps[n_occ - 1] - eps[0]), 0.01)
 
 
-def sternheimer_dense(H, eps, U, n_occ, dV, omega, alpha, miller, L, N, return_dpsi=False):
+def sternheimer_dense(H, eps, U, n_occ, dV, omega, alpha, miller, L, N, return_dpsi=False, occupation=2.0):
     """Brute force: for each (i, v) solve (H - eps_v - i omega + alpha P_v) x = -P_c b_iv with LAPACK."""
     idx = gsphere.fft_index(miller, N)
     vol = float(L) ** 3
@@ -70,8 +72,18 @@ def sternheimer_dense(H, eps, U, n_occ, dV, omega, alpha, miller, L, N, return_d
         dpsi[:, v, :] = x
     for i in range(len(dV)):
         du = ham.to_real_space(dpsi[i], idx, N)
-        dn[i] = (4.0 / vol) * np.real(np.sum(np.conj(u_occ) * du, axis=0))
+        dn[i] = (2.0 * occupation / vol) * np.real(np.sum(np.conj(u_occ) * du, axis=0))
     return (dn, dpsi) if return_dpsi else dn
+
+
+def chi0_spin_polarised(channels, dV, omegas, miller, L, N):
+    """N_spin = 2 (Tables 3, 5, 7 list N_spin): each channel sigma has its own h^sigma, hence its own
+    (eps, U, n_occ) = channels[sigma]; Eq. 10 is solved per channel with P_c^sigma, and Eq. 11 sums the channels, each orbital
+    holding one electron:  dn = sum_sigma (2 / Omega) Re sum_v conj(u_v^sigma) du_v^sigma."""
+    dn = 0.0
+    for eps, U, n_occ in channels:
+        dn = dn + chi0_sum_over_states(eps, U, n_occ, dV, omegas, miller, L, N, occupation=1.0)
+    return dn
 
 
 def dn_from_dpsi(U_occ, dpsi, miller, L, N):

@@ -19,4 +19,5 @@ from .fields import (  # noqa: F401
     vloc_for,
     atoms_for,
     dense_grid,
+    spin_splitting_field,
 )

@@ -57,5 +57,5 @@ def get_config(name):
 
 
 def seed_for(cfg_id, k):
-    """Seeds 1000*cfg + k.  k: 0 V_loc noise, 1 atom positions, 2.. dV stream, 99 random test vectors."""
+    """Seeds 1000*cfg + k.  k: 0 V_loc noise, 1 atom positions, 2.. dV stream, 98 spin splitting field, 99 random test vectors."""
     return 1000 * int(cfg_id) + int(k)

@@ -140,3 +140,9 @@ def dense_grid(n, n_batch=1, seed=7000):
     rng = np.random.Generator(np.random.PCG64(seed + n))
     x = rng.standard_normal((n_batch, n, n, n)) + 1j * rng.standard_normal((n_batch, n, n, n))
     return np.ascontiguousarray(x)
+
+
+def spin_splitting_field(cfg):
+    """B(r) of the spin-polarised workload (N_spin = 2): V_up = V_loc + B, V_down = V_loc - B with B a smooth
+    field (sigma 1.5 bohr, rms 0.03 Ry, seed stream 98); both channels keep n_occ orbitals, so both keep a gap."""
+    return smooth_field(cfg["N"], cfg["L"], 1.5, 0.03, make_rng(cfg["cfg"], 98))

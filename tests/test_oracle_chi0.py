@@ -115,3 +115,47 @@ def test_eq11_is_real_and_dn_from_dpsi_matches():
     assert np.max(np.abs(eq11.imag)) < 1e-15 * np.max(np.abs(eq11.real))
     assert _relmax(eq11.real, dn[0, 0]) < 1e-14
     assert _relmax(ochi0.dn_from_dpsi(Uo, dpsi[0, 0], p.miller, p.L, p.N), dn[0, 0]) < 1e-14
+
+
+def _spin_channels(p, n_occ_up=None, n_occ_dn=None):
+    import synth
+    B = synth.spin_splitting_field(p.cfg)
+    ch = []
+    for sgn, n_occ in ((+1, n_occ_up or p.n_occ), (-1, n_occ_dn or p.n_occ)):
+        H = oham.dense_h(p.miller, p.L, p.N, p.vloc + sgn * B, p.beta, p.dcoef)
+        eps, U = np.linalg.eigh(H)
+        ch.append((eps, U, n_occ, H))
+    return B, ch
+
+
+def test_spin_polarised_finite_field_derivative_and_limits():
+    """N_spin = 2: dn = d/d lambda of n(r) = (1/Omega) sum_sigma sum_v |u_v^sigma|^2 with h^sigma = T + V_loc +- B + lambda dV + V_NL,
+    different occupations in the two channels; identical channels reduce to the unpolarised result; an empty channel adds nothing."""
+    p = op.build("cfg1")
+    dV = p.dV[1]
+    B, ch = _spin_channels(p, n_occ_up=p.n_occ + 1, n_occ_dn=p.n_occ - 1)
+    lam = 2e-4
+
+    def density(lmb):
+        n = 0.0
+        for sgn, n_occ in ((+1, p.n_occ + 1), (-1, p.n_occ - 1)):
+            H = oham.dense_h(p.miller, p.L, p.N, p.vloc + sgn * B + lmb * dV, p.beta, p.dcoef)
+            _, U = np.linalg.eigh(H)
+            u = oham.to_real_space(U[:, :n_occ].T, p.fft_idx, p.N)
+            n = n + (1.0 / p.L ** 3) * np.sum(np.abs(u) ** 2, axis=0)
+        return n
+
+    ff = (density(lam) - density(-lam)) / (2 * lam)
+    dn = ochi0.chi0_spin_polarised([c[:3] for c in ch], dV[None], [0.0], p.miller, p.L, p.N)[0, 0]
+    assert _relmax(dn, ff) < 5e-6
+    # per channel: dense Sternheimer solve with that channel's own H and projector
+    for eps, U, n_occ, H in ch:
+        a = ochi0.chi0_sum_over_states(eps, U, n_occ, dV[None], [0.3], p.miller, p.L, p.N, occupation=1.0)[0]
+        b = ochi0.sternheimer_dense(H, eps, U, n_occ, dV[None], 0.3, 1.7, p.miller, p.L, p.N, occupation=1.0)
+        assert _relmax(b, a) < 1e-11
+    same = ochi0.chi0_spin_polarised([(p.eps, p.U, p.n_occ)] * 2, dV[None], [0.0, 0.5], p.miller, p.L, p.N)
+    unpol = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, dV[None], [0.0, 0.5], p.miller, p.L, p.N)
+    assert _relmax(same, unpol) < 1e-13
+    one = ochi0.chi0_spin_polarised([ch[0][:3], (ch[1][0], ch[1][1], 0)], dV[None], [0.0], p.miller, p.L, p.N)
+    up = ochi0.chi0_sum_over_states(*ch[0][:3], dV[None], [0.0], p.miller, p.L, p.N, occupation=1.0)
+    assert _relmax(one, up) < 1e-14
