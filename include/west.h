@@ -80,6 +80,9 @@ typedef struct {
     int32_t solver;     /* 0: one preconditioned PCG (omega = 0) / COCG (omega > 0) solve per frequency (R7);
                            1: multi-shift CG (WEST_GAMMA only, <= 16 frequencies): all frequencies from ONE unpreconditioned Krylov
                               sequence of the real seed operator H - eps_v + alpha P_v, one H*psi per iteration for every omega */
+    double  occupation; /* electrons per orbital in Eq. 11: 2 = spin-unpolarised (0 selects this default), 1 = ONE channel of a
+                           spin-polarised system (N_spin = 2): dn = (2 occupation / Omega) Re sum_v ... */
+    int32_t dn_accumulate; /* 0: dn is overwritten; 1: dn += this call's response (second spin channel: the sum over sigma) */
 } west_cg_opts;
 
 typedef struct {            /* host struct, filled when non-NULL (forces one stream synchronisation) */

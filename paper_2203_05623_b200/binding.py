@@ -24,7 +24,7 @@ class west_cell(C.Structure):
 
 class west_cg_opts(C.Structure):
     _fields_ = [("max_iter", C.c_int32), ("tol", C.c_double), ("alpha_pv", C.c_double), ("precond", C.c_int32),
-                ("check_every", C.c_int32), ("solver", C.c_int32)]
+                ("check_every", C.c_int32), ("solver", C.c_int32), ("occupation", C.c_double), ("dn_accumulate", C.c_int32)]
 
 
 class west_stats(C.Structure):
@@ -194,7 +194,9 @@ class West:
         return out
 
     def chi0_apply(self, dV, omegas, tol=1e-12, max_iter=500, alpha_pv=1.0, precond=1, check_every=4, precision=WEST_FP64, solver=0,
-                   dn=None, want_dpsi=False, n_occ=None, want_stats=True):
+                   dn=None, want_dpsi=False, n_occ=None, want_stats=True, occupation=2.0, accumulate=False):
+        """occupation / accumulate: the sum over spin channels of Eq. 11 (one context per channel, occupation=1, the second call
+        with accumulate=True and the first call's dn); see chi0_apply_spin."""
         import torch
         N = self.N
         n_pert = int(dV.shape[0])
@@ -207,7 +209,7 @@ class West:
             assert n_occ is not None
             shape = (n_freq, n_pert, n_occ, 2, self.n_g) if self.mode == WEST_GAMMA else (n_freq, n_pert, n_occ, self.n_g)
             dpsi = torch.empty(shape, dtype=torch.complex128, device=dV.device)
-        opts = west_cg_opts(int(max_iter), float(tol), float(alpha_pv), int(precond), int(check_every), int(solver))
+        opts = west_cg_opts(int(max_iter), float(tol), float(alpha_pv), int(precond), int(check_every), int(solver), float(occupation), int(bool(accumulate)))
         st = west_stats()
         rc = self._ck(self.lib.west_chi0_apply(self.ctx, precision, n_pert, _dev(dV, torch.float64), n_freq, om.ctypes.data, C.byref(opts),
                                                _dev(dn, torch.float64), _dev(dpsi) if dpsi is not None else None,
@@ -215,6 +217,19 @@ class West:
         stats = {k: getattr(st, k) for k, _ in west_stats._fields_}
         stats["rc"] = rc
         return dn, dpsi, stats
+
+    @staticmethod
+    def chi0_apply_spin(channels, dV, omegas, **kw):
+        """N_spin = 2: channels = [West_up, West_down], each holding its own V_loc^sigma, projectors and
+        occupied orbitals.  dn = sum over channels, each with one electron per orbital.  alpha_pv may be a pair (one per channel).
+        Returns dn and the list of per-channel stats."""
+        alpha = kw.pop("alpha_pv", 1.0)
+        alphas = list(alpha) if isinstance(alpha, (list, tuple)) else [alpha] * len(channels)
+        dn, stats = None, []
+        for k, w in enumerate(channels):
+            dn, _, st = w.chi0_apply(dV, omegas, dn=dn, occupation=1.0, accumulate=k > 0, alpha_pv=alphas[k], **kw)
+            stats.append(st)
+        return dn, stats
 
     def lanczos(self, phi, n_steps, n_occ, want_brakets=False, precision=WEST_FP64):
         """alpha, beta [n_pert][n_occ][n_steps], norm [n_pert][n_occ], brakets [n_occ][n_steps][n_pert][n_pert] or None."""

@@ -161,7 +161,7 @@ __global__ void nat_to_pos_real(int N, int N1, int N2, long long total, const do
     out[i] = (T)in[b * n3 + ((long long)ix * N + iy) * N + iz];
 }
 // position order real [b][pz][py][px] -> natural [b][ix][iy][iz]
-__global__ void pos_to_nat_real(int N, int N1, int N2, long long total, const double* in, double* out) {
+__global__ void pos_to_nat_real(int N, int N1, int N2, long long total, const double* in, double* out, int acc = 0) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
     const long long n3 = (long long)N * N * N, b = i / n3;
@@ -169,7 +169,8 @@ __global__ void pos_to_nat_real(int N, int N1, int N2, long long total, const do
     const int iz = (int)(r % N); r /= N;
     const int iy = (int)(r % N); const int ix = (int)(r / N);
     const int px = N2 * (ix % N1) + ix / N1, py = N2 * (iy % N1) + iy / N1, pz = N2 * (iz % N1) + iz / N1;
-    out[i] = in[b * n3 + ((long long)pz * N + py) * N + px];
+    const double v = in[b * n3 + ((long long)pz * N + py) * N + px];
+    out[i] = acc ? out[i] + v : v;
 }
 // complex position-order slots [s][N^3] -> user grids.  gamma: real grids 2s (Re), 2s+1 (Im); full: complex grid s
 __global__ void pos_to_user(int N, int N1, int N2, int gamma, int slot0, int n_slots, int n_batch, const cx<double>* R, double* out) {
@@ -833,7 +834,7 @@ int add_deflated(west_ctx* c, int n_col, int in_nvpc, int out_nvpc, double omega
 }
 
 // a10: dn_i(r) = (4/Omega) Re sum_v conj(u_v) du_iv from X ([n_col][nvpc][n_g]) into dn_out ([n_pert][N^3], natural order)
-int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_out) {
+int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_out, double occupation, int accumulate) {
     const int gamma = is_gamma(c), N = c->cell.N, n_col = n_pert * c->n_occ, n_vec = n_col * nvpc;
     const long long n3 = n3_of(c);
     const double vol = c->cell.L * c->cell.L * c->cell.L;
@@ -844,7 +845,7 @@ int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_o
     CK(cudaMemsetAsync(c->dnpos.p, 0, sizeof(double) * n3 * n_pert, c->st));
     VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
     K2Any a{};
-    a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dn = (double*)c->dnpos.p; a.n_uslots = n_uslots; a.fac = 4.0 / vol;
+    a.W = c->W.p; a.ucache = (const cx<double>*)c->ucache.p; a.dn = (double*)c->dnpos.p; a.n_uslots = n_uslots; a.fac = 2.0 * occupation / vol;
     for (int s0 = 0; s0 < n_rslots; s0 += chunk) {
         const int ns = std::min(chunk, n_rslots - s0);
         vm.slot0 = s0; a.slot0 = s0;
@@ -853,7 +854,7 @@ int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_o
         CK(c->ops->k2(0, K2_DN, ns, c->st, c->geom, a));
         c->launches += 2;
     }
-    pos_to_nat_real<<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, (const double*)c->dnpos.p, dn_out);
+    pos_to_nat_real<<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, (const double*)c->dnpos.p, dn_out, accumulate);
     CK(cudaGetLastError());
     c->launches += 1;
     return WEST_OK;
@@ -925,7 +926,10 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
-    if (opts->max_iter < 1 || !(opts->tol > 0) || (opts->solver != 0 && opts->solver != 1)) return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
+    if (opts->max_iter < 1 || !(opts->tol > 0) || (opts->solver != 0 && opts->solver != 1) || opts->occupation < 0 || opts->occupation > 2 ||
+        (opts->dn_accumulate != 0 && opts->dn_accumulate != 1))
+        return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
+    const double occ = opts->occupation > 0 ? opts->occupation : 2.0;
     if (opts->solver == 1 && (c->cell.mode != WEST_GAMMA || n_freq > wcg::MS_MAX_SHIFTS))
         return fail(c, WEST_EINVAL, "west_chi0_apply: the multi-shift solver needs WEST_GAMMA and at most %d frequencies", wcg::MS_MAX_SHIFTS);
     const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
@@ -1037,7 +1041,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         for (int w = 0; w < n_freq; ++w) {
             cx<double>* Xw = (cx<double>*)c->xs.p + (size_t)w * per;
             if ((rc = add_deflated(c, n_col, 1, 2, omega_host[w], d_eps, Xw))) return rc;
-            if ((rc = chi0_dn(c, n_pert, 2, Xw, dn + (long long)w * n_pert * n3))) return rc;
+            if ((rc = chi0_dn(c, n_pert, 2, Xw, dn + (long long)w * n_pert * n3, occ, opts->dn_accumulate))) return rc;
             if (dpsi_opt && (rc = copy_dpsi(w, 1, Xw))) return rc;
         }
         if ((rc = ensure(c, c->misc, 64))) return rc;
@@ -1072,7 +1076,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         if (rc) return rc;
         if ((rc = add_deflated(c, n_col, nvpc, nvpc, omega, d_eps, X))) return rc;
         if (stats) CK(cudaEventRecord(ev[2], c->st));
-        if ((rc = chi0_dn(c, n_pert, nvpc, X, dn + (long long)w * n_pert * n3))) return rc;
+        if ((rc = chi0_dn(c, n_pert, nvpc, X, dn + (long long)w * n_pert * n3, occ, opts->dn_accumulate))) return rc;
         if (dpsi_opt && (rc = copy_dpsi(w, mode, X))) return rc;
         if (stats) {
             CK(cudaEventRecord(ev[3], c->st));
