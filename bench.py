@@ -41,8 +41,10 @@ def parse():
     ap.add_argument("--check-every", type=int, default=1, help="CG convergence poll / compaction period")
     ap.add_argument("--precond", type=int, default=1, help="0 none, 1 R4 default, 2 Teter-Payne-Allan")
     ap.add_argument("--solver", type=int, default=-1, help="0 per-frequency PCG/COCG, 1 multi-shift CG; -1 = 1 for cfg3, else 0")
-    ap.add_argument("--op", default="chi0", choices=["chi0", "lanczos", "pdep"],
-                    help="chi0 = the hot path (default); lanczos = Eq. 15-19 chains; pdep = Davidson shell for chi0bar (widening rows)")
+    ap.add_argument("--op", default="chi0", choices=["chi0", "lanczos", "pdep", "fft", "spin"],
+                    help="chi0 = the hot path (default); lanczos = Eq. 15-19 chains; pdep = Davidson shell for chi0bar; fft = the dense "
+                         "C2C FFT of Fig. 3 (--workload fft128 | fft256, --precision); spin = N_spin = 2 chi0 (widening rows)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"], help="--op fft only")
     ap.add_argument("--deflate", type=int, default=0, help="number of conduction eigenstates handed to west_set_deflation (0 = off)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
     return ap.parse_args()
@@ -95,7 +97,7 @@ def build_inputs(cfg):
     return atoms, vloc
 
 
-def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0):
+def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0, vloc_add=None):
     import torch
     import synth
     import paper_2203_05623_b200 as wb
@@ -106,6 +108,8 @@ def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0):
         w.set_fft_chunk(chunk)
     miller, _, _, g2 = w.gsphere()
     atoms, vloc = build_inputs(cfg)
+    if vloc_add is not None:
+        vloc = vloc + vloc_add
     beta, dcoef = synth.kb_projectors(miller, cfg["L"], atoms, 0.8, cfg["projectors"])
     if mode == wb.WEST_GAMMA:
         # synth normalises over the rows it is given (the half sphere); rescale to sum over the FULL sphere = 1
@@ -174,6 +178,8 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     import synth
+    if a.op == "fft":
+        return bench_fft(a, rank, world, local)
     cfg = synth.get_config(a.workload)
     n_pert = a.n_pert or cfg.get("pert_batch", cfg["n_pert"])
     omegas = [0.0] if a.workload != "cfg3" else list(cfg["omegas"])
@@ -211,6 +217,9 @@ def main():
         return bench_lanczos(a, cfg, w, dV, n_pert, rank, world, barrier)
     if a.op == "pdep":
         return bench_pdep(a, cfg, w, alpha, n_pert, rank, world, barrier)
+    if a.op == "spin":
+        w.close()
+        return bench_spin(a, cfg, dV, n_pert, rank, world, barrier, kw)
     stats = None
     for _ in range(a.warmup):
         _, _, stats = w.chi0_apply(dV, omegas, **kw)
@@ -344,6 +353,149 @@ def bench_pdep(a, cfg, w, alpha, n_pdep, rank, world, barrier):
                       "config": {"workload": a.workload, "op": "pdep", "n_pdep": n_pdep, "chi0_applications": int(n_app),
                                  "lambda_min": float(lam[0]), "lambda_max_kept": float(lam[-1]), "max_residual": float(res.max())},
                       "chi0_applications_per_s": n_app / dt}))
+
+
+def bench_spin(a, cfg, dV, n_pert, rank, world, barrier, kw):
+    """Widening row SURVEY 8(f)-4, second half: the same cell with N_spin = 2.  h^sigma = T + V_loc +- B + V_NL (synth.spin_splitting_field),
+    n_occ orbitals per channel with one electron each; a step = chi0*dV summed over both channels (two Sternheimer batches)."""
+    import torch
+    import synth
+    import paper_2203_05623_b200 as wb
+    B = synth.spin_splitting_field(cfg)
+    ws, alphas, gaps = [], [], []
+    for sgn in (+1, -1):
+        w, _, alpha, aux = setup_gpu(cfg, 1, a.chunk, verbose=(rank == 0), vloc_add=sgn * B)
+        ws.append(w); alphas.append(alpha); gaps.append(aux["gap"])
+    kw = dict(kw, alpha_pv=alphas)
+    kw.pop("dn")
+    stats = None
+    for _ in range(a.warmup):
+        _, stats = wb.West.chi0_apply_spin(ws, dV, [0.0], **kw)
+    barrier()
+    l0 = sum(w.launch_count() for w in ws)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(a.steps):
+        _, stats = wb.West.chi0_apply_spin(ws, dV, [0.0], **kw)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    if rank != 0:
+        return
+    print(json.dumps({"metric": "spin-polarised chi0*dV perturbations/s (N_spin = 2, PCG to tol %.0e)" % TOL, "value": n_pert * world * a.steps / (ms * 1e-3),
+                      "unit": "perturbations/s", "n_gpus": world, "steps": a.steps, "warmup": a.warmup, "ms_per_step": ms / a.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": a.workload, "op": "spin", "n_spin": 2, "n_pert_per_gpu": n_pert, "n_occ_per_channel": cfg["n_occ"],
+                                 "gaps_ry": gaps, "cg_iters": [st["iters"] for st in stats], "unconverged": [st["n_unconverged"] for st in stats]},
+                      "h_apply_per_s": sum(st["n_h_apply"] for st in stats) * world / (ms / a.steps * 1e-3),
+                      "gpu_launches": int(sum(w.launch_count() for w in ws) - l0), "device_gb": sum(w.device_bytes() for w in ws) / 1e9}))
+
+
+def bench_fft(a, rank, world, local):
+    """Widening row SURVEY 8(f)-4, first half: Fig. 3 of the paper - ONE dense C2C FFT of a 128^3 or 256^3 grid, FP64 or
+    FP32, data resident on the device, mean over the timed steps (the paper averages 100: run with --steps 100).  Each step is timed
+    with its own CUDA-event pair and a 256 MB L2 flush in between, because the 128^3 grid fits the 126 MB L2.  N > 1: replicas."""
+    import torch
+    import torch.distributed as dist
+    import synth
+    import paper_2203_05623_b200 as wb
+    n = {"fft128": 128, "fft256": 256, "fft64": 64}.get(a.workload)
+    if n is None:
+        raise SystemExit("--op fft needs --workload fft64 | fft128 | fft256")
+    if a.impl == "reference":
+        if rank == 0:
+            from oracle import fft_dense as ofd
+            ts = []
+            ns = min(n, 128)
+            xs = synth.dense_grid(ns, 1)[0]
+            for _ in range(a.warmup + a.steps):
+                t0 = time.time()
+                ofd.dft3(xs, -1)
+                ts.append((time.time() - t0) * (n / ns) ** 4)
+            v = float(np.mean(ts[a.warmup:])) * 1e3
+            print(json.dumps({"impl": "reference", "metric": "time of one dense C2C 3D FFT (Fig. 3)", "value": v, "unit": "ms", "n_gpus": a.gpus,
+                              "steps": a.steps, "warmup": a.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+                              "dtype": "f64", "data": "synthetic", "config": {"workload": a.workload, "op": "fft", "n": n},
+                              "cpu_baseline": {"value": v, "unit": "ms", "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+                                               "sample": "oracle.fft_dense.dft3 on the whole grid" if n <= 128 else "dft3 on a 128^3 grid, time scaled by 16 (its cost is 3 n^4)"},
+                              "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cdt, esz = (torch.complex128, 16) if a.precision == "fp64" else (torch.complex64, 8)
+    x_np = synth.dense_grid(n, 1)
+    x = torch.from_numpy(x_np).to("cuda", dtype=cdt)
+    y = torch.empty_like(x)
+    w = wb.West(10.0, 25, 24, wb.WEST_FULL)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn, k):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        for e0, e1 in ev:
+            flush.zero_()
+            e0.record(); fn(); e1.record()
+        torch.cuda.synchronize()
+        return [e0.elapsed_time(e1) for e0, e1 in ev]
+
+    for _ in range(max(a.warmup, 3)):
+        w.fft3d_dense(x, -1, out=y)
+        torch.fft.fftn(x, dim=(1, 2, 3), out=y)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = w.launch_count()
+    t = timed(lambda: w.fft3d_dense(x, -1, out=y), a.steps)
+    launches = w.launch_count() - l0
+    sampler.stop_flag.set(); sampler.join()
+    t_lib = timed(lambda: torch.fft.fftn(x, dim=(1, 2, 3), out=y), a.steps)
+    # end to end: pinned host grid -> device, transform, result -> pinned host
+    hx = torch.from_numpy(x_np[...]).to(cdt).pin_memory()
+    hy = torch.empty_like(hx).pin_memory()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        x.copy_(hx, non_blocking=True)
+        w.fft3d_dense(x, -1, out=y)
+        hy.copy_(y, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / a.steps
+    ms = float(np.mean(t))
+    tt = torch.tensor([ms, e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dist.destroy_process_group()
+    ms, e2e_ms = float(tt[0]), float(tt[1])
+    if rank != 0:
+        return
+    hbm_peak, peak_src = peaks()
+    alg = 2.0 * n ** 3 * esz
+    line = {"metric": "time of one dense C2C 3D FFT (Fig. 3)", "value": ms, "unit": "ms", "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
+            "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if esz == 16 else "f32", "data": "synthetic (seeded complex normal grid)",
+            "config": {"workload": a.workload, "op": "fft", "n": n, "precision": a.precision, "l2": "256 MB flush between timed steps", "replicas": world},
+            "ffts_per_s": world * 1e3 / ms, "ms_median": float(np.median(t)),
+            "library": {"what": "cuFFT through torch.fft.fftn, same buffers, same timing loop", "ms_mean": float(np.mean(t_lib)), "ratio": float(np.mean(t_lib)) / ms},
+            "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(x.numel() * esz), "d2h_bytes_per_step": int(y.numel() * esz)},
+            "gpu_launches": int(launches), "clocks": sampler.summary(),
+            "roofline": {"kernel": "dense_axis_pass (3 launches per FFT)", "bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": alg / (ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src, "traffic": None,
+                         "algorithmic_bytes": alg, "note": "algorithmic = read the grid once + write it once; the three axis passes move 3x that "
+                                                         "(through HBM at 256^3, mostly through L2 at 128^3): three_pass_frac = %.3f" % (3 * alg / (ms * 1e-3) / 1e9 / hbm_peak)}}
+    if world == 1 and not a.no_cpu_baseline:
+        from oracle import fft_dense as ofd
+        # the DFT-matrix definition costs 3 n^4 complex multiply-adds: 256^3 takes ~50 s, so it is sampled on the 128^3 grid and scaled by 16
+        ns = min(n, 128)
+        xs = x_np[0] if ns == n else synth.dense_grid(ns, 1)[0]
+        t0 = time.time()
+        ofd.dft3(xs, -1)
+        dt = (time.time() - t0) * (n / ns) ** 4
+        sample = "oracle.fft_dense.dft3 (DFT matrices) on the whole %d^3 grid" % n if ns == n else \
+                 "oracle.fft_dense.dft3 on a 128^3 grid, time scaled by (256/128)^4 = 16 (its cost is 3 n^4)"
+        line["cpu_baseline"] = {"value": dt * 1e3, "unit": "ms", "cores": len(os.sched_getaffinity(0)), "kind": "oracle", "sample": sample}
+    print(json.dumps(line))
 
 
 def aux_ncols(cfg):
