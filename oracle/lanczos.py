@@ -65,3 +65,21 @@ def tridiagonal(alpha, beta):
     for l in range(L - 1):
         T[l, l + 1] = T[l + 1, l] = beta[l]
     return T
+
+
+def eig_tridiagonal(alpha, beta):
+    """d^{l'} and U^{l l'} of Eq. 19: eigenvalues (ascending) and orthonormal eigenvectors (columns) of the tridiagonal
+    matrix with alpha^l on the diagonal and beta^l on the sub- and super-diagonal, T = U diag(d) U^T.  LAPACK through numpy.linalg.eigh
+    is the step; the sign of each eigenvector is fixed by U[0, l'] >= 0 (the first component of an eigenvector of an unreduced
+    tridiagonal matrix is never zero), which is what makes U unique when the eigenvalues are simple."""
+    T = tridiagonal(np.asarray(alpha, dtype=np.float64), np.asarray(beta, dtype=np.float64))
+    d, U = np.linalg.eigh(T)
+    U = U * np.where(U[0] < 0, -1.0, 1.0)[None, :]
+    return d, U
+
+
+def resolvent_column(alpha, beta, z):
+    """x = (T - z)^{-1} e_1 by a dense solve: the vector Eq. 19 evaluates as x_l = sum_l' U^{l l'} U^{1 l'} / (d^{l'} - z)."""
+    T = tridiagonal(np.asarray(alpha, dtype=np.float64), np.asarray(beta, dtype=np.float64)).astype(np.complex128)
+    e1 = np.zeros(len(alpha), dtype=np.complex128); e1[0] = 1.0
+    return np.linalg.solve(T - z * np.eye(len(alpha)), e1)
