@@ -168,6 +168,15 @@ int  west_chi0_apply(west_ctx* ctx, int32_t precision, int32_t n_pert, const dou
 int  west_lanczos(west_ctx* ctx, int32_t precision, int32_t n_pert, const double* phi, int32_t n_steps, double* alpha, double* beta,
                   double* norm, double* braket_opt);
 
+/* d and U of Eq. 19: "the eigenvalues and the eigenvectors of the tri-diagonal matrix that has alpha^l along the diagonal
+ * and beta^l along the sub- and super-diagonal", for n_chain chains at once (one warp per matrix, implicit-shift QL with accumulated
+ * plane rotations).  alpha, beta [n_chain][n_steps] f64 (device) exactly as west_lanczos returns them (beta[..][l] couples rows l and
+ * l+1; the last entry of each row is not part of T).  d [n_chain][n_steps] ascending; U [n_chain][n_steps][n_steps] row-major,
+ * U[l][l'] = component l of the eigenvector of d[l'], orthonormal, sign fixed by U[0][l'] >= 0.  sweeps_opt NULL or [n_chain] i32
+ * (device): QL sweeps used, -1 = not converged.  1 <= n_steps <= 64.  Synchronises the stream once (to return WEST_NOTCONVERGED). */
+int  west_lanczos_diag(west_ctx* ctx, int32_t n_chain, int32_t n_steps, const double* alpha, const double* beta, double* d, double* U,
+                       int32_t* sweeps_opt);
+
 /* Dense contraction building blocks (FP64 DMMA), exported for tests and the roofline bench.
  * C[m][n] = sum_k A[m][k] B[n][k]          (west_gemm_tn: both operands K-contiguous, row-major [rows][ld])
  * Y[n][k] += sum_m C[m][n] A[m][k]          (west_gemm_update)

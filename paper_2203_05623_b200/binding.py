@@ -33,7 +33,7 @@ class west_stats(C.Structure):
 
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
-           "west_fft3d", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
+           "west_fft3d", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_lanczos_diag", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
            "west_launch_count", "west_set_fft_chunk", "west_set_profile", "west_get_profile"]
 
 
@@ -56,6 +56,7 @@ def load_library():
     lib.west_h_apply.argtypes = [vp, i32, i32, vp, vp]
     lib.west_chi0_apply.argtypes = [vp, i32, i32, vp, i32, vp, C.POINTER(west_cg_opts), vp, vp, C.POINTER(west_stats)]
     lib.west_lanczos.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp, vp]
+    lib.west_lanczos_diag.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.west_gemm_tn.argtypes = [vp, i32, i32, i64, vp, i64, vp, i64, vp, i64]
     lib.west_gemm_update.argtypes = [vp, i32, i32, i64, vp, i64, vp, i64, vp, i64]
     lib.west_device_bytes.argtypes = [vp]
@@ -243,6 +244,19 @@ class West:
         self._ck(self.lib.west_lanczos(self.ctx, precision, n_pert, _dev(phi, torch.float64), int(n_steps), _dev(alpha), _dev(beta),
                                        _dev(norm), _dev(br) if br is not None else None))
         return alpha, beta, norm, br
+
+    def lanczos_diag(self, alpha, beta, want_sweeps=False):
+        """d [..., n_steps] ascending and U [..., n_steps, n_steps] (columns = eigenvectors, U[..., 0, :] >= 0) of the tridiagonal
+        matrices of Eq. 19; alpha, beta [..., n_steps] as returned by lanczos()."""
+        import torch
+        n = int(alpha.shape[-1])
+        n_chain = int(alpha.numel() // n) if n else 0
+        d = torch.empty_like(alpha)
+        U = torch.empty(tuple(alpha.shape) + (n,), dtype=torch.float64, device=alpha.device)
+        sw = torch.empty(tuple(alpha.shape[:-1]), dtype=torch.int32, device=alpha.device) if want_sweeps else None
+        self._ck(self.lib.west_lanczos_diag(self.ctx, n_chain, n, _dev(alpha, torch.float64), _dev(beta, torch.float64), _dev(d), _dev(U),
+                                            _dev(sw) if sw is not None else None))
+        return (d, U, sw) if want_sweeps else (d, U)
 
     def gemm_tn(self, A, B, out=None):
         """C[m][n] = sum_k A[m][k] B[n][k], f64 row-major."""

@@ -79,4 +79,107 @@ __global__ void braket_fix(int n_batch, int n, long long sC, double* C, const do
     *c = 2.0 * (*c) - A[(long long)b * sAB + (long long)row * ld] * B[(long long)b * sAB + (long long)colm * ld];
 }
 
+// Eigenvalues d and eigenvectors U of the Lanczos tridiagonal matrices of Eq. 19, one WARP per chain:
+//   T = tridiag(beta^2 .. beta^L ; alpha^1 .. alpha^L ; beta^2 .. beta^L),  T = U diag(d) U^T,  d ascending, U[0][l'] >= 0.
+// Implicit-shift QL iteration (Wilkinson shift, Givens chase from the bottom of the unreduced block to its top), the
+// textbook method for symmetric tridiagonal matrices.  The scalar recurrence on d, e is carried redundantly by every lane (warp-uniform
+// control flow); each plane rotation is applied to the eigenvector matrix with one row per lane (n <= 64: two rows per lane).
+// alpha, beta: [n_chain][n] as west_lanczos writes them (beta[l] = the off-diagonal between l and l+1; beta[n-1] is not part of T).
+// d_out [n_chain][n]; U_out [n_chain][n][n] row-major, U[l][l'] = component l of eigenvector l'; status[chain] = sweeps used, or -1
+// if some eigenvalue did not converge in 60 sweeps.
+constexpr int TRI_MAX = 64, TRI_WARPS = 4;
+__global__ void __launch_bounds__(32 * TRI_WARPS) tridiag_eig(int n_chain, int n, const double* __restrict__ alpha, const double* __restrict__ beta,
+                                                              double* __restrict__ d_out, double* __restrict__ U_out, int* __restrict__ status, int* __restrict__ n_failed) {
+    extern __shared__ double sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chain = blockIdx.x * TRI_WARPS + warp;
+    if (chain >= n_chain) return;                               // whole warps leave together; only __syncwarp below
+    double* d = sm + (size_t)warp * (2 * TRI_MAX + (size_t)n * (n + 1));
+    double* e = d + TRI_MAX;
+    double* Z = e + TRI_MAX;                                    // [n][n + 1]: row k at pitch n + 1 (conflict-free column access)
+    const int P = n + 1;
+    for (int i = lane; i < n; i += 32) {
+        d[i] = alpha[(long long)chain * n + i];
+        e[i] = i + 1 < n ? beta[(long long)chain * n + i] : 0.0;
+    }
+    for (int i = lane; i < n * P; i += 32) Z[i] = 0.0;
+    __syncwarp();
+    for (int i = lane; i < n; i += 32) Z[i * P + i] = 1.0;
+    __syncwarp();
+    int sweeps = 0;
+    bool ok = true;
+    for (int l = 0; l < n && ok; ++l) {
+        int iter = 0;
+        while (true) {
+            int m = l;
+            for (; m < n - 1; ++m) {
+                const double dd = fabs(d[m]) + fabs(d[m + 1]);
+                if (fabs(e[m]) <= 2.220446049250313e-16 * dd) break;
+            }
+            if (m == l) break;
+            if (++iter > 60) { ok = false; break; }
+            ++sweeps;
+            double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+            double r = hypot(g, 1.0);
+            g = d[m] - d[l] + e[l] / (g + copysign(r, g));
+            double sn = 1.0, cs = 1.0, pp = 0.0;
+            int i = m - 1;
+            bool deflated = false;
+            __syncwarp();
+            for (; i >= l; --i) {
+                double f = sn * e[i];
+                const double b = cs * e[i];
+                r = hypot(f, g);
+                double e_next = r;
+                if (r == 0.0) {                                 // the chase recovered a zero off-diagonal: split here
+                    __syncwarp();
+                    if (lane == 0) { e[i + 1] = 0.0; d[i + 1] -= pp; e[m] = 0.0; }
+                    deflated = true;
+                    break;
+                }
+                sn = f / r; cs = g / r;
+                g = d[i + 1] - pp;
+                r = (d[i] - g) * sn + 2.0 * cs * b;
+                pp = sn * r;
+                const double d_next = g + pp;
+                g = cs * r - b;
+                __syncwarp();                                   // every lane has read e[i], d[i], d[i + 1]
+                if (lane == 0) { e[i + 1] = e_next; d[i + 1] = d_next; }
+                for (int k = lane; k < n; k += 32) {            // rotate columns i, i + 1 of Z
+                    f = Z[k * P + i + 1];
+                    const double zi = Z[k * P + i];
+                    Z[k * P + i + 1] = sn * zi + cs * f;
+                    Z[k * P + i] = cs * zi - sn * f;
+                }
+                __syncwarp();
+            }
+            __syncwarp();
+            if (!deflated) {
+                if (lane == 0) { d[l] -= pp; e[l] = g; e[m] = 0.0; }
+            }
+            __syncwarp();
+        }
+    }
+    __syncwarp();
+    // ascending order by rank (ties by index), sign U[0][l'] >= 0, written straight to the output
+    for (int j = lane; j < n; j += 32) {
+        const double dj = d[j];
+        int rank = 0;
+        for (int i = 0; i < n; ++i) rank += (d[i] < dj) || (d[i] == dj && i < j);
+        e[j] = (double)rank;                                    // e is free now
+        d_out[(long long)chain * n + rank] = dj;
+    }
+    __syncwarp();
+    double* U = U_out + (long long)chain * n * n;
+    for (int idx = lane; idx < n * n; idx += 32) {
+        const int k = idx / n, j = idx - k * n;
+        const double sgn = Z[j] < 0.0 ? -1.0 : 1.0;             // Z[0][j]
+        U[(long long)k * n + (int)e[j]] = sgn * Z[k * P + j];
+    }
+    if (lane == 0) {
+        if (status) status[chain] = ok ? sweeps : -1;
+        if (!ok) atomicAdd(n_failed, 1);
+    }
+}
+
 }  // namespace wlz

@@ -1161,3 +1161,28 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     }
     return WEST_OK;
 }
+
+extern "C" int west_lanczos_diag(west_ctx* c, int32_t n_chain, int32_t n_steps, const double* alpha, const double* beta, double* d, double* U,
+                                 int32_t* sweeps_opt) {
+    if (!c || n_chain < 0 || n_steps < 1 || n_steps > wlz::TRI_MAX || (n_chain > 0 && (!alpha || !beta || !d || !U)))
+        return fail(c, WEST_EINVAL, "west_lanczos_diag: bad argument (1 <= n_steps <= %d)", wlz::TRI_MAX);
+    if (n_chain == 0) return WEST_OK;
+    int rc;
+    if ((rc = ensure(c, c->misc, 256))) return rc;
+    int* n_failed = (int*)c->misc.p;
+    CK(cudaMemsetAsync(n_failed, 0, sizeof(int), c->st));
+    const size_t bytes = sizeof(double) * wlz::TRI_WARPS * (2 * wlz::TRI_MAX + (size_t)n_steps * (n_steps + 1));
+    if (bytes > 48 * 1024) CK(cudaFuncSetAttribute(wlz::tridiag_eig, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    {
+        Prof p_(c, PC_MISC);
+        wlz::tridiag_eig<<<(n_chain + wlz::TRI_WARPS - 1) / wlz::TRI_WARPS, 32 * wlz::TRI_WARPS, bytes, c->st>>>(n_chain, n_steps, alpha, beta, d, U,
+                                                                                                       sweeps_opt, n_failed);
+        CK(cudaGetLastError());
+        c->launches += 1;
+    }
+    CK(cudaMemcpyAsync(c->h_pinned, n_failed, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (c->h_pinned[0] > 0)
+        return fail(c, WEST_NOTCONVERGED, "west_lanczos_diag: %d of %d matrices did not converge in 60 QL sweeps per eigenvalue", c->h_pinned[0], n_chain);
+    return WEST_OK;
+}

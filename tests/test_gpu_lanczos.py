@@ -66,3 +66,80 @@ def test_lanczos_cfg2_size_sampled_chains():
     G = (np.conj(q1[:, 0]) @ q1[:, 0].T).real
     assert np.max(np.abs(br[5, 0].cpu().numpy() - G)) < 1e-10
     w.close()
+
+
+def _diag_ctx():
+    import paper_2203_05623_b200 as wb
+    return wb.West(10.0, 25, 24, wb.WEST_FULL)
+
+
+def _check_diag(alpha, beta, d, U, tol=1e-12):
+    """Against oracle.lanczos.eig_tridiagonal: what is unique (eigenvalues; the spectral sum of Eq. 19) is compared, the rest
+    (orthonormal eigenvectors of T, sign convention) is checked for validity; eigenvectors themselves only when the spectrum is simple."""
+    for c in range(alpha.shape[0]):
+        T = olz.tridiagonal(alpha[c], beta[c])
+        scale = max(np.max(np.abs(T)), 1e-300)
+        d_ref, U_ref = olz.eig_tridiagonal(alpha[c], beta[c])
+        assert np.max(np.abs(d[c] - d_ref)) < tol * scale * len(d_ref)
+        assert np.all(np.diff(d[c]) >= 0)
+        assert np.max(np.abs(U[c].T @ U[c] - np.eye(len(d_ref)))) < 1e-12
+        assert np.max(np.abs(T @ U[c] - U[c] * d[c][None, :])) < 1e-12 * scale * len(d_ref)
+        assert np.all(U[c][0] >= 0)
+        if len(d_ref) > 1 and np.min(np.diff(d_ref)) > 1e-3 * scale:
+            # the sign rule binds only where the first component is not at rounding level; elsewhere compare up to the sign
+            fixed = np.abs(U_ref[0]) > 1e-8
+            assert np.max(np.abs(U[c][:, fixed] - U_ref[:, fixed])) < 1e-9
+            sgn = np.sign(np.sum(U[c] * U_ref, axis=0))
+            assert np.max(np.abs(U[c] * sgn[None, :] - U_ref)) < 1e-9
+        for z in (0.3j, 0.1 + 2.0j):
+            x = (U[c] * U[c][0][None, :]) @ (1.0 / (d[c] - z))
+            assert np.max(np.abs(x - olz.resolvent_column(alpha[c], beta[c], z))) < 1e-11
+
+
+@pytest.mark.parametrize("n", [1, 2, 7, 30, 33, 64])
+def test_tridiagonal_eigensolver_random_and_special_matrices(n):
+    import torch
+    rng = np.random.Generator(np.random.PCG64(100 + n))
+    n_chain = 37
+    alpha = rng.standard_normal((n_chain, n))
+    beta = np.abs(rng.standard_normal((n_chain, n))) + 0.05
+    alpha[0], beta[0] = 0.3, 0.7                                   # Toeplitz: closed-form spectrum
+    if n > 4:
+        beta[1, n // 2] = 0.0                                      # reducible: two independent blocks
+        alpha[2] = 1.0; beta[2] = 1e-9                             # nearly diagonal, clustered eigenvalues
+        beta[3] *= 1e3; alpha[3] *= 1e-3                           # badly scaled
+    w = _diag_ctx()
+    d, U, sw = w.lanczos_diag(torch.from_numpy(alpha).cuda(), torch.from_numpy(beta).cuda(), want_sweeps=True)
+    assert int(sw.min()) >= 0
+    d, U = d.cpu().numpy(), U.cpu().numpy()
+    if n > 4:
+        # row 1 is reducible: first components of the second block's eigenvectors are exactly zero, the sign rule does not bind
+        keep = [c for c in range(n_chain) if c != 1]
+        T = olz.tridiagonal(alpha[1], beta[1])
+        assert np.max(np.abs(np.sort(np.linalg.eigvalsh(T)) - d[1])) < 1e-12 * n
+        assert np.max(np.abs(T @ U[1] - U[1] * d[1][None, :])) < 1e-12 * n
+    else:
+        keep = list(range(n_chain))
+    _check_diag(alpha[keep], beta[keep], d[keep], U[keep])
+    k = np.arange(1, n + 1)
+    assert np.max(np.abs(d[0] - np.sort(0.3 + 1.4 * np.cos(k * np.pi / (n + 1))))) < 1e-13 * n
+    w.close()
+
+
+def test_tridiagonal_eigensolver_on_real_chains_and_errors():
+    """alpha, beta of oracle chains (cfg 1, 30 steps, where orthogonality is already lost and Ritz values cluster) as the input of both sides."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build("cfg1")
+    q1, _ = olz.start_vectors(p.U[:, :p.n_occ], p.dV[:2], p.fft_idx, p.N)
+    ab = [olz.chain(lambda y: p.H @ y, q1[m, i], 30) for m in range(2) for i in range(p.n_occ)]
+    alpha = np.array([x[0] for x in ab]); beta = np.array([x[1] for x in ab])
+    w = _diag_ctx()
+    d, U = w.lanczos_diag(torch.from_numpy(alpha).cuda(), torch.from_numpy(beta).cuda())
+    _check_diag(alpha, beta, d.cpu().numpy(), U.cpu().numpy())
+    with pytest.raises(wb.WestError) as e:
+        w.lanczos_diag(torch.zeros((2, 65), dtype=torch.float64, device="cuda"), torch.zeros((2, 65), dtype=torch.float64, device="cuda"))
+    assert e.value.code == wb.binding.WEST_EINVAL
+    d0, U0 = w.lanczos_diag(torch.zeros((0, 30), dtype=torch.float64, device="cuda"), torch.zeros((0, 30), dtype=torch.float64, device="cuda"))
+    assert d0.shape == (0, 30) and U0.shape == (0, 30, 30)
+    w.close()
