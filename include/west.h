@@ -106,7 +106,8 @@ int  west_gsphere(const west_ctx* ctx, int64_t* n_g, int32_t* miller, int32_t* f
 /* Operator data (device pointers, copied).  vloc [N^3] f64.  beta [n_proj][n_g] c128 in the storage of cell.mode
  * (in GAMMA mode each projector must be a real function of r), dcoef [n_proj] f64 HOST: V_NL = sum_k |beta_k> D_k <beta_k|
  * (Kleinman-Bylander, R12).  psi [n_occ][n_g] c128 orthonormal occupied orbitals (sum_G |c|^2 = 1 over the FULL sphere),
- * eps [n_occ] f64 HOST eigenvalues in Ry: the inputs psi_i, eps_i of Eq. 10. n_proj = 0 removes V_NL. */
+ * eps [n_occ] f64 HOST eigenvalues in Ry: the inputs psi_i, eps_i of Eq. 10. n_proj = 0 removes V_NL.
+ * n_occ may be odd in either mode (WEST_GAMMA pads internally with a zero orbital, which no output ever contains). */
 int  west_set_vloc  (west_ctx* ctx, const double* vloc);
 int  west_set_kb    (west_ctx* ctx, int32_t n_proj, const void* beta, const double* dcoef_host);
 int  west_set_states(west_ctx* ctx, int32_t n_occ, const void* psi, const double* eps_host);

@@ -51,7 +51,8 @@ struct west_ctx {
     double* d_vpos = nullptr;          // V_loc, position order, f64
     float* d_vpos_f = nullptr;         // same, f32 (WEST_MIXED)
     bool have_vloc = false;
-    int n_proj = 0, n_occ = 0;
+    int n_proj = 0, n_occ = 0;         // n_occ: orbitals the solvers run over (WEST_GAMMA pads an odd count with one zero orbital)
+    int n_occ_user = 0;                // orbitals the caller handed to west_set_states (layout of dpsi / Lanczos outputs)
     int rows_kb = 0, rows_psi = 0;     // rows of the stacked real operator matrix (x2 in WEST_FULL)
     int n_defl = 0, rows_defl = 0;     // optional deflation states (lowest conduction orbitals), stacked after the psi rows
     DevBuf A_defl, eps_defl, craw, dcoef_defl;
@@ -546,28 +547,40 @@ int west_set_kb(west_ctx* c, int32_t n_proj, const void* beta, const double* dco
     return WEST_OK;
 }
 
-int west_set_states(west_ctx* c, int32_t n_occ, const void* psi, const double* eps_host) {
-    if (!c || n_occ <= 0 || !psi || !eps_host) return fail(c, WEST_EINVAL, "west_set_states: bad argument");
+int west_set_states(west_ctx* c, int32_t n_occ_user, const void* psi, const double* eps_host) {
+    if (!c || n_occ_user <= 0 || !psi || !eps_host) return fail(c, WEST_EINVAL, "west_set_states: bad argument");
     const int full = !is_gamma(c);
     const long long n_g = c->hs.n_g, n3 = n3_of(c);
+    // WEST_GAMMA transforms two real orbitals per complex FFT: an odd count gets one ZERO orbital appended (R15).  Its right-hand
+    // sides, solutions and density contributions are identically zero (the CG marks zero columns inactive at start), its row in
+    // the P_v GEMMs is zero, and it never appears in an output.
+    const int n_occ = (!full && (n_occ_user & 1)) ? n_occ_user + 1 : n_occ_user;
     c->n_occ = n_occ;
+    c->n_occ_user = n_occ_user;
     c->rows_psi = n_occ * (full ? 2 : 1);
     c->A_dirty = true;
-    c->h_eps.assign(eps_host, eps_host + n_occ);
+    c->h_eps.assign(eps_host, eps_host + n_occ_user);
+    if (n_occ > n_occ_user) c->h_eps.push_back(eps_host[n_occ_user - 1]);
     int rc = ensure(c, c->A_psi, (size_t)c->rows_psi * 2 * n_g * sizeof(double));
     if (rc) return rc;
-    stack_rows<<<blocks_for(n_g * n_occ, 256), 256, 0, c->st>>>(n_g, n_occ, full, (const cx<double>*)psi, (double*)c->A_psi.p);
+    if (n_occ > n_occ_user) CK(cudaMemsetAsync(c->A_psi.p, 0, (size_t)c->rows_psi * 2 * n_g * sizeof(double), c->st));
+    stack_rows<<<blocks_for(n_g * n_occ_user, 256), 256, 0, c->st>>>(n_g, n_occ_user, full, (const cx<double>*)psi, (double*)c->A_psi.p);
     CK(cudaGetLastError());
     if ((rc = ensure(c, c->tk, sizeof(double) * n_occ))) return rc;
-    kinetic_expect<<<n_occ, 256, 0, c->st>>>(n_g, is_gamma(c), c->d_g2, (const cx<double>*)psi, (double*)c->tk.p);
+    kinetic_expect<<<n_occ_user, 256, 0, c->st>>>(n_g, is_gamma(c), c->d_g2, (const cx<double>*)psi, (double*)c->tk.p);
     CK(cudaGetLastError());
+    if (n_occ > n_occ_user) {
+        const double one = 1.0;        // finite preconditioner for the zero orbital's (never active) columns
+        CK(cudaMemcpyAsync((double*)c->tk.p + n_occ_user, &one, sizeof(double), cudaMemcpyHostToDevice, c->st));
+        CK(cudaStreamSynchronize(c->st));
+    }
     c->launches += 2;
     // u_v(r) cache in position order: GAMMA packs (v, v+1) as u_v + i u_{v+1}
     c->n_uslots = full ? n_occ : (n_occ + 1) / 2;
     if ((rc = ensure(c, c->ucache, sizeof(cx<double>) * n3 * c->n_uslots))) return rc;
     const int chunk = std::max(1, std::min(c->n_uslots, chunk_slots(c, 0)));
     if ((rc = ensure_W(c, chunk, 0))) return rc;
-    VecMap vm{full ? 1 : 2, full ? 0 : 1, n_occ, 0};
+    VecMap vm{full ? 1 : 2, full ? 0 : 1, n_occ_user, 0};       // vectors >= n_vec read as zero: the padding orbital
     for (int s0 = 0; s0 < c->n_uslots; s0 += chunk) {
         const int ns = std::min(chunk, c->n_uslots - s0);
         vm.slot0 = s0;
@@ -933,7 +946,6 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     if (opts->solver == 1 && (c->cell.mode != WEST_GAMMA || n_freq > wcg::MS_MAX_SHIFTS))
         return fail(c, WEST_EINVAL, "west_chi0_apply: the multi-shift solver needs WEST_GAMMA and at most %d frequencies", wcg::MS_MAX_SHIFTS);
     const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
-    if (gamma && (n_occ & 1)) return fail(c, WEST_EINVAL, "west_chi0_apply: WEST_GAMMA needs an even number of occupied states (two per FFT)");
     for (int w = 0; w < n_freq; ++w) {
         if (omega_host[w] < 0) return fail(c, WEST_EINVAL, "west_chi0_apply: omega must be >= 0");
         if (omega_host[w] > 0 && !gamma) return fail(c, WEST_EINVAL, "west_chi0_apply: omega > 0 needs WEST_GAMMA (COCG needs real orbitals, R7)");
@@ -982,15 +994,23 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     if (stats) for (auto& e : ev.e) CK(cudaEventCreate(&e));
     int ret = WEST_OK;
     auto copy_dpsi = [&](int w, int mode, const cx<double>* Xw) -> int {
-        // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 (per-frequency solver) the imaginary part is zero
-        const long long per = n_g * n_col * (gamma ? 2 : 1);
+        // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 (per-frequency solver) the imaginary part is zero.
+        // n_occ here is the caller's count: the columns of the padding orbital (odd counts, R15) are skipped.
+        const int n_user = c->n_occ_user;
+        const long long per = n_g * n_pert * n_user * (gamma ? 2 : 1);
         cx<double>* dst = (cx<double>*)dpsi_opt + (long long)w * per;
         if (gamma && mode == 0) {
             CK(cudaMemsetAsync(dst, 0, sizeof(cx<double>) * per, c->st));
-            CK(cudaMemcpy2DAsync(dst, sizeof(cx<double>) * 2 * n_g, Xw, sizeof(cx<double>) * n_g, sizeof(cx<double>) * n_g, n_col,
-                                 cudaMemcpyDeviceToDevice, c->st));
+            for (int i = 0; i < (n_user == n_occ ? 1 : n_pert); ++i) {
+                const int rows = n_user == n_occ ? n_col : n_user;
+                CK(cudaMemcpy2DAsync(dst + (long long)i * n_user * 2 * n_g, sizeof(cx<double>) * 2 * n_g, Xw + (long long)i * n_occ * n_g,
+                                     sizeof(cx<double>) * n_g, sizeof(cx<double>) * n_g, rows, cudaMemcpyDeviceToDevice, c->st));
+            }
         } else {
-            CK(cudaMemcpyAsync(dst, Xw, sizeof(cx<double>) * per, cudaMemcpyDeviceToDevice, c->st));
+            const long long vpc = gamma ? 2 : 1;       // vectors per column
+            if (n_user == n_occ) CK(cudaMemcpyAsync(dst, Xw, sizeof(cx<double>) * per, cudaMemcpyDeviceToDevice, c->st));
+            else CK(cudaMemcpy2DAsync(dst, sizeof(cx<double>) * n_user * vpc * n_g, Xw, sizeof(cx<double>) * n_occ * vpc * n_g,
+                                      sizeof(cx<double>) * n_user * vpc * n_g, n_pert, cudaMemcpyDeviceToDevice, c->st));
         }
         return WEST_OK;
     };
@@ -1107,7 +1127,6 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_lanczos: bad precision %d", precision);
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_lanczos: west_set_vloc and west_set_states are required");
     const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
-    if (gamma && (n_occ & 1)) return fail(c, WEST_EINVAL, "west_lanczos: WEST_GAMMA needs an even number of occupied states");
     if (braket_opt && !gamma) return fail(c, WEST_EINVAL, "west_lanczos: brakets are implemented for WEST_GAMMA only");
     if (n_pert == 0) return WEST_OK;
     const long long n_g = c->hs.n_g, n3 = n3_of(c), K = 2 * n_g;
@@ -1121,6 +1140,13 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     cx<double>* Q = (cx<double>*)c->vecs[0].p; cx<double>* QP = (cx<double>*)c->vecs[1].p;
     cx<double>* HQ = (cx<double>*)c->vecs[2].p; cx<double>* Q1 = (cx<double>*)c->vecs[3].p;
     double* beta_prev = (double*)c->scal.p;
+    // odd orbital count in WEST_GAMMA (R15): the chains run over the padded column set into scratch arrays, the caller's are filled at the end
+    const int n_user = c->n_occ_user;
+    double *alpha_out = alpha, *beta_out = beta, *norm_out = norm;
+    if (n_user != n_occ) {
+        if ((rc = ensure(c, c->msst, sizeof(double) * (size_t)n_col * (2 * n_steps + 1)))) return rc;
+        alpha = (double*)c->msst.p; beta = alpha + (size_t)n_col * n_steps; norm = beta + (size_t)n_col * n_steps;
+    }
     nat_to_pos_real<double><<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, phi, (double*)c->dVpos.p);
     CK(cudaGetLastError());
     c->launches += 1;
@@ -1131,7 +1157,7 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     else wlz::lz_normalize<false><<<n_col, wcg::NT, 0, c->st>>>(n_g, (double2*)Q, nullptr, norm, beta_prev);
     CK(cudaGetLastError());
     c->launches += 1;
-    if (braket_opt) CK(cudaMemsetAsync(braket_opt, 0, sizeof(double) * (size_t)n_occ * n_steps * n_pert * n_pert, c->st));
+    if (braket_opt) CK(cudaMemsetAsync(braket_opt, 0, sizeof(double) * (size_t)n_user * n_steps * n_pert * n_pert, c->st));
     const int f32 = precision == WEST_MIXED;
     VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_col, 0};
     const int n_slots = gamma ? (n_col + 1) / 2 : n_col;
@@ -1141,9 +1167,9 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
             double* C = braket_opt + (size_t)l * n_pert * n_pert;
             const long long sC = (long long)n_steps * n_pert * n_pert;
             if ((rc = launch_gemm_tn(c, n_pert, n_pert, K, (const double*)Q1, (long long)n_occ * K, (const double*)Q, (long long)n_occ * K, C,
-                                     n_pert, n_occ, K, K, sC, false)))
+                                     n_pert, n_user, K, K, sC, false)))
                 return rc;
-            wlz::braket_fix<<<blocks_for((long long)n_occ * n_pert * n_pert, 256), 256, 0, c->st>>>(n_occ, n_pert, sC, C, (const double*)Q1,
+            wlz::braket_fix<<<blocks_for((long long)n_user * n_pert * n_pert, 256), 256, 0, c->st>>>(n_user, n_pert, sC, C, (const double*)Q1,
                                                                                                   (const double*)Q, (long long)n_occ * K, K);
             CK(cudaGetLastError());
             c->launches += 1;
@@ -1158,6 +1184,12 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
             c->launches += 1;
         }
         std::swap(Q, QP);          // QP now holds q^l (the next q^{l-1}), Q holds q^{l+1}
+    }
+    if (n_user != n_occ) {
+        const size_t w = sizeof(double) * n_steps;
+        CK(cudaMemcpy2DAsync(alpha_out, w * n_user, alpha, w * n_occ, w * n_user, n_pert, cudaMemcpyDeviceToDevice, c->st));
+        CK(cudaMemcpy2DAsync(beta_out, w * n_user, beta, w * n_occ, w * n_user, n_pert, cudaMemcpyDeviceToDevice, c->st));
+        CK(cudaMemcpy2DAsync(norm_out, sizeof(double) * n_user, norm, sizeof(double) * n_occ, sizeof(double) * n_user, n_pert, cudaMemcpyDeviceToDevice, c->st));
     }
     return WEST_OK;
 }
