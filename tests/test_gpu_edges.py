@@ -51,19 +51,6 @@ def test_error_codes():
     w.close()
 
 
-def test_odd_state_count_rejected_in_gamma_mode():
-    import torch
-    import paper_2203_05623_b200 as wb
-    p = oracle_problem.build("mini2")
-    w, sel = make_west(p, with_states=False)
-    psi = np.ascontiguousarray(p.U[:, :p.n_occ - 1].T[:, sel])
-    w.set_states(torch.from_numpy(psi).cuda(), p.eps[:p.n_occ - 1])
-    with pytest.raises(wb.WestError) as e:
-        w.chi0_apply(torch.from_numpy(np.ascontiguousarray(p.dV[:1])).cuda(), [0.0], alpha_pv=p.alpha)
-    assert e.value.code == wb.binding.WEST_EINVAL
-    w.close()
-
-
 def test_constant_perturbation_gives_zero_response_and_linearity():
     import torch
     p = oracle_problem.build("mini2")
