@@ -36,6 +36,9 @@ template <typename T> WHD cx<T> cvt(cx<double> a) { return mk<T>((T)a.x, (T)a.y)
 template <typename T> WHD cx<double> cvd(cx<T> a) { return mk<double>((double)a.x, (double)a.y); }
 WHD int wrap_signed(int n, int N) { return n < N / 2 ? n : n - N; }
 
+#ifndef WEST_ZFUSE
+#define WEST_ZFUSE 1      // 1: fused z-stick kernels (K1: combine while loading, store from registers; K3: load + contiguous pass fused)
+#endif
 #ifndef WEST_TW_POW
 #define WEST_TW_POW 1     // 1: level twiddles w^(m k) as powers of ONE table entry per thread (FP64 work traded for L1TEX wavefronts)
 #endif
@@ -133,6 +136,78 @@ if (WEST_TW_POW) {
             }
         }
     }
+    // ---- fused variant (WEST_ZFUSE): two phases, one barrier, the line buffer is written once and read once.
+    // GAMMA: the two lines of a unit are formed WHILE LOADING as  line 2ul = a(n) + i b(n)  and  line 2ul+1 = conj(a(-n)) + i conj(b(-n)),
+    // whose transforms are S+ = A + iB and S- = conj(A) + i conj(B) themselves, so phase BC stores its registers straight to the
+    // column cp and its mirror.  FULL: phaseA as above, then phaseBC.
+    static WHD cx<T> coef(const cx<double>* src, int m, int zmax, bool half00) {
+        if (half00) {                                   // column (0,0): only n_z >= 0 is stored, c(-n) = conj(c(n)), c(0) real
+            const cx<double> c = src[m >= 0 ? m : -m];
+            return mk<T>((T)c.x, m == 0 ? (T)0 : (T)(m > 0 ? c.y : -c.y));
+        }
+        return cvt<T>(src[m + zmax]);
+    }
+    static WHD void phaseA2(int tid, int nthr, cx<T>* lines, const cx<T>* tw, const WestGeom& g, VecMap vm, int slot, int u0,
+                            const cx<double>* X) {
+        if (!GAMMA) { phaseA(tid, nthr, lines, tw, g, vm, slot, u0, X); return; }
+        for (int it = tid; it < NL * N2; it += nthr) {
+            const int line = it / N2, n2 = it - line * N2;
+            const int u = u0 + line / 2, sgn = line & 1;
+            cx<T> v[N1];
+            const long long vec0 = (long long)(vm.slot0 + slot) * vm.vstride, vec1 = vec0 + vm.voffb;
+            // column 0 is its own mirror: its minus line is never stored
+            if (u < g.n_units && vec0 < vm.n_vec && !(u == 0 && sgn)) {
+                const int zmax = g.unit_zmax[u];
+                const bool half00 = u == 0, has_b = vec1 < vm.n_vec;
+                const cx<double>* sa = X + vec0 * g.n_g + g.unit_off[u];
+                const cx<double>* sb = X + vec1 * g.n_g + g.unit_off[u];
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    const int nz = wrap_signed(N2 * n1 + n2, N);
+                    cx<T> val = mk<T>(0, 0);
+                    if (keep_n1<N1, N2>(n1) && nz <= zmax && nz >= -zmax) {
+                        const int m = sgn ? -nz : nz;
+                        const cx<T> a = coef(sa, m, zmax, half00);
+                        const cx<T> b = has_b ? coef(sb, m, zmax, half00) : mk<T>(0, 0);
+                        val = sgn ? mk<T>(a.x + b.y, b.x - a.y) : mk<T>(a.x - b.y, a.y + b.x);
+                    }
+                    v[n1] = val;
+                }
+                Dft<T, N1, +1>::run(v);
+            } else {
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) v[n1] = mk<T>(0, 0);
+            }
+            cx<T>* dst = lines + line * PITCH + n2;
+            if (WEST_TW_POW) {
+                cx<T> zp[N1];
+                tw_powers<T, N1>(tw[N2 + n2], zp);
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
+            } else {
+#pragma unroll
+                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+            }
+        }
+    }
+    // contiguous DFT-N2 of (line, k1), registers straight to W; lanes run over the lines, i.e. over consecutive columns
+    static WHD void phaseBC(int tid, int nthr, const cx<T>* lines, const WestGeom& g, int slot, int u0, cx<T>* W) {
+        for (int it = tid; it < NL * N1; it += nthr) {
+            const int k1 = it / NL, line = it - k1 * NL;
+            const int u = u0 + line / NF, sgn = GAMMA ? (line & 1) : 0;
+            if (u >= g.n_units || (GAMMA && sgn && u == 0)) continue;
+            const cx<T>* p = lines + line * PITCH + N2 * k1;
+            cx<T> v[N2];
+#pragma unroll
+            for (int j = 0; j < N2; ++j) v[j] = p[j];
+            Dft<T, N2, +1>::run(v);
+            const int cp = GAMMA ? u + (g.n_cols - g.n_units) : u;
+            const int col = sgn ? g.n_cols - 1 - cp : cp;
+            cx<T>* dst = W + ((long long)slot * N + N2 * k1) * g.n_cols + col;
+#pragma unroll
+            for (int j = 0; j < N2; ++j) dst[(long long)j * g.n_cols] = v[j];
+        }
+    }
 };
 
 // ---------------------------------------------------------------------------------------------------------------- K3
@@ -196,6 +271,50 @@ struct K3 {
             for (int j = 0; j < N2; ++j) v[j] = p[j];
             Dft<T, N2, -1>::run(v);
 if (WEST_TW_POW) {
+                cx<T> zp[N2];
+                tw_powers<T, N2>(tw[N + N1 + k1], zp);
+#pragma unroll
+                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+            }
+        }
+    }
+    // ---- fused variant (WEST_ZFUSE): W -> registers -> (GAMMA: separate the two real functions with the partner lane) -> DFT-N2,
+    // twiddle -> line buffer; replaces phaseA + phaseB and one barrier.  Item (k1, line), lanes over the lines: lane pair (2m, 2m+1)
+    // holds column cp (S+) and its mirror (S-) of the same unit at the same N2 positions.  On the host (stepped test) the
+    // partner's values are simply loaded again.
+    static WHD void phaseAB(int tid, int nthr, cx<T>* lines, const cx<T>* tw, const WestGeom& g, int slot, int u0, const cx<T>* W) {
+        constexpr int ITEMS = NL * N1, ROUND = (ITEMS + 31) / 32 * 32;       // whole warps take part in the exchange
+        for (int it = tid; it < ROUND; it += nthr) {
+            const int k1 = it / NL, line = it - k1 * NL;
+            const int u = u0 + line / NF, sgn = GAMMA ? (line & 1) : 0;
+            const bool valid = it < ITEMS && u < g.n_units;
+            cx<T> v[N2];
+            const int cp = GAMMA ? u + (g.n_cols - g.n_units) : u;
+            const int mirror = (GAMMA && u != 0) ? g.n_cols - 1 - cp : cp;     // column 0 is its own mirror
+            const cx<T>* src = W + ((long long)slot * N + N2 * k1) * g.n_cols;
+#pragma unroll
+            for (int j = 0; j < N2; ++j) v[j] = valid ? src[(long long)j * g.n_cols + (sgn ? mirror : cp)] : mk<T>(0, 0);
+            if (GAMMA) {
+#pragma unroll
+                for (int j = 0; j < N2; ++j) {
+                    cx<T> o;
+#ifdef __CUDA_ARCH__
+                    o.x = __shfl_xor_sync(0xffffffffu, v[j].x, 1);
+                    o.y = __shfl_xor_sync(0xffffffffu, v[j].y, 1);
+#else
+                    o = valid ? src[(long long)j * g.n_cols + (sgn ? cp : mirror)] : mk<T>(0, 0);
+#endif
+                    // sgn 0 holds S+ and receives S-: a = (S+ + conj S-)/2 ; sgn 1 holds S- and receives S+: b = (S+ - conj S-)/(2i)
+                    v[j] = sgn ? mk<T>((T)0.5 * (o.y + v[j].y), (T)0.5 * (v[j].x - o.x)) : mk<T>((T)0.5 * (v[j].x + o.x), (T)0.5 * (v[j].y - o.y));
+                }
+            }
+            if (it >= ITEMS) continue;
+            Dft<T, N2, -1>::run(v);
+            cx<T>* p = lines + line * PITCH + N2 * k1;
+            if (WEST_TW_POW) {
                 cx<T> zp[N2];
                 tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
@@ -487,11 +606,17 @@ __global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k1_g2r_z(WestGeom g, Vec
     load_tw<T, N1, N2>(tw, g.tw);
     __syncthreads();
     const int slot = blockIdx.y, u0 = blockIdx.x * CU;
+#if WEST_ZFUSE
+    K::phaseA2(threadIdx.x, blockDim.x, lines, tw, g, vm, slot, u0, X);
+    __syncthreads();
+    K::phaseBC(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
+#else
     K::phaseA(threadIdx.x, blockDim.x, lines, tw, g, vm, slot, u0, X);
     __syncthreads();
     K::phaseB(threadIdx.x, blockDim.x, lines);
     __syncthreads();
     K::phaseC(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
+#endif
 }
 
 template <typename T, int N1, int N2, bool GAMMA, int CU>
@@ -512,10 +637,16 @@ __global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k3_r2g_z(WestGeom g, Vec
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(e.X + vec * g.n_g + g.unit_off[u] + seg * 8));
         }
     }
+#if WEST_ZFUSE
+    __syncthreads();                                   // twiddles
+    K::phaseAB(threadIdx.x, blockDim.x, lines, tw, g, slot, u0, W);
+    __syncthreads();
+#else
     K::phaseA(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
     __syncthreads();
     K::phaseB(threadIdx.x, blockDim.x, lines, tw);
     __syncthreads();
+#endif
     K::phaseC(threadIdx.x, blockDim.x, lines, g, vm, slot, u0, e, Y);
 }
 

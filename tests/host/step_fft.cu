@@ -1,12 +1,14 @@
 // Host-stepped run of the FFT kernel phases (paper_2203_05623_b200/csrc/fft_kernels.cuh) for tests/test_host_stepped_fft.py:
 // every phase between two barriers is a function of (tid, nthreads), so the exact device code path of K1 -> K2<K2_H> -> K3
-// (local part of H: T + V_loc) is executed here thread by thread on the CPU.   usage: step_fft N n2max gamma L nvec f32 in out
+// (local part of H: T + V_loc) is executed here thread by thread on the CPU.   usage: step_fft N n2max gamma L nvec f32 in out [fused]
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <vector>
 #include "../../paper_2203_05623_b200/csrc/fft_kernels.cuh"
 #include "../../paper_2203_05623_b200/csrc/gsphere.hpp"
+
+static int g_fused = 0;      // 1: the fused z-stick phases (K1 phaseA2/phaseBC, K3 phaseAB; the lane exchange is replaced by a reload)
 
 template <typename T, int N1, int N2, bool GAMMA>
 void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V, std::vector<double>& Y) {
@@ -33,6 +35,11 @@ void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V
     using KA = K1<T, N1, N2, GAMMA, CU>; using KC = K3<T, N1, N2, GAMMA, CU>; using KB = K2<T, N1, N2, K2_H, LC>;
     std::vector<cx<T>> lines(KA::NL * KA::PITCH);
     for (int slot = 0; slot < nslots; slot++) for (int u0 = 0; u0 < s.n_units; u0 += CU) {
+        if (g_fused) {
+            for (int t = 0; t < NT; t++) KA::phaseA2(t, NT, lines.data(), tw.data(), g, vm, slot, u0, (const cx<double>*)X.data());
+            for (int t = 0; t < NT; t++) KA::phaseBC(t, NT, lines.data(), g, slot, u0, W.data());
+            continue;
+        }
         for (int t = 0; t < NT; t++) KA::phaseA(t, NT, lines.data(), tw.data(), g, vm, slot, u0, (const cx<double>*)X.data());
         for (int t = 0; t < NT; t++) KA::phaseB(t, NT, lines.data());
         for (int t = 0; t < NT; t++) KA::phaseC(t, NT, lines.data(), g, slot, u0, W.data());
@@ -56,8 +63,12 @@ void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V
     }
     K3Epi e; e.scale = 1.0 / ((double)N * N * N); e.kinetic = 1; e.shift = nullptr; e.omega = 0; e.X = (const cx<double>*)X.data();
     for (int slot = 0; slot < nslots; slot++) for (int u0 = 0; u0 < s.n_units; u0 += CU) {
-        for (int t = 0; t < NT; t++) KC::phaseA(t, NT, lines.data(), g, slot, u0, W.data());
-        for (int t = 0; t < NT; t++) KC::phaseB(t, NT, lines.data(), tw.data());
+        if (g_fused) {
+            for (int t = 0; t < NT; t++) KC::phaseAB(t, NT, lines.data(), tw.data(), g, slot, u0, W.data());
+        } else {
+            for (int t = 0; t < NT; t++) KC::phaseA(t, NT, lines.data(), g, slot, u0, W.data());
+            for (int t = 0; t < NT; t++) KC::phaseB(t, NT, lines.data(), tw.data());
+        }
         for (int t = 0; t < NT; t++) KC::phaseC(t, NT, lines.data(), g, vm, slot, u0, e, (cx<double>*)Y.data());
     }
 }
@@ -67,6 +78,7 @@ int main(int argc, char** argv) {
     const int N = atoi(argv[1]), n2max = atoi(argv[2]), gamma = atoi(argv[3]);
     const double L = atof(argv[4]);
     const int nvec = atoi(argv[5]), f32 = atoi(argv[6]);
+    if (argc > 9) g_fused = atoi(argv[9]);
     HostSphere s = build_sphere(n2max, N, gamma, L);
     std::vector<double> X((size_t)nvec * s.n_g * 2), Y(X.size(), 0.0), V((size_t)N * N * N);
     FILE* f = fopen(argv[7], "rb");
