@@ -58,6 +58,13 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def sm_clock_mhz():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p)).get("sm_max_mhz", 1965.0))
+    return 1965.0
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks / throttle reasons sampled during the timed region."""
 
@@ -554,6 +561,15 @@ def roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, mixed, w, f
                         "peak_source": fp64_src + ("; x2 for the FP32 path" if mixed else ""),
                         "algorithmic_flops_per_slot": fl_slot, "algorithmic_bytes_per_slot": per_slot,
                         "hbm_view": {"achieved_gbs": gbs, "peak_gbs": hbm_peak, "frac": gbs / hbm_peak, "peak_source": peak_src}})
+            # shared-memory view: the four two-stage 1D passes move 8 nr N + 4 N^2 elements per plane through shared
+            # memory; peak = 128 B/clk/SM x 148 SMs x the SM clock.  Removing FP64 work from this kernel does not shorten it, removing
+            # shared-memory wavefronts does (profiles/r01_k2_l1tex_bound.md), so this is the pipe that binds
+            smem_slot = N * (8 * nr * N + 4 * N * N) * csz
+            smem_peak = 128.0 * 148 * sm_clock_mhz() * 1e6 / 1e9
+            smem_gbs = smem_slot * slots / t / 1e9
+            out["smem_view"] = {"achieved_gbs": smem_gbs, "peak_gbs": smem_peak, "frac": smem_gbs / smem_peak,
+                                "algorithmic_smem_bytes_per_slot": smem_slot,
+                                "peak_source": "128 B/clk/SM x 148 SMs x max SM clock (MEASURED_PEAKS.json sm_max_mhz, else 1965 MHz)"}
             if N == 72 and not mixed:
                 out["traffic"] = NCU_K2_DRAM_BYTES_PER_SLOT_CFG2 * slots / spans
                 out["traffic_note"] = "ncu dram bytes per slot (51-slot capture, cold L2) x slots per launch; algorithmic = %.3e B/slot" % per_slot

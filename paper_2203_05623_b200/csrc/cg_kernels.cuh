@@ -203,6 +203,100 @@ __global__ void __launch_bounds__(NT) cg_step(long long n_g, int n_occ, const do
     }
 }
 
+// The same iteration with the column RESIDENT on the SM (MODE 0 and 2, n_g <= EPT * NTR): cg_step's second touches of p, Ap and r
+// were meant to hit L2, but 8 CTAs x 148 SMs x 4 vectors x 146 KB (cfg 2) is 690 MB of columns in flight against a 126 MB L2, so
+// they came from HBM again (11 vector passes per iteration instead of 7).  Here one CTA of NTR threads owns a column, thread t
+// owns elements g = e NTR + t: Ap, then the new r, stay in its registers and p in its own shared-memory slots (each thread reads
+// back only what it wrote, so no barrier guards them), and HBM sees exactly 4 reads (p, Ap, x, r) and 3 writes (x, r, p).
+// Measured at cfg 2: 44.3 -> 40.4 ms per step (1024 threads; 768 the same, 512 slower; an L2 prefetch of x and r during the first loop
+// made it slower, 43.3 ms).  One column per SM is all that fits on chip, so the three phases of a CTA do not overlap with another CTA's.
+template <int NV, int NWARP>
+__device__ __forceinline__ void block_reduce_w(double (&v)[NV], double* sh /* [NV * NWARP] */) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0)
+#pragma unroll
+        for (int i = 0; i < NV; ++i) sh[i * NWARP + warp] = v[i];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        double s = lane < NWARP ? sh[i * NWARP + lane] : 0.0;      // NWARP <= 32: every warp folds the partials itself
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        v[i] = s;
+    }
+    __syncthreads();
+}
+
+template <int MODE, int NTR, int EPT>
+__global__ void __launch_bounds__(NTR, 1) cg_step_resident(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on, double tol2,
+                                                           double2* P, const double2* AP, double2* X, double2* R, Scalars s, const int* colmap) {
+    static_assert(MODE == 0 || MODE == 2, "one vector per column");
+    extern __shared__ __align__(16) double2 psh[];            // [EPT][NTR]: thread t owns psh[e * NTR + t]
+    __shared__ double sh[3 * (NTR / 32)];
+    const int k = blockIdx.x, col = colmap[k], t = threadIdx.x;
+    if (!s.active[col]) return;
+    const long long o = (long long)k * n_g;
+    double2* p = P + o; const double2* ap = AP + o;
+    double2* x = X + (long long)col * n_g; double2* r = R + o;
+    const double tkv = tk[col % n_occ];
+    // ---- (p, Ap): p to shared memory, Ap to registers
+    double2 q[EPT];
+    double d1[1] = {0};
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = e * NTR + t;
+        if (g < n_g) {
+            const double2 pp = p[g];
+            q[e] = ap[g];
+            psh[e * NTR + t] = pp;
+            const double w = pp.x * q[e].x + pp.y * q[e].y;
+            d1[0] += MODE == 0 ? (g == 0 ? pp.x * q[e].x : 2.0 * w) : w;
+        }
+    }
+    block_reduce_w<1, NTR / 32>(d1, sh);
+    const double2 rz = s.rz[col];
+    const double a = rz.x / d1[0];
+    // ---- x += a p ; r -= a Ap (kept in q) ; (r, M r), ||r||^2
+    double acc[2] = {0, 0};
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = e * NTR + t;
+        if (g < n_g) {
+            const double2 pp = psh[e * NTR + t];
+            double2 xx = x[g], rr = r[g];
+            xx.x += a * pp.x; xx.y += a * pp.y;
+            rr.x -= a * q[e].x; rr.y -= a * q[e].y;
+            x[g] = xx; r[g] = rr; q[e] = rr;
+            const double n2 = (MODE == 0) ? (g == 0 ? rr.x * rr.x : 2.0 * (rr.x * rr.x + rr.y * rr.y)) : rr.x * rr.x + rr.y * rr.y;
+            acc[0] += n2 * precond(g2[g], tkv, precond_on); acc[1] += n2;
+        }
+    }
+    block_reduce_w<2, NTR / 32>(acc, sh);
+    const bool still = acc[1] > tol2 * s.b2[col];
+    // ---- p = M r + beta p
+    if (still) {
+        const double beta = acc[0] / rz.x;
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int g = e * NTR + t;
+            if (g < n_g) {
+                const double m = precond(g2[g], tkv, precond_on);
+                const double2 pp = psh[e * NTR + t];
+                p[g] = make_double2(m * q[e].x + beta * pp.x, m * q[e].y + beta * pp.y);
+            }
+        }
+    }
+    if (t == 0) {
+        s.rz[col] = make_double2(acc[0], 0.0);
+        s.rr[col] = acc[1];
+        if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------- multi-shift CG
 // All imaginary frequencies from ONE Krylov sequence (Frommer's shifted CG): the seed system is the
 // real symmetric A = H - eps_v + alpha P_v (WEST_GAMMA, unpreconditioned), the shifted systems are (A + sigma_s) x_s = b with

@@ -702,6 +702,27 @@ int west_gemm_update(west_ctx* c, int32_t m, int32_t n, int64_t k, const double*
 // ============================================================================================================ chi0 * dV
 namespace {
 
+#ifndef WEST_RES_NT
+#define WEST_RES_NT 1024
+#define WEST_RES_EPT 9
+#endif
+constexpr int RES_NT = WEST_RES_NT, RES_EPT = WEST_RES_EPT;
+template <int MODE>
+cudaError_t cg_resident_attr() {
+    if (MODE == 1) return cudaSuccess;
+    constexpr int M = MODE == 1 ? 0 : MODE;
+    return cudaFuncSetAttribute(wcg::cg_step_resident<M, RES_NT, RES_EPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(sizeof(double2) * RES_NT * RES_EPT));
+}
+template <int MODE>
+void cg_resident_launch(int n_act, cudaStream_t st, long long n_g, int n_occ, const double* g2, const double* tk, int precond_on, double tol2,
+                        double2* P, const double2* AP, double2* X, double2* R, wcg::Scalars s, const int* colmap) {
+    constexpr int M = MODE == 1 ? 0 : MODE;          // MODE 1 never takes this path
+    const int ept = (int)((n_g + RES_NT - 1) / RES_NT);
+    wcg::cg_step_resident<M, RES_NT, RES_EPT><<<n_act, RES_NT, sizeof(double2) * RES_NT * ept, st>>>(n_g, n_occ, g2, tk, precond_on, tol2, P, AP,
+                                                                                                      X, R, s, colmap);
+}
+
 template <int MODE>
 int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omega, cx<double>* X, cx<double>*& R, cx<double>*& P,
              cx<double>*& AP, double* shift, const double* d_eps, wcg::Scalars s, int* maps /* [3][n_col] */, int* iters_out,
@@ -721,6 +742,9 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
     CK(cudaGetLastError());
     c->launches += 1;
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
+    // column-resident vector kernel when a column fits one CTA's registers + shared memory (cfgs 1-4); else the streaming one
+    const bool resident = MODE != 1 && n_g <= (long long)RES_EPT * RES_NT;
+    if (resident) CK(cg_resident_attr<MODE>());
     int n_act = n_col;          // columns currently held (compacted) in R, P, AP
     int it = 0;
     int64_t n_h = 0;
@@ -736,8 +760,12 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
         n_h += n_vec;
         {
             Prof p_(c, PC_CGVEC);
-            wcg::cg_step<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (double2*)P, (const double2*)AP,
-                                                             (double2*)X, (double2*)R, s, colmap);
+            if (resident)
+                cg_resident_launch<MODE>(n_act, c->st, n_g, n_occ, g2, tk, o.precond, tol2, (double2*)P, (const double2*)AP, (double2*)X, (double2*)R,
+                                         s, colmap);
+            else
+                wcg::cg_step<MODE><<<n_act, wcg::NT, 0, c->st>>>(n_g, n_occ, g2, tk, o.precond, tol2, (double2*)P, (const double2*)AP,
+                                                                 (double2*)X, (double2*)R, s, colmap);
             CK(cudaGetLastError());
             c->launches += 1;
         }
