@@ -61,7 +61,9 @@ def build(force=False, verbose=False):
     jobs = []
     for n1, n2, n, nw, minb, cu, zminb, znt in FFT_SIZES:
         o = os.path.join(OBJ, "fft_%d.o" % n)
-        extra = ["-DWEST_NW_H=6", "-DWEST_MINB_H=3", "-DWEST_GW_H=2"] if n == 72 else []      # measured: 6 warps x 3 CTAs is 3 % faster for the H*psi planes at N = 72 (16-24 resident warps all give 215-217 ms: pipe-bound)
+        # WEST_K2H="NW,MINB,GW,HOIST" overrides the H*psi plane-kernel shape at N = 72 (experiments of profiles/r01_k2_pipe_experiments.md)
+        k2h = [int(x) for x in os.environ.get("WEST_K2H", "6,3,2,0").split(",")]
+        extra = ["-DWEST_NW_H=%d" % k2h[0], "-DWEST_MINB_H=%d" % k2h[1], "-DWEST_GW_H=%d" % k2h[2], "-DWEST_TW_HOIST=%d" % k2h[3]] if n == 72 else []      # measured: 6 warps x 3 CTAs is 3 % faster for the H*psi planes at N = 72 (16-24 resident warps all give 215-217 ms: pipe-bound)
         jobs.append((o, [nvcc] + NVCC_FLAGS + extra + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_NW=%d" % nw, "-DWEST_MINB=%d" % minb, "-DWEST_CU=%d" % cu, "-DWEST_ZMINB=%d" % zminb, "-DWEST_ZNT=%d" % znt,
                                                "-c", os.path.join(CSRC, "fft_n.cu"), "-o", o]))
     o = os.path.join(OBJ, "fft_dense.o")

@@ -42,6 +42,9 @@ WHD int wrap_signed(int n, int N) { return n < N / 2 ? n : n - N; }
 #ifndef WEST_TW_POW
 #define WEST_TW_POW 1     // 1: level twiddles w^(m k) as powers of ONE table entry per thread (FP64 work traded for L1TEX wavefronts)
 #endif
+#ifndef WEST_TW_HOIST
+#define WEST_TW_HOIST 0   // 1: the H*psi plane kernel keeps each thread's level-twiddle powers in registers for the whole kernel
+#endif
 // zp[m] = z^m for m = 1 .. R-1 by binary splitting (dependency depth log2 R)
 template <typename T, int R> WHD void tw_powers(cx<T> z, cx<T> (&zp)[R]) {
     zp[0] = mk<T>(1, 0);
@@ -398,7 +401,10 @@ struct K2 {
         return (ny <= ymax && ny >= -ymax) ? Wp[c0 + ny + ymax] : mk<T>(0, 0);
     }
     // y inverse, pass A: rows of the disc straight from W
-    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp, int row0, int nrow) {
+    // zpre (yA, xA: powers of tw[N2 + n2]; xB, yC: powers of tw[N + N1 + k1]): the caller's hoisted level twiddles when every thread keeps
+    // the same n2 / k1 for the whole kernel (WEST_TW_HOIST), else NULL and the powers are formed here
+    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp, int row0, int nrow,
+                       const cx<T>* zpre = nullptr) {
         for (int it = tid; it < nrow * N2; it += nthr) {
             const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
             cx<T> v[N1];
@@ -408,7 +414,10 @@ struct K2 {
             cx<T>* dst = S + row * PITCH + n2;
 if (WEST_TW_POW) {
                 cx<T> zp[N1];
-                tw_powers<T, N1>(tw[N2 + n2], zp);
+                if (zpre) {
+#pragma unroll
+                    for (int k1 = 0; k1 < N1; ++k1) zp[k1] = zpre[k1];
+                } else tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
                 for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
             } else {
@@ -430,7 +439,7 @@ if (WEST_TW_POW) {
         }
     }
     // x inverse, pass A: gather the 2 n_max + 1 non-zero inputs of LC lines from S
-    static WHD void xA(int tid, int nthr, const cx<T>* S, cx<T>* X, const cx<T>* tw, const WestGeom& g, int py0) {
+    static WHD void xA(int tid, int nthr, const cx<T>* S, cx<T>* X, const cx<T>* tw, const WestGeom& g, int py0, const cx<T>* zpre = nullptr) {
         for (int it = tid; it < LC * N2; it += nthr) {
             const int l = it / N2, n2 = it - l * N2;
             const int py = py0 + l;
@@ -445,7 +454,10 @@ if (WEST_TW_POW) {
             cx<T>* dst = X + l * PITCH + n2;
 if (WEST_TW_POW) {
                 cx<T> zp[N1];
-                tw_powers<T, N1>(tw[N2 + n2], zp);
+                if (zpre) {
+#pragma unroll
+                    for (int k1 = 0; k1 < N1; ++k1) zp[k1] = zpre[k1];
+                } else tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
                 for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
             } else {
@@ -455,7 +467,7 @@ if (WEST_TW_POW) {
         }
     }
     // x inverse pass B, the real-space operation, x forward pass B' - all on the same N2 contiguous values
-    static WHD void xB(int tid, int nthr, cx<T>* X, const cx<T>* tw, const K2Args<T>& a, int slot, int pz, int py0) {
+    static WHD void xB(int tid, int nthr, cx<T>* X, const cx<T>* tw, const K2Args<T>& a, int slot, int pz, int py0, const cx<T>* zpre = nullptr) {
         for (int it = tid; it < LC * N1; it += nthr) {
             const int l = it / N1, k1 = it - l * N1;
             const int py = py0 + l;
@@ -511,7 +523,10 @@ if (WEST_TW_POW) {
             Dft<T, N2, -1>::run(v);
 if (WEST_TW_POW) {
                 cx<T> zp[N2];
-                tw_powers<T, N2>(tw[N + N1 + k1], zp);
+                if (zpre) {
+#pragma unroll
+                    for (int j = 0; j < N2; ++j) zp[j] = zpre[j];
+                } else tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
             } else {
@@ -539,7 +554,7 @@ if (WEST_TW_POW) {
             }
         }
     }
-    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, int row0, int nrow) {
+    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, int row0, int nrow, const cx<T>* zpre = nullptr) {
         for (int it = tid; it < nrow * N1; it += nthr) {
             const int rl = it / N1, k1 = it - rl * N1, row = row0 + rl;
             cx<T>* p = S + row * PITCH + N2 * k1;
@@ -549,7 +564,10 @@ if (WEST_TW_POW) {
             Dft<T, N2, -1>::run(v);
 if (WEST_TW_POW) {
                 cx<T> zp[N2];
-                tw_powers<T, N2>(tw[N + N1 + k1], zp);
+                if (zpre) {
+#pragma unroll
+                    for (int j = 0; j < N2; ++j) zp[j] = zpre[j];
+                } else tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
             } else {
@@ -678,10 +696,21 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T>
     const int pz = blockIdx.x, slot = blockIdx.y;
     cx<T>* Wp = a.W + ((long long)slot * N + pz) * g.n_cols;
     __syncthreads();
+    // WEST_TW_HOIST (experiment, off: profiles/r01_k2_pipe_experiments.md): when a group's GT threads cover one round of its LPG lines
+    // in every pass, a thread keeps n2 = gt % N2 (strided passes) and k1 = gt % N1 (contiguous passes) for the whole kernel, and the
+    // powers of its two table entries can stay in registers.  14 % fewer FP64 instructions, same time: the kernel is not FP64-bound.
+    constexpr bool HOIST = WEST_TW_HOIST && WEST_TW_POW && MODE == K2_H && LPG * N2 <= GT && LPG * N1 <= GT;
+    cx<T> zA[N1], zB[N2];
+    if (HOIST) {
+        tw_powers<T, N1>(tw[N2 + gt % N2], zA);
+        tw_powers<T, N2>(tw[N + N1 + gt % N1], zB);
+    }
+    const cx<T>* zAp = HOIST ? zA : nullptr;
+    const cx<T>* zBp = HOIST ? zB : nullptr;
     if (MODE != K2_FROMR) {
         for (int r0 = group * LPG; r0 < g.nr; r0 += NG * LPG) {
             const int nrow = g.nr - r0 < LPG ? g.nr - r0 : LPG;
-            K::yA(gt, GT, S, tw, g, Wp, r0, nrow);
+            K::yA(gt, GT, S, tw, g, Wp, r0, nrow, zAp);
             group_sync<GW>(group);
             K::yB(gt, GT, S, g, r0, nrow);
         }
@@ -689,10 +718,10 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T>
     }
     for (int py0 = group * LPG; py0 < N; py0 += NG * LPG) {
         if (MODE != K2_FROMR) {
-            K::xA(gt, GT, S, Xw, tw, g, py0);
+            K::xA(gt, GT, S, Xw, tw, g, py0, zAp);
             group_sync<GW>(group);
         }
-        K::xB(gt, GT, Xw, tw, a, slot, pz, py0);
+        K::xB(gt, GT, Xw, tw, a, slot, pz, py0, zBp);
         if (MODE == K2_H || MODE == K2_FROMR) {
             group_sync<GW>(group);
             K::xC(gt, GT, S, Xw, g, py0);
@@ -703,7 +732,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T>
         __syncthreads();
         for (int r0 = group * LPG; r0 < g.nr; r0 += NG * LPG) {
             const int nrow = g.nr - r0 < LPG ? g.nr - r0 : LPG;
-            K::yC(gt, GT, S, tw, g, r0, nrow);
+            K::yC(gt, GT, S, tw, g, r0, nrow, zBp);
             group_sync<GW>(group);
             K::yD(gt, GT, S, g, Wp, r0, nrow);
         }
