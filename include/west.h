@@ -59,7 +59,8 @@ extern "C" {
 #define WEST_GAMMA  1
 
 #define WEST_FP64   0   /* everything in FP64 */
-#define WEST_MIXED  1   /* FFT + real-space multiply inside H*psi in FP32; vectors, GEMMs, dots, dn in FP64 */
+#define WEST_MIXED  1   /* inside H*psi: FFT + real-space multiply in FP32, KB / P_v projector GEMMs as 3xTF32 tensor-core products
+                           (FP32 class, FP64 operands in memory); vectors, CG dots, RHS projection, dn in FP64 */
 #define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
 typedef struct west_ctx west_ctx;

@@ -37,8 +37,53 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
+// WEST_MIXED variants (template parameter TF32 = true; "matrix multiplication or FFTs ... carried out using FP32"): the same
+// FP64 operands and the same cp.async staging, but the products run on the TF32 tensor path as 3xTF32 - every operand is rounded to
+// FP32 and split into hi + lo TF32 parts, lo*hi + hi*lo + hi*hi accumulate in FP32 (error ~2^-22 per product, FP32 class) - with
+// mma.sync.m16n8k8; warp tile 64 x 32 = 4 x 4 MMA tiles.  Partial sums leave the kernel in FP64 (atomics / the FP64 vector block).
+__device__ __forceinline__ void split_tf32(double x, uint32_t& hi, uint32_t& lo) {
+    const float f = (float)x;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(f));
+    const float r = f - __uint_as_float(hi);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(r));
+}
+__device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+// one k = 8 step of a 64 x 32 warp tile: A-operand element (row, k) at pa[row * sa_row + k * sa_k], B-operand element (k, col) at
+// pb[col * sb_col + k * sb_k]; lane = 4 g + t holds rows g, g + 8 and k = t, t + 4 (A), k = t, t + 4 and col g (B)
+__device__ __forceinline__ void tf32x3_step(float (&acc)[4][4][4], const double* pa, int sa_row, int sa_k, const double* pb, int sb_col,
+                                            int sb_k, int g, int t) {
+    uint32_t ah[4][4], al[4][4], bh[4][2], bl[4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double* q = pa + (i * 16 + g) * sa_row + t * sa_k;
+        split_tf32(q[0], ah[i][0], al[i][0]);
+        split_tf32(q[8 * sa_row], ah[i][1], al[i][1]);
+        split_tf32(q[4 * sa_k], ah[i][2], al[i][2]);
+        split_tf32(q[8 * sa_row + 4 * sa_k], ah[i][3], al[i][3]);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const double* q = pb + (j * 8 + g) * sb_col + t * sb_k;
+        split_tf32(q[0], bh[j][0], bl[j][0]);
+        split_tf32(q[4 * sb_k], bh[j][1], bl[j][1]);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            mma_tf32(acc[i][j], al[i], bh[j]);
+            mma_tf32(acc[i][j], ah[i], bl[j]);
+            mma_tf32(acc[i][j], ah[i], bh[j]);
+        }
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // C[m][n] += sum_{k in this split} A[m][k] B[n][k].   lda, ldb even (16-byte aligned rows), A and B 16-byte aligned.
+template <bool TF32>
 __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, long long K, const double* __restrict__ A, long long lda,
                                                            const double* __restrict__ B, long long ldb, double* __restrict__ C,
                                                            long long ldc, long long k_per_split, int use_atomic, int splits,
@@ -56,11 +101,19 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
     long long ke = kb + k_per_split; if (ke > K) ke = K;
     const int nk = (int)((ke - kb + BK - 1) / BK);
 
-    double acc[8][4][2];
+    constexpr int NA = TF32 ? 1 : 8;
+    double acc[NA][4][2];
+    float accf[TF32 ? 4 : 1][4][4];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < NA; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll
+    for (int i = 0; i < (TF32 ? 4 : 1); ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) accf[i][j][q] = 0.f;
 
     auto load_stage = [&](int stage, int kt) {
         const long long k0 = kb + (long long)kt * BK;
@@ -92,6 +145,14 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
         cp_commit();
         const double* as = As + (size_t)(kt % STAGES) * BM * PITCH_TN + (wm * 64 + (lane >> 2)) * PITCH_TN + (lane & 3);
         const double* bs = Bs + (size_t)(kt % STAGES) * BN * PITCH_TN + (wn * 32 + (lane >> 2)) * PITCH_TN + (lane & 3);
+        if constexpr (TF32) {
+            const double* ta = As + (size_t)(kt % STAGES) * BM * PITCH_TN + wm * 64 * PITCH_TN;
+            const double* tb = Bs + (size_t)(kt % STAGES) * BN * PITCH_TN + wn * 32 * PITCH_TN;
+#pragma unroll
+            for (int kk = 0; kk < BK; kk += 8)
+                tf32x3_step(reinterpret_cast<float (&)[4][4][4]>(accf), ta + kk, PITCH_TN, 1, tb + kk, PITCH_TN, 1, lane >> 2, lane & 3);
+            continue;
+        }
 #pragma unroll
         for (int kk = 0; kk < BK; kk += 4) {
             double a[8], b[4];
@@ -106,9 +167,33 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
         }
     }
     cp_wait<0>();
+    if constexpr (TF32) {
+        // C fragment of m16n8: rows g, g + 8; cols 2 t, 2 t + 1
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int m = m0 + wm * 64 + i * 16 + h * 8 + (lane >> 2);
+                if (m >= M) continue;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int n = n0 + wn * 32 + j * 8 + 2 * (lane & 3);
+                    double* c = C + (long long)m * ldc + n;
+                    const double v0 = (double)accf[TF32 ? i : 0][j][2 * h], v1 = (double)accf[TF32 ? i : 0][j][2 * h + 1];
+                    if (use_atomic) {
+                        if (n < Nn) atomicAdd(c, v0);
+                        if (n + 1 < Nn) atomicAdd(c + 1, v1);
+                    } else {
+                        if (n < Nn) c[0] = v0;
+                        if (n + 1 < Nn) c[1] = v1;
+                    }
+                }
+            }
+        return;
+    }
     // C fragment: row = lane/4, cols 2*(lane%4), +1
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
+    for (int i = 0; i < NA; ++i) {
         const int m = m0 + wm * 64 + i * 8 + (lane >> 2);
         if (m >= M) continue;
 #pragma unroll
@@ -129,6 +214,7 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
 // ---------------------------------------------------------------------------------------------------------------------
 // Y[n][k] += sum_m C[m][n] A[m][k].  Output tile: 128 vectors (n) x 128 reals (k).  MMA roles: rows = n, cols = k,
 // contraction = m.  A-operand element (n, m) = C[m][n] (n contiguous), B-operand element (m, k) = A[m][k] (k contiguous).
+template <bool TF32>
 __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int Nn, long long K, const double* __restrict__ C, long long ldc,
                                                                const double* __restrict__ A, long long lda, double* __restrict__ Y,
                                                                long long ldy) {
@@ -141,11 +227,19 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int 
     const long long k0 = (long long)blockIdx.x * BN;
     const int nm = (M + BK - 1) / BK;
 
-    double acc[8][4][2];
+    constexpr int NA = TF32 ? 1 : 8;
+    double acc[NA][4][2];
+    float accf[TF32 ? 4 : 1][4][4];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < NA; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll
+    for (int i = 0; i < (TF32 ? 4 : 1); ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) accf[i][j][q] = 0.f;
 
     auto load_stage = [&](int stage, int mt) {
         const int mb = mt * BK;
@@ -176,6 +270,16 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int 
         // A-operand (row n = lane/4, contraction m = lane%4): Cs[m][n];  B-operand (m = lane%4, col k = lane/4): As[m][k]
         const double* cs = Cs + (size_t)(mt % STAGES) * BK * PITCH_UPC + (lane & 3) * PITCH_UPC + wm * 64 + (lane >> 2);
         const double* as = As + (size_t)(mt % STAGES) * BK * PITCH_UPA + (lane & 3) * PITCH_UPA + wn * 32 + (lane >> 2);
+        if constexpr (TF32) {
+            // MMA rows = n (A-operand element (n, m) = Cs[m][n]), cols = k (B-operand element (m, k) = As[m][k]), contraction = m
+            const double* ta = Cs + (size_t)(mt % STAGES) * BK * PITCH_UPC + wm * 64;
+            const double* tb = As + (size_t)(mt % STAGES) * BK * PITCH_UPA + wn * 32;
+#pragma unroll
+            for (int mm = 0; mm < BK; mm += 8)
+                tf32x3_step(reinterpret_cast<float (&)[4][4][4]>(accf), ta + mm * PITCH_UPC, 1, PITCH_UPC, tb + mm * PITCH_UPA, 1, PITCH_UPA,
+                            lane >> 2, lane & 3);
+            continue;
+        }
 #pragma unroll
         for (int mm = 0; mm < BK; mm += 4) {
             double a[8], b[4];
@@ -190,8 +294,28 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int 
         }
     }
     cp_wait<0>();
+    if constexpr (TF32) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int n = n0 + wm * 64 + i * 16 + h * 8 + (lane >> 2);
+                if (n >= Nn) continue;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const long long k = k0 + wn * 32 + j * 8 + 2 * (lane & 3);
+                    if (k < K) {
+                        double2* y = reinterpret_cast<double2*>(Y + (long long)n * ldy + k);
+                        double2 v = *y;
+                        v.x += (double)accf[TF32 ? i : 0][j][2 * h]; v.y += (double)accf[TF32 ? i : 0][j][2 * h + 1];
+                        *y = v;
+                    }
+                }
+            }
+        return;
+    }
+#pragma unroll
+    for (int i = 0; i < NA; ++i) {
         const int n = n0 + wm * 64 + i * 8 + (lane >> 2);
         if (n >= Nn) continue;
 #pragma unroll

@@ -274,16 +274,25 @@ int ensure_W(west_ctx* c, int n_slots, int f32) {
     return ensure(c, c->W, (size_t)n_slots * c->cell.N * c->hs.n_cols * (f32 ? 8 : 16));
 }
 
+// opt-in to the GEMM kernels' dynamic shared memory (all four instantiations), once per process
+cudaError_t gemm_attrs() {
+    using namespace wgemm;
+    static bool done = false;
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(gemm_tn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TN);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tn_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TN);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_update_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_update_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP);
+    done = e == cudaSuccess;
+    return e;
+}
+
 int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, long long lda, const double* B, long long ldb,
-                   double* C, long long ldc, int n_batch = 1, long long sA = 0, long long sB = 0, long long sC = 0, bool zero_c = true) {
+                   double* C, long long ldc, int n_batch = 1, long long sA = 0, long long sB = 0, long long sC = 0, bool zero_c = true,
+                   bool tf32 = false) {
     using namespace wgemm;
     if (M <= 0 || Nn <= 0) return WEST_OK;
-    static bool attr = false;
-    if (!attr) {
-        CK(cudaFuncSetAttribute(gemm_tn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TN));
-        CK(cudaFuncSetAttribute(gemm_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP));
-        attr = true;
-    }
+    CK(gemm_attrs());
     const int tm = (M + BM - 1) / BM, tn = (Nn + BN - 1) / BN;
     // split K so that the CTA count fills whole waves of the 148 SMs (MINB CTAs per SM): pick the split count with
     // the best wave efficiency, each split keeping at least 32 k-steps
@@ -302,24 +311,21 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
     if (zero_c) CK(cudaMemsetAsync(C, 0, (size_t)M * ldc * sizeof(double), c->st));     // batched callers zero their own output
     dim3 grid(tn, tm, (unsigned)(splits * n_batch));
     Prof prof_(c, PC_GEMM_TN);
-    gemm_tn_kernel<<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1, (int)splits, sA, sB, sC);
+    if (tf32) gemm_tn_kernel<true><<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1, (int)splits, sA, sB, sC);
+    else gemm_tn_kernel<false><<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1, (int)splits, sA, sB, sC);
     CK(cudaGetLastError());
     c->launches += 1;
     return WEST_OK;
 }
 int launch_gemm_update(west_ctx* c, int M, int Nn, long long K, const double* C, long long ldc, const double* A, long long lda,
-                       double* Y, long long ldy) {
+                       double* Y, long long ldy, bool tf32 = false) {
     using namespace wgemm;
     if (M <= 0 || Nn <= 0) return WEST_OK;
-    static bool attr = false;
-    if (!attr) {
-        CK(cudaFuncSetAttribute(gemm_tn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TN));
-        CK(cudaFuncSetAttribute(gemm_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_UP));
-        attr = true;
-    }
+    CK(gemm_attrs());
     dim3 grid((unsigned)((K + BN - 1) / BN), (unsigned)((Nn + BM - 1) / BM));
     Prof prof_(c, PC_GEMM_UP);
-    gemm_update_kernel<<<grid, NTHREADS, SMEM_UP, c->st>>>(M, Nn, K, C, ldc, A, lda, Y, ldy);
+    if (tf32) gemm_update_kernel<true><<<grid, NTHREADS, SMEM_UP, c->st>>>(M, Nn, K, C, ldc, A, lda, Y, ldy);
+    else gemm_update_kernel<false><<<grid, NTHREADS, SMEM_UP, c->st>>>(M, Nn, K, C, ldc, A, lda, Y, ldy);
     CK(cudaGetLastError());
     c->launches += 1;
     return WEST_OK;
@@ -354,7 +360,8 @@ int ensure_opmatrix(west_ctx* c, double alpha) {
 
 // Y += sum_{m in [r0, r0+nr)} coef_m A_m <A_m, X>   for n_vec real-function / complex vectors (as 2 n_g reals each).
 // coef_override: if non-NULL use this constant instead of the stored coefficients (RHS projection: -1).
-int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const double* coef_dev) {
+// tf32: the WEST_MIXED path of H*psi (3xTF32 tensor-core products, FP32 class) - never the RHS projection or the deflation
+int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const double* coef_dev, bool tf32 = false) {
     if (nr <= 0 || n_vec <= 0) return WEST_OK;
     const long long K = 2 * c->hs.n_g;
     const long long ldc = (n_vec + 1) / 2 * 2;
@@ -362,12 +369,12 @@ int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, doubl
     if (rc) return rc;
     const double* A = (const double*)c->A_all.p + (size_t)r0 * K;
     double* C = (double*)c->Cbuf.p;
-    rc = launch_gemm_tn(c, nr, n_vec, K, A, K, X, K, C, ldc);
+    rc = launch_gemm_tn(c, nr, n_vec, K, A, K, X, K, C, ldc, 1, 0, 0, 0, true, tf32);
     if (rc) return rc;
     wcg::lowrank_fix<<<blocks_for((long long)nr * n_vec, 256), 256, 0, c->st>>>(nr, n_vec, ldc, C, A, K, X, K, coef_dev, is_gamma(c) ? 1 : 0);
     CK(cudaGetLastError());
     c->launches += 1;
-    return launch_gemm_update(c, nr, n_vec, K, C, ldc, A, K, Y, K);
+    return launch_gemm_update(c, nr, n_vec, K, C, ldc, A, K, Y, K, tf32);
 }
 
 // local part of (H - shift - i omega) on vectors: Y = T x + V_loc x - shift x -+ omega terms   (no KB, no P_v)
@@ -683,7 +690,7 @@ int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, v
     if (rc) return rc;
     if (c->rows_kb > 0) {
         if ((rc = ensure_opmatrix(c, 0.0))) return rc;
-        rc = lowrank_apply(c, 0, c->rows_kb, n_vec, (const double*)x, (double*)y, (const double*)c->coef_all.p);
+        rc = lowrank_apply(c, 0, c->rows_kb, n_vec, (const double*)x, (double*)y, (const double*)c->coef_all.p, precision == WEST_MIXED);
     }
     return rc;
 }
@@ -755,7 +762,7 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
         const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
         int rc = hloc_apply(c, f32, vm, n_slots, P, AP, shift, omega);
         if (rc) return rc;
-        rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, (const double*)c->coef_all.p);
+        rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, (const double*)c->coef_all.p, f32 != 0);
         if (rc) return rc;
         n_h += n_vec;
         {
@@ -922,7 +929,7 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
         VecMap vm{2, 1, n_act, 0};
         int rc = hloc_apply(c, f32, vm, (n_act + 1) / 2, P, AP, shift, 0.0);
         if (rc) return rc;
-        rc = lowrank_apply(c, 0, rows, n_act, (const double*)P, (double*)AP, (const double*)c->coef_all.p);
+        rc = lowrank_apply(c, 0, rows, n_act, (const double*)P, (double*)AP, (const double*)c->coef_all.p, f32 != 0);
         if (rc) return rc;
         n_h += n_act;
         {
@@ -1203,7 +1210,7 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
             c->launches += 1;
         }
         if ((rc = hloc_apply(c, f32, vm, n_slots, Q, HQ, nullptr, 0.0))) return rc;
-        if (c->rows_kb > 0 && (rc = lowrank_apply(c, 0, c->rows_kb, n_col, (const double*)Q, (double*)HQ, (const double*)c->coef_all.p))) return rc;
+        if (c->rows_kb > 0 && (rc = lowrank_apply(c, 0, c->rows_kb, n_col, (const double*)Q, (double*)HQ, (const double*)c->coef_all.p, f32 != 0))) return rc;
         {
             Prof p_(c, PC_CGVEC);
             if (gamma) wlz::lz_step<true><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_steps, l, (const double2*)Q, (const double2*)HQ, (double2*)QP, alpha, beta, beta_prev);
