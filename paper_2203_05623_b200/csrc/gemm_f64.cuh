@@ -75,9 +75,15 @@ __device__ __forceinline__ void tf32x3_step(float (&acc)[4][4][4], const double*
     for (int i = 0; i < 4; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            mma_tf32(acc[i][j], al[i], bh[j]);
-            mma_tf32(acc[i][j], ah[i], bl[j]);
-            mma_tf32(acc[i][j], ah[i], bh[j]);
+            // the tensor core adds into its accumulator with truncation, a bias that grows with the number of accumulations (measured:
+            // 2e-5 relative after ~750); so the three products of a k = 8 step meet in a zeroed temporary and join the running sum
+            // through one round-to-nearest FADD per element (random-walk error, ~3e-6 at K = 18 278)
+            float tmp[4] = {0.f, 0.f, 0.f, 0.f};
+            mma_tf32(tmp, al[i], bh[j]);
+            mma_tf32(tmp, ah[i], bl[j]);
+            mma_tf32(tmp, ah[i], bh[j]);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[i][j][q] += tmp[q];
         }
 }
 

@@ -81,6 +81,29 @@ def test_h_apply_vs_matrix_free(name, n_vec):
     w.close()
 
 
+@pytest.mark.parametrize("name,n_vec", [("cfg1", 5), ("mini2", 9), ("cfg2", 70)])
+def test_mixed_nonlocal_term_is_fp32_class(name, n_vec):
+    """WEST_MIXED applies the KB projectors as 3xTF32 tensor-core GEMMs (FP32 matrix multiplication).  The nonlocal
+    term in isolation - H*psi with projectors minus H*psi without, both through the mixed path, whose local part is deterministic -
+    must agree with the oracle's sum_k beta_k D_k <beta_k|c> to FP32 class: one dropped lo*hi term, a single-pass TF32
+    product (2^-11) or a running sum kept in the tensor core's truncating accumulator would leave 1e-5 .. 5e-4."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build(name, dense=False)
+    c, cfull = random_vectors(p, n_vec, 96)
+    x = torch.from_numpy(c).cuda()
+    w, sel = make_west(p, with_states=False)
+    y_kb = w.h_apply(x, precision=wb.WEST_MIXED).cpu().numpy()
+    w.close()
+    w0, _ = make_west(p, with_states=False, with_kb=False)
+    y_loc = w0.h_apply(x, precision=wb.WEST_MIXED).cpu().numpy()
+    w0.close()
+    ref = (cfull @ np.conj(p.beta).T * np.asarray(p.dcoef)) @ p.beta
+    err = relmax(y_kb - y_loc, ref[:, sel])
+    assert err < 2e-6, err      # measured 2.4e-7 .. 4.8e-7; 7e-6 .. 2e-5 when the tensor core's truncating accumulator carried the sum
+    assert err > 1e-13          # it did not run in FP64
+
+
 @pytest.mark.parametrize("m,n,k", [(10, 32, 1030), (384, 1000, 18278), (130, 257, 4098)])
 def test_gemm_tn_and_update(m, n, k):
     import torch
