@@ -7,7 +7,7 @@ import synth
 from . import WEST_GAMMA, West
 
 
-def main(n_vec=8192, reps=5, workload="cfg2"):
+def main(n_vec=8192, reps=5, workload="cfg2", precision=0):
     cfg = synth.get_config(workload)
     w = West(cfg["L"], cfg["n2max"], cfg["N"], WEST_GAMMA)
     g = torch.Generator(device="cuda").manual_seed(1)
@@ -15,10 +15,10 @@ def main(n_vec=8192, reps=5, workload="cfg2"):
     x = torch.randn((n_vec, w.n_g), dtype=torch.float64, device="cuda", generator=g) + 0j
     y = torch.empty_like(x)
     for _ in range(2):
-        w.h_apply(x, y)
+        w.h_apply(x, y, precision=precision)
     w.set_profile(True)
     for _ in range(reps):
-        w.h_apply(x, y)
+        w.h_apply(x, y, precision=precision)
     p = w.get_profile()
     print({k: round(v["ms"] / reps, 3) for k, v in p.items() if v["spans"]})
     w.close()
@@ -28,5 +28,7 @@ if __name__ == "__main__":
     import sys
     if len(sys.argv) > 1 and sys.argv[1] == "cfg5":
         main(n_vec=1024, reps=3, workload="cfg5")
+    elif len(sys.argv) > 1 and sys.argv[1] == "mixed":
+        main(precision=1)
     else:
         main()
