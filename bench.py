@@ -47,6 +47,7 @@ def parse():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"], help="--op fft only")
     ap.add_argument("--deflate", type=int, default=0, help="number of conduction eigenstates handed to west_set_deflation (0 = off)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
+    ap.add_argument("--cg-kernel", type=int, default=0, help="west_set_cg_kernel: 0 automatic (column-resident where it fits), 1 streaming")
     return ap.parse_args()
 
 
@@ -206,6 +207,7 @@ def main():
     precision = wb.WEST_MIXED if cfg["precision"] == "mixed" else wb.WEST_FP64
     # every rank: same cell and orbitals, its own block of perturbations (seeded stream offset by rank)
     w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0), n_defl=a.deflate)
+    w.set_cg_kernel(a.cg_kernel)
     if world > 1:
         dV_np = synth.perturbations(cfg, n_pert=n_pert, first=rank * n_pert)
     dev = torch.device("cuda")

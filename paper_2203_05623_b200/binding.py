@@ -34,7 +34,7 @@ class west_stats(C.Structure):
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
            "west_fft3d", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_lanczos_diag", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
-           "west_launch_count", "west_set_fft_chunk", "west_set_profile", "west_get_profile"]
+           "west_launch_count", "west_set_fft_chunk", "west_set_cg_kernel", "west_set_profile", "west_get_profile"]
 
 
 def load_library():
@@ -64,6 +64,7 @@ def load_library():
     lib.west_launch_count.argtypes = [vp]
     lib.west_launch_count.restype = i64
     lib.west_set_fft_chunk.argtypes = [vp, i32]
+    lib.west_set_cg_kernel.argtypes = [vp, i32]
     lib.west_set_profile.argtypes = [vp, i32]
     lib.west_get_profile.argtypes = [vp, vp, vp]
     for name in EXPORTS:
@@ -283,6 +284,9 @@ class West:
 
     def launch_count(self):
         return int(self.lib.west_launch_count(self.ctx))
+
+    def set_cg_kernel(self, which):
+        self._ck(self.lib.west_set_cg_kernel(self.ctx, int(which)))
 
     def set_fft_chunk(self, n):
         self._ck(self.lib.west_set_fft_chunk(self.ctx, int(n)))

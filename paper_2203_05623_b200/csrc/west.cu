@@ -40,6 +40,7 @@ struct west_ctx {
     int64_t launches = 0;
     int64_t dev_bytes = 0;
     int fft_chunk = 0;
+    int cg_kernel = 0;                 // west_set_cg_kernel: 0 automatic, 1 always streaming
     std::vector<void*> owned;          // every cudaMalloc of this context
 
     // geometry tables
@@ -424,6 +425,11 @@ int west_get_profile(west_ctx* c, double* ms, int64_t* count) {
     c->ev_used = 0;
     return WEST_OK;
 }
+int west_set_cg_kernel(west_ctx* c, int32_t which) {
+    if (!c || (which != 0 && which != 1)) return WEST_EINVAL;
+    c->cg_kernel = which;
+    return WEST_OK;
+}
 int west_set_fft_chunk(west_ctx* c, int32_t n) {
     if (!c || n < 0 || n > 65535) return WEST_EINVAL;
     c->fft_chunk = n;
@@ -750,7 +756,7 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
     c->launches += 1;
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     // column-resident vector kernel when a column fits one CTA's registers + shared memory (cfgs 1-4); else the streaming one
-    const bool resident = MODE != 1 && n_g <= (long long)RES_EPT * RES_NT;
+    const bool resident = MODE != 1 && n_g <= (long long)RES_EPT * RES_NT && c->cg_kernel == 0;
     if (resident) CK(cg_resident_attr<MODE>());
     int n_act = n_col;          // columns currently held (compacted) in R, P, AP
     int it = 0;

@@ -11,11 +11,12 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-9
 
 
-def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500, n_defl=0):
+def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500, n_defl=0, cg_kernel=0):
     import torch
     import paper_2203_05623_b200 as wb
     p = oracle_problem.build(name)
     w, sel = make_west(p)
+    w.set_cg_kernel(cg_kernel)
     if n_defl:
         w.set_deflation(torch.from_numpy(np.ascontiguousarray(p.U[:, p.n_occ:p.n_occ + n_defl].T[:, sel])).cuda(), p.eps[p.n_occ:p.n_occ + n_defl])
     dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
@@ -107,3 +108,16 @@ def test_chi0_with_deflated_conduction_states(name, solver, omegas):
     _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
     # at omega = 0 the smallest eigenvalue of the operator is the gap and deflation must help; large omega already lifts the spectrum
     assert st["iters"] <= st0["iters"] and (omegas is not None or name == "mini3" or st["iters"] < st0["iters"])
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mini2"])
+def test_chi0_streaming_cg_kernel(name):
+    """west_set_cg_kernel(1): the streaming vector kernel (the one cfg 5 and the COCG pairs use) on cells where the default is the
+    column-resident kernel; same parity bar against the sum over states (Eq. 10-11), same iteration count."""
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run(name, cg_kernel=1, omegas=[0.0])
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    assert relmax(dn, ref_dn) < 1e-9
+    _check_dpsi(p, sel, dpsi, ref_dpsi, 1e-9)
+    _, _, dn0, _, st0, _, _ = _run(name, cg_kernel=0, omegas=[0.0])
+    assert st0["iters"] == st["iters"]
+    assert relmax(dn, dn0) < 1e-12
