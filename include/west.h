@@ -203,8 +203,9 @@ int  west_get_profile(west_ctx* ctx, double* ms, int64_t* count);
  * intermediate of a chunk is sized to stay L2-resident between the three FFT kernels. */
 int  west_set_fft_chunk(west_ctx* ctx, int32_t n_slots);
 /* Tuning knob: vector kernel of the CG iteration (steps a8 + a9).  0 (default): the column-resident kernel where a column fits one SM
- * (n_g <= 9216, omega = 0), else the streaming one; 1: always the streaming kernel.  Same results up to summation order.
- * Errors: WEST_EINVAL (NULL ctx, which not 0 / 1). */
+ * (n_g <= 9216, omega = 0), else the streaming one; 1: always the streaming kernel; 2: the resident kernel with each column split
+ * over a cluster of two CTAs (partial sums through distributed shared memory; same size limit).  Same results up to summation order.
+ * Errors: WEST_EINVAL (NULL ctx, which not 0 / 1 / 2). */
 int  west_set_cg_kernel(west_ctx* ctx, int32_t which);
 
 #ifdef __cplusplus

@@ -7,6 +7,7 @@
 // One CTA per column; vectors are [col][nvpc][n_g] complex128, nvpc = 2 in MODE 1 else 1.
 #pragma once
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 
 namespace wcg {
 
@@ -293,6 +294,91 @@ __global__ void __launch_bounds__(NTR, 1) cg_step_resident(long long n_g, int n_
     if (t == 0) {
         s.rz[col] = make_double2(acc[0], 0.0);
         s.rr[col] = acc[1];
+        if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
+    }
+}
+
+// The resident iteration with the column split over a thread-block CLUSTER of CL CTAs (distributed shared memory carries the partial
+// sums): a CTA holds 1 / CL of the column (p in shared memory, Ap / r in registers), so two CTAs of different columns share an SM and
+// one's reduction latency and store drain overlap the other's loads.  Element g = (e CL + rank) NTR + t.
+template <int MODE, int NTR, int EPT, int CL>
+__global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__(NTR, 2)
+cg_step_cluster(long long n_g, int n_occ, const double* g2, const double* tk, int precond_on, double tol2, double2* P, const double2* AP,
+                double2* X, double2* R, Scalars s, const int* colmap) {
+    static_assert(MODE == 0 || MODE == 2, "one vector per column");
+    namespace cgr = cooperative_groups;
+    cgr::cluster_group cluster = cgr::this_cluster();
+    extern __shared__ __align__(16) double2 psh[];            // [EPT][NTR]
+    __shared__ double sh[3 * (NTR / 32)];
+    __shared__ double part[3];                                // this CTA's partial sums: (p, Ap) | (r, M r), ||r||^2
+    const int rank = (int)cluster.block_rank();
+    const int k = blockIdx.x / CL, col = colmap[k], t = threadIdx.x;
+    if (!s.active[col]) return;                               // the whole cluster reads the same flag; it changes only at the very end
+    const long long o = (long long)k * n_g;
+    double2* p = P + o; const double2* ap = AP + o;
+    double2* x = X + (long long)col * n_g; double2* r = R + o;
+    const double tkv = tk[col % n_occ];
+    double2 q[EPT];
+    double d1[1] = {0};
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = (e * CL + rank) * NTR + t;
+        if (g < n_g) {
+            const double2 pp = p[g];
+            q[e] = ap[g];
+            psh[e * NTR + t] = pp;
+            const double w = pp.x * q[e].x + pp.y * q[e].y;
+            d1[0] += MODE == 0 ? (g == 0 ? pp.x * q[e].x : 2.0 * w) : w;
+        }
+    }
+    block_reduce_w<1, NTR / 32>(d1, sh);
+    if (t == 0) part[0] = d1[0];
+    cluster.sync();
+    double pap = 0;
+#pragma unroll
+    for (int c = 0; c < CL; ++c) pap += *cluster.map_shared_rank(&part[0], c);
+    const double2 rz = s.rz[col];
+    const double a = rz.x / pap;
+    double acc[2] = {0, 0};
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = (e * CL + rank) * NTR + t;
+        if (g < n_g) {
+            const double2 pp = psh[e * NTR + t];
+            double2 xx = x[g], rr = r[g];
+            xx.x += a * pp.x; xx.y += a * pp.y;
+            rr.x -= a * q[e].x; rr.y -= a * q[e].y;
+            x[g] = xx; r[g] = rr; q[e] = rr;
+            const double n2 = (MODE == 0) ? (g == 0 ? rr.x * rr.x : 2.0 * (rr.x * rr.x + rr.y * rr.y)) : rr.x * rr.x + rr.y * rr.y;
+            acc[0] += n2 * precond(g2[g], tkv, precond_on); acc[1] += n2;
+        }
+    }
+    block_reduce_w<2, NTR / 32>(acc, sh);
+    if (t == 0) { part[1] = acc[0]; part[2] = acc[1]; }
+    cluster.sync();
+    double rzn = 0, rrn = 0;
+#pragma unroll
+    for (int c = 0; c < CL; ++c) {
+        const double* pc = cluster.map_shared_rank(&part[0], c);
+        rzn += pc[1]; rrn += pc[2];
+    }
+    const bool still = rrn > tol2 * s.b2[col];
+    if (still) {
+        const double beta = rzn / rz.x;
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int g = (e * CL + rank) * NTR + t;
+            if (g < n_g) {
+                const double m = precond(g2[g], tkv, precond_on);
+                const double2 pp = psh[e * NTR + t];
+                p[g] = make_double2(m * q[e].x + beta * pp.x, m * q[e].y + beta * pp.y);
+            }
+        }
+    }
+    cluster.sync();                                           // no CTA leaves while a partner may still read its partial sums
+    if (rank == 0 && t == 0) {
+        s.rz[col] = make_double2(rzn, 0.0);
+        s.rr[col] = rrn;
         if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
     }
 }

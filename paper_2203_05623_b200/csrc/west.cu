@@ -426,7 +426,7 @@ int west_get_profile(west_ctx* c, double* ms, int64_t* count) {
     return WEST_OK;
 }
 int west_set_cg_kernel(west_ctx* c, int32_t which) {
-    if (!c || (which != 0 && which != 1)) return WEST_EINVAL;
+    if (!c || which < 0 || which > 2) return WEST_EINVAL;
     c->cg_kernel = which;
     return WEST_OK;
 }
@@ -727,6 +727,21 @@ cudaError_t cg_resident_attr() {
     return cudaFuncSetAttribute(wcg::cg_step_resident<M, RES_NT, RES_EPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)(sizeof(double2) * RES_NT * RES_EPT));
 }
+constexpr int CLU_NT = 512, CLU_EPT = 9, CLU_CL = 2;
+template <int MODE>
+cudaError_t cg_cluster_attr() {
+    constexpr int M = MODE == 1 ? 0 : MODE;
+    return cudaFuncSetAttribute(wcg::cg_step_cluster<M, CLU_NT, CLU_EPT, CLU_CL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(sizeof(double2) * CLU_NT * CLU_EPT));
+}
+template <int MODE>
+void cg_cluster_launch(int n_act, cudaStream_t st, long long n_g, int n_occ, const double* g2, const double* tk, int precond_on, double tol2,
+                       double2* P, const double2* AP, double2* X, double2* R, wcg::Scalars s, const int* colmap) {
+    constexpr int M = MODE == 1 ? 0 : MODE;
+    const int ept = (int)((n_g + (long long)CLU_NT * CLU_CL - 1) / ((long long)CLU_NT * CLU_CL));
+    wcg::cg_step_cluster<M, CLU_NT, CLU_EPT, CLU_CL><<<n_act * CLU_CL, CLU_NT, sizeof(double2) * CLU_NT * ept, st>>>(
+        n_g, n_occ, g2, tk, precond_on, tol2, P, AP, X, R, s, colmap);
+}
 template <int MODE>
 void cg_resident_launch(int n_act, cudaStream_t st, long long n_g, int n_occ, const double* g2, const double* tk, int precond_on, double tol2,
                         double2* P, const double2* AP, double2* X, double2* R, wcg::Scalars s, const int* colmap) {
@@ -757,7 +772,9 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     // column-resident vector kernel when a column fits one CTA's registers + shared memory (cfgs 1-4); else the streaming one
     const bool resident = MODE != 1 && n_g <= (long long)RES_EPT * RES_NT && c->cg_kernel == 0;
+    const bool clustered = MODE != 1 && n_g <= (long long)CLU_EPT * CLU_NT * CLU_CL && c->cg_kernel == 2;
     if (resident) CK(cg_resident_attr<MODE>());
+    if (clustered) CK(cg_cluster_attr<MODE>());
     int n_act = n_col;          // columns currently held (compacted) in R, P, AP
     int it = 0;
     int64_t n_h = 0;
@@ -773,7 +790,10 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
         n_h += n_vec;
         {
             Prof p_(c, PC_CGVEC);
-            if (resident)
+            if (clustered)
+                cg_cluster_launch<MODE>(n_act, c->st, n_g, n_occ, g2, tk, o.precond, tol2, (double2*)P, (const double2*)AP, (double2*)X, (double2*)R,
+                                        s, colmap);
+            else if (resident)
                 cg_resident_launch<MODE>(n_act, c->st, n_g, n_occ, g2, tk, o.precond, tol2, (double2*)P, (const double2*)AP, (double2*)X, (double2*)R,
                                          s, colmap);
             else

@@ -111,10 +111,12 @@ def test_chi0_with_deflated_conduction_states(name, solver, omegas):
 
 
 @pytest.mark.parametrize("name", ["cfg1", "mini2"])
-def test_chi0_streaming_cg_kernel(name):
-    """west_set_cg_kernel(1): the streaming vector kernel (the one cfg 5 and the COCG pairs use) on cells where the default is the
-    column-resident kernel; same parity bar against the sum over states (Eq. 10-11), same iteration count."""
-    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run(name, cg_kernel=1, omegas=[0.0])
+@pytest.mark.parametrize("which", [1, 2])
+def test_chi0_other_cg_kernels(name, which):
+    """west_set_cg_kernel(1): the streaming vector kernel (the one cfg 5 and the COCG pairs use); (2): the column split over a 2-CTA
+    cluster, on cells where the default is the column-resident kernel; same parity bar against the sum over states (Eq. 10-11),
+    same iteration count."""
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run(name, cg_kernel=which, omegas=[0.0])
     assert st["rc"] == 0 and st["n_unconverged"] == 0
     assert relmax(dn, ref_dn) < 1e-9
     _check_dpsi(p, sel, dpsi, ref_dpsi, 1e-9)
