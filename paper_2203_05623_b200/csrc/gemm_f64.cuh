@@ -7,6 +7,7 @@
 //   gemm_update Y[n][k] += sum_m C[m][n] A[m][k]        rank-m update of the vector block
 // Warp tile 64 x 32 (64 accumulators / thread), k step 16 through a cp.async ring.  Shared-memory rows are padded by 4
 // doubles so every fragment load is bank-conflict free.  Yardstick on the same box: cuBLAS DGEMM 35-36 TFLOP/s on these shapes.
+// Both kernels are templates on TF32: false = the FP64 DMMA path above, true = the 3xTF32 path of WEST_MIXED (see split_tf32 below).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
             const double* tb = Bs + (size_t)(kt % STAGES) * BN * PITCH_TN + wn * 32 * PITCH_TN;
 #pragma unroll
             for (int kk = 0; kk < BK; kk += 8)
-                tf32x3_step(reinterpret_cast<float (&)[4][4][4]>(accf), ta + kk, PITCH_TN, 1, tb + kk, PITCH_TN, 1, lane >> 2, lane & 3);
+                tf32x3_step(accf, ta + kk, PITCH_TN, 1, tb + kk, PITCH_TN, 1, lane >> 2, lane & 3);
             continue;
         }
 #pragma unroll
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
                 for (int j = 0; j < 4; ++j) {
                     const int n = n0 + wn * 32 + j * 8 + 2 * (lane & 3);
                     double* c = C + (long long)m * ldc + n;
-                    const double v0 = (double)accf[TF32 ? i : 0][j][2 * h], v1 = (double)accf[TF32 ? i : 0][j][2 * h + 1];
+                    const double v0 = (double)accf[i][j][2 * h], v1 = (double)accf[i][j][2 * h + 1];
                     if (use_atomic) {
                         if (n < Nn) atomicAdd(c, v0);
                         if (n + 1 < Nn) atomicAdd(c + 1, v1);
@@ -282,7 +283,7 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int 
             const double* tb = As + (size_t)(mt % STAGES) * BK * PITCH_UPA + wn * 32;
 #pragma unroll
             for (int mm = 0; mm < BK; mm += 8)
-                tf32x3_step(reinterpret_cast<float (&)[4][4][4]>(accf), ta + mm * PITCH_UPC, 1, PITCH_UPC, tb + mm * PITCH_UPA, 1, PITCH_UPA,
+                tf32x3_step(accf, ta + mm * PITCH_UPC, 1, PITCH_UPC, tb + mm * PITCH_UPA, 1, PITCH_UPA,
                             lane >> 2, lane & 3);
             continue;
         }
@@ -313,7 +314,7 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int 
                     if (k < K) {
                         double2* y = reinterpret_cast<double2*>(Y + (long long)n * ldy + k);
                         double2 v = *y;
-                        v.x += (double)accf[TF32 ? i : 0][j][2 * h]; v.y += (double)accf[TF32 ? i : 0][j][2 * h + 1];
+                        v.x += (double)accf[i][j][2 * h]; v.y += (double)accf[i][j][2 * h + 1];
                         *y = v;
                     }
                 }
