@@ -395,6 +395,12 @@ struct K2 {
     static constexpr int N = N1 * N2, PITCH = N + WEST_PAD;
     static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + 2 * N); }
 
+    // layout of V_loc for the K2_H variant: position (pz, py = py0 + l, px = N2 k1 + k2), py0 a multiple of LC
+    static constexpr int NCH = (N + LC - 1) / LC;
+    static WHD size_t vloc_elems() { return (size_t)N * NCH * N2 * LC * N1; }
+    static WHD long long vloc_index(int pz, int py0, int l, int k1, int k2) {
+        return ((((long long)pz * NCH + py0 / LC) * N2 + k2) * LC + l) * N1 + k1;
+    }
     static WHD cx<T> load_disc(const cx<T>* Wp, const WestGeom& g, int row, int n) {
         const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
         const int ny = wrap_signed(n, N);
@@ -482,11 +488,11 @@ if (WEST_TW_POW) {
                 Dft<T, N2, +1>::run(v);
             }
             if (MODE == K2_H) {
-                // V_loc is stored with the x position transposed inside each line ([pz][py][k2][k1] instead of [k1][k2]) so that for
-                // a fixed j the lanes of a line (k1 = 0..N1-1) read consecutive words: whole sectors instead of one word per sector
-                const T* V = a.V + ((long long)pz * N + py) * N + k1;
+                // V_loc is stored per chunk of LC lines as [pz][py0 / LC][k2][l][k1] (vloc_index below): for a fixed j = k2 the LC * N1
+                // threads of a line group read LC * N1 consecutive words - whole 128-byte lines instead of one 8 N1-byte piece per line
+                const T* V = a.V + vloc_index(pz, py0, l, k1, 0);
 #pragma unroll
-                for (int j = 0; j < N2; ++j) { const T w = V[j * N1]; v[j].x *= w; v[j].y *= w; }
+                for (int j = 0; j < N2; ++j) { const T w = V[j * (LC * N1)]; v[j].x *= w; v[j].y *= w; }
             } else if (MODE == K2_TOR) {
                 cx<double>* R = a.R + (long long)slot * n3 + r0;
 #pragma unroll

@@ -95,7 +95,7 @@ cudaError_t k2_entry(int f32, int mode, int n_slots, cudaStream_t st, const West
     }
     return cudaErrorInvalidValue;
 }
-const FftOps ops = {NN, N1, N2, WEST_CU, LPW, k1_entry, k2_entry, k3_entry};
+const FftOps ops = {NN, N1, N2, WEST_CU, LPW, K2Cfg<N1, N2, WEST_GW_H>::LPW, k1_entry, k2_entry, k3_entry};
 }  // namespace
 
 #define WEST_CAT2(a, b) a##b

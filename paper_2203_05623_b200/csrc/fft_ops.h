@@ -17,6 +17,7 @@ struct K2Any {                 // K2Args<T> with untyped W / V
 
 struct FftOps {
     int N, N1, N2, CU, LC;
+    int LC_H;      // lines per group of the H*psi plane kernel: fixes the V_loc layout (K2::vloc_index)
     // grid.y = slots in every launch; slot0 offsets are applied by the caller through pointer arithmetic / VecMap
     cudaError_t (*k1)(int f32, int gamma, int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, const cx<double>* X, void* W);
     cudaError_t (*k2)(int f32, int mode, int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a);

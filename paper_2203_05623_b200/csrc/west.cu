@@ -162,6 +162,18 @@ __global__ void nat_to_pos_real(int N, int N1, int N2, long long total, const do
     const int ix = j_of_p(px, N1, N2), iy = j_of_p(py, N1, N2), iz = j_of_p(pz, N1, N2);
     out[i] = (T)in[b * n3 + ((long long)ix * N + iy) * N + iz];
 }
+// V_loc, natural [ix][iy][iz] -> the plane kernel's layout [pz][py / LC][k2][py % LC][k1] (K2::vloc_index; px = N2 k1 + k2)
+template <typename T>
+__global__ void vloc_layout(int N, int N1, int N2, int LC, const double* in, T* out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)N * N * N) return;
+    long long r = i;
+    const int iz = (int)(r % N); r /= N;
+    const int iy = (int)(r % N); const int ix = (int)(r / N);
+    const int k1 = ix % N1, k2 = ix / N1, py = N2 * (iy % N1) + iy / N1, pz = N2 * (iz % N1) + iz / N1;
+    const int nch = (N + LC - 1) / LC;
+    out[((((long long)pz * nch + py / LC) * N2 + k2) * LC + py % LC) * N1 + k1] = (T)in[i];
+}
 // position order real [b][pz][py][px] -> natural [b][ix][iy][iz]
 __global__ void pos_to_nat_real(int N, int N1, int N2, long long total, const double* in, double* out, int acc = 0) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -527,12 +539,16 @@ int west_set_vloc(west_ctx* c, const double* vloc) {
     if (!c || !vloc) return fail(c, WEST_EINVAL, "west_set_vloc: NULL argument");
     const long long n3 = n3_of(c);
     int rc;
+    const int lch = c->ops->LC_H, N_ = c->cell.N;
+    const size_t nv = (size_t)N_ * ((N_ + lch - 1) / lch) * c->ops->N2 * lch * c->ops->N1;      // K2::vloc_elems(): chunks padded to LC lines
     if (!c->d_vpos) {
-        if ((rc = dev_alloc(c, (void**)&c->d_vpos, sizeof(double) * n3))) return rc;
-        if ((rc = dev_alloc(c, (void**)&c->d_vpos_f, sizeof(float) * n3))) return rc;
+        if ((rc = dev_alloc(c, (void**)&c->d_vpos, sizeof(double) * nv))) return rc;
+        if ((rc = dev_alloc(c, (void**)&c->d_vpos_f, sizeof(float) * nv))) return rc;
+        CK(cudaMemsetAsync(c->d_vpos, 0, sizeof(double) * nv, c->st));
+        CK(cudaMemsetAsync(c->d_vpos_f, 0, sizeof(float) * nv, c->st));
     }
-    nat_to_pos_real<double><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos, 1);
-    nat_to_pos_real<float><<<blocks_for(n3, 256), 256, 0, c->st>>>(c->cell.N, c->ops->N1, c->ops->N2, n3, vloc, c->d_vpos_f, 1);
+    vloc_layout<double><<<blocks_for(n3, 256), 256, 0, c->st>>>(N_, c->ops->N1, c->ops->N2, lch, vloc, c->d_vpos);
+    vloc_layout<float><<<blocks_for(n3, 256), 256, 0, c->st>>>(N_, c->ops->N1, c->ops->N2, lch, vloc, c->d_vpos_f);
     CK(cudaGetLastError());
     c->launches += 2;
     c->have_vloc = true;

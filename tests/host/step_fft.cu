@@ -28,11 +28,11 @@ void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V
     const int nslots = GAMMA ? (nvec + 1) / 2 : nvec;
     VecMap vm{GAMMA ? 2 : 1, GAMMA ? 1 : 0, nvec, 0};
     std::vector<cx<T>> W((size_t)nslots * N * s.n_cols);
-    std::vector<T> Vp((size_t)N * N * N);
-    auto jof = [&](int p) { return p / N2 + N1 * (p % N2); };
-    for (int pz = 0; pz < N; pz++) for (int py = 0; py < N; py++) for (int px = 0; px < N; px++)
-        Vp[((size_t)pz * N + py) * N + (px % N2) * N1 + px / N2] = (T)V[((size_t)jof(px) * N + jof(py)) * N + jof(pz)];   // x transposed in-line
     using KA = K1<T, N1, N2, GAMMA, CU>; using KC = K3<T, N1, N2, GAMMA, CU>; using KB = K2<T, N1, N2, K2_H, LC>;
+    std::vector<T> Vp(KB::vloc_elems(), (T)0);
+    auto jof = [&](int p) { return p / N2 + N1 * (p % N2); };
+    for (int pz = 0; pz < N; pz++) for (int py = 0; py < N; py++) for (int px = 0; px < N; px++)     // px = N2 k1 + k2
+        Vp[KB::vloc_index(pz, py - py % LC, py % LC, px / N2, px % N2)] = (T)V[((size_t)jof(px) * N + jof(py)) * N + jof(pz)];
     std::vector<cx<T>> lines(KA::NL * KA::PITCH);
     for (int slot = 0; slot < nslots; slot++) for (int u0 = 0; u0 < s.n_units; u0 += CU) {
         if (g_fused) {
