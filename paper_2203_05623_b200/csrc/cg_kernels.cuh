@@ -12,6 +12,9 @@
 namespace wcg {
 
 constexpr int NT = 256;
+#ifndef WEST_PC_C
+#define WEST_PC_C 1.35      // crossover of the default diagonal preconditioner in units of <psi_v|T|psi_v> (reading R4)
+#endif
 
 struct Scalars {
     double2* rz;      // (r, z)
@@ -60,7 +63,7 @@ __device__ __forceinline__ double precond(double g2, double tk, int on) {
         const double num = 27.0 + x * (18.0 + x * (12.0 + 8.0 * x));
         return num / (num + 16.0 * x * x * x * x);
     }
-    const double q = g2 / (1.35 * tk);
+    const double q = g2 / (WEST_PC_C * tk);
     return 1.0 / fmax(1.0, q);
 }
 
