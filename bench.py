@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"], help="--op fft only")
     ap.add_argument("--deflate", type=int, default=0, help="number of conduction eigenstates handed to west_set_deflation (0 = off)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
+    ap.add_argument("--alpha-factor", type=float, default=1.5, help="alpha_pv = factor x (eps_Nv - eps_1), reading R3 (the result does not depend on it; "
+                                                                         "must exceed 1; measured at cfg 2: 1.25 fastest, 1.5 keeps half a band width of margin, DESIGN.md R3)")
     ap.add_argument("--cg-kernel", type=int, default=0, help="west_set_cg_kernel: 0 automatic (column-resident where it fits), 1 streaming, 2 column split over a 2-CTA cluster")
     return ap.parse_args()
 
@@ -105,7 +107,7 @@ def build_inputs(cfg):
     return atoms, vloc
 
 
-def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0, vloc_add=None):
+def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0, vloc_add=None, alpha_factor=1.5):
     import torch
     import synth
     import paper_2203_05623_b200 as wb
@@ -136,7 +138,7 @@ def setup_gpu(cfg, n_pert, chunk, verbose, n_defl=0, vloc_add=None):
     if verbose:
         print("# eigensolver: %.1f s, residual %.2e, gap %.4f Ry" % (time.time() - t0, res, gap), file=sys.stderr)
     w.set_states(psi, eps[:cfg["n_occ"]])
-    alpha = max(2.0 * float(eps[cfg["n_occ"] - 1] - eps[0]), 0.01)
+    alpha = max(alpha_factor * float(eps[cfg["n_occ"] - 1] - eps[0]), 0.01)
     dV = synth.perturbations(cfg, n_pert=n_pert)
     return w, dV, alpha, dict(eps=eps, psi=psi, gap=gap, res=res, miller=miller, vloc=vloc, beta=beta, dcoef=dcoef)
 
@@ -206,7 +208,7 @@ def main():
     import paper_2203_05623_b200 as wb
     precision = wb.WEST_MIXED if cfg["precision"] == "mixed" else wb.WEST_FP64
     # every rank: same cell and orbitals, its own block of perturbations (seeded stream offset by rank)
-    w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0), n_defl=a.deflate)
+    w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0), n_defl=a.deflate, alpha_factor=a.alpha_factor)
     w.set_cg_kernel(a.cg_kernel)
     if world > 1:
         dV_np = synth.perturbations(cfg, n_pert=n_pert, first=rank * n_pert)
@@ -291,7 +293,7 @@ def main():
         "dtype": "f64" if precision == wb.WEST_FP64 else "f32 FFT / f64 vectors",
         "data": "synthetic (seeded Si-like cell, GPU-computed orbitals)",
         "config": {"workload": a.workload, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": len(omegas),
-                   "n_proj": cfg["n_proj"], "n_deflated": a.deflate, "tol": TOL, "solver": "multi-shift CG" if solver == 1 else "PCG/COCG per frequency", "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
+                   "n_proj": cfg["n_proj"], "n_deflated": a.deflate, "alpha_pv_factor": a.alpha_factor, "tol": TOL, "solver": "multi-shift CG" if solver == 1 else "PCG/COCG per frequency", "cg_iters": stats["iters"], "unconverged": stats["n_unconverged"],
                    "gap_ry": aux["gap"], "l2": "inputs per step (4 vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
         "h_apply_per_s": n_h * world / (ms * 1e-3),
         "e2e": {"value": units * a.steps / (e2e_ms * 1e-3), "unit": "perturbations/s",
