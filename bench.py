@@ -566,8 +566,8 @@ def roofline(cfg, top, prof, n_h, stats, hbm_peak, peak_src, n_cols, mixed, w, f
                         "algorithmic_flops_per_slot": fl_slot, "algorithmic_bytes_per_slot": per_slot,
                         "hbm_view": {"achieved_gbs": gbs, "peak_gbs": hbm_peak, "frac": gbs / hbm_peak, "peak_source": peak_src}})
             # shared-memory view: the four two-stage 1D passes move 8 nr N + 4 N^2 elements per plane through shared
-            # memory; peak = 128 B/clk/SM x 148 SMs x the SM clock.  Removing FP64 work from this kernel does not shorten it, removing
-            # shared-memory wavefronts does (profiles/r01_k2_l1tex_bound.md), so this is the pipe that binds
+            # memory; peak = 128 B/clk/SM x 148 SMs x the SM clock.  Removing FP64 work from this kernel does not shorten it; this is the
+            # more loaded of its two pipes (profiles/r01_k2_pipe_experiments.md)
             smem_slot = N * (8 * nr * N + 4 * N * N) * csz
             smem_peak = 128.0 * 148 * sm_clock_mhz() * 1e6 / 1e9
             smem_gbs = smem_slot * slots / t / 1e9
