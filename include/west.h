@@ -25,12 +25,30 @@
  *     supported N: 24, 36, 48, 72, 144.
  *
  * Ownership and streams
- *   Every pointer is a DEVICE pointer owned by the caller unless marked "host".  The library allocates device
- *   memory only in west_create / west_set_* / the first call of an operation at a larger batch size (internal
- *   workspace, grown lazily, never shrunk, freed by west_destroy).  All work is enqueued on the CUDA stream given to
- *   west_create (a cudaStream_t passed as void*; NULL = the legacy default stream).  Calls are asynchronous with
- *   respect to the host except where stated.  Pointers given to west_set_* are COPIED (the caller may free them after
- *   the call returns; the copy is enqueued on the stream).  A context is not thread-safe.
+ *   Every pointer is a DEVICE pointer owned by the caller unless marked "host".  Device memory is allocated only by
+ *   west_create and west_set_* (operator data: COPIES of what the caller passes, so the caller may free its arrays
+ *   after the call returns; the copy is enqueued on the stream).  The HOT calls (west_fft3d, west_h_apply,
+ *   west_chi0_apply, west_lanczos, west_lanczos_diag, the GEMMs, west_fft3d_dense) take all scratch memory from ONE
+ *   workspace block:
+ *     - west_set_workspace(ctx, ws, bytes): the caller's block.  A hot call then performs no cudaMalloc, no cudaFree
+ *       and no implicit stream synchronisation for memory; it fails with WEST_EWORKSPACE if the block is too small
+ *       (west_workspace_bytes gives the size; west_chi0_apply also accepts a smaller block and then walks the
+ *       perturbations in sub-blocks, as long as one perturbation fits).
+ *     - no workspace set (the default, convenient for tests): the context owns the block and regrows it when a call needs
+ *       more (that call synchronises the stream, frees and reallocates); west_chi0_apply sizes its sub-blocks by the
+ *       device's free memory (cudaMemGetInfo).
+ *   All work is enqueued on the CUDA stream given to west_create (a cudaStream_t passed as void*; NULL = the legacy
+ *   default stream).  Calls are asynchronous with respect to the host except: west_chi0_apply returns after its last CG
+ *   iteration has been QUEUED and the one before has FINISHED (the host reads one live-column counter per poll, one
+ *   iteration late, through an event - it never drains the stream inside the solve; with stats_opt != NULL or the
+ *   multi-shift solver it synchronises once per frequency / sub-block to read the report); west_lanczos_diag
+ *   synchronises once; west_get_profile synchronises.  A context is not thread-safe; distinct contexts are independent.
+ *
+ * Determinism
+ *   west_fft3d, west_h_apply's FFT part, the CG vector kernels and the per-column scalars are deterministic.  Two places
+ *   use FP64 atomicAdd, so their results can differ in the last bits (<= 1e-15 relative) from run to run: the dn
+ *   accumulation over the occupied states (step a10), and the split-K partial sums of west_gemm_tn (KB / P_v overlaps)
+ *   whenever the contraction is split over more than one CTA (the CG iterates, and hence dpsi and dn, inherit that).
  *
  * Errors
  *   Every int-returning call returns 0 on success, a negative WEST_E* on a hard error (nothing useful written) or the
@@ -54,6 +72,7 @@ extern "C" {
 #define WEST_ECUDA        -2
 #define WEST_ESTATE       -3   /* a required west_set_* has not been called */
 #define WEST_ENOMEM       -4
+#define WEST_EWORKSPACE   -5   /* the workspace set by west_set_workspace is too small for this call */
 
 #define WEST_FULL   0
 #define WEST_GAMMA  1
@@ -61,6 +80,14 @@ extern "C" {
 #define WEST_FP64   0   /* everything in FP64 */
 #define WEST_MIXED  1   /* inside H*psi: FFT + real-space multiply in FP32, KB / P_v projector GEMMs as 3xTF32 tensor-core products
                            (FP32 class, FP64 operands in memory); vectors, CG dots, RHS projection, dn in FP64 */
+/* operations of west_workspace_bytes */
+#define WEST_OP_FFT3D            0   /* west_fft3d,      n_pert = n_batch */
+#define WEST_OP_H_APPLY          1   /* west_h_apply,    n_pert = n_vec */
+#define WEST_OP_CHI0             2   /* west_chi0_apply, solver 0, every omega = 0 (PCG) */
+#define WEST_OP_CHI0_IW          3   /* west_chi0_apply, solver 0, some omega > 0 (COCG: two real vectors per column) */
+#define WEST_OP_CHI0_MULTISHIFT  4   /* west_chi0_apply, solver 1, n_freq frequencies */
+#define WEST_OP_LANCZOS          5   /* west_lanczos, n_freq = n_steps */
+
 #define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
 typedef struct west_ctx west_ctx;
@@ -75,7 +102,10 @@ typedef struct {
 typedef struct {
     int32_t max_iter;   /* iteration cap per column (R5), e.g. 500 */
     double  tol;        /* stop when ||r||_2 <= tol * ||b||_2 per column (R5) */
-    double  alpha_pv;   /* alpha of the alpha*P_v term (R3); the converged result does not depend on it */
+    double  alpha_pv;   /* alpha of the alpha*P_v term (R3); the converged result does not depend on it.  > 0: one constant for every
+                           column; it must exceed the occupied band width eps_max - eps_min (else H - eps_v + alpha P_v is indefinite
+                           and CG can converge to a wrong answer: WEST_EINVAL).  <= 0: the per-orbital default
+                           alpha_v = (eps_v - eps_min) + (eps_max - eps_min)/2 */
     int32_t precond;    /* 0: none; 1: M_v(G) = 1/max(1, |G|^2/(1.35 <psi_v|T|psi_v>)) (R4); 2: Teter-Payne-Allan polynomial form */
     int32_t check_every;/* host polls convergence every this many iterations (>=1) */
     int32_t solver;     /* 0: one preconditioned PCG (omega = 0) / COCG (omega > 0) solve per frequency (R7);
@@ -86,8 +116,10 @@ typedef struct {
     int32_t dn_accumulate; /* 0: dn is overwritten; 1: dn += this call's response (second spin channel: the sum over sigma) */
 } west_cg_opts;
 
-typedef struct {            /* host struct, filled when non-NULL (forces one stream synchronisation) */
-    int32_t iters;          /* iterations executed (max over columns) */
+typedef struct {            /* host struct, filled when non-NULL (one stream synchronisation per frequency and sub-block) */
+    int32_t iters;          /* CG iterations launched (max over frequencies / sub-blocks; with the lagged poll one more than the slowest column needed) */
+    int32_t iters_min;      /* fewest iterations any (non-zero) column took part in before it converged */
+    int32_t n_sub_blocks;   /* perturbation sub-blocks the call was split into to fit the workspace (1 = none) */
     int32_t n_unconverged;  /* columns above tol at exit */
     double  resid_max;      /* max over columns of ||r|| / ||b|| (recurrence residual) */
     int64_t n_h_apply;      /* vectors pushed through H in this call (real functions in GAMMA mode) */
@@ -98,6 +130,17 @@ typedef struct {            /* host struct, filled when non-NULL (forces one str
 int  west_create (west_ctx** ctx, const west_cell* cell, void* cuda_stream);
 int  west_destroy(west_ctx* ctx);
 const char* west_last_error(const west_ctx* ctx);   /* ctx may be NULL: last error of a failed west_create */
+
+/* Workspace of the hot calls (the paper's rule behind it: "data are copied to the GPU once ... and copied back only
+ * for I/O", PAPER.md:171, 183 - nothing is allocated or moved inside the solve).
+ * west_workspace_bytes: bytes the operation `op` (WEST_OP_*) needs for n_pert perturbations (vectors / grids for the FFT and H ops) and
+ *   n_freq frequencies (Lanczos: steps) at `precision`, with the operator data currently set (call it after west_set_kb / west_set_states /
+ *   west_set_deflation).  0 for a bad argument.  For the chi0 ops this is the size that runs all n_pert perturbations as ONE block.
+ * west_set_workspace: ws = DEVICE block of `bytes` bytes, 256-byte aligned, owned by the caller and retained until replaced or
+ *   west_destroy; ws = NULL returns to the context-owned lazy block.  Not a hot call (it may free the context's own block).
+ *   Errors: WEST_EINVAL (NULL ctx, misaligned block). */
+size_t west_workspace_bytes(const west_ctx* ctx, int32_t op, int32_t n_pert, int32_t n_freq, int32_t precision);
+int    west_set_workspace(west_ctx* ctx, void* ws, size_t bytes);
 
 /* Step a0 - the sphere S and its maps, computed on the HOST with integer arithmetic only.
  * All output pointers are HOST pointers, any may be NULL.  miller [n_g][3]; fft_index[n_g] = ((n_x mod N) N + (n_y mod N)) N
@@ -152,7 +195,10 @@ int  west_h_apply(west_ctx* ctx, int32_t precision, int32_t n_vec, const void* x
  *             WEST_GAMMA [n_freq][n_pert][n_occ][2][n_g] c128 - real part and imaginary part of dpsi as two real functions
  *   stats_opt NULL or HOST struct.
  * For every (frequency w, perturbation i, occupied state v) it forms b = -P_c (dV_i psi_v), solves
- * (H - eps_v - i omega_w + alpha P_v) dpsi = b by batched (one recurrence per column) preconditioned CG and accumulates dn. */
+ * (H - eps_v - i omega_w + alpha P_v) dpsi = b by batched (one recurrence per column) preconditioned CG and accumulates dn.
+ * If the workspace cannot hold all n_pert perturbations at once they are processed in sub-blocks (stats: n_sub_blocks); the result
+ * does not depend on the split.  Errors: WEST_EINVAL, WEST_ESTATE, WEST_EWORKSPACE / WEST_ENOMEM (not even one perturbation fits),
+ * WEST_ECUDA; WEST_NOTCONVERGED (> 0) when a column hit max_iter. */
 int  west_chi0_apply(west_ctx* ctx, int32_t precision, int32_t n_pert, const double* dV,
                      int32_t n_freq, const double* omega_host, const west_cg_opts* opts,
                      double* dn, void* dpsi_opt, west_stats* stats_opt);

@@ -13,7 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libwest.so")
 
 WEST_OK, WEST_NOTCONVERGED = 0, 1
-WEST_EINVAL, WEST_ECUDA, WEST_ESTATE, WEST_ENOMEM = -1, -2, -3, -4
+WEST_EINVAL, WEST_ECUDA, WEST_ESTATE, WEST_ENOMEM, WEST_EWORKSPACE = -1, -2, -3, -4, -5
+WEST_OP_FFT3D, WEST_OP_H_APPLY, WEST_OP_CHI0, WEST_OP_CHI0_IW, WEST_OP_CHI0_MULTISHIFT, WEST_OP_LANCZOS = 0, 1, 2, 3, 4, 5
 WEST_FULL, WEST_GAMMA = 0, 1
 WEST_FP64, WEST_MIXED, WEST_FP32 = 0, 1, 2
 
@@ -28,13 +29,13 @@ class west_cg_opts(C.Structure):
 
 
 class west_stats(C.Structure):
-    _fields_ = [("iters", C.c_int32), ("n_unconverged", C.c_int32), ("resid_max", C.c_double), ("n_h_apply", C.c_int64),
+    _fields_ = [("iters", C.c_int32), ("iters_min", C.c_int32), ("n_sub_blocks", C.c_int32), ("n_unconverged", C.c_int32), ("resid_max", C.c_double), ("n_h_apply", C.c_int64),
                 ("ms_rhs", C.c_float), ("ms_cg", C.c_float), ("ms_dn", C.c_float)]
 
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
            "west_fft3d", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_lanczos_diag", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
-           "west_launch_count", "west_set_fft_chunk", "west_set_cg_kernel", "west_set_profile", "west_get_profile"]
+           "west_launch_count", "west_workspace_bytes", "west_set_workspace", "west_set_fft_chunk", "west_set_cg_kernel", "west_set_profile", "west_get_profile"]
 
 
 def load_library():
@@ -63,13 +64,16 @@ def load_library():
     lib.west_device_bytes.restype = i64
     lib.west_launch_count.argtypes = [vp]
     lib.west_launch_count.restype = i64
+    lib.west_workspace_bytes.argtypes = [vp, i32, i32, i32, i32]
+    lib.west_workspace_bytes.restype = C.c_size_t
+    lib.west_set_workspace.argtypes = [vp, vp, C.c_size_t]
     lib.west_set_fft_chunk.argtypes = [vp, i32]
     lib.west_set_cg_kernel.argtypes = [vp, i32]
     lib.west_set_profile.argtypes = [vp, i32]
     lib.west_get_profile.argtypes = [vp, vp, vp]
     for name in EXPORTS:
         getattr(lib, name)
-        if name not in ("west_last_error", "west_device_bytes", "west_launch_count"):
+        if name not in ("west_last_error", "west_device_bytes", "west_launch_count", "west_workspace_bytes"):
             getattr(lib, name).restype = C.c_int
     return lib
 
@@ -110,6 +114,8 @@ class West:
         self._ck(self.lib.west_gsphere(self.ctx, C.byref(n_g), None, None, None, None))
         self.n_g = int(n_g.value)
         self.N, self.mode, self.L = int(N), int(mode), float(L)
+        self.n_occ = None          # set by set_states
+        self._ws = None            # the caller's workspace tensor (kept alive while it is set)
 
     def _ck(self, rc):
         if rc < 0:
@@ -154,6 +160,7 @@ class West:
         e = np.ascontiguousarray(eps, dtype=np.float64)
         assert psi.shape[1] == self.n_g and len(e) == psi.shape[0]
         self._ck(self.lib.west_set_states(self.ctx, int(psi.shape[0]), _dev(psi, torch.complex128), e.ctypes.data))
+        self.n_occ = int(psi.shape[0])
 
     def set_deflation(self, psi_c, eps_c):
         """n_defl eigenstates directly above the occupied ones (or None / empty to switch deflation off)."""
@@ -195,20 +202,37 @@ class West:
         self._ck(self.lib.west_h_apply(self.ctx, precision, int(x.shape[0]), _dev(x, torch.complex128), _dev(out, torch.complex128)))
         return out
 
-    def chi0_apply(self, dV, omegas, tol=1e-12, max_iter=500, alpha_pv=1.0, precond=1, check_every=4, precision=WEST_FP64, solver=0,
+    def workspace_bytes(self, op, n_pert, n_freq=1, precision=WEST_FP64):
+        return int(self.lib.west_workspace_bytes(self.ctx, int(op), int(n_pert), int(n_freq), int(precision)))
+
+    def set_workspace(self, ws):
+        """ws: a CUDA uint8 tensor the caller owns (hot calls then never allocate), or None for the context-owned lazy block."""
+        import torch
+        if ws is None:
+            self._ck(self.lib.west_set_workspace(self.ctx, None, 0))
+        else:
+            self._ck(self.lib.west_set_workspace(self.ctx, _dev(ws, torch.uint8), int(ws.numel())))
+        self._ws = ws
+
+    def chi0_apply(self, dV, omegas, tol=1e-12, max_iter=500, alpha_pv=0.0, precond=1, check_every=4, precision=WEST_FP64, solver=0,
                    dn=None, want_dpsi=False, n_occ=None, want_stats=True, occupation=2.0, accumulate=False):
-        """occupation / accumulate: the sum over spin channels of Eq. 11 (one context per channel, occupation=1, the second call
-        with accumulate=True and the first call's dn); see chi0_apply_spin."""
+        """alpha_pv <= 0 selects the library's per-orbital default (west.h).  occupation / accumulate: the sum over spin channels
+        of Eq. 11 (one context per channel, occupation=1, the second call with accumulate=True and the first call's dn); see
+        chi0_apply_spin."""
         import torch
         N = self.N
         n_pert = int(dV.shape[0])
+        assert tuple(dV.shape[1:]) == (N, N, N)
         om = np.ascontiguousarray(omegas, dtype=np.float64)
         n_freq = len(om)
         if dn is None:
             dn = torch.empty((n_freq, n_pert, N, N, N), dtype=torch.float64, device=dV.device)
+        assert tuple(dn.shape) == (n_freq, n_pert, N, N, N), "dn must be [n_freq][n_pert][N][N][N]"
         dpsi = None
         if want_dpsi:
-            assert n_occ is not None
+            # the library writes with the orbital count given to set_states: size the block from that
+            assert self.n_occ is not None and (n_occ is None or int(n_occ) == self.n_occ), "n_occ differs from set_states"
+            n_occ = self.n_occ
             shape = (n_freq, n_pert, n_occ, 2, self.n_g) if self.mode == WEST_GAMMA else (n_freq, n_pert, n_occ, self.n_g)
             dpsi = torch.empty(shape, dtype=torch.complex128, device=dV.device)
         opts = west_cg_opts(int(max_iter), float(tol), float(alpha_pv), int(precond), int(check_every), int(solver), float(occupation), int(bool(accumulate)))
@@ -225,7 +249,7 @@ class West:
         """N_spin = 2: channels = [West_up, West_down], each holding its own V_loc^sigma, projectors and
         occupied orbitals.  dn = sum over channels, each with one electron per orbital.  alpha_pv may be a pair (one per channel).
         Returns dn and the list of per-channel stats."""
-        alpha = kw.pop("alpha_pv", 1.0)
+        alpha = kw.pop("alpha_pv", 0.0)
         alphas = list(alpha) if isinstance(alpha, (list, tuple)) else [alpha] * len(channels)
         dn, stats = None, []
         for k, w in enumerate(channels):

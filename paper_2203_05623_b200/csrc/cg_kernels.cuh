@@ -21,6 +21,7 @@ struct Scalars {
     double*  rr;      // Hermitian ||r||^2
     double*  b2;      // ||b||^2
     int*     active;  // 1 while ||r|| > tol ||b||
+    int*     iters;   // iterations this column took part in
     int*     counters;   // [0] number of active columns after the last p-update
 };
 
@@ -130,6 +131,7 @@ __global__ void __launch_bounds__(NT) cg_init(long long n_g, int n_occ, const do
         s.rr[col] = acc[2];
         const int act = acc[2] > 0.0;
         s.active[col] = act;
+        s.iters[col] = 0;
         if (act) atomicAdd(s.counters, 1);
     }
 }
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(NT) cg_step(long long n_g, int n_occ, const do
                                               double2* P, const double2* AP, double2* X, double2* R, Scalars s, const int* colmap) {
     __shared__ double sh[32];
     const int k = blockIdx.x, col = colmap[k], nvpc = MODE == 1 ? 2 : 1;
-    if (!s.active[col]) return;
+    if (col < 0 || !s.active[col]) return;       // col < 0: inert padding of a lagged compaction (cg_compact_map)
     const long long o = (long long)k * nvpc * n_g;
     double2* p = P + o; const double2* ap = AP + o;
     double2* x = X + (long long)col * nvpc * n_g; double2* r = R + o;
@@ -203,6 +205,7 @@ __global__ void __launch_bounds__(NT) cg_step(long long n_g, int n_occ, const do
     if (threadIdx.x == 0) {
         s.rz[col] = rznew;
         s.rr[col] = acc[2];
+        s.iters[col] += 1;
         if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
     }
 }
@@ -242,7 +245,7 @@ __global__ void __launch_bounds__(NTR, 1) cg_step_resident(long long n_g, int n_
     extern __shared__ __align__(16) double2 psh[];            // [EPT][NTR]: thread t owns psh[e * NTR + t]
     __shared__ double sh[3 * (NTR / 32)];
     const int k = blockIdx.x, col = colmap[k], t = threadIdx.x;
-    if (!s.active[col]) return;
+    if (col < 0 || !s.active[col]) return;
     const long long o = (long long)k * n_g;
     double2* p = P + o; const double2* ap = AP + o;
     double2* x = X + (long long)col * n_g; double2* r = R + o;
@@ -297,6 +300,7 @@ __global__ void __launch_bounds__(NTR, 1) cg_step_resident(long long n_g, int n_
     if (t == 0) {
         s.rz[col] = make_double2(acc[0], 0.0);
         s.rr[col] = acc[1];
+        s.iters[col] += 1;
         if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
     }
 }
@@ -316,7 +320,7 @@ cg_step_cluster(long long n_g, int n_occ, const double* g2, const double* tk, in
     __shared__ double part[3];                                // this CTA's partial sums: (p, Ap) | (r, M r), ||r||^2
     const int rank = (int)cluster.block_rank();
     const int k = blockIdx.x / CL, col = colmap[k], t = threadIdx.x;
-    if (!s.active[col]) return;                               // the whole cluster reads the same flag; it changes only at the very end
+    if (col < 0 || !s.active[col]) return;                    // the whole cluster reads the same flag; it changes only at the very end
     const long long o = (long long)k * n_g;
     double2* p = P + o; const double2* ap = AP + o;
     double2* x = X + (long long)col * n_g; double2* r = R + o;
@@ -382,6 +386,7 @@ cg_step_cluster(long long n_g, int n_occ, const double* g2, const double* tk, in
     if (rank == 0 && t == 0) {
         s.rz[col] = make_double2(rzn, 0.0);
         s.rr[col] = rrn;
+        s.iters[col] += 1;
         if (!still) { s.active[col] = 0; atomicSub(s.counters, 1); }
     }
 }
@@ -406,6 +411,7 @@ struct MsState {
     double2* zeta_prev;  // [n_shift][n_col]
     double*  res2;       // [n_shift][n_col] |zeta|^2 rr / b2 at the moment the shift was frozen (or now)
     int*     active;     // [n_col]
+    int*     iters;      // [n_col] iterations this column took part in
     int*     sactive;    // [n_shift][n_col]
     int*     counters;   // [0] live columns
 };
@@ -439,6 +445,7 @@ __global__ void __launch_bounds__(NT) ms_init(long long n_g, int n_col, MsShifts
         st.rr[col] = acc[0]; st.b2[col] = acc[0]; st.a_prev[col] = 1.0; st.b_prev[col] = 0.0;
         const int act = acc[0] > 0.0;
         st.active[col] = act;
+        st.iters[col] = 0;
         if (act) atomicAdd(st.counters, 1);
         for (int s = 0; s < sh.n; ++s) {
             const long long i = (long long)s * n_col + col;
@@ -454,7 +461,7 @@ __global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts
     __shared__ double2 s_zn[MS_MAX_SHIFTS], s_as[MS_MAX_SHIFTS], s_bs[MS_MAX_SHIFTS];
     __shared__ int s_on[MS_MAX_SHIFTS];
     const int k = blockIdx.x, col = colmap[k];
-    if (!st.active[col]) return;
+    if (col < 0 || !st.active[col]) return;
     double2* p = P + (long long)k * n_g; const double2* ap = AP + (long long)k * n_g; double2* r = R + (long long)k * n_g;
     // ---- a_k
     double acc[1] = {0};
@@ -525,49 +532,53 @@ __global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts
     __syncthreads();
     if (threadIdx.x == 0) {
         st.a_prev[col] = a; st.b_prev[col] = b; st.rr[col] = rrn;
+        st.iters[col] += 1;
         int any = 0;
         for (int s = 0; s < sh.n; ++s) any |= st.sactive[(long long)s * n_col + col];
         if (!any) { st.active[col] = 0; atomicSub(st.counters, 1); }
     }
 }
 
-// per-frequency report of the multi-shift solve: out[0] = max relative residual, out[1] = number of unconverged (col, shift)
+// block-wide min / max / sum helpers of the final reports (one CTA of NT threads)
+__device__ __forceinline__ void report_reduce(double m, int c, int lo, int hi, double* out) {
+    __shared__ double shm[NT]; __shared__ int shc[NT], shlo[NT], shhi[NT];
+    shm[threadIdx.x] = m; shc[threadIdx.x] = c; shlo[threadIdx.x] = lo; shhi[threadIdx.x] = hi;
+    __syncthreads();
+    for (int o = NT / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            shm[threadIdx.x] = fmax(shm[threadIdx.x], shm[threadIdx.x + o]); shc[threadIdx.x] += shc[threadIdx.x + o];
+            shlo[threadIdx.x] = min(shlo[threadIdx.x], shlo[threadIdx.x + o]); shhi[threadIdx.x] = max(shhi[threadIdx.x], shhi[threadIdx.x + o]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[0] = sqrt(shm[0]); out[1] = (double)shc[0]; out[2] = (double)(shlo[0] == 0x7fffffff ? 0 : shlo[0]); out[3] = (double)shhi[0]; }
+}
+// final report, out[4]: max relative residual, number of unconverged (column[, shift]) pairs, min and max over the non-zero columns of
+// the iterations a column took part in
 __global__ void ms_report(int n_col, int n_shift, double tol2, MsState st, double* out) {
-    __shared__ double shm[NT]; __shared__ int shc[NT];
-    double m = 0; int c = 0;
+    double m = 0; int c = 0, lo = 0x7fffffff, hi = 0;
     for (long long i = threadIdx.x; i < (long long)n_col * n_shift; i += NT) {
         const double q = st.res2[i];
         m = fmax(m, q); c += q > tol2;
     }
-    shm[threadIdx.x] = m; shc[threadIdx.x] = c;
-    __syncthreads();
-    for (int o = NT / 2; o > 0; o >>= 1) {
-        if (threadIdx.x < o) { shm[threadIdx.x] = fmax(shm[threadIdx.x], shm[threadIdx.x + o]); shc[threadIdx.x] += shc[threadIdx.x + o]; }
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) { out[0] = sqrt(shm[0]); out[1] = (double)shc[0]; }
+    for (int i = threadIdx.x; i < n_col; i += NT)
+        if (st.b2[i] > 0) { lo = min(lo, st.iters[i]); hi = max(hi, st.iters[i]); }
+    report_reduce(m, c, lo, hi, out);
 }
-
-// max over columns of sqrt(rr/b2), and count of columns above tol (final report)
-__global__ void cg_report(int n_col, double tol2, Scalars s, double* out /* [2]: resid_max, n_unconverged */) {
-    __shared__ double shm[NT]; __shared__ int shc[NT];
-    double m = 0; int c = 0;
+__global__ void cg_report(int n_col, double tol2, Scalars s, double* out) {
+    double m = 0; int c = 0, lo = 0x7fffffff, hi = 0;
     for (int i = threadIdx.x; i < n_col; i += NT) {
         const double b2 = s.b2[i];
-        if (b2 > 0) { const double q = s.rr[i] / b2; m = fmax(m, q); c += q > tol2; }
+        if (b2 > 0) { const double q = s.rr[i] / b2; m = fmax(m, q); c += q > tol2; lo = min(lo, s.iters[i]); hi = max(hi, s.iters[i]); }
     }
-    shm[threadIdx.x] = m; shc[threadIdx.x] = c;
-    __syncthreads();
-    for (int o = NT / 2; o > 0; o >>= 1) {
-        if (threadIdx.x < o) { shm[threadIdx.x] = fmax(shm[threadIdx.x], shm[threadIdx.x + o]); shc[threadIdx.x] += shc[threadIdx.x + o]; }
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) { out[0] = sqrt(shm[0]); out[1] = (double)shc[0]; }
+    report_reduce(m, c, lo, hi, out);
 }
 
 // Compaction of the active columns (order preserving).  One CTA: new_map[j] = original column of the j-th still-active
-// entry of old_map[0..n_old), src[j] = its old compacted position.
-__global__ void __launch_bounds__(1024) cg_compact_map(int n_old, const int* old_map, const int* active, int* new_map, int* src) {
+// entry of old_map[0..n_old), src[j] = its old compacted position.  The host asks for n_new columns, the count it read one
+// iteration ago (lagged poll); columns that converged since leave fewer, and the rest is padded with inert entries
+// (new_map = -1: skipped by the vector kernels; src = 0: a copy of finite data for the FFT / GEMM batches).
+__global__ void __launch_bounds__(1024) cg_compact_map(int n_old, const int* old_map, const int* active, int* new_map, int* src, int n_new) {
     __shared__ int warp_sums[32];
     __shared__ int base;
     if (threadIdx.x == 0) base = 0;
@@ -589,11 +600,12 @@ __global__ void __launch_bounds__(1024) cg_compact_map(int n_old, const int* old
         }
         __syncthreads();
         const int before = base + v - flag + ((threadIdx.x >> 5) ? warp_sums[(threadIdx.x >> 5) - 1] : 0);
-        if (flag) { new_map[before] = col; src[before] = i; }
+        if (flag && before < n_new) { new_map[before] = col; src[before] = i; }
         __syncthreads();
         if (threadIdx.x == 0) base += warp_sums[31];
         __syncthreads();
     }
+    for (int j = base + threadIdx.x; j < n_new; j += 1024) { new_map[j] = -1; src[j] = 0; }
 }
 // dst[j] = src_vec[src[j]] for whole columns (nvpc * n_g complex each)
 __global__ void __launch_bounds__(NT) cg_gather_cols(long long len, const int* src, const double2* in, double2* out) {
@@ -602,15 +614,25 @@ __global__ void __launch_bounds__(NT) cg_gather_cols(long long len, const int* s
     for (long long g = threadIdx.x; g < len; g += NT) b[g] = a[g];
 }
 
-// C[m][n] <- coef[m] * (gamma ? 2 C[m][n] - A[m][0] X[n][0] : C[m][n])      (A[m][0], X[n][0]: real part of G = 0)
+// C[m][n] <- coef(m, n) * (gamma ? 2 C[m][n] - A[m][0] X[n][0] : C[m][n])      (A[m][0], X[n][0]: real part of G = 0)
+// coef(m, n) = dcoef[m] for the first n_rows_d rows (KB: D_k); for the others alpha_vec[orbital of column n] if given (alpha_v P_v,
+// reading R3; colmap: compacted -> original column, nvpc vectors per column, orbital = column mod n_occ), else alpha_const.
 __global__ void lowrank_fix(int M, int Nn, long long ldc, double* C, const double* A, long long lda, const double* X, long long ldx,
-                            const double* coef, int gamma) {
+                            const double* dcoef, int n_rows_d, double alpha_const, const double* alpha_vec, const int* colmap, int nvpc,
+                            int n_occ, int gamma) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= (long long)M * Nn) return;
     const int m = (int)(i / Nn), n = (int)(i - (long long)m * Nn);
     double c = C[(long long)m * ldc + n];
     if (gamma) c = 2.0 * c - A[(long long)m * lda] * X[(long long)n * ldx];
-    C[(long long)m * ldc + n] = coef[m] * c;
+    double coef;
+    if (m < n_rows_d) coef = dcoef[m];
+    else if (alpha_vec) {
+        int col = n / nvpc;
+        if (colmap) { col = colmap[col]; if (col < 0) col = 0; }
+        coef = alpha_vec[col % n_occ];
+    } else coef = alpha_const;
+    C[(long long)m * ldc + n] = coef * c;
 }
 
 }  // namespace wcg

@@ -26,6 +26,18 @@ std::string g_create_error;
 struct DevBuf {
     void* p = nullptr;
     size_t bytes = 0;
+    uint64_t epoch = 0;        // hot buffers only: the arena epoch (= hot call) this carve-out belongs to
+};
+
+// Workspace arena of the hot calls ("the caller allocates every device buffer including the workspace; the library never
+// allocates or frees in a hot call").  Either the caller's block (west_set_workspace) or, while none is set, a block the context owns and
+// grows on demand (the documented lazy mode: growth synchronises the stream, frees and reallocates).  Every hot call starts a new epoch
+// and carves its buffers from offset 0 (bump allocation, 256-byte alignment).
+struct Arena {
+    char* base = nullptr;
+    size_t cap = 0, off = 0;
+    bool user = false;
+    uint64_t epoch = 0;
 };
 
 }  // namespace
@@ -56,11 +68,13 @@ struct west_ctx {
     int n_occ_user = 0;                // orbitals the caller handed to west_set_states (layout of dpsi / Lanczos outputs)
     int rows_kb = 0, rows_psi = 0;     // rows of the stacked real operator matrix (x2 in WEST_FULL)
     int n_defl = 0, rows_defl = 0;     // optional deflation states (lowest conduction orbitals), stacked after the psi rows
-    DevBuf A_defl, eps_defl, craw, dcoef_defl;
+    DevBuf A_defl, eps_defl;           // operator data (west_set_deflation)
+    DevBuf dcoef_dev, eps_dev;         // operator data: device copies of D_k and eps_v
+    DevBuf craw, dcoef_defl;           // hot
     long long craw_ld = 0;
     std::vector<double> h_eps_defl;
     DevBuf A_kb, A_psi;                // [rows][2 n_g] f64 each (kept apart; concatenated lazily into A_all)
-    DevBuf A_all, coef_all;            // [rows_kb + rows_psi][2 n_g], coef [rows]
+    DevBuf A_all;                      // [rows_kb + rows_psi + rows_defl][2 n_g]
     bool A_dirty = true;
     std::vector<double> h_dcoef;       // per stacked KB row
     std::vector<double> h_eps;
@@ -69,9 +83,15 @@ struct west_ctx {
     int n_uslots = 0;
     std::map<int, void*> dense_tw;     // twiddle tables of west_fft3d_dense, one per grid size used
 
-    // workspaces (grown lazily)
-    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst;
-    int* h_pinned = nullptr;           // pinned host scratch for convergence polling / reports
+    double* d_dcoef = nullptr;         // [rows_kb] D_k per stacked KB row (device copy made in west_set_kb)
+    double* d_eps = nullptr;           // [n_occ] eigenvalues (device copy made in west_set_states)
+    double eps_min = 0, eps_max = 0;   // extent of the occupied band (alpha_pv validation / the per-orbital default)
+
+    // hot-call workspaces: carved from the arena at the start of every hot call (hot_begin / hot)
+    Arena arena;
+    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk;
+    int* h_pinned = nullptr;           // pinned host scratch (64 ints): lagged convergence polls [0], [1]; reports [8..]
+    cudaEvent_t ev_poll[2] = {nullptr, nullptr};
 
     // optional per-kernel-class timing (west_set_profile): CUDA events on the context's stream around every launch
     bool profile = false;
@@ -123,6 +143,54 @@ int ensure(west_ctx* c, DevBuf& b, size_t bytes) {
     int rc = dev_alloc(c, &b.p, bytes);
     if (rc == WEST_OK) b.bytes = bytes;
     return rc;
+}
+
+inline size_t al256(size_t b) { return (std::max<size_t>(b, 16) + 255) & ~(size_t)255; }
+
+// Start of a hot call that needs `need` bytes of workspace (the sum of al256 over its buffers).
+int hot_begin(west_ctx* c, size_t need) {
+    Arena& a = c->arena;
+    a.epoch += 1;
+    a.off = 0;
+    if (need <= a.cap) return WEST_OK;
+    if (a.user)
+        return fail(c, WEST_EWORKSPACE, "the workspace set by west_set_workspace holds %zu bytes, this call needs %zu (west_workspace_bytes)", a.cap, need);
+    // lazy mode: the context owns the arena and regrows it (synchronises the stream; documented in west.h)
+    if (a.base) {
+        cudaStreamSynchronize(c->st);
+        cudaFree(a.base);
+        c->dev_bytes -= (int64_t)a.cap;
+        a.base = nullptr; a.cap = 0;
+    }
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, need);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, WEST_ENOMEM, "cudaMalloc of a %zu-byte workspace failed: %s", need, cudaGetErrorString(e));
+    }
+    a.base = (char*)p; a.cap = need;
+    c->dev_bytes += (int64_t)need;
+    return WEST_OK;
+}
+// Carve (or re-use within the same hot call) a workspace buffer.
+int hot(west_ctx* c, DevBuf& b, size_t bytes) {
+    Arena& a = c->arena;
+    if (b.epoch == a.epoch && b.p && b.bytes >= bytes) return WEST_OK;
+    const size_t n = al256(bytes);
+    if (a.off + n > a.cap)
+        return fail(c, WEST_EWORKSPACE, "workspace exhausted: %zu + %zu > %zu bytes (a sizing error of the library, or a workspace smaller than west_workspace_bytes)", a.off, n, a.cap);
+    b.p = a.base + a.off; b.bytes = n; b.epoch = a.epoch;
+    a.off += n;
+    return WEST_OK;
+}
+// bytes the hot arena may take: the caller's block, or (lazy mode) what the device has free plus what the context's own arena holds
+size_t arena_budget(const west_ctx* c) {
+    if (c->arena.user) return c->arena.cap;
+    size_t fr = 0, tot = 0;
+    if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return c->arena.cap; }
+    const size_t margin = (size_t)1 << 30;      // leave 1 GB to the caller / allocator granularity
+    const size_t avail = fr + c->arena.cap;
+    return avail > margin ? avail - margin : 0;
 }
 
 // profiling classes
@@ -262,7 +330,11 @@ __global__ void kinetic_expect(long long n_g, int gamma, const double* g2, const
 }
 __global__ void fill_shift(int n_vec, int nvpc, int n_occ, const double* eps, double* shift, const int* colmap) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_vec) shift[i] = eps[(colmap ? colmap[i / nvpc] : i / nvpc) % n_occ];
+    if (i < n_vec) {
+        int col = i / nvpc;
+        if (colmap) { col = colmap[col]; if (col < 0) col = 0; }      // -1: inert padding column of a lagged compaction
+        shift[i] = eps[col % n_occ];
+    }
 }
 
 inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
@@ -283,9 +355,12 @@ int chunk_slots(const west_ctx* c, int f32) {
     if (n > 32768) n = 32768;
     return (int)n;
 }
-int ensure_W(west_ctx* c, int n_slots, int f32) {
-    return ensure(c, c->W, (size_t)n_slots * c->cell.N * c->hs.n_cols * (f32 ? 8 : 16));
+size_t bytes_W(const west_ctx* c, long long n_slots, int f32) {
+    const long long n = std::max<long long>(1, std::min<long long>(chunk_slots(c, f32), n_slots));
+    return (size_t)n * c->cell.N * c->hs.n_cols * (f32 ? 8 : 16);
 }
+int ensure_W(west_ctx* c, long long n_slots, int f32) { return hot(c, c->W, bytes_W(c, n_slots, f32)); }
+size_t bytes_C(int rows, long long n_vec) { return (size_t)rows * (size_t)((n_vec + 1) / 2 * 2) * sizeof(double); }
 
 // opt-in to the GEMM kernels' dynamic shared memory (all four instantiations), once per process
 cudaError_t gemm_attrs() {
@@ -344,47 +419,47 @@ int launch_gemm_update(west_ctx* c, int M, int Nn, long long K, const double* C,
     return WEST_OK;
 }
 
-// (re)build the concatenated operator matrix [KB rows ; psi rows] and its coefficient vector
-int ensure_opmatrix(west_ctx* c, double alpha) {
+// (re)build the concatenated operator matrix [KB rows ; psi rows ; deflation rows] (operator data: grown outside the hot arena, only
+// after a west_set_* call changed it)
+int ensure_opmatrix(west_ctx* c) {
     const long long K = 2 * c->hs.n_g;
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
-    if (rows == 0) return WEST_OK;
-    if (c->A_dirty) {
-        int rc = ensure(c, c->A_all, (size_t)rows * K * sizeof(double));
-        if (rc) return rc;
-        rc = ensure(c, c->coef_all, (size_t)rows * sizeof(double));
-        if (rc) return rc;
-        if (c->rows_kb) CK(cudaMemcpyAsync(c->A_all.p, c->A_kb.p, (size_t)c->rows_kb * K * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
-        if (c->rows_psi)
-            CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)c->rows_kb * K, c->A_psi.p, (size_t)c->rows_psi * K * sizeof(double),
-                               cudaMemcpyDeviceToDevice, c->st));
-        if (c->rows_defl)
-            CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)(c->rows_kb + c->rows_psi) * K, c->A_defl.p,
-                               (size_t)c->rows_defl * K * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
-        c->A_dirty = false;
-    }
-    std::vector<double> coef(rows);
-    for (int i = 0; i < c->rows_kb; ++i) coef[i] = c->h_dcoef[i];
-    for (int i = 0; i < c->rows_psi + c->rows_defl; ++i) coef[c->rows_kb + i] = alpha;     // alpha (P_v + P_deflated)
-    // stream-ordered copy from a pageable vector is synchronous with respect to the host buffer: safe
-    CK(cudaMemcpyAsync(c->coef_all.p, coef.data(), rows * sizeof(double), cudaMemcpyHostToDevice, c->st));
+    if (rows == 0 || !c->A_dirty) return WEST_OK;
+    int rc = ensure(c, c->A_all, (size_t)rows * K * sizeof(double));
+    if (rc) return rc;
+    if (c->rows_kb) CK(cudaMemcpyAsync(c->A_all.p, c->A_kb.p, (size_t)c->rows_kb * K * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+    if (c->rows_psi)
+        CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)c->rows_kb * K, c->A_psi.p, (size_t)c->rows_psi * K * sizeof(double),
+                           cudaMemcpyDeviceToDevice, c->st));
+    if (c->rows_defl)
+        CK(cudaMemcpyAsync((double*)c->A_all.p + (size_t)(c->rows_kb + c->rows_psi) * K, c->A_defl.p,
+                           (size_t)c->rows_defl * K * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+    c->A_dirty = false;
     return WEST_OK;
 }
 
+// coefficients of the low-rank terms (applied by wcg::lowrank_fix to the overlap block C[m][n]):
+//   rows [0, n_rows_d) of the block take dcoef[m] (the KB D_k); the remaining rows (psi / deflation rows) take alpha_vec[orbital of
+//   column n] if alpha_vec is given, else the constant alpha_const (RHS projection: -1)
+struct LowrankCoef {
+    const double* dcoef = nullptr; int n_rows_d = 0;
+    double alpha_const = 0.0; const double* alpha_vec = nullptr; const int* colmap = nullptr; int nvpc = 1, n_occ = 1;
+};
+
 // Y += sum_{m in [r0, r0+nr)} coef_m A_m <A_m, X>   for n_vec real-function / complex vectors (as 2 n_g reals each).
-// coef_override: if non-NULL use this constant instead of the stored coefficients (RHS projection: -1).
 // tf32: the WEST_MIXED path of H*psi (3xTF32 tensor-core products, FP32 class) - never the RHS projection or the deflation
-int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const double* coef_dev, bool tf32 = false) {
+int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const LowrankCoef& lc, bool tf32 = false) {
     if (nr <= 0 || n_vec <= 0) return WEST_OK;
     const long long K = 2 * c->hs.n_g;
     const long long ldc = (n_vec + 1) / 2 * 2;
-    int rc = ensure(c, c->Cbuf, (size_t)nr * ldc * sizeof(double));
+    int rc = hot(c, c->Cbuf, bytes_C(nr, n_vec));
     if (rc) return rc;
     const double* A = (const double*)c->A_all.p + (size_t)r0 * K;
     double* C = (double*)c->Cbuf.p;
     rc = launch_gemm_tn(c, nr, n_vec, K, A, K, X, K, C, ldc, 1, 0, 0, 0, true, tf32);
     if (rc) return rc;
-    wcg::lowrank_fix<<<blocks_for((long long)nr * n_vec, 256), 256, 0, c->st>>>(nr, n_vec, ldc, C, A, K, X, K, coef_dev, is_gamma(c) ? 1 : 0);
+    wcg::lowrank_fix<<<blocks_for((long long)nr * n_vec, 256), 256, 0, c->st>>>(nr, n_vec, ldc, C, A, K, X, K, lc.dcoef, lc.n_rows_d, lc.alpha_const,
+                                                                             lc.alpha_vec, lc.colmap, lc.nvpc, lc.n_occ, is_gamma(c) ? 1 : 0);
     CK(cudaGetLastError());
     c->launches += 1;
     return launch_gemm_update(c, nr, n_vec, K, C, ldc, A, K, Y, K, tf32);
@@ -409,6 +484,28 @@ int hloc_apply(west_ctx* c, int f32, VecMap vm, int n_slots, const cx<double>* X
         c->launches += 3;
     }
     return WEST_OK;
+}
+
+// ---- workspace plans: the sum of al256(bytes) over the buffers a hot call carves (west_workspace_bytes returns exactly these)
+int fft3d_chunk(const west_ctx* c, int n_slots) { return std::max(1, std::min(n_slots, std::min(chunk_slots(c, 0), 64))); }
+size_t plan_fft3d(const west_ctx* c, int n_batch) {
+    const int n_slots = is_gamma(c) ? (n_batch + 1) / 2 : n_batch;
+    const int chunk = fft3d_chunk(c, n_slots);
+    return al256(bytes_W(c, chunk, 0)) + al256(sizeof(cx<double>) * (size_t)n3_of(c) * chunk);
+}
+size_t plan_lanczos(const west_ctx* c, int n_pert, int n_steps, int f32) {
+    const size_t n_col = (size_t)n_pert * c->n_occ;
+    const long long slots_h = is_gamma(c) ? ((long long)n_col + 1) / 2 : (long long)n_col, slots_r = (long long)n_pert * c->n_uslots;
+    size_t t = 4 * al256(sizeof(cx<double>) * (size_t)c->hs.n_g * n_col) + al256(sizeof(double) * (size_t)n3_of(c) * n_pert) + al256(sizeof(double) * n_col + 64) +
+               al256(bytes_W(c, std::max(slots_h, slots_r), 0)) + al256(256);
+    if (c->rows_kb > 0) t += al256(bytes_C(c->rows_kb, (long long)n_col));
+    if (c->n_occ_user != c->n_occ) t += al256(sizeof(double) * n_col * (2 * (size_t)n_steps + 1));
+    (void)f32;
+    return t;
+}
+size_t plan_happly(const west_ctx* c, long long n_vec, int f32) {
+    const long long n_slots = is_gamma(c) ? (n_vec + 1) / 2 : n_vec;
+    return al256(bytes_W(c, n_slots, f32)) + (c->rows_kb > 0 ? al256(bytes_C(c->rows_kb, n_vec)) : 0);
 }
 
 }  // namespace
@@ -499,8 +596,23 @@ int west_create(west_ctx** out, const west_cell* cell, void* stream) {
     if (e == cudaSuccess) e = cudaMemcpy(c->d_unit_zmax, s.unit_zmax.data(), sizeof(int) * s.n_units, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(c->d_tw, tw.data(), sizeof(cx<double>) * s.N, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(c->d_g2, s.g2.data(), sizeof(double) * s.n_g, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_pinned, 64);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_pinned, 64 * sizeof(int));
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_poll[0], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_poll[1], cudaEventDisableTiming);
     if (e != cudaSuccess) { fail(c, WEST_ECUDA, "west_create: %s", cudaGetErrorString(e)); return bail(WEST_ECUDA); }
+    // twiddle tables of west_fft3d_dense (all three grid sizes, 7 KB): no allocation in the hot call
+    for (int n : {64, 128, 256}) {
+        std::vector<cx<double>> dtw(n);
+        for (int i = 0; i < n; ++i) {
+            const double a = 2.0 * 3.14159265358979323846264338327950288 * (double)i / (double)n;
+            dtw[i].x = std::cos(a); dtw[i].y = std::sin(a);
+        }
+        dtw[0] = mk<double>(1, 0); dtw[n / 4] = mk<double>(0, 1); dtw[n / 2] = mk<double>(-1, 0); dtw[3 * n / 4] = mk<double>(0, -1);
+        void* d = nullptr;
+        if ((rc = dev_alloc(c, &d, sizeof(cx<double>) * n))) return bail(rc);
+        if (cudaMemcpy(d, dtw.data(), sizeof(cx<double>) * n, cudaMemcpyHostToDevice) != cudaSuccess) { fail(c, WEST_ECUDA, "west_create: twiddle copy"); return bail(WEST_ECUDA); }
+        c->dense_tw.emplace(n, d);
+    }
     WestGeom& g = c->geom;
     g.N = s.N; g.n_max = s.n_max; g.nr = s.nr; g.n_cols = s.n_cols; g.n_units = s.n_units; g.gamma = s.gamma; g.n_g = s.n_g;
     g.row_off = c->d_row_off; g.unit_off = c->d_unit_off; g.unit_zmax = c->d_unit_zmax; g.tw = c->d_tw; g.g2 = c->d_g2;
@@ -512,7 +624,9 @@ int west_destroy(west_ctx* c) {
     if (!c) return WEST_OK;
     cudaStreamSynchronize(c->st);
     for (void* p : c->owned) cudaFree(p);
+    if (c->arena.base && !c->arena.user) cudaFree(c->arena.base);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_poll) if (e) cudaEventDestroy(e);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     delete c;
     return WEST_OK;
@@ -570,6 +684,9 @@ int west_set_kb(west_ctx* c, int32_t n_proj, const void* beta, const double* dco
     if (n_proj == 0) return WEST_OK;
     int rc = ensure(c, c->A_kb, (size_t)c->rows_kb * 2 * n_g * sizeof(double));
     if (rc) return rc;
+    if ((rc = ensure(c, c->dcoef_dev, sizeof(double) * c->rows_kb))) return rc;
+    c->d_dcoef = (double*)c->dcoef_dev.p;
+    CK(cudaMemcpy(c->d_dcoef, c->h_dcoef.data(), sizeof(double) * c->rows_kb, cudaMemcpyHostToDevice));
     stack_rows<<<blocks_for(n_g * n_proj, 256), 256, 0, c->st>>>(n_g, n_proj, full, (const cx<double>*)beta, (double*)c->A_kb.p);
     CK(cudaGetLastError());
     c->launches += 1;
@@ -596,6 +713,11 @@ int west_set_states(west_ctx* c, int32_t n_occ_user, const void* psi, const doub
     stack_rows<<<blocks_for(n_g * n_occ_user, 256), 256, 0, c->st>>>(n_g, n_occ_user, full, (const cx<double>*)psi, (double*)c->A_psi.p);
     CK(cudaGetLastError());
     if ((rc = ensure(c, c->tk, sizeof(double) * n_occ))) return rc;
+    if ((rc = ensure(c, c->eps_dev, sizeof(double) * n_occ))) return rc;
+    c->d_eps = (double*)c->eps_dev.p;
+    CK(cudaMemcpy(c->d_eps, c->h_eps.data(), sizeof(double) * n_occ, cudaMemcpyHostToDevice));
+    c->eps_min = *std::min_element(eps_host, eps_host + n_occ_user);
+    c->eps_max = *std::max_element(eps_host, eps_host + n_occ_user);
     kinetic_expect<<<n_occ_user, 256, 0, c->st>>>(n_g, is_gamma(c), c->d_g2, (const cx<double>*)psi, (double*)c->tk.p);
     CK(cudaGetLastError());
     if (n_occ > n_occ_user) {
@@ -607,18 +729,25 @@ int west_set_states(west_ctx* c, int32_t n_occ_user, const void* psi, const doub
     // u_v(r) cache in position order: GAMMA packs (v, v+1) as u_v + i u_{v+1}
     c->n_uslots = full ? n_occ : (n_occ + 1) / 2;
     if ((rc = ensure(c, c->ucache, sizeof(cx<double>) * n3 * c->n_uslots))) return rc;
-    const int chunk = std::max(1, std::min(c->n_uslots, chunk_slots(c, 0)));
-    if ((rc = ensure_W(c, chunk, 0))) return rc;
+    // a set-up call may allocate: the stick intermediate of this one transform is a temporary of its own (not the hot arena)
+    const int chunk = std::max(1, std::min(c->n_uslots, std::min(chunk_slots(c, 0), 256)));
+    void* Wtmp = nullptr;
+    cudaError_t e = cudaMalloc(&Wtmp, bytes_W(c, chunk, 0));
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(c, WEST_ENOMEM, "west_set_states: cudaMalloc of the transform buffer failed: %s", cudaGetErrorString(e)); }
     VecMap vm{full ? 1 : 2, full ? 0 : 1, n_occ_user, 0};       // vectors >= n_vec read as zero: the padding orbital
-    for (int s0 = 0; s0 < c->n_uslots; s0 += chunk) {
+    cudaError_t ke = cudaSuccess;
+    for (int s0 = 0; s0 < c->n_uslots && ke == cudaSuccess; s0 += chunk) {
         const int ns = std::min(chunk, c->n_uslots - s0);
         vm.slot0 = s0;
         K2Any a{};
-        a.W = c->W.p; a.R = (cx<double>*)c->ucache.p + (long long)s0 * n3;
-        CK(c->ops->k1(0, is_gamma(c), ns, c->st, c->geom, vm, (const cx<double>*)psi, c->W.p));
-        CK(c->ops->k2(0, K2_TOR, ns, c->st, c->geom, a));
+        a.W = Wtmp; a.R = (cx<double>*)c->ucache.p + (long long)s0 * n3;
+        ke = c->ops->k1(0, is_gamma(c), ns, c->st, c->geom, vm, (const cx<double>*)psi, Wtmp);
+        if (ke == cudaSuccess) ke = c->ops->k2(0, K2_TOR, ns, c->st, c->geom, a);
         c->launches += 2;
     }
+    cudaStreamSynchronize(c->st);
+    cudaFree(Wtmp);
+    if (ke != cudaSuccess) return fail(c, WEST_ECUDA, "west_set_states: %s", cudaGetErrorString(ke));
     return WEST_OK;
 }
 
@@ -648,10 +777,11 @@ int west_fft3d(west_ctx* c, int32_t dir, int32_t precision, int32_t n_batch, con
     const int gamma = is_gamma(c), N = c->cell.N;
     const long long n3 = n3_of(c);
     const int n_slots = gamma ? (n_batch + 1) / 2 : n_batch;
-    const int chunk = std::max(1, std::min(n_slots, std::min(chunk_slots(c, 0), 64)));
+    const int chunk = fft3d_chunk(c, n_slots);
     int rc;
+    if ((rc = hot_begin(c, plan_fft3d(c, n_batch)))) return rc;
     if ((rc = ensure_W(c, chunk, 0))) return rc;
-    if ((rc = ensure(c, c->Rbuf, sizeof(cx<double>) * n3 * chunk))) return rc;
+    if ((rc = hot(c, c->Rbuf, sizeof(cx<double>) * n3 * chunk))) return rc;
     VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_batch, 0};
     K2Any a{};
     a.W = c->W.p; a.R = (cx<double>*)c->Rbuf.p;
@@ -681,19 +811,7 @@ int west_fft3d_dense(west_ctx* c, int32_t n, int32_t sign, int32_t precision, in
     if (!west_dense_fft_supported(n)) return fail(c, WEST_EINVAL, "west_fft3d_dense: n = %d is not built (64, 128, 256)", n);
     if (n_batch == 0) return WEST_OK;
     auto it = c->dense_tw.find(n);
-    if (it == c->dense_tw.end()) {
-        std::vector<cx<double>> tw(n);
-        for (int i = 0; i < n; ++i) {
-            const double a = 2.0 * 3.14159265358979323846264338327950288 * (double)i / (double)n;
-            tw[i].x = std::cos(a); tw[i].y = std::sin(a);
-        }
-        tw[0] = mk<double>(1, 0); tw[n / 4] = mk<double>(0, 1); tw[n / 2] = mk<double>(-1, 0); tw[3 * n / 4] = mk<double>(0, -1);
-        void* d = nullptr;
-        int rc = dev_alloc(c, &d, sizeof(cx<double>) * n);
-        if (rc) return rc;
-        CK(cudaMemcpy(d, tw.data(), sizeof(cx<double>) * n, cudaMemcpyHostToDevice));
-        it = c->dense_tw.emplace(n, d).first;
-    }
+    if (it == c->dense_tw.end()) return fail(c, WEST_EINVAL, "west_fft3d_dense: no twiddle table for n = %d", n);
     Prof pf(c, PC_FFT_OTHER);
     CK(west_dense_fft3d(n, precision == WEST_FP32, sign, n_batch, c->st, in, out, it->second));
     c->launches += 3;
@@ -708,11 +826,13 @@ int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, v
     const int gamma = is_gamma(c);
     const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
     VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
-    int rc = hloc_apply(c, precision == WEST_MIXED, vm, n_slots, (const cx<double>*)x, (cx<double>*)y, nullptr, 0.0);
-    if (rc) return rc;
+    int rc;
+    if ((rc = ensure_opmatrix(c))) return rc;
+    if ((rc = hot_begin(c, plan_happly(c, n_vec, precision == WEST_MIXED)))) return rc;
+    if ((rc = hloc_apply(c, precision == WEST_MIXED, vm, n_slots, (const cx<double>*)x, (cx<double>*)y, nullptr, 0.0))) return rc;
     if (c->rows_kb > 0) {
-        if ((rc = ensure_opmatrix(c, 0.0))) return rc;
-        rc = lowrank_apply(c, 0, c->rows_kb, n_vec, (const double*)x, (double*)y, (const double*)c->coef_all.p, precision == WEST_MIXED);
+        LowrankCoef lc; lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb;
+        rc = lowrank_apply(c, 0, c->rows_kb, n_vec, (const double*)x, (double*)y, lc, precision == WEST_MIXED);
     }
     return rc;
 }
@@ -767,10 +887,45 @@ void cg_resident_launch(int n_act, cudaStream_t st, long long n_g, int n_occ, co
                                                                                                       X, R, s, colmap);
 }
 
+// Lagged convergence poll (reading R5 allows late masking): the live-column count written by iteration k is copied to pinned host memory
+// behind iteration k's kernels and READ by the host only after iteration k+1 has been queued, so the stream never drains inside the
+// solve.  The host's column count n_act is therefore an upper bound of the device's (cg_compact_map pads the difference with inert
+// columns), and the iteration after the last live column converged is launched on inactive columns (its kernels change nothing).
+struct Poller {
+    int slot = 0, pending = -1;
+    cudaError_t post(west_ctx* c, const int* dev_counter) {
+        cudaError_t e = cudaMemcpyAsync(c->h_pinned + slot, dev_counter, sizeof(int), cudaMemcpyDeviceToHost, c->st);
+        if (e == cudaSuccess) e = cudaEventRecord(c->ev_poll[slot], c->st);
+        pending = slot; slot ^= 1;
+        return e;
+    }
+    bool ready() const { return pending >= 0; }
+    int collect(west_ctx* c) {
+        cudaEventSynchronize(c->ev_poll[pending]);
+        const int v = c->h_pinned[pending];
+        pending = -1;
+        return v;
+    }
+};
+
+// drop converged columns from the working set (r -> AP buffer, p -> old r buffer; rotation by the caller)
+int compact_columns(west_ctx* c, int n_act, int n_new, long long len, int*& colmap, int*& newmap, int* src, const int* active, cx<double>*& R,
+                    cx<double>*& P, cx<double>*& AP) {
+    Prof p_(c, PC_CGVEC);
+    wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, colmap, active, newmap, src, n_new);
+    wcg::cg_gather_cols<<<n_new, wcg::NT, 0, c->st>>>(len, src, (const double2*)R, (double2*)AP);
+    wcg::cg_gather_cols<<<n_new, wcg::NT, 0, c->st>>>(len, src, (const double2*)P, (double2*)R);
+    CK(cudaGetLastError());
+    c->launches += 3;
+    cx<double>* oldR = R; cx<double>* oldP = P;
+    R = AP; P = oldR; AP = oldP;           // AP (scratch) now holds r, the old r buffer holds p
+    std::swap(colmap, newmap);
+    return WEST_OK;
+}
+
 template <int MODE>
 int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omega, cx<double>* X, cx<double>*& R, cx<double>*& P,
-             cx<double>*& AP, double* shift, const double* d_eps, wcg::Scalars s, int* maps /* [3][n_col] */, int* iters_out,
-             int64_t* n_h_out) {
+             cx<double>*& AP, double* shift, wcg::Scalars s, int* maps /* [3][n_col] */, int* iters_out, int64_t* n_h_out, int* live_out) {
     const long long n_g = c->hs.n_g;
     const int nvpc = MODE == 1 ? 2 : 1, n_occ = c->n_occ;
     const long long len = (long long)nvpc * n_g;
@@ -791,17 +946,21 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
     const bool clustered = MODE != 1 && n_g <= (long long)CLU_EPT * CLU_NT * CLU_CL && c->cg_kernel == 2;
     if (resident) CK(cg_resident_attr<MODE>());
     if (clustered) CK(cg_cluster_attr<MODE>());
-    int n_act = n_col;          // columns currently held (compacted) in R, P, AP
-    int it = 0;
+    int n_act = n_col;          // columns currently held (compacted) in R, P, AP: an upper bound of the device's live count
+    int it = 0, live = n_col;
     int64_t n_h = 0;
-    for (; it < o.max_iter; ++it) {
+    Poller poll;
+    bool done = false;
+    for (; it < o.max_iter && !done; ++it) {
         // slots of the H application: GAMMA pairs vectors (2s, 2s+1) - in MODE 1 these are (Re, Im) of one column
         const int n_vec = n_act * nvpc;
         VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
         const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
         int rc = hloc_apply(c, f32, vm, n_slots, P, AP, shift, omega);
         if (rc) return rc;
-        rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, (const double*)c->coef_all.p, f32 != 0);
+        LowrankCoef lc;
+        lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb; lc.alpha_vec = (const double*)c->alpha_v.p; lc.colmap = colmap; lc.nvpc = nvpc; lc.n_occ = n_occ;
+        rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)AP, lc, f32 != 0);
         if (rc) return rc;
         n_h += n_vec;
         {
@@ -818,32 +977,36 @@ int cg_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, double omeg
             CK(cudaGetLastError());
             c->launches += 1;
         }
-        if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
-            CK(cudaMemcpyAsync(c->h_pinned, s.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
-            CK(cudaStreamSynchronize(c->st));
-            const int live = c->h_pinned[0];
-            if (live <= 0) { ++it; break; }
+        if (poll.ready()) {                       // the count as of the previous polled iteration; this iteration is already queued
+            live = poll.collect(c);
+            if (live <= 0) done = true;
             // drop converged columns from the working set when that removes at least ~6 % of it (a1-a9 then run on fewer vectors)
-            if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
-                Prof p_(c, PC_CGVEC);
-                wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, colmap, s.active, newmap, src);
-                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(len, src, (const double2*)R, (double2*)AP);
-                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(len, src, (const double2*)P, (double2*)R);
-                CK(cudaGetLastError());
-                c->launches += 3;
-                cx<double>* oldR = R; cx<double>* oldP = P;
-                R = AP; P = oldR; AP = oldP;           // rotate: AP (scratch) now holds r, the old r buffer holds p
-                std::swap(colmap, newmap);
+            else if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
+                if ((rc = compact_columns(c, n_act, live, len, colmap, newmap, src, s.active, R, P, AP))) return rc;
                 n_act = live;
-                fill_shift<<<blocks_for(n_act * nvpc, 256), 256, 0, c->st>>>(n_act * nvpc, nvpc, n_occ, d_eps, shift, colmap);
+                fill_shift<<<blocks_for(n_act * nvpc, 256), 256, 0, c->st>>>(n_act * nvpc, nvpc, n_occ, c->d_eps, shift, colmap);
                 CK(cudaGetLastError());
                 c->launches += 1;
             }
         }
+        if (!done && ((it + 1) % every == 0 || it + 1 == o.max_iter)) CK(poll.post(c, s.counters));
     }
+    if (poll.ready()) live = poll.collect(c);     // cap reached: the exact final count
     *iters_out = it;
     *n_h_out = n_h;
+    *live_out = live;
     return WEST_OK;
+}
+
+__global__ void fill_const(int n, double v, double* out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = v;
+}
+// alpha_v of the alpha P_v term (reading R3): the caller's constant, or (alpha_user <= 0) the per-orbital default
+// alpha_v = (eps_v - eps_min) + W/2, W the occupied band width: H - eps_v + alpha_v P_v is then >= W/2 on the occupied space for every v
+__global__ void fill_alpha(int n_occ, const double* eps, double eps_min, double width, double alpha_user, double* out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_occ) out[i] = alpha_user > 0 ? alpha_user : fmax(eps[i] - eps_min + 0.5 * width, 0.01);
 }
 
 // a1: b = -P_c (dV_i psi_v) written into R ([n_col][nvpc][n_g]; the imaginary-part vectors of nvpc = 2 stay zero)
@@ -852,7 +1015,7 @@ int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R, double sign = -1.
     const long long n_g = c->hs.n_g;
     const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
     const int chunk = std::max(1, chunk_slots(c, 0));
-    int rc = ensure_W(c, std::min(chunk, std::max(n_rslots, 1)), 0);
+    int rc = ensure_W(c, std::max(n_rslots, 1), 0);
     if (rc) return rc;
     if (nvpc == 2) CK(cudaMemsetAsync(R, 0, sizeof(cx<double>) * n_g * n_vec, c->st));
     // slot (i, us) -> columns i*n_occ + 2us (+1)  [GAMMA] or i*n_occ + us
@@ -869,17 +1032,14 @@ int chi0_rhs(west_ctx* c, int n_pert, int nvpc, cx<double>* R, double sign = -1.
         c->launches += 2;
     }
     if (!project) return WEST_OK;
-    // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows
-    const int rows_p = c->rows_psi + c->rows_defl;        // P_v and, if set, the deflated conduction states
-    if ((rc = ensure(c, c->misc, sizeof(double) * std::max(rows_p, 8)))) return rc;
-    std::vector<double> m1(rows_p, -1.0);
-    CK(cudaMemcpyAsync(c->misc.p, m1.data(), sizeof(double) * rows_p, cudaMemcpyHostToDevice, c->st));
-    CK(cudaStreamSynchronize(c->st));     // m1 is a stack-lifetime pageable buffer
-    if ((rc = lowrank_apply(c, c->rows_kb, rows_p, n_vec, (const double*)R, (double*)R, (const double*)c->misc.p))) return rc;
+    // R <- R - Psi (Psi^T R): coefficient -1 on the psi rows (and, if set, the deflated conduction states)
+    const int rows_p = c->rows_psi + c->rows_defl;
+    LowrankCoef lc; lc.alpha_const = -1.0;
+    if ((rc = lowrank_apply(c, c->rows_kb, rows_p, n_vec, (const double*)R, (double*)R, lc))) return rc;
     if (c->rows_defl > 0) {
         // Cbuf now holds <psi_m | dV psi_v> for every projector row: keep the deflation rows for the closed-form part of the solution
         const long long ldc = (n_vec + 1) / 2 * 2;
-        if ((rc = ensure(c, c->craw, sizeof(double) * (size_t)c->rows_defl * ldc))) return rc;
+        if ((rc = hot(c, c->craw, sizeof(double) * (size_t)c->rows_defl * ldc))) return rc;
         c->craw_ld = ldc;
         CK(cudaMemcpyAsync(c->craw.p, (const double*)c->Cbuf.p + (size_t)c->rows_psi * ldc, sizeof(double) * (size_t)c->rows_defl * ldc,
                            cudaMemcpyDeviceToDevice, c->st));
@@ -906,17 +1066,17 @@ __global__ void defl_coef(int rows, int mult, int n_col, int in_nvpc, int out_nv
     D[(long long)m * ld_out + n] = d;
 }
 
-int add_deflated(west_ctx* c, int n_col, int in_nvpc, int out_nvpc, double omega, const double* d_eps, cx<double>* X) {
+int add_deflated(west_ctx* c, int n_col, int in_nvpc, int out_nvpc, double omega, cx<double>* X) {
     if (c->rows_defl == 0) return WEST_OK;
     const long long K = 2 * c->hs.n_g;
     const int n_out = n_col * out_nvpc;
     const long long ldo = (n_out + 1) / 2 * 2;
-    int rc = ensure(c, c->dcoef_defl, sizeof(double) * (size_t)c->rows_defl * ldo);
+    int rc = hot(c, c->dcoef_defl, sizeof(double) * (size_t)c->rows_defl * ldo);
     if (rc) return rc;
     CK(cudaMemsetAsync(c->dcoef_defl.p, 0, sizeof(double) * (size_t)c->rows_defl * ldo, c->st));
     defl_coef<<<blocks_for((long long)c->rows_defl * n_out, 256), 256, 0, c->st>>>(
         c->rows_defl, is_gamma(c) ? 1 : 2, n_col, in_nvpc, out_nvpc, c->n_occ, c->craw_ld, (const double*)c->craw.p, ldo,
-        (double*)c->dcoef_defl.p, (const double*)c->eps_defl.p, d_eps, omega);
+        (double*)c->dcoef_defl.p, (const double*)c->eps_defl.p, c->d_eps, omega);
     CK(cudaGetLastError());
     c->launches += 1;
     const double* A = (const double*)c->A_all.p + (size_t)(c->rows_kb + c->rows_psi) * K;
@@ -930,7 +1090,7 @@ int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_o
     const double vol = c->cell.L * c->cell.L * c->cell.L;
     const int n_uslots = c->n_uslots, n_rslots = n_pert * n_uslots;
     const int chunk = std::max(1, chunk_slots(c, 0));
-    int rc = ensure_W(c, std::min(chunk, std::max(n_rslots, 1)), 0);
+    int rc = ensure_W(c, std::max(n_rslots, 1), 0);
     if (rc) return rc;
     CK(cudaMemsetAsync(c->dnpos.p, 0, sizeof(double) * n3 * n_pert, c->st));
     VecMap vm{gamma ? 2 * nvpc : 1, gamma ? nvpc : 0, n_vec, 0};
@@ -950,10 +1110,23 @@ int chi0_dn(west_ctx* c, int n_pert, int nvpc, const cx<double>* X, double* dn_o
     return WEST_OK;
 }
 
+// converged solutions -> the caller's dpsi block of this (frequency, perturbation sub-block): out column (i, v < n_user), parts_out
+// vectors per column; the solver's column (i, v) holds parts_in vectors (parts beyond it are written as zero)
+__global__ void __launch_bounds__(wcg::NT) dpsi_gather(long long n_g, int n_occ, int n_user, int parts_in, int parts_out, const double2* X, double2* out) {
+    const int b = blockIdx.x;                      // (i * n_user + v) * parts_out + q
+    const int q = b % parts_out, cv = b / parts_out, v = cv % n_user, i = cv / n_user;
+    double2* dst = out + (long long)b * n_g;
+    if (q < parts_in) {
+        const double2* src = X + (((long long)i * n_occ + v) * parts_in + q) * n_g;
+        for (long long g = threadIdx.x; g < n_g; g += wcg::NT) dst[g] = src[g];
+    } else {
+        for (long long g = threadIdx.x; g < n_g; g += wcg::NT) dst[g] = make_double2(0.0, 0.0);
+    }
+}
+
 // multi-shift CG (WEST_GAMMA): all frequencies from one unpreconditioned Krylov sequence of the real seed operator
 int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::MsShifts& sh, cx<double>*& R, cx<double>*& P, cx<double>*& AP,
-             cx<double>* XS, cx<double>* PS, int want_imag, double* shift, const double* d_eps, wcg::MsState st, int* maps, int* iters_out,
-             int64_t* n_h_out) {
+             cx<double>* XS, cx<double>* PS, int want_imag, double* shift, wcg::MsState st, int* maps, int* iters_out, int64_t* n_h_out) {
     const long long n_g = c->hs.n_g;
     const int n_occ = c->n_occ;
     const double tol2 = o.tol * o.tol;
@@ -967,11 +1140,15 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     int n_act = n_col, it = 0;
     int64_t n_h = 0;
-    for (; it < o.max_iter; ++it) {
+    Poller poll;
+    bool done = false;
+    for (; it < o.max_iter && !done; ++it) {
         VecMap vm{2, 1, n_act, 0};
         int rc = hloc_apply(c, f32, vm, (n_act + 1) / 2, P, AP, shift, 0.0);
         if (rc) return rc;
-        rc = lowrank_apply(c, 0, rows, n_act, (const double*)P, (double*)AP, (const double*)c->coef_all.p, f32 != 0);
+        LowrankCoef lc;
+        lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb; lc.alpha_vec = (const double*)c->alpha_v.p; lc.colmap = colmap; lc.nvpc = 1; lc.n_occ = n_occ;
+        rc = lowrank_apply(c, 0, rows, n_act, (const double*)P, (double*)AP, lc, f32 != 0);
         if (rc) return rc;
         n_h += n_act;
         {
@@ -981,31 +1158,65 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
             CK(cudaGetLastError());
             c->launches += 1;
         }
-        if ((it + 1) % every == 0 || it + 1 == o.max_iter) {
-            CK(cudaMemcpyAsync(c->h_pinned, st.counters, sizeof(int), cudaMemcpyDeviceToHost, c->st));
-            CK(cudaStreamSynchronize(c->st));
-            const int live = c->h_pinned[0];
-            if (live <= 0) { ++it; break; }
-            if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
-                Prof p_(c, PC_CGVEC);
-                wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, colmap, st.active, newmap, src);
-                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(n_g, src, (const double2*)R, (double2*)AP);
-                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(n_g, src, (const double2*)P, (double2*)R);
-                CK(cudaGetLastError());
-                c->launches += 3;
-                cx<double>* oldR = R; cx<double>* oldP = P;
-                R = AP; P = oldR; AP = oldP;
-                std::swap(colmap, newmap);
+        if (poll.ready()) {
+            const int live = poll.collect(c);
+            if (live <= 0) done = true;
+            else if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
+                if ((rc = compact_columns(c, n_act, live, n_g, colmap, newmap, src, st.active, R, P, AP))) return rc;
                 n_act = live;
-                fill_shift<<<blocks_for(n_act, 256), 256, 0, c->st>>>(n_act, 1, n_occ, d_eps, shift, colmap);
+                fill_shift<<<blocks_for(n_act, 256), 256, 0, c->st>>>(n_act, 1, n_occ, c->d_eps, shift, colmap);
                 CK(cudaGetLastError());
                 c->launches += 1;
             }
         }
+        if (!done && ((it + 1) % every == 0 || it + 1 == o.max_iter)) CK(poll.post(c, st.counters));
     }
+    if (poll.ready()) poll.collect(c);
     *iters_out = it;
     *n_h_out = n_h;
     return WEST_OK;
+}
+
+// ---- workspace plan of west_chi0_apply for a sub-block of pb perturbations
+struct Chi0Plan {
+    int solver = 0, nvpc = 1, n_freq = 1, pb = 0;
+    size_t vec = 0, xs = 0, shift = 0, grid = 0, scal = 0, maps = 0, misc = 0, W = 0, C = 0, msst = 0, craw = 0, dcoefd = 0, alpha = 0;
+    size_t total() const {
+        size_t t = (solver == 1 ? 3 : 4) * al256(vec) + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) +
+                   al256(C) + al256(alpha);
+        if (solver == 1) t += 2 * al256(xs) + al256(msst);
+        if (craw) t += al256(craw) + al256(dcoefd);
+        return t;
+    }
+};
+Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb) {
+    Chi0Plan p;
+    p.solver = solver; p.nvpc = nvpc; p.n_freq = n_freq; p.pb = pb;
+    const size_t n_g = (size_t)c->hs.n_g, n3 = (size_t)n3_of(c);
+    const size_t n_col = (size_t)pb * c->n_occ;
+    const int vp = solver == 1 ? 1 : nvpc;                     // vectors per column in the working sets r, p, Ap (, x)
+    p.vec = sizeof(cx<double>) * n_g * n_col * vp;
+    p.shift = sizeof(double) * n_col * vp;
+    p.grid = sizeof(double) * n3 * pb;
+    p.scal = n_col * (sizeof(double2) + 2 * sizeof(double) + 2 * sizeof(int)) + 64;
+    p.maps = sizeof(int) * 3 * n_col;
+    p.misc = 256;
+    const long long n_vec = (long long)n_col * vp;
+    const long long slots_h = is_gamma(c) ? (n_vec + 1) / 2 : n_vec, slots_r = (long long)pb * c->n_uslots;
+    p.W = bytes_W(c, std::max(slots_h, slots_r), 0);
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
+    p.C = bytes_C(rows, n_vec);
+    p.alpha = sizeof(double) * c->n_occ;
+    if (solver == 1) {
+        p.xs = sizeof(cx<double>) * n_g * n_col * 2 * n_freq;
+        const size_t ncs = n_col * n_freq;
+        p.msst = sizeof(double) * 4 * n_col + sizeof(double2) * 2 * ncs + sizeof(double) * ncs + sizeof(int) * (2 * n_col + ncs) + 64;
+    }
+    if (c->rows_defl > 0) {
+        p.craw = sizeof(double) * (size_t)c->rows_defl * (size_t)((n_vec + 1) / 2 * 2);
+        p.dcoefd = sizeof(double) * (size_t)c->rows_defl * (size_t)((n_col * (solver == 1 ? 2 : nvpc) + 1) / 2 * 2);
+    }
+    return p;
 }
 
 }  // namespace
@@ -1019,10 +1230,15 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     if (opts->max_iter < 1 || !(opts->tol > 0) || (opts->solver != 0 && opts->solver != 1) || opts->occupation < 0 || opts->occupation > 2 ||
         (opts->dn_accumulate != 0 && opts->dn_accumulate != 1))
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
+    // H - eps_v + alpha P_v is positive on the occupied space only if alpha > eps_v - eps_min for every v (reading R3): a smaller
+    // constant would make CG break down or converge to a wrong answer silently
+    if (opts->alpha_pv > 0 && !(opts->alpha_pv > c->eps_max - c->eps_min))
+        return fail(c, WEST_EINVAL, "west_chi0_apply: alpha_pv = %g Ry does not exceed the occupied band width %g Ry (pass alpha_pv <= 0 for the per-orbital default)",
+                    opts->alpha_pv, c->eps_max - c->eps_min);
     const double occ = opts->occupation > 0 ? opts->occupation : 2.0;
     if (opts->solver == 1 && (c->cell.mode != WEST_GAMMA || n_freq > wcg::MS_MAX_SHIFTS))
         return fail(c, WEST_EINVAL, "west_chi0_apply: the multi-shift solver needs WEST_GAMMA and at most %d frequencies", wcg::MS_MAX_SHIFTS);
-    const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
+    const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ, n_user = c->n_occ_user;
     for (int w = 0; w < n_freq; ++w) {
         if (omega_host[w] < 0) return fail(c, WEST_EINVAL, "west_chi0_apply: omega must be >= 0");
         if (omega_host[w] > 0 && !gamma) return fail(c, WEST_EINVAL, "west_chi0_apply: omega > 0 needs WEST_GAMMA (COCG needs real orbitals, R7)");
@@ -1031,35 +1247,47 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     if (n_pert == 0 || n_freq == 0) return WEST_OK;
     const int f32 = precision == WEST_MIXED;
     const long long n_g = c->hs.n_g, n3 = n3_of(c);
-    const int n_col = n_pert * n_occ;
-    const double vol = c->cell.L * c->cell.L * c->cell.L;
     bool any_omega = false;
     for (int w = 0; w < n_freq; ++w) any_omega |= omega_host[w] > 0;
     const int nvpc_max = any_omega ? 2 : 1;
     int rc;
-    if ((rc = ensure_opmatrix(c, opts->alpha_pv))) return rc;
-    for (int i = 0; i < 4; ++i)
-        if ((rc = ensure(c, c->vecs[i], sizeof(cx<double>) * n_g * n_col * nvpc_max))) return rc;
-    if ((rc = ensure(c, c->shift, sizeof(double) * ((size_t)n_col * nvpc_max + n_occ)))) return rc;
-    if ((rc = ensure(c, c->dVpos, sizeof(double) * n3 * n_pert))) return rc;
-    if ((rc = ensure(c, c->dnpos, sizeof(double) * n3 * n_pert))) return rc;
-    if ((rc = ensure(c, c->scal, (size_t)n_col * (3 * sizeof(double2) + 2 * sizeof(double) + sizeof(int)) + 64))) return rc;
-    if ((rc = ensure(c, c->maps, sizeof(int) * 3 * (size_t)n_col))) return rc;
-    wcg::Scalars s;
-    {
-        char* p = (char*)c->scal.p;
-        s.rz = (double2*)p; p += sizeof(double2) * n_col;
-        s.rr = (double*)p; p += sizeof(double) * n_col;
-        s.b2 = (double*)p; p += sizeof(double) * n_col;
-        s.active = (int*)p; p += sizeof(int) * n_col;
-        p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
-        s.counters = (int*)p;
+    if ((rc = ensure_opmatrix(c))) return rc;
+
+    // ---- workspace: the largest perturbation sub-block whose buffers fit the arena (the caller's, or what the device has free)
+    const size_t budget = arena_budget(c);
+    Chi0Plan plan;
+    int pb = n_pert;
+    for (int nb = 1;; ++nb) {
+        pb = (n_pert + nb - 1) / nb;
+        plan = chi0_plan(c, opts->solver, nvpc_max, n_freq, pb);
+        if (plan.total() <= budget || pb == 1) break;
     }
-    cx<double>* X = (cx<double>*)c->vecs[0].p; cx<double>* R = (cx<double>*)c->vecs[1].p;
-    cx<double>* P = (cx<double>*)c->vecs[2].p; cx<double>* AP = (cx<double>*)c->vecs[3].p;
-    double* d_eps = (double*)c->shift.p + (size_t)n_col * nvpc_max;
-    CK(cudaMemcpyAsync(d_eps, c->h_eps.data(), sizeof(double) * n_occ, cudaMemcpyHostToDevice, c->st));
-    nat_to_pos_real<double><<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, dV, (double*)c->dVpos.p);
+    if (plan.total() > budget)
+        return fail(c, c->arena.user ? WEST_EWORKSPACE : WEST_ENOMEM, "west_chi0_apply: one perturbation needs %zu bytes of workspace, %zu available",
+                    plan.total(), budget);
+    if ((rc = hot_begin(c, plan.total()))) return rc;
+    const int n_vecsets = opts->solver == 1 ? 3 : 4;
+    for (int i = 4 - n_vecsets; i < 4; ++i)
+        if ((rc = hot(c, c->vecs[i], plan.vec))) return rc;
+    if ((rc = hot(c, c->shift, plan.shift))) return rc;
+    if ((rc = hot(c, c->dVpos, plan.grid))) return rc;
+    if ((rc = hot(c, c->dnpos, plan.grid))) return rc;
+    if ((rc = hot(c, c->scal, plan.scal))) return rc;
+    if ((rc = hot(c, c->maps, plan.maps))) return rc;
+    if ((rc = hot(c, c->misc, plan.misc))) return rc;
+    if ((rc = hot(c, c->W, plan.W))) return rc;
+    if ((rc = hot(c, c->Cbuf, plan.C))) return rc;
+    if ((rc = hot(c, c->alpha_v, plan.alpha))) return rc;
+    if (opts->solver == 1) {
+        if ((rc = hot(c, c->xs, plan.xs))) return rc;
+        if ((rc = hot(c, c->ps, plan.xs))) return rc;
+        if ((rc = hot(c, c->msst, plan.msst))) return rc;
+    }
+    if (plan.craw) {
+        if ((rc = hot(c, c->craw, plan.craw))) return rc;
+        if ((rc = hot(c, c->dcoef_defl, plan.dcoefd))) return rc;
+    }
+    fill_alpha<<<blocks_for(n_occ, 256), 256, 0, c->st>>>(n_occ, c->d_eps, c->eps_min, c->eps_max - c->eps_min, opts->alpha_pv, (double*)c->alpha_v.p);
     CK(cudaGetLastError());
     c->launches += 1;
 
@@ -1070,27 +1298,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     } ev;
     if (stats) for (auto& e : ev.e) CK(cudaEventCreate(&e));
     int ret = WEST_OK;
-    auto copy_dpsi = [&](int w, int mode, const cx<double>* Xw) -> int {
-        // GAMMA layout [n_freq][n_pert][n_occ][2][n_g]; at omega = 0 (per-frequency solver) the imaginary part is zero.
-        // n_occ here is the caller's count: the columns of the padding orbital (odd counts, R15) are skipped.
-        const int n_user = c->n_occ_user;
-        const long long per = n_g * n_pert * n_user * (gamma ? 2 : 1);
-        cx<double>* dst = (cx<double>*)dpsi_opt + (long long)w * per;
-        if (gamma && mode == 0) {
-            CK(cudaMemsetAsync(dst, 0, sizeof(cx<double>) * per, c->st));
-            for (int i = 0; i < (n_user == n_occ ? 1 : n_pert); ++i) {
-                const int rows = n_user == n_occ ? n_col : n_user;
-                CK(cudaMemcpy2DAsync(dst + (long long)i * n_user * 2 * n_g, sizeof(cx<double>) * 2 * n_g, Xw + (long long)i * n_occ * n_g,
-                                     sizeof(cx<double>) * n_g, sizeof(cx<double>) * n_g, rows, cudaMemcpyDeviceToDevice, c->st));
-            }
-        } else {
-            const long long vpc = gamma ? 2 : 1;       // vectors per column
-            if (n_user == n_occ) CK(cudaMemcpyAsync(dst, Xw, sizeof(cx<double>) * per, cudaMemcpyDeviceToDevice, c->st));
-            else CK(cudaMemcpy2DAsync(dst, sizeof(cx<double>) * n_user * vpc * n_g, Xw, sizeof(cx<double>) * n_occ * vpc * n_g,
-                                      sizeof(cx<double>) * n_user * vpc * n_g, n_pert, cudaMemcpyDeviceToDevice, c->st));
-        }
-        return WEST_OK;
-    };
+    int it_min = INT32_MAX;
     auto add_times = [&]() {
         float t;
         cudaEventElapsedTime(&t, ev[0], ev[1]); stats->ms_rhs += t;
@@ -1098,103 +1306,163 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         cudaEventElapsedTime(&t, ev[2], ev[3]); stats->ms_dn += t;
     };
 
-    if (opts->solver == 1) {
-        // ------------------------------------------------------------ multi-shift CG: every frequency from one Krylov sequence
-        wcg::MsShifts sh;
-        sh.n = n_freq;
-        for (int w = 0; w < n_freq; ++w) sh.omega[w] = omega_host[w];
-        const size_t per = (size_t)n_g * n_col * 2;                       // complex-valued solution of one frequency
-        if ((rc = ensure(c, c->xs, sizeof(cx<double>) * per * n_freq))) return rc;
-        if ((rc = ensure(c, c->ps, sizeof(cx<double>) * per * n_freq))) return rc;
-        const size_t ncs = (size_t)n_col * n_freq;
-        if ((rc = ensure(c, c->msst, sizeof(double) * 4 * n_col + sizeof(double2) * 2 * ncs + sizeof(double) * ncs + sizeof(int) * (n_col + ncs) + 64)))
-            return rc;
-        wcg::MsState st;
-        {
-            char* p = (char*)c->msst.p;
-            st.zeta = (double2*)p; p += sizeof(double2) * ncs;
-            st.zeta_prev = (double2*)p; p += sizeof(double2) * ncs;
-            st.a_prev = (double*)p; p += sizeof(double) * n_col;
-            st.b_prev = (double*)p; p += sizeof(double) * n_col;
-            st.rr = (double*)p; p += sizeof(double) * n_col;
-            st.b2 = (double*)p; p += sizeof(double) * n_col;
-            st.res2 = (double*)p; p += sizeof(double) * ncs;
-            st.active = (int*)p; p += sizeof(int) * n_col;
-            st.sactive = (int*)p; p += sizeof(int) * ncs;
-            p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
-            st.counters = (int*)p;
-        }
-        fill_shift<<<blocks_for(n_col, 256), 256, 0, c->st>>>(n_col, 1, n_occ, d_eps, (double*)c->shift.p, nullptr);
+    for (int p0 = 0; p0 < n_pert; p0 += pb) {
+        const int np = std::min(pb, n_pert - p0);           // perturbations of this sub-block
+        const int n_col = np * n_occ;
+        cx<double>* X = (cx<double>*)c->vecs[0].p; cx<double>* R = (cx<double>*)c->vecs[1].p;
+        cx<double>* P = (cx<double>*)c->vecs[2].p; cx<double>* AP = (cx<double>*)c->vecs[3].p;
+        nat_to_pos_real<double><<<blocks_for(n3 * np, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * np, dV + (long long)p0 * n3, (double*)c->dVpos.p);
         CK(cudaGetLastError());
-        if (stats) CK(cudaEventRecord(ev[0], c->st));
-        if ((rc = chi0_rhs(c, n_pert, 1, R))) return rc;
-        if (stats) CK(cudaEventRecord(ev[1], c->st));
-        int iters = 0;
-        int64_t n_h = 0;
-        if ((rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, dpsi_opt != nullptr, (double*)c->shift.p, d_eps, st,
-                           (int*)c->maps.p, &iters, &n_h)))
-            return rc;
-        if (stats) CK(cudaEventRecord(ev[2], c->st));
-        for (int w = 0; w < n_freq; ++w) {
-            cx<double>* Xw = (cx<double>*)c->xs.p + (size_t)w * per;
-            if ((rc = add_deflated(c, n_col, 1, 2, omega_host[w], d_eps, Xw))) return rc;
-            if ((rc = chi0_dn(c, n_pert, 2, Xw, dn + (long long)w * n_pert * n3, occ, opts->dn_accumulate))) return rc;
-            if (dpsi_opt && (rc = copy_dpsi(w, 1, Xw))) return rc;
-        }
-        if ((rc = ensure(c, c->misc, 64))) return rc;
-        wcg::ms_report<<<1, wcg::NT, 0, c->st>>>(n_col, n_freq, opts->tol * opts->tol, st, (double*)c->misc.p);
-        double h[2];
-        if (stats) CK(cudaEventRecord(ev[3], c->st));
-        CK(cudaMemcpyAsync(h, c->misc.p, sizeof h, cudaMemcpyDeviceToHost, c->st));
-        CK(cudaStreamSynchronize(c->st));
-        if (h[1] > 0) ret = WEST_NOTCONVERGED;
-        if (stats) {
-            add_times();
-            stats->iters = iters; stats->n_unconverged = (int)h[1]; stats->resid_max = h[0]; stats->n_h_apply = n_h;
-        }
-        return ret;
-    }
+        c->launches += 1;
+        // [n_freq][n_pert][n_occ(caller's)][parts][n_g]: block of (frequency w, perturbation p0)
+        const int parts_out = gamma ? 2 : 1;
+        auto dpsi_block = [&](int w) { return (double2*)dpsi_opt + ((long long)w * n_pert + p0) * n_user * parts_out * n_g; };
 
-    for (int w = 0; w < n_freq; ++w) {
-        const double omega = omega_host[w];
-        const int mode = gamma ? (omega > 0 ? 1 : 0) : 2;
-        const int nvpc = mode == 1 ? 2 : 1, n_vec = n_col * nvpc;
-        fill_shift<<<blocks_for(n_vec, 256), 256, 0, c->st>>>(n_vec, nvpc, n_occ, d_eps, (double*)c->shift.p, nullptr);
-        CK(cudaGetLastError());
-        if (stats) CK(cudaEventRecord(ev[0], c->st));
-        if ((rc = chi0_rhs(c, n_pert, nvpc, R))) return rc;
-        if (stats) CK(cudaEventRecord(ev[1], c->st));
-        // ---- a2-a9: batched PCG / COCG
-        int iters = 0;
-        int64_t n_h = 0;
-        if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
-        else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
-        else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, d_eps, s, (int*)c->maps.p, &iters, &n_h);
-        if (rc) return rc;
-        if ((rc = add_deflated(c, n_col, nvpc, nvpc, omega, d_eps, X))) return rc;
-        if (stats) CK(cudaEventRecord(ev[2], c->st));
-        if ((rc = chi0_dn(c, n_pert, nvpc, X, dn + (long long)w * n_pert * n3, occ, opts->dn_accumulate))) return rc;
-        if (dpsi_opt && (rc = copy_dpsi(w, mode, X))) return rc;
-        if (stats) {
-            CK(cudaEventRecord(ev[3], c->st));
-            if ((rc = ensure(c, c->misc, 64))) return rc;
+        if (opts->solver == 1) {
+            // -------------------------------------------------------- multi-shift CG: every frequency from one Krylov sequence
+            wcg::MsShifts sh;
+            sh.n = n_freq;
+            for (int w = 0; w < n_freq; ++w) sh.omega[w] = omega_host[w];
+            const size_t per = (size_t)n_g * n_col * 2;                       // complex-valued solution of one frequency
+            const size_t ncs = (size_t)n_col * n_freq;
+            wcg::MsState st;
+            {
+                char* p = (char*)c->msst.p;
+                st.zeta = (double2*)p; p += sizeof(double2) * ncs;
+                st.zeta_prev = (double2*)p; p += sizeof(double2) * ncs;
+                st.a_prev = (double*)p; p += sizeof(double) * n_col;
+                st.b_prev = (double*)p; p += sizeof(double) * n_col;
+                st.rr = (double*)p; p += sizeof(double) * n_col;
+                st.b2 = (double*)p; p += sizeof(double) * n_col;
+                st.res2 = (double*)p; p += sizeof(double) * ncs;
+                st.active = (int*)p; p += sizeof(int) * n_col;
+                st.iters = (int*)p; p += sizeof(int) * n_col;
+                st.sactive = (int*)p; p += sizeof(int) * ncs;
+                p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
+                st.counters = (int*)p;
+            }
+            fill_shift<<<blocks_for(n_col, 256), 256, 0, c->st>>>(n_col, 1, n_occ, c->d_eps, (double*)c->shift.p, nullptr);
+            CK(cudaGetLastError());
+            if (stats) CK(cudaEventRecord(ev[0], c->st));
+            if ((rc = chi0_rhs(c, np, 1, R))) return rc;
+            if (stats) CK(cudaEventRecord(ev[1], c->st));
+            int iters = 0;
+            int64_t n_h = 0;
+            if ((rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, dpsi_opt != nullptr, (double*)c->shift.p, st,
+                               (int*)c->maps.p, &iters, &n_h)))
+                return rc;
+            if (stats) CK(cudaEventRecord(ev[2], c->st));
+            for (int w = 0; w < n_freq; ++w) {
+                cx<double>* Xw = (cx<double>*)c->xs.p + (size_t)w * per;
+                if ((rc = add_deflated(c, n_col, 1, 2, omega_host[w], Xw))) return rc;
+                if ((rc = chi0_dn(c, np, 2, Xw, dn + ((long long)w * n_pert + p0) * n3, occ, opts->dn_accumulate))) return rc;
+                if (dpsi_opt) {
+                    dpsi_gather<<<np * n_user * 2, wcg::NT, 0, c->st>>>(n_g, n_occ, n_user, 2, 2, (const double2*)Xw, dpsi_block(w));
+                    CK(cudaGetLastError());
+                    c->launches += 1;
+                }
+            }
+            // convergence report: the return code needs it, so this is the call's one stream synchronisation
             double* rep = (double*)c->misc.p;
-            wcg::cg_report<<<1, wcg::NT, 0, c->st>>>(n_col, opts->tol * opts->tol, s, rep);
-            double h[2];
-            CK(cudaMemcpyAsync(h, rep, sizeof h, cudaMemcpyDeviceToHost, c->st));
+            wcg::ms_report<<<1, wcg::NT, 0, c->st>>>(n_col, n_freq, opts->tol * opts->tol, st, rep);
+            if (stats) CK(cudaEventRecord(ev[3], c->st));
+            double* h = (double*)(c->h_pinned + 8);
+            CK(cudaMemcpyAsync(h, rep, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
             CK(cudaStreamSynchronize(c->st));
-            add_times();
-            stats->iters = std::max(stats->iters, iters);
-            stats->n_unconverged += (int)h[1];
-            stats->resid_max = std::max(stats->resid_max, h[0]);
-            stats->n_h_apply += n_h;
             if (h[1] > 0) ret = WEST_NOTCONVERGED;
-        } else {
-            // convergence status without stats: the last polled counter
-            if (c->h_pinned[0] > 0) ret = WEST_NOTCONVERGED;
+            if (stats) {
+                add_times();
+                stats->iters = std::max(stats->iters, iters); stats->n_unconverged += (int)h[1]; stats->resid_max = std::max(stats->resid_max, h[0]);
+                stats->n_h_apply += n_h;
+                it_min = std::min(it_min, (int)h[2]);
+            }
+            continue;
         }
+
+        wcg::Scalars s;
+        {
+            char* p = (char*)c->scal.p;
+            s.rz = (double2*)p; p += sizeof(double2) * n_col;
+            s.rr = (double*)p; p += sizeof(double) * n_col;
+            s.b2 = (double*)p; p += sizeof(double) * n_col;
+            s.active = (int*)p; p += sizeof(int) * n_col;
+            s.iters = (int*)p; p += sizeof(int) * n_col;
+            p = (char*)(((uintptr_t)p + 15) & ~(uintptr_t)15);
+            s.counters = (int*)p;
+        }
+        for (int w = 0; w < n_freq; ++w) {
+            const double omega = omega_host[w];
+            const int mode = gamma ? (omega > 0 ? 1 : 0) : 2;
+            const int nvpc = mode == 1 ? 2 : 1, n_vec = n_col * nvpc;
+            fill_shift<<<blocks_for(n_vec, 256), 256, 0, c->st>>>(n_vec, nvpc, n_occ, c->d_eps, (double*)c->shift.p, nullptr);
+            CK(cudaGetLastError());
+            if (stats) CK(cudaEventRecord(ev[0], c->st));
+            if ((rc = chi0_rhs(c, np, nvpc, R))) return rc;
+            if (stats) CK(cudaEventRecord(ev[1], c->st));
+            // ---- a2-a9: batched PCG / COCG
+            int iters = 0, live = 0;
+            int64_t n_h = 0;
+            if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
+            else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
+            else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
+            if (rc) return rc;
+            if (live > 0) ret = WEST_NOTCONVERGED;
+            if ((rc = add_deflated(c, n_col, nvpc, nvpc, omega, X))) return rc;
+            if (stats) CK(cudaEventRecord(ev[2], c->st));
+            if ((rc = chi0_dn(c, np, nvpc, X, dn + ((long long)w * n_pert + p0) * n3, occ, opts->dn_accumulate))) return rc;
+            if (dpsi_opt) {
+                dpsi_gather<<<np * n_user * parts_out, wcg::NT, 0, c->st>>>(n_g, n_occ, n_user, nvpc, parts_out, (const double2*)X, dpsi_block(w));
+                CK(cudaGetLastError());
+                c->launches += 1;
+            }
+            if (stats) {
+                CK(cudaEventRecord(ev[3], c->st));
+                double* rep = (double*)c->misc.p;
+                wcg::cg_report<<<1, wcg::NT, 0, c->st>>>(n_col, opts->tol * opts->tol, s, rep);
+                double* h = (double*)(c->h_pinned + 8);
+                CK(cudaMemcpyAsync(h, rep, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+                CK(cudaStreamSynchronize(c->st));
+                add_times();
+                stats->iters = std::max(stats->iters, iters);
+                stats->n_unconverged += (int)h[1];
+                stats->resid_max = std::max(stats->resid_max, h[0]);
+                stats->n_h_apply += n_h;
+                it_min = std::min(it_min, (int)h[2]);
+            }
+        }
+    }
+    if (stats) {
+        stats->iters_min = it_min == INT32_MAX ? 0 : it_min;
+        stats->n_sub_blocks = (n_pert + pb - 1) / pb;
     }
     return ret;
+}
+
+extern "C" size_t west_workspace_bytes(const west_ctx* c, int32_t op, int32_t n_pert, int32_t n_freq, int32_t precision) {
+    if (!c || n_pert <= 0) return 0;
+    const int f32 = precision == WEST_MIXED;
+    switch (op) {
+        case WEST_OP_FFT3D: return plan_fft3d(c, n_pert);
+        case WEST_OP_H_APPLY: return plan_happly(c, n_pert, f32);
+        case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert).total();
+        case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert).total();
+        case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert).total();
+        case WEST_OP_LANCZOS: return plan_lanczos(c, n_pert, std::max(1, n_freq), f32);
+    }
+    return 0;
+}
+
+extern "C" int west_set_workspace(west_ctx* c, void* ws, size_t bytes) {
+    if (!c || (ws && ((uintptr_t)ws & 255))) return fail(c, WEST_EINVAL, "west_set_workspace: NULL context or a block that is not 256-byte aligned");
+    Arena& a = c->arena;
+    if (a.base && !a.user) {             // drop the context's own arena: not a hot call, may synchronise and free
+        cudaStreamSynchronize(c->st);
+        cudaFree(a.base);
+        c->dev_bytes -= (int64_t)a.cap;
+    }
+    a.base = (char*)ws; a.cap = ws ? bytes : 0; a.user = ws != nullptr; a.off = 0;
+    a.epoch += 1;
+    return WEST_OK;
 }
 
 // ============================================================================================================ Lanczos chains
@@ -1209,11 +1477,16 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     const long long n_g = c->hs.n_g, n3 = n3_of(c), K = 2 * n_g;
     const int n_col = n_pert * n_occ;
     int rc;
-    if (c->rows_kb > 0 && (rc = ensure_opmatrix(c, 0.0))) return rc;
+    if ((rc = ensure_opmatrix(c))) return rc;
+    if ((rc = hot_begin(c, plan_lanczos(c, n_pert, n_steps, precision == WEST_MIXED)))) return rc;
     for (int i = 0; i < 4; ++i)
-        if ((rc = ensure(c, c->vecs[i], sizeof(cx<double>) * n_g * n_col))) return rc;
-    if ((rc = ensure(c, c->dVpos, sizeof(double) * n3 * n_pert))) return rc;
-    if ((rc = ensure(c, c->scal, sizeof(double) * n_col + 64))) return rc;
+        if ((rc = hot(c, c->vecs[i], sizeof(cx<double>) * n_g * n_col))) return rc;
+    if ((rc = hot(c, c->dVpos, sizeof(double) * n3 * n_pert))) return rc;
+    if ((rc = hot(c, c->scal, sizeof(double) * n_col + 64))) return rc;
+    {
+        const long long slots_h = gamma ? ((long long)n_col + 1) / 2 : (long long)n_col, slots_r = (long long)n_pert * c->n_uslots;
+        if ((rc = hot(c, c->W, bytes_W(c, std::max(slots_h, slots_r), 0)))) return rc;
+    }
     cx<double>* Q = (cx<double>*)c->vecs[0].p; cx<double>* QP = (cx<double>*)c->vecs[1].p;
     cx<double>* HQ = (cx<double>*)c->vecs[2].p; cx<double>* Q1 = (cx<double>*)c->vecs[3].p;
     double* beta_prev = (double*)c->scal.p;
@@ -1221,7 +1494,7 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     const int n_user = c->n_occ_user;
     double *alpha_out = alpha, *beta_out = beta, *norm_out = norm;
     if (n_user != n_occ) {
-        if ((rc = ensure(c, c->msst, sizeof(double) * (size_t)n_col * (2 * n_steps + 1)))) return rc;
+        if ((rc = hot(c, c->msst, sizeof(double) * (size_t)n_col * (2 * n_steps + 1)))) return rc;
         alpha = (double*)c->msst.p; beta = alpha + (size_t)n_col * n_steps; norm = beta + (size_t)n_col * n_steps;
     }
     nat_to_pos_real<double><<<blocks_for(n3 * n_pert, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, n3 * n_pert, phi, (double*)c->dVpos.p);
@@ -1252,7 +1525,10 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
             c->launches += 1;
         }
         if ((rc = hloc_apply(c, f32, vm, n_slots, Q, HQ, nullptr, 0.0))) return rc;
-        if (c->rows_kb > 0 && (rc = lowrank_apply(c, 0, c->rows_kb, n_col, (const double*)Q, (double*)HQ, (const double*)c->coef_all.p, f32 != 0))) return rc;
+        if (c->rows_kb > 0) {
+            LowrankCoef lc; lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb;
+            if ((rc = lowrank_apply(c, 0, c->rows_kb, n_col, (const double*)Q, (double*)HQ, lc, f32 != 0))) return rc;
+        }
         {
             Prof p_(c, PC_CGVEC);
             if (gamma) wlz::lz_step<true><<<n_col, wcg::NT, 0, c->st>>>(n_g, n_steps, l, (const double2*)Q, (const double2*)HQ, (double2*)QP, alpha, beta, beta_prev);
@@ -1277,7 +1553,8 @@ extern "C" int west_lanczos_diag(west_ctx* c, int32_t n_chain, int32_t n_steps, 
         return fail(c, WEST_EINVAL, "west_lanczos_diag: bad argument (1 <= n_steps <= %d)", wlz::TRI_MAX);
     if (n_chain == 0) return WEST_OK;
     int rc;
-    if ((rc = ensure(c, c->misc, 256))) return rc;
+    if ((rc = hot_begin(c, al256(256)))) return rc;
+    if ((rc = hot(c, c->misc, 256))) return rc;
     int* n_failed = (int*)c->misc.p;
     CK(cudaMemsetAsync(n_failed, 0, sizeof(int), c->st));
     const size_t bytes = sizeof(double) * wlz::TRI_WARPS * (2 * wlz::TRI_MAX + (size_t)n_steps * (n_steps + 1));

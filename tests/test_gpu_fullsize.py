@@ -88,7 +88,7 @@ def test_invariants_on_the_full_batch(big):
     p, U = big["p"], big["U"]
     dn = big["dn"]
     scale = np.max(np.abs(dn))
-    assert np.max(np.abs(dn.reshape(64, -1).sum(axis=1))) < 1e-9 * scale * p.N ** 3 ** 0.5      # charge conservation
+    assert np.max(np.abs(dn.reshape(64, -1).sum(axis=1))) < 1e-9 * scale * (p.N ** 3) ** 0.5    # charge conservation
     M = ochi0.response_matrix(p.dV, dn, p.L)
     assert np.max(np.abs(M - M.T)) < 1e-9 * np.max(np.abs(M))                                    # chi0 is symmetric
     assert np.max(np.linalg.eigvalsh(0.5 * (M + M.T))) < 0.0                                     # and negative definite
