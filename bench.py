@@ -417,6 +417,8 @@ def chi0_op(wb, solver, omegas):
     B = wb.binding
     if solver == 1:
         return B.WEST_OP_CHI0_MULTISHIFT
+    if solver == 2 and max(omegas) == 0:
+        return B.WEST_OP_CHI0_BLOCK
     return B.WEST_OP_CHI0_IW if max(omegas) > 0 else B.WEST_OP_CHI0
 
 

@@ -87,6 +87,7 @@ extern "C" {
 #define WEST_OP_CHI0_IW          3   /* west_chi0_apply, solver 0, some omega > 0 (COCG: two real vectors per column) */
 #define WEST_OP_CHI0_MULTISHIFT  4   /* west_chi0_apply, solver 1, n_freq frequencies */
 #define WEST_OP_LANCZOS          5   /* west_lanczos, n_freq = n_steps */
+#define WEST_OP_CHI0_BLOCK       6   /* west_chi0_apply, solver 2, every omega = 0 (block CG: five vector sets) */
 
 #define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
@@ -110,7 +111,11 @@ typedef struct {
     int32_t check_every;/* host polls convergence every this many iterations (>=1) */
     int32_t solver;     /* 0: one preconditioned PCG (omega = 0) / COCG (omega > 0) solve per frequency (R7);
                            1: multi-shift CG (WEST_GAMMA only, <= 16 frequencies): all frequencies from ONE unpreconditioned Krylov
-                              sequence of the real seed operator H - eps_v + alpha P_v, one H*psi per iteration for every omega */
+                              sequence of the real seed operator H - eps_v + alpha P_v, one H*psi per iteration for every omega;
+                           2: block CG: at omega = 0 the n_pert right-hand sides of one orbital share ONE Krylov space (Gram
+                              matrices of the search block, rank-revealing pivoted-Cholesky solves that drop dependent directions, csrc/
+                              bcg_kernels.cuh); same dpsi, fewer H*psi.  Blocks of 2 .. 128 perturbations (per sub-block); frequencies
+                              omega > 0 and other block sizes run as solver 0 */
     double  occupation; /* electrons per orbital in Eq. 11: 2 = spin-unpolarised (0 selects this default), 1 = ONE channel of a
                            spin-polarised system (N_spin = 2): dn = (2 occupation / Omega) Re sum_v ... */
     int32_t dn_accumulate; /* 0: dn is overwritten; 1: dn += this call's response (second spin channel: the sum over sigma) */
@@ -242,7 +247,8 @@ int64_t west_launch_count(const west_ctx* ctx);
  * events on the context's stream.  west_get_profile synchronises the stream, writes the summed milliseconds and span
  * counts of the 8 classes into the HOST arrays ms[8], count[8] and resets the record.  Classes: 0 K1 (sphere -> z sticks,
  * H*psi), 1 K2 (planes: y/x inverse, x V_loc, x/y forward), 2 K3 (z sticks -> sphere + kinetic), 3 gemm_tn, 4 gemm_update,
- * 5 CG vector kernel (fused step; compaction launches included), 6 FFT kernels of the RHS / dn stages (two launches per span), 7 unused. */
+ * 5 CG vector kernel (fused step; compaction launches included), 6 FFT kernels of the RHS / dn stages (two launches per span), 7 block-CG Gram /
+ * coefficient / block-update kernels and the tridiagonal eigensolver. */
 int  west_set_profile(west_ctx* ctx, int32_t on);
 int  west_get_profile(west_ctx* ctx, double* ms, int64_t* count);
 /* Tuning knob: how many FFT slots (complex transforms) are processed per internal chunk (0 = default).  The stick

@@ -18,6 +18,7 @@
 #include "gemm_f64.cuh"
 #include "gsphere.hpp"
 #include "lanczos_kernels.cuh"
+#include "bcg_kernels.cuh"
 
 namespace {
 
@@ -89,7 +90,7 @@ struct west_ctx {
 
     // hot-call workspaces: carved from the arena at the start of every hot call (hot_begin / hot)
     Arena arena;
-    DevBuf W, Cbuf, Rbuf, vecs[4], shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk;
+    DevBuf W, Cbuf, Rbuf, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk;
     int* h_pinned = nullptr;           // pinned host scratch (64 ints): lagged convergence polls [0], [1]; reports [8..]
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
 
@@ -1177,12 +1178,159 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
     return WEST_OK;
 }
 
+// ---- block CG (solver 2, omega = 0): one Krylov space per orbital shared by its s = np right-hand sides (bcg_kernels.cuh)
+size_t bcg_small_bytes(int n_occ, int s) {
+    const size_t ss = (size_t)s * s, no = (size_t)n_occ, nc = no * s;
+    return al256(sizeof(double) * 4 * no * ss) + al256(sizeof(double) * no * s) + al256(sizeof(int) * (no * s + no)) + al256(sizeof(double) * 2 * nc) +
+           al256(sizeof(int) * 3 * no + 64) + al256(sizeof(int) * (3 * no + nc));
+}
+template <int TS>
+void gram_launch(west_ctx* c, int s, long long K, int n_act, const int* orbmap, const double* A, const double* B, double* C, int gamma) {
+    const int tiles = (s + TS - 1) / TS, t2 = tiles * tiles;
+    long long splits = std::max<long long>(1, std::min<long long>(K / 2048, (592 + (long long)n_act * t2 - 1) / ((long long)n_act * t2)));
+    long long kps = ((K + splits - 1) / splits + 31) / 32 * 32;
+    splits = (K + kps - 1) / kps;
+    if (splits > 1) cudaMemsetAsync(C, 0, sizeof(double) * (size_t)n_act * s * s, c->st);
+    wbcg::gram_kernel<TS><<<dim3(n_act, (unsigned)(t2 * splits)), 256, 0, c->st>>>(s, K, n_act, orbmap, A, B, C, gamma, (int)splits, kps);
+}
+int bcg_gram(west_ctx* c, int s, long long K, int n_act, const int* orbmap, const cx<double>* A, const cx<double>* B, double* C) {
+    Prof p_(c, PC_MISC);
+    const int gamma = is_gamma(c) ? 1 : 0;
+    if (s <= 16) gram_launch<16>(c, s, K, n_act, orbmap, (const double*)A, (const double*)B, C, gamma);
+    else if (s <= 32) gram_launch<32>(c, s, K, n_act, orbmap, (const double*)A, (const double*)B, C, gamma);
+    else gram_launch<64>(c, s, K, n_act, orbmap, (const double*)A, (const double*)B, C, gamma);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+int bcg_update(west_ctx* c, int s, long long K, int n_act, const int* orbmap, const double* C, const cx<double>* P, cx<double>* Y, long long out_stride,
+               const int* out_orb, double sign) {
+    Prof p_(c, PC_MISC);
+    const unsigned gx = (unsigned)((K / 2 + 255) / 256);
+    if (s <= 16)
+        wbcg::update_kernel<16><<<dim3(gx, n_act, 1), 256, sizeof(double) * s * 16, c->st>>>(s, K, n_act, orbmap, C, (const double*)P, (double*)Y, out_stride, out_orb, sign);
+    else
+        wbcg::update_kernel<32><<<dim3(gx, n_act, (s + 31) / 32), 256, sizeof(double) * s * 32, c->st>>>(s, K, n_act, orbmap, C, (const double*)P, (double*)Y, out_stride,
+                                                                                                      out_orb, sign);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+
+int bcg_solve(west_ctx* c, int f32, int s, const west_cg_opts& o, cx<double>* X, cx<double>* R, cx<double>* P, cx<double>* Q, cx<double>* Z, double* shift,
+              double* rep_dev, int* iters_out, int64_t* n_h_out, int* live_out) {
+    const long long n_g = c->hs.n_g, K = 2 * n_g;
+    const int n_occ = c->n_occ, gamma = is_gamma(c), n_col = s * n_occ;
+    const double tol2 = o.tol * o.tol;
+    const int every = std::max(1, o.check_every);
+    const double* tk = (const double*)c->tk.p;
+    // carve the small buffers
+    char* p = (char*)c->blk.p;
+    auto take = [&](size_t bytes) { char* q = p; p += al256(bytes); return q; };
+    const size_t ss = (size_t)s * s;
+    double* G = (double*)take(sizeof(double) * 4 * n_occ * ss);
+    double* T = G + n_occ * ss; double* C = T + n_occ * ss;
+    wbcg::Fac fac;
+    fac.L = C + n_occ * ss;
+    fac.D = (double*)take(sizeof(double) * n_occ * s);
+    fac.order = (int*)take(sizeof(int) * ((size_t)n_occ * s + n_occ));
+    fac.rank = fac.order + (size_t)n_occ * s;
+    wbcg::State st;
+    st.b2 = (double*)take(sizeof(double) * 2 * n_col); st.rr = st.b2 + n_col;
+    st.n_open = (int*)take(sizeof(int) * 3 * n_occ + 64); st.active = st.n_open + n_occ; st.iters = st.active + n_occ; st.counters = st.iters + n_occ;
+    int* orbmap = (int*)take(sizeof(int) * (3 * (size_t)n_occ + n_col));
+    int* newmap = orbmap + n_occ; int* src = newmap + n_occ; int* colmap = src + n_occ;
+    const size_t csm = wbcg::coef_smem(s);
+    if (csm > 48 * 1024) CK(cudaFuncSetAttribute(wbcg::coef_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)csm));
+
+    CK(cudaMemsetAsync(st.n_open, 0, sizeof(int) * 3 * n_occ + 64, c->st));
+    CK(cudaMemsetAsync(X, 0, sizeof(cx<double>) * n_g * n_col, c->st));
+    // identity orbital map; Z = M R goes straight into P (the first search block); b2, flags
+    wbcg::colmap_kernel<<<blocks_for(n_occ, 256), 256, 0, c->st>>>(n_occ, 1, n_occ, nullptr, orbmap);
+    wbcg::zr_kernel<<<n_col, 256, 0, c->st>>>(n_g, n_occ, n_occ, gamma, orbmap, c->d_g2, tk, o.precond, tol2, 1, (const double2*)R, (double2*)P, st);
+    wbcg::flags_kernel<<<blocks_for(n_occ, 256), 256, 0, c->st>>>(n_occ, orbmap, 1, st);
+    wbcg::colmap_kernel<<<blocks_for(n_col, 256), 256, 0, c->st>>>(n_occ, s, n_occ, orbmap, colmap);
+    CK(cudaGetLastError());
+    c->launches += 4;
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
+    int n_act = n_occ, it = 0, live = n_occ;
+    int64_t n_h = 0;
+    Poller poll;
+    bool done = false;
+    for (; it < o.max_iter && !done; ++it) {
+        const int n_vec = n_act * s;
+        VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
+        const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
+        int rc = hloc_apply(c, f32, vm, n_slots, P, Q, shift, 0.0);
+        if (rc) return rc;
+        LowrankCoef lc;
+        lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb; lc.alpha_vec = (const double*)c->alpha_v.p; lc.colmap = colmap; lc.nvpc = 1; lc.n_occ = n_occ;
+        if ((rc = lowrank_apply(c, 0, rows, n_vec, (const double*)P, (double*)Q, lc, f32 != 0))) return rc;
+        n_h += n_vec;
+        if ((rc = bcg_gram(c, s, K, n_act, orbmap, P, Q, G))) return rc;
+        if ((rc = bcg_gram(c, s, K, n_act, orbmap, P, R, T))) return rc;
+        {
+            Prof p_(c, PC_MISC);
+            wbcg::coef_kernel<<<n_act, 256, csm, c->st>>>(s, 0, orbmap, G, T, C, fac, 1e-12, 1.0);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        if ((rc = bcg_update(c, s, K, n_act, orbmap, C, P, X, n_occ, orbmap, 1.0))) return rc;        // x += P alpha   (original column order)
+        if ((rc = bcg_update(c, s, K, n_act, orbmap, C, Q, R, n_act, nullptr, -1.0))) return rc;      // r -= Q alpha
+        {
+            Prof p_(c, PC_CGVEC);
+            wbcg::zr_kernel<<<n_vec, 256, 0, c->st>>>(n_g, n_act, n_occ, gamma, orbmap, c->d_g2, tk, o.precond, tol2, 0, (const double2*)R, (double2*)Z, st);
+            wbcg::flags_kernel<<<blocks_for(n_act, 256), 256, 0, c->st>>>(n_act, orbmap, 0, st);
+            CK(cudaGetLastError());
+            c->launches += 2;
+        }
+        if ((rc = bcg_gram(c, s, K, n_act, orbmap, Q, Z, T))) return rc;
+        {
+            Prof p_(c, PC_MISC);
+            wbcg::coef_kernel<<<n_act, 256, csm, c->st>>>(s, 1, orbmap, G, T, C, fac, 1e-12, -1.0);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        if ((rc = bcg_update(c, s, K, n_act, orbmap, C, P, Z, n_act, nullptr, 1.0))) return rc;       // p_new = z - P beta
+        std::swap(P, Z);
+        if (poll.ready()) {
+            live = poll.collect(c);
+            if (live <= 0) done = true;
+            else if (it + 1 < o.max_iter && live <= n_act - std::max(1, n_act / 16)) {
+                Prof p_(c, PC_CGVEC);
+                wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, orbmap, st.active, newmap, src, live);
+                wbcg::gather_blocks<<<live * s, 256, 0, c->st>>>(n_g, live, n_act, src, (const double2*)R, (double2*)Q);
+                wbcg::gather_blocks<<<live * s, 256, 0, c->st>>>(n_g, live, n_act, src, (const double2*)P, (double2*)Z);
+                cx<double>* oldR = R; cx<double>* oldP = P;
+                R = Q; P = Z; Q = oldR; Z = oldP;
+                std::swap(orbmap, newmap);
+                n_act = live;
+                wbcg::colmap_kernel<<<blocks_for(n_act * s, 256), 256, 0, c->st>>>(n_act, s, n_occ, orbmap, colmap);
+                fill_shift<<<blocks_for(n_act * s, 256), 256, 0, c->st>>>(n_act * s, 1, n_occ, c->d_eps, shift, colmap);
+                CK(cudaGetLastError());
+                c->launches += 5;
+            }
+        }
+        if (!done && ((it + 1) % every == 0 || it + 1 == o.max_iter)) CK(poll.post(c, st.counters));
+    }
+    if (poll.ready()) live = poll.collect(c);
+    if (rep_dev) {
+        wbcg::report_kernel<<<1, 256, 0, c->st>>>(n_col, n_occ, tol2, st, rep_dev);
+        CK(cudaGetLastError());
+    }
+    *iters_out = it;
+    *n_h_out = n_h;
+    *live_out = live;
+    return WEST_OK;
+}
+
 // ---- workspace plan of west_chi0_apply for a sub-block of pb perturbations
 struct Chi0Plan {
     int solver = 0, nvpc = 1, n_freq = 1, pb = 0;
+    size_t blk = 0;        // block CG: Gram / coefficient / factor blocks and flags (already a sum of al256 pieces)
     size_t vec = 0, xs = 0, shift = 0, grid = 0, scal = 0, maps = 0, misc = 0, W = 0, C = 0, msst = 0, craw = 0, dcoefd = 0, alpha = 0;
     size_t total() const {
-        size_t t = (solver == 1 ? 3 : 4) * al256(vec) + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) +
+        size_t t = (solver == 1 ? 3 : (solver == 2 ? 5 : 4)) * al256(vec) + blk + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) +
                    al256(C) + al256(alpha);
         if (solver == 1) t += 2 * al256(xs) + al256(msst);
         if (craw) t += al256(craw) + al256(dcoefd);
@@ -1207,6 +1355,7 @@ Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb) 
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     p.C = bytes_C(rows, n_vec);
     p.alpha = sizeof(double) * c->n_occ;
+    if (solver == 2) p.blk = bcg_small_bytes(c->n_occ, pb);
     if (solver == 1) {
         p.xs = sizeof(cx<double>) * n_g * n_col * 2 * n_freq;
         const size_t ncs = n_col * n_freq;
@@ -1227,7 +1376,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
-    if (opts->max_iter < 1 || !(opts->tol > 0) || (opts->solver != 0 && opts->solver != 1) || opts->occupation < 0 || opts->occupation > 2 ||
+    if (opts->max_iter < 1 || !(opts->tol > 0) || opts->solver < 0 || opts->solver > 2 || opts->occupation < 0 || opts->occupation > 2 ||
         (opts->dn_accumulate != 0 && opts->dn_accumulate != 1))
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad cg options");
     // H - eps_v + alpha P_v is positive on the occupied space only if alpha > eps_v - eps_min for every v (reading R3): a smaller
@@ -1278,6 +1427,10 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     if ((rc = hot(c, c->W, plan.W))) return rc;
     if ((rc = hot(c, c->Cbuf, plan.C))) return rc;
     if ((rc = hot(c, c->alpha_v, plan.alpha))) return rc;
+    if (opts->solver == 2) {
+        if ((rc = hot(c, c->vec5, plan.vec))) return rc;
+        if ((rc = hot(c, c->blk, plan.blk))) return rc;
+    }
     if (opts->solver == 1) {
         if ((rc = hot(c, c->xs, plan.xs))) return rc;
         if ((rc = hot(c, c->ps, plan.xs))) return rc;
@@ -1402,7 +1555,10 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             // ---- a2-a9: batched PCG / COCG
             int iters = 0, live = 0;
             int64_t n_h = 0;
-            if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
+            // solver 2: block CG over the np right-hand sides of every orbital (omega = 0; blocks of 2 .. 128 perturbations)
+            const bool block = opts->solver == 2 && mode != 1 && np >= 2 && np <= wbcg::SMAX;
+            if (block) rc = bcg_solve(c, f32, np, *opts, X, R, P, AP, (cx<double>*)c->vec5.p, (double*)c->shift.p, stats ? (double*)c->misc.p : nullptr, &iters, &n_h, &live);
+            else if (mode == 0) rc = cg_solve<0>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
             else if (mode == 1) rc = cg_solve<1>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
             else rc = cg_solve<2>(c, f32, n_col, *opts, omega, X, R, P, AP, (double*)c->shift.p, s, (int*)c->maps.p, &iters, &n_h, &live);
             if (rc) return rc;
@@ -1418,7 +1574,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             if (stats) {
                 CK(cudaEventRecord(ev[3], c->st));
                 double* rep = (double*)c->misc.p;
-                wcg::cg_report<<<1, wcg::NT, 0, c->st>>>(n_col, opts->tol * opts->tol, s, rep);
+                if (!block) wcg::cg_report<<<1, wcg::NT, 0, c->st>>>(n_col, opts->tol * opts->tol, s, rep);
                 double* h = (double*)(c->h_pinned + 8);
                 CK(cudaMemcpyAsync(h, rep, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
                 CK(cudaStreamSynchronize(c->st));
@@ -1447,6 +1603,7 @@ extern "C" size_t west_workspace_bytes(const west_ctx* c, int32_t op, int32_t n_
         case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert).total();
         case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert).total();
         case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert).total();
+        case WEST_OP_CHI0_BLOCK: return chi0_plan(c, 2, 1, std::max(1, n_freq), n_pert).total();
         case WEST_OP_LANCZOS: return plan_lanczos(c, n_pert, std::max(1, n_freq), f32);
     }
     return 0;

@@ -123,3 +123,42 @@ def test_chi0_other_cg_kernels(name, which):
     _, _, dn0, _, st0, _, _ = _run(name, cg_kernel=0, omegas=[0.0])
     assert st0["iters"] == st["iters"]
     assert relmax(dn, dn0) < 1e-12
+
+
+@pytest.mark.parametrize("name,omegas", [("cfg1", None), ("mini2", None), ("mini3", [0.0, 0.6947]), ("mini48", None)])
+def test_chi0_block_cg_same_answer_fewer_h_applications(name, omegas):
+    """solver = 2 (second half): the perturbations of one orbital share one Krylov space.  Same parity bar against the
+    sum over states (Eq. 10-11); at omega > 0 (mini3's second frequency) the call falls back to COCG; H*psi count below solver 0's."""
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run(name, solver=2, omegas=omegas)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0 and st["resid_max"] <= 1e-12
+    for w in range(dn.shape[0]):
+        assert relmax(dn[w], ref_dn[w]) < TOL
+    _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+    _, _, dn0, _, st0, _, _ = _run(name, solver=0, omegas=omegas)
+    assert relmax(dn, dn0) < TOL
+    assert st["n_h_apply"] < st0["n_h_apply"]
+    assert 0 < st["iters_min"] <= st["iters"]
+
+
+def test_chi0_block_cg_mixed_precision_and_deflation():
+    import paper_2203_05623_b200 as wb
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini4", precision=wb.WEST_MIXED, tol_cg=1e-6, solver=2)
+    assert st["rc"] == 0 and relmax(dn, ref_dn) < 1e-4
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini2", solver=2, n_defl=12)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0 and relmax(dn, ref_dn) < TOL
+
+
+def test_chi0_block_cg_degenerate_blocks():
+    """Linearly dependent and zero right-hand sides inside one block (the rank-revealing solve must drop them), and a block of one."""
+    import torch
+    p = oracle_problem.build("mini2")
+    w, _ = make_west(p)
+    N = p.N
+    dV = np.concatenate([p.dV[:2], 2.0 * p.dV[:1] - 0.5 * p.dV[1:2], np.full((1, N, N, N), 0.3), p.dV[:1]])     # rank 2 of 5, one zero response
+    ref = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, dV, [0.0], p.miller, p.L, p.N)
+    dn, _, st = w.chi0_apply(torch.from_numpy(np.ascontiguousarray(dV)).cuda(), [0.0], tol=1e-12, alpha_pv=p.alpha, solver=2)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    assert relmax(dn.cpu().numpy(), ref) < TOL and np.max(np.abs(dn[0, 3].cpu().numpy())) < 1e-12 * np.max(np.abs(ref))
+    dn1, _, st1 = w.chi0_apply(torch.from_numpy(np.ascontiguousarray(dV[:1])).cuda(), [0.0], tol=1e-12, alpha_pv=p.alpha, solver=2)
+    assert st1["rc"] == 0 and relmax(dn1.cpu().numpy()[0, 0], ref[0, 0]) < TOL
+    w.close()

@@ -146,3 +146,28 @@ def test_cfg4_mixed_precision_sampled_columns(states):
     # dn of the mixed path against the FP64 path of the same library (itself pinned to the oracle above) and Eq. 11 by the oracle
     assert relmax(dn.cpu().numpy(), dn64.cpu().numpy()) < 1e-4
     assert relmax(dn[0, 0].cpu().numpy(), ochi0.dn_from_dpsi(U, _full(p, dpsi[0, :, 0]), p.miller, p.L, p.N)) < 1e-12
+
+
+def test_cfg2_block_cg_sampled_columns(states):
+    """solver = 2 at config-2 size (64 right-hand sides per orbital block, 128 blocks): sampled columns against the oracle's PCG, true
+    residuals with the oracle's H, and the H*psi count against the per-column solver in the bench's configuration (tol 1e-8)."""
+    import torch
+    p, eps, U, alpha, w, dev = (states[k] for k in ("p", "eps", "U", "alpha", "w", "dev"))
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV)).to(dev)
+    dn, dpsi, st = w.chi0_apply(dV, [0.0], tol=1e-12, max_iter=500, alpha_pv=alpha, want_dpsi=True, solver=2)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    dpsi = dpsi.cpu().numpy()[0]
+    apply_H = lambda y: oham.apply_h(y, p.miller, p.L, p.N, p.vloc, p.beta, p.dcoef)
+    for i, v in ((0, 0), (31, 64), (63, p.n_occ - 1)):
+        b = ochi0.rhs_vectors(U[:, v:v + 1], p.dV[i:i + 1], p.fft_idx, p.N)[0, 0]
+        x, it, rel = oit.pcg_sternheimer(apply_H, U, eps[v], v, b, p.g2, alpha, tol=1e-12, max_iter=500)
+        got = _full(p, dpsi[i, v, 0])
+        assert relmax(got, x) < 1e-9
+        A = apply_H(got) - eps[v] * got + alpha * (U @ (U.conj().T @ got))
+        rhs = -(b - U @ (U.conj().T @ b))
+        assert np.linalg.norm(A - rhs) / np.linalg.norm(rhs) < 1e-10
+    assert relmax(dn[0, 37].cpu().numpy(), ochi0.dn_from_dpsi(U, _full(p, dpsi[37, :, 0]), p.miller, p.L, p.N)) < 1e-12
+    del dpsi
+    _, _, st2 = w.chi0_apply(dV, [0.0], tol=1e-8, max_iter=300, alpha_pv=0.0, check_every=1, solver=2)
+    _, _, st0 = w.chi0_apply(dV, [0.0], tol=1e-8, max_iter=300, alpha_pv=0.0, check_every=1, solver=0)
+    assert st2["rc"] == 0 and st0["rc"] == 0 and st2["n_h_apply"] < 0.9 * st0["n_h_apply"]
