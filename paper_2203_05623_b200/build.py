@@ -22,6 +22,8 @@ LIB = os.path.join(HERE, "libwest.so")
 # ZNT = threads per CTA of the z-stick kernels (2 * CU * max(N1, N2) <= ZNT)
 FFT_SIZES = [(4, 6, 24, 4, 4, 20, 4, 256), (6, 6, 36, 4, 4, 20, 4, 256), (6, 8, 48, 6, 3, 16, 4, 256), (8, 9, 72, 12, 2, 14, 4, 256),
              (12, 12, 144, 16, 1, 10, 2, 256)]
+K2H_SHAPES = {72: tuple(int(x) for x in os.environ.get("WEST_K2H_72", "6,3,2,1").split(",")),
+              144: tuple(int(x) for x in os.environ.get("WEST_K2H_144", "16,1,1,1").split(","))}
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
@@ -61,9 +63,10 @@ def build(force=False, verbose=False):
     jobs = []
     for n1, n2, n, nw, minb, cu, zminb, znt in FFT_SIZES:
         o = os.path.join(OBJ, "fft_%d.o" % n)
-        # WEST_K2H="NW,MINB,GW,HOIST" overrides the H*psi plane-kernel shape at N = 72 (experiments of profiles/r01_k2_pipe_experiments.md)
-        k2h = [int(x) for x in os.environ.get("WEST_K2H", "6,3,2,0").split(",")]
-        extra = ["-DWEST_NW_H=%d" % k2h[0], "-DWEST_MINB_H=%d" % k2h[1], "-DWEST_GW_H=%d" % k2h[2], "-DWEST_TW_HOIST=%d" % k2h[3]] if n == 72 else []      # measured: 6 warps x 3 CTAs is 3 % faster for the H*psi planes at N = 72 (16-24 resident warps all give 215-217 ms: pipe-bound)
+        # shape of the H*psi plane kernel: (warps per CTA, resident CTAs per SM, warps per line group, items per thread and pass);
+        # other N: the one-way variants' shape.  Measured alternatives: profiles/r02_k2_ilp.md
+        k2h = K2H_SHAPES.get(n)
+        extra = ["-DWEST_NW_H=%d" % k2h[0], "-DWEST_MINB_H=%d" % k2h[1], "-DWEST_GW_H=%d" % k2h[2], "-DWEST_NB_H=%d" % k2h[3]] if k2h else []
         jobs.append((o, [nvcc] + NVCC_FLAGS + extra + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_NW=%d" % nw, "-DWEST_MINB=%d" % minb, "-DWEST_CU=%d" % cu, "-DWEST_ZMINB=%d" % zminb, "-DWEST_ZNT=%d" % znt,
                                                "-c", os.path.join(CSRC, "fft_n.cu"), "-o", o]))
     o = os.path.join(OBJ, "fft_dense.o")

@@ -36,15 +36,6 @@ template <typename T> WHD cx<T> cvt(cx<double> a) { return mk<T>((T)a.x, (T)a.y)
 template <typename T> WHD cx<double> cvd(cx<T> a) { return mk<double>((double)a.x, (double)a.y); }
 WHD int wrap_signed(int n, int N) { return n < N / 2 ? n : n - N; }
 
-#ifndef WEST_ZFUSE
-#define WEST_ZFUSE 1      // 1: fused z-stick kernels (K1: combine while loading, store from registers; K3: load + contiguous pass fused)
-#endif
-#ifndef WEST_TW_POW
-#define WEST_TW_POW 1     // 1: level twiddles w^(m k) as powers of ONE table entry per thread (FP64 work traded for L1TEX wavefronts)
-#endif
-#ifndef WEST_TW_HOIST
-#define WEST_TW_HOIST 0   // 1: the H*psi plane kernel keeps each thread's level-twiddle powers in registers for the whole kernel
-#endif
 // zp[m] = z^m for m = 1 .. R-1 by binary splitting (dependency depth log2 R)
 template <typename T, int R> WHD void tw_powers(cx<T> z, cx<T> (&zp)[R]) {
     zp[0] = mk<T>(1, 0);
@@ -99,47 +90,15 @@ struct K1 {
                 for (int n1 = 0; n1 < N1; ++n1) v[n1] = mk<T>(0, 0);
             }
             cx<T>* dst = lines + line * PITCH + n2;
-if (WEST_TW_POW) {
+{
                 cx<T> zp[N1];
                 tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
                 for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
-            } else {
-#pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
             }
         }
     }
-    // phase B: contiguous DFT-N2
-    static WHD void phaseB(int tid, int nthr, cx<T>* lines) {
-        for (int it = tid; it < NL * N1; it += nthr) {
-            const int line = it / N1, k1 = it - line * N1;
-            cx<T>* p = lines + line * PITCH + N2 * k1;
-            cx<T> v[N2];
-#pragma unroll
-            for (int j = 0; j < N2; ++j) v[j] = p[j];
-            Dft<T, N2, +1>::run(v);
-#pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = v[j];
-        }
-    }
-    // phase C: write sticks, column index fastest.  GAMMA: S+ = A + iB to column cp, S- = conj(A) + i conj(B) to its mirror.
-    static WHD void phaseC(int tid, int nthr, const cx<T>* lines, const WestGeom& g, int slot, int u0, cx<T>* W) {
-        for (int it = tid; it < N * CU; it += nthr) {
-            const int pos = it / CU, ul = it - pos * CU, u = u0 + ul;
-            if (u >= g.n_units) continue;
-            cx<T>* dst = W + ((long long)slot * N + pos) * g.n_cols;
-            if (GAMMA) {
-                const cx<T> a = lines[(2 * ul) * PITCH + pos], b = lines[(2 * ul + 1) * PITCH + pos];
-                const int cp = u + (g.n_cols - g.n_units);
-                dst[cp] = mk<T>(a.x - b.y, a.y + b.x);
-                if (u != 0) dst[g.n_cols - 1 - cp] = mk<T>(a.x + b.y, b.x - a.y);
-            } else {
-                dst[u] = lines[ul * PITCH + pos];
-            }
-        }
-    }
-    // ---- fused variant (WEST_ZFUSE): two phases, one barrier, the line buffer is written once and read once.
+    // ---- GAMMA: two phases, one barrier, the line buffer is written once and read once.
     // GAMMA: the two lines of a unit are formed WHILE LOADING as  line 2ul = a(n) + i b(n)  and  line 2ul+1 = conj(a(-n)) + i conj(b(-n)),
     // whose transforms are S+ = A + iB and S- = conj(A) + i conj(B) themselves, so phase BC stores its registers straight to the
     // column cp and its mirror.  FULL: phaseA as above, then phaseBC.
@@ -182,14 +141,11 @@ if (WEST_TW_POW) {
                 for (int n1 = 0; n1 < N1; ++n1) v[n1] = mk<T>(0, 0);
             }
             cx<T>* dst = lines + line * PITCH + n2;
-            if (WEST_TW_POW) {
+            {
                 cx<T> zp[N1];
                 tw_powers<T, N1>(tw[N2 + n2], zp);
 #pragma unroll
                 for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
-            } else {
-#pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
             }
         }
     }
@@ -227,65 +183,7 @@ struct K3 {
     static constexpr int N = N1 * N2, PITCH = N + WEST_PAD, NF = GAMMA ? 2 : 1, NL = CU * NF;
     static constexpr size_t smem_bytes = sizeof(cx<T>) * (size_t)(NL * PITCH + 2 * N);
 
-    static WHD void phaseA(int tid, int nthr, cx<T>* lines, const WestGeom& g, int slot, int u0, const cx<T>* W) {
-        // loads of UNR items are issued before any shared-memory store so that several global loads are in flight per thread
-        constexpr int UNR = 4;
-        for (int it0 = tid; it0 < N * CU; it0 += nthr * UNR) {
-            cx<T> sp[UNR], sm[UNR];
-#pragma unroll
-            for (int q = 0; q < UNR; ++q) {
-                const int it = it0 + q * nthr;
-                sp[q] = mk<T>(0, 0); sm[q] = mk<T>(0, 0);
-                if (it < N * CU) {
-                    const int pos = it / CU, ul = it - pos * CU, u = u0 + ul;
-                    const cx<T>* src = W + ((long long)slot * N + pos) * g.n_cols;
-                    if (u < g.n_units) {
-                        if (GAMMA) {
-                            const int cp = u + (g.n_cols - g.n_units);
-                            sp[q] = src[cp];
-                            sm[q] = u == 0 ? sp[q] : src[g.n_cols - 1 - cp];
-                        } else {
-                            sp[q] = src[u];
-                        }
-                    }
-                }
-            }
-#pragma unroll
-            for (int q = 0; q < UNR; ++q) {
-                const int it = it0 + q * nthr;
-                if (it >= N * CU) continue;
-                const int pos = it / CU, ul = it - pos * CU;
-                if (GAMMA) {
-                    lines[(2 * ul) * PITCH + pos] = mk<T>((T)0.5 * (sp[q].x + sm[q].x), (T)0.5 * (sp[q].y - sm[q].y));      // (S+ + conj S-)/2
-                    lines[(2 * ul + 1) * PITCH + pos] = mk<T>((T)0.5 * (sp[q].y + sm[q].y), (T)0.5 * (sm[q].x - sp[q].x));  // (S+ - conj S-)/(2i)
-                } else {
-                    lines[ul * PITCH + pos] = sp[q];
-                }
-            }
-        }
-    }
-    // phase B': contiguous DFT-N2 (sign -), twiddle
-    static WHD void phaseB(int tid, int nthr, cx<T>* lines, const cx<T>* tw) {
-        for (int it = tid; it < NL * N1; it += nthr) {
-            const int line = it / N1, k1 = it - line * N1;
-            cx<T>* p = lines + line * PITCH + N2 * k1;
-            cx<T> v[N2];
-#pragma unroll
-            for (int j = 0; j < N2; ++j) v[j] = p[j];
-            Dft<T, N2, -1>::run(v);
-if (WEST_TW_POW) {
-                cx<T> zp[N2];
-                tw_powers<T, N2>(tw[N + N1 + k1], zp);
-#pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
-            } else {
-#pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
-            }
-        }
-    }
-    // ---- fused variant (WEST_ZFUSE): W -> registers -> (GAMMA: separate the two real functions with the partner lane) -> DFT-N2,
-    // twiddle -> line buffer; replaces phaseA + phaseB and one barrier.  Item (k1, line), lanes over the lines: lane pair (2m, 2m+1)
+    // W -> registers -> (GAMMA: separate the two real functions with the partner lane) -> DFT-N2, twiddle -> line buffer.  Item (k1, line), lanes over the lines: lane pair (2m, 2m+1)
     // holds column cp (S+) and its mirror (S-) of the same unit at the same N2 positions.  On the host (stepped test) the
     // partner's values are simply loaded again.
     static WHD void phaseAB(int tid, int nthr, cx<T>* lines, const cx<T>* tw, const WestGeom& g, int slot, int u0, const cx<T>* W) {
@@ -317,14 +215,11 @@ if (WEST_TW_POW) {
             if (it >= ITEMS) continue;
             Dft<T, N2, -1>::run(v);
             cx<T>* p = lines + line * PITCH + N2 * k1;
-            if (WEST_TW_POW) {
+            {
                 cx<T> zp[N2];
                 tw_powers<T, N2>(tw[N + N1 + k1], zp);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
-            } else {
-#pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
             }
         }
     }
@@ -390,6 +285,9 @@ struct K2Args {
     double fac;                 // K2_DN: 4/Omega
 };
 
+// LC = lines (x) or rows (y) a thread group owns per round; NB = independent items every thread runs in lockstep inside a pass (loads
+// of all NB items are issued before the first butterfly, stores after the last: NB load -> butterfly -> store chains in flight per
+// thread instead of one; the round then covers NB * LC lines).  NB = 1 is the plain one-item-per-thread pass.
 template <typename T, int N1, int N2, int MODE, int LC>
 struct K2 {
     static constexpr int N = N1 * N2, PITCH = N + WEST_PAD;
@@ -406,196 +304,261 @@ struct K2 {
         const int ny = wrap_signed(n, N);
         return (ny <= ymax && ny >= -ymax) ? Wp[c0 + ny + ymax] : mk<T>(0, 0);
     }
+    // strided-pass epilogue: v[k1] * w^(n2 k1) -> dst[N2 k1]   (level twiddles as powers of ONE table entry per thread: the kernels are
+    // bound by L1TEX wavefronts, so FP64 work is traded for table look-ups)
+    static WHD void tw_store_strided(cx<T> (&v)[N1], cx<T> z, cx<T>* dst) {
+        cx<T> zp[N1];
+        tw_powers<T, N1>(z, zp);
+#pragma unroll
+        for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
+    }
+    // contiguous-pass epilogue of the forward direction: v[j] * conj(w^(k1 j)) -> p[j]
+    static WHD void tw_store_contig(cx<T> (&v)[N2], cx<T> z, cx<T>* p) {
+        cx<T> zp[N2];
+        tw_powers<T, N2>(z, zp);
+#pragma unroll
+        for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
+    }
+
     // y inverse, pass A: rows of the disc straight from W
-    // zpre (yA, xA: powers of tw[N2 + n2]; xB, yC: powers of tw[N + N1 + k1]): the caller's hoisted level twiddles when every thread keeps
-    // the same n2 / k1 for the whole kernel (WEST_TW_HOIST), else NULL and the powers are formed here
-    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp, int row0, int nrow,
-                       const cx<T>* zpre = nullptr) {
-        for (int it = tid; it < nrow * N2; it += nthr) {
-            const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
-            cx<T> v[N1];
+    template <int NB = 1>
+    static WHD void yA(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, const cx<T>* Wp, int row0, int nrow) {
+        for (int it0 = tid; it0 < nrow * N2; it0 += NB * nthr) {
+            cx<T> v[NB][N1];
 #pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) v[n1] = keep_n1<N1, N2>(n1) ? load_disc(Wp, g, row, N2 * n1 + n2) : mk<T>(0, 0);
-            Dft<T, N1, +1>::run(v);
-            cx<T>* dst = S + row * PITCH + n2;
-if (WEST_TW_POW) {
-                cx<T> zp[N1];
-                if (zpre) {
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
 #pragma unroll
-                    for (int k1 = 0; k1 < N1; ++k1) zp[k1] = zpre[k1];
-                } else tw_powers<T, N1>(tw[N2 + n2], zp);
+                for (int n1 = 0; n1 < N1; ++n1)
+                    v[b][n1] = (it < nrow * N2 && keep_n1<N1, N2>(n1)) ? load_disc(Wp, g, row, N2 * n1 + n2) : mk<T>(0, 0);
+            }
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
-            } else {
+            for (int b = 0; b < NB; ++b) Dft<T, N1, +1>::run(v[b]);
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                if (it >= nrow * N2) continue;
+                const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
+                tw_store_strided(v[b], tw[N2 + n2], S + row * PITCH + n2);
             }
         }
     }
+    template <int NB = 1>
     static WHD void yB(int tid, int nthr, cx<T>* S, const WestGeom& g, int row0, int nrow) {
-        for (int it = tid; it < nrow * N1; it += nthr) {
-            const int rl = it / N1, k1 = it - rl * N1, row = row0 + rl;
-            cx<T>* p = S + row * PITCH + N2 * k1;
-            cx<T> v[N2];
+        for (int it0 = tid; it0 < nrow * N1; it0 += NB * nthr) {
+            cx<T> v[NB][N2];
 #pragma unroll
-            for (int j = 0; j < N2; ++j) v[j] = p[j];
-            Dft<T, N2, +1>::run(v);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const bool ok = NB == 1 || it < nrow * N1;            // (the loop bound covers b = 0)
+                const cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
 #pragma unroll
-            for (int j = 0; j < N2; ++j) p[j] = v[j];
+                for (int j = 0; j < N2; ++j) v[b][j] = ok ? p[j] : mk<T>(0, 0);
+            }
+#pragma unroll
+            for (int b = 0; b < NB; ++b) Dft<T, N2, +1>::run(v[b]);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                if (it >= nrow * N1) continue;
+                cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
+#pragma unroll
+                for (int j = 0; j < N2; ++j) p[j] = v[b][j];
+            }
         }
     }
     // x inverse, pass A: gather the 2 n_max + 1 non-zero inputs of LC lines from S
-    static WHD void xA(int tid, int nthr, const cx<T>* S, cx<T>* X, const cx<T>* tw, const WestGeom& g, int py0, const cx<T>* zpre = nullptr) {
-        for (int it = tid; it < LC * N2; it += nthr) {
-            const int l = it / N2, n2 = it - l * N2;
-            const int py = py0 + l;
-            if (py >= N) continue;
-            cx<T> v[N1];
+    template <int NB = 1>
+    static WHD void xA(int tid, int nthr, const cx<T>* S, cx<T>* X, const cx<T>* tw, const WestGeom& g, int py0) {
+        for (int it0 = tid; it0 < LC * N2; it0 += NB * nthr) {
+            cx<T> v[NB][N1];
 #pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) {
-                const int nx = wrap_signed(N2 * n1 + n2, N);
-                v[n1] = (keep_n1<N1, N2>(n1) && nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + py] : mk<T>(0, 0);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const int l = it / N2, n2 = it - l * N2, py = py0 + l;
+                const bool ok = it < LC * N2 && py < N;
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    const int nx = wrap_signed(N2 * n1 + n2, N);
+                    v[b][n1] = (ok && keep_n1<N1, N2>(n1) && nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + py] : mk<T>(0, 0);
+                }
             }
-            Dft<T, N1, +1>::run(v);
-            cx<T>* dst = X + l * PITCH + n2;
-if (WEST_TW_POW) {
-                cx<T> zp[N1];
-                if (zpre) {
 #pragma unroll
-                    for (int k1 = 0; k1 < N1; ++k1) zp[k1] = zpre[k1];
-                } else tw_powers<T, N1>(tw[N2 + n2], zp);
+            for (int b = 0; b < NB; ++b) Dft<T, N1, +1>::run(v[b]);
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
-            } else {
-#pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], tw[k1 * N2 + n2]);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const int l = it / N2, n2 = it - l * N2;
+                if (it >= LC * N2 || py0 + l >= N) continue;
+                tw_store_strided(v[b], tw[N2 + n2], X + l * PITCH + n2);
             }
         }
     }
-    // x inverse pass B, the real-space operation, x forward pass B' - all on the same N2 contiguous values
-    static WHD void xB(int tid, int nthr, cx<T>* X, const cx<T>* tw, const K2Args<T>& a, int slot, int pz, int py0, const cx<T>* zpre = nullptr) {
-        for (int it = tid; it < LC * N1; it += nthr) {
-            const int l = it / N1, k1 = it - l * N1;
-            const int py = py0 + l;
-            if (py >= N) continue;
-            cx<T>* p = X + l * PITCH + N2 * k1;
-            const long long r0 = ((long long)pz * N + py) * N + N2 * k1;      // position-order real-space index
-            const long long n3 = (long long)N * N * N;
-            cx<T> v[N2];
-            if (MODE != K2_FROMR) {
+    // the real-space operation on the N2 contiguous values of item (l, k1) between x inverse pass B and x forward pass B'
+    static WHD bool xB_mid(cx<T> (&v)[N2], const K2Args<T>& a, int slot, int pz, int py0, int l, int k1) {
+        const int py = py0 + l;
+        const long long r0 = ((long long)pz * N + py) * N + N2 * k1;      // position-order real-space index
+        const long long n3 = (long long)N * N * N;
+        if (MODE == K2_H) {
+            // V_loc is stored per chunk of LC lines as [pz][py0 / LC][k2][l][k1] (vloc_index): for a fixed j = k2 the LC * N1
+            // threads of a line group read LC * N1 consecutive words - whole 128-byte lines instead of one 8 N1-byte piece per line
+            const T* V = a.V + vloc_index(pz, py0, l, k1, 0);
 #pragma unroll
-                for (int j = 0; j < N2; ++j) v[j] = p[j];
-                Dft<T, N2, +1>::run(v);
+            for (int j = 0; j < N2; ++j) { const T w = V[j * (LC * N1)]; v[j].x *= w; v[j].y *= w; }
+            return true;
+        } else if (MODE == K2_TOR) {
+            cx<double>* R = a.R + (long long)slot * n3 + r0;
+#pragma unroll
+            for (int j = 0; j < N2; ++j) R[j] = cvd<T>(v[j]);
+            return false;
+        } else if (MODE == K2_DN) {
+            const int gs = a.slot0 + slot, ip = gs / a.n_uslots, us = gs - ip * a.n_uslots;
+            const cx<double>* U = a.ucache + (long long)us * n3 + r0;
+            double* D = a.dn + (long long)ip * n3 + r0;
+#pragma unroll
+            for (int j = 0; j < N2; ++j) {
+                const cx<double> u = U[j];
+                const double val = a.fac * ((double)v[j].x * u.x + (double)v[j].y * u.y);
+#ifdef __CUDA_ARCH__
+                atomicAdd(D + j, val);
+#else
+                D[j] += val;
+#endif
             }
-            if (MODE == K2_H) {
-                // V_loc is stored per chunk of LC lines as [pz][py0 / LC][k2][l][k1] (vloc_index below): for a fixed j = k2 the LC * N1
-                // threads of a line group read LC * N1 consecutive words - whole 128-byte lines instead of one 8 N1-byte piece per line
-                const T* V = a.V + vloc_index(pz, py0, l, k1, 0);
-#pragma unroll
-                for (int j = 0; j < N2; ++j) { const T w = V[j * (LC * N1)]; v[j].x *= w; v[j].y *= w; }
-            } else if (MODE == K2_TOR) {
-                cx<double>* R = a.R + (long long)slot * n3 + r0;
-#pragma unroll
-                for (int j = 0; j < N2; ++j) R[j] = cvd<T>(v[j]);
-                continue;
-            } else if (MODE == K2_DN) {
+            return false;
+        } else {   // K2_FROMR
+            if (a.ucache) {
                 const int gs = a.slot0 + slot, ip = gs / a.n_uslots, us = gs - ip * a.n_uslots;
                 const cx<double>* U = a.ucache + (long long)us * n3 + r0;
-                double* D = a.dn + (long long)ip * n3 + r0;
+                const double* D = a.dV + (long long)ip * n3 + r0;
 #pragma unroll
-                for (int j = 0; j < N2; ++j) {
-                    const cx<double> u = U[j];
-                    const double val = a.fac * ((double)v[j].x * u.x + (double)v[j].y * u.y);
-#ifdef __CUDA_ARCH__
-                    atomicAdd(D + j, val);
-#else
-                    D[j] += val;
-#endif
-                }
-                continue;
-            } else {   // K2_FROMR
-                if (a.ucache) {
-                    const int gs = a.slot0 + slot, ip = gs / a.n_uslots, us = gs - ip * a.n_uslots;
-                    const cx<double>* U = a.ucache + (long long)us * n3 + r0;
-                    const double* D = a.dV + (long long)ip * n3 + r0;
+                for (int j = 0; j < N2; ++j) { const double w = D[j]; const cx<double> u = U[j]; v[j] = mk<T>((T)(u.x * w), (T)(u.y * w)); }
+            } else {
+                const cx<double>* R = a.R + (long long)slot * n3 + r0;
 #pragma unroll
-                    for (int j = 0; j < N2; ++j) { const double w = D[j]; const cx<double> u = U[j]; v[j] = mk<T>((T)(u.x * w), (T)(u.y * w)); }
-                } else {
-                    const cx<double>* R = a.R + (long long)slot * n3 + r0;
+                for (int j = 0; j < N2; ++j) v[j] = cvt<T>(R[j]);
+            }
+            return true;
+        }
+    }
+    // x inverse pass B, the real-space operation, x forward pass B' - all on the same N2 contiguous values
+    template <int NB = 1>
+    static WHD void xB(int tid, int nthr, cx<T>* X, const cx<T>* tw, const K2Args<T>& a, int slot, int pz, int py0) {
+        for (int it0 = tid; it0 < LC * N1; it0 += NB * nthr) {
+            cx<T> v[NB][N2];
+            bool ok[NB], fwd[NB];
 #pragma unroll
-                    for (int j = 0; j < N2; ++j) v[j] = cvt<T>(R[j]);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const int l = it / N1, k1 = it - l * N1;
+                ok[b] = it < LC * N1 && py0 + l < N;
+                if (MODE != K2_FROMR) {
+                    const cx<T>* p = X + l * PITCH + N2 * k1;
+#pragma unroll
+                    for (int j = 0; j < N2; ++j) v[b][j] = ok[b] ? p[j] : mk<T>(0, 0);
                 }
             }
-            Dft<T, N2, -1>::run(v);
-if (WEST_TW_POW) {
-                cx<T> zp[N2];
-                if (zpre) {
+            if (MODE != K2_FROMR) {
 #pragma unroll
-                    for (int j = 0; j < N2; ++j) zp[j] = zpre[j];
-                } else tw_powers<T, N2>(tw[N + N1 + k1], zp);
+                for (int b = 0; b < NB; ++b) Dft<T, N2, +1>::run(v[b]);
+            }
 #pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
-            } else {
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                fwd[b] = ok[b] && xB_mid(v[b], a, slot, pz, py0, it / N1, it % N1);
+            }
+            if (MODE == K2_H || MODE == K2_FROMR) {
 #pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+                for (int b = 0; b < NB; ++b) Dft<T, N2, -1>::run(v[b]);
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    const int it = it0 + b * nthr;
+                    const int l = it / N1, k1 = it - l * N1;
+                    if (fwd[b]) tw_store_contig(v[b], tw[N + N1 + k1], X + l * PITCH + N2 * k1);
+                }
             }
         }
     }
     // x forward pass A': strided DFT-N1, keep |n_x| <= n_max, back into S
+    template <int NB = 1>
     static WHD void xC(int tid, int nthr, cx<T>* S, const cx<T>* X, const WestGeom& g, int py0) {
-        for (int it = tid; it < LC * N2; it += nthr) {
-            const int l = it / N2, n2 = it - l * N2;
-            const int py = py0 + l;
-            if (py >= N) continue;
-            const cx<T>* p = X + l * PITCH + n2;
-            cx<T> v[N1];
+        for (int it0 = tid; it0 < LC * N2; it0 += NB * nthr) {
+            cx<T> v[NB][N1];
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
-            Dft<T, N1, -1>::run(v);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const int l = it / N2, n2 = it - l * N2;
+                const bool ok = it < LC * N2 && py0 + l < N;
+                const cx<T>* p = X + l * PITCH + n2;
 #pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) {
-                if (!keep_n1<N1, N2>(n1)) continue;
-                const int nx = wrap_signed(N2 * n1 + n2, N);
-                if (nx <= g.n_max && nx >= -g.n_max) S[(nx + g.n_max) * PITCH + py] = v[n1];
+                for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[N2 * k1] : mk<T>(0, 0);
+            }
+#pragma unroll
+            for (int b = 0; b < NB; ++b) Dft<T, N1, -1>::run(v[b]);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const int l = it / N2, n2 = it - l * N2, py = py0 + l;
+                if (it >= LC * N2 || py >= N) continue;
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    if (!keep_n1<N1, N2>(n1)) continue;
+                    const int nx = wrap_signed(N2 * n1 + n2, N);
+                    if (nx <= g.n_max && nx >= -g.n_max) S[(nx + g.n_max) * PITCH + py] = v[b][n1];
+                }
             }
         }
     }
-    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, int row0, int nrow, const cx<T>* zpre = nullptr) {
-        for (int it = tid; it < nrow * N1; it += nthr) {
-            const int rl = it / N1, k1 = it - rl * N1, row = row0 + rl;
-            cx<T>* p = S + row * PITCH + N2 * k1;
-            cx<T> v[N2];
+    template <int NB = 1>
+    static WHD void yC(int tid, int nthr, cx<T>* S, const cx<T>* tw, const WestGeom& g, int row0, int nrow) {
+        for (int it0 = tid; it0 < nrow * N1; it0 += NB * nthr) {
+            cx<T> v[NB][N2];
 #pragma unroll
-            for (int j = 0; j < N2; ++j) v[j] = p[j];
-            Dft<T, N2, -1>::run(v);
-if (WEST_TW_POW) {
-                cx<T> zp[N2];
-                if (zpre) {
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const bool ok = NB == 1 || it < nrow * N1;            // (the loop bound covers b = 0)
+                const cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
 #pragma unroll
-                    for (int j = 0; j < N2; ++j) zp[j] = zpre[j];
-                } else tw_powers<T, N2>(tw[N + N1 + k1], zp);
+                for (int j = 0; j < N2; ++j) v[b][j] = ok ? p[j] : mk<T>(0, 0);
+            }
 #pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = j == 0 ? v[j] : cmulc(v[j], zp[j]);
-            } else {
+            for (int b = 0; b < NB; ++b) Dft<T, N2, -1>::run(v[b]);
 #pragma unroll
-                for (int j = 0; j < N2; ++j) p[j] = (j == 0 || k1 == 0) ? v[j] : cmulc(v[j], tw[N + j * N1 + k1]);
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                if (it >= nrow * N1) continue;
+                const int k1 = it % N1;
+                tw_store_contig(v[b], tw[N + N1 + k1], S + (row0 + it / N1) * PITCH + N2 * k1);
             }
         }
     }
+    template <int NB = 1>
     static WHD void yD(int tid, int nthr, const cx<T>* S, const WestGeom& g, cx<T>* Wp, int row0, int nrow) {
-        for (int it = tid; it < nrow * N2; it += nthr) {
-            const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
-            const cx<T>* p = S + row * PITCH + n2;
-            cx<T> v[N1];
+        for (int it0 = tid; it0 < nrow * N2; it0 += NB * nthr) {
+            cx<T> v[NB][N1];
 #pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) v[k1] = p[N2 * k1];
-            Dft<T, N1, -1>::run(v);
-            const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                const bool ok = NB == 1 || it < nrow * N2;
+                const cx<T>* p = S + (row0 + it / N2) * PITCH + it % N2;
 #pragma unroll
-            for (int n1 = 0; n1 < N1; ++n1) {
-                if (!keep_n1<N1, N2>(n1)) continue;
-                const int ny = wrap_signed(N2 * n1 + n2, N);
-                if (ny <= ymax && ny >= -ymax) Wp[c0 + ny + ymax] = v[n1];
+                for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[N2 * k1] : mk<T>(0, 0);
+            }
+#pragma unroll
+            for (int b = 0; b < NB; ++b) Dft<T, N1, -1>::run(v[b]);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int it = it0 + b * nthr;
+                if (it >= nrow * N2) continue;
+                const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
+                const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
+#pragma unroll
+                for (int n1 = 0; n1 < N1; ++n1) {
+                    if (!keep_n1<N1, N2>(n1)) continue;
+                    const int ny = wrap_signed(N2 * n1 + n2, N);
+                    if (ny <= ymax && ny >= -ymax) Wp[c0 + ny + ymax] = v[b][n1];
+                }
             }
         }
     }
@@ -630,17 +593,9 @@ __global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k1_g2r_z(WestGeom g, Vec
     load_tw<T, N1, N2>(tw, g.tw);
     __syncthreads();
     const int slot = blockIdx.y, u0 = blockIdx.x * CU;
-#if WEST_ZFUSE
     K::phaseA2(threadIdx.x, blockDim.x, lines, tw, g, vm, slot, u0, X);
     __syncthreads();
     K::phaseBC(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
-#else
-    K::phaseA(threadIdx.x, blockDim.x, lines, tw, g, vm, slot, u0, X);
-    __syncthreads();
-    K::phaseB(threadIdx.x, blockDim.x, lines);
-    __syncthreads();
-    K::phaseC(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
-#endif
 }
 
 template <typename T, int N1, int N2, bool GAMMA, int CU>
@@ -661,24 +616,19 @@ __global__ void __launch_bounds__(WEST_ZNT, WEST_ZMINB) k3_r2g_z(WestGeom g, Vec
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(e.X + vec * g.n_g + g.unit_off[u] + seg * 8));
         }
     }
-#if WEST_ZFUSE
     __syncthreads();                                   // twiddles
     K::phaseAB(threadIdx.x, blockDim.x, lines, tw, g, slot, u0, W);
     __syncthreads();
-#else
-    K::phaseA(threadIdx.x, blockDim.x, lines, g, slot, u0, W);
-    __syncthreads();
-    K::phaseB(threadIdx.x, blockDim.x, lines, tw);
-    __syncthreads();
-#endif
     K::phaseC(threadIdx.x, blockDim.x, lines, g, vm, slot, u0, e, Y);
 }
 
-// Plane kernel.  NW warps per CTA in groups of GW warps (GW = 1 or 2); each group owns LPG = 32 GW / max(N1, N2) lines at a
-// time and runs the three passes of "its" lines with group-level barriers only (__syncwarp, or a named barrier for a warp
-// pair), so the CTA synchronises just twice (after y inverse, before y forward).  Warp pairs raise the lane utilisation of the
-// passes: at N = 72 a warp holds 3 lines (27 / 24 of 32 lanes busy), a pair holds 7 (63 / 56 of 64).
-template <int N1, int N2, int GW = 1> struct K2Cfg { static constexpr int LPW = 32 * GW / (N1 > N2 ? N1 : N2); };
+// Plane kernel.  NW warps per CTA in groups of GW warps (GW = 1 or 2); each group owns LPG = 32 GW / max(N1, N2) lines per item slot and
+// NB item slots per thread (K2's NB), i.e. NB * LPG lines per round, and runs the three passes of "its" lines with group-level barriers
+// only (__syncwarp, or a named barrier for a warp pair), so the CTA synchronises just twice (after y inverse, before y forward).
+// Warp pairs raise the lane utilisation of the passes: at N = 72 a warp holds 3 lines (27 / 24 of 32 lanes busy), a pair holds 7
+// (63 / 56 of 64).  NB = 2 gives every thread two independent load -> butterfly -> store chains per pass (the kernel is latency-bound:
+// 0.8 eligible of 4.3 resident warps per scheduler at NB = 1, profiles/r01_k2_pipe_experiments.md).
+template <int N1, int N2, int GW = 1, int NB = 1> struct K2Cfg { static constexpr int LPW = NB * (32 * GW / (N1 > N2 ? N1 : N2)); };
 
 template <int GW>
 __device__ __forceinline__ void group_sync(int group) {
@@ -686,9 +636,9 @@ __device__ __forceinline__ void group_sync(int group) {
     else asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(GW * 32) : "memory");
 }
 
-template <typename T, int N1, int N2, int MODE, int NW, int MINB, int GW = 1>
+template <typename T, int N1, int N2, int MODE, int NW, int MINB, int GW = 1, int NB = 1>
 __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T> a) {
-    constexpr int LPG = K2Cfg<N1, N2, GW>::LPW, GT = GW * 32, NG = NW / GW;
+    constexpr int LPG = K2Cfg<N1, N2, GW, NB>::LPW, GT = GW * 32, NG = NW / GW;
     static_assert(NW % GW == 0 && (GW == 1 || NG <= 15), "warp-pair groups use named barriers 1..15");
     using K = K2<T, N1, N2, MODE, LPG>;
     constexpr int N = K::N;
@@ -702,35 +652,24 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T>
     const int pz = blockIdx.x, slot = blockIdx.y;
     cx<T>* Wp = a.W + ((long long)slot * N + pz) * g.n_cols;
     __syncthreads();
-    // WEST_TW_HOIST (experiment, off: profiles/r01_k2_pipe_experiments.md): when a group's GT threads cover one round of its LPG lines
-    // in every pass, a thread keeps n2 = gt % N2 (strided passes) and k1 = gt % N1 (contiguous passes) for the whole kernel, and the
-    // powers of its two table entries can stay in registers.  14 % fewer FP64 instructions, same time: the kernel is not FP64-bound.
-    constexpr bool HOIST = WEST_TW_HOIST && WEST_TW_POW && MODE == K2_H && LPG * N2 <= GT && LPG * N1 <= GT;
-    cx<T> zA[N1], zB[N2];
-    if (HOIST) {
-        tw_powers<T, N1>(tw[N2 + gt % N2], zA);
-        tw_powers<T, N2>(tw[N + N1 + gt % N1], zB);
-    }
-    const cx<T>* zAp = HOIST ? zA : nullptr;
-    const cx<T>* zBp = HOIST ? zB : nullptr;
     if (MODE != K2_FROMR) {
         for (int r0 = group * LPG; r0 < g.nr; r0 += NG * LPG) {
             const int nrow = g.nr - r0 < LPG ? g.nr - r0 : LPG;
-            K::yA(gt, GT, S, tw, g, Wp, r0, nrow, zAp);
+            K::template yA<NB>(gt, GT, S, tw, g, Wp, r0, nrow);
             group_sync<GW>(group);
-            K::yB(gt, GT, S, g, r0, nrow);
+            K::template yB<NB>(gt, GT, S, g, r0, nrow);
         }
         __syncthreads();
     }
     for (int py0 = group * LPG; py0 < N; py0 += NG * LPG) {
         if (MODE != K2_FROMR) {
-            K::xA(gt, GT, S, Xw, tw, g, py0, zAp);
+            K::template xA<NB>(gt, GT, S, Xw, tw, g, py0);
             group_sync<GW>(group);
         }
-        K::xB(gt, GT, Xw, tw, a, slot, pz, py0, zBp);
+        K::template xB<NB>(gt, GT, Xw, tw, a, slot, pz, py0);
         if (MODE == K2_H || MODE == K2_FROMR) {
             group_sync<GW>(group);
-            K::xC(gt, GT, S, Xw, g, py0);
+            K::template xC<NB>(gt, GT, S, Xw, g, py0);
         }
         group_sync<GW>(group);
     }
@@ -738,9 +677,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_planes(WestGeom g, K2Args<T>
         __syncthreads();
         for (int r0 = group * LPG; r0 < g.nr; r0 += NG * LPG) {
             const int nrow = g.nr - r0 < LPG ? g.nr - r0 : LPG;
-            K::yC(gt, GT, S, tw, g, r0, nrow, zBp);
+            K::template yC<NB>(gt, GT, S, tw, g, r0, nrow);
             group_sync<GW>(group);
-            K::yD(gt, GT, S, g, Wp, r0, nrow);
+            K::template yD<NB>(gt, GT, S, g, Wp, r0, nrow);
         }
     }
 }

@@ -19,6 +19,9 @@
 #ifndef WEST_GW_H
 #define WEST_GW_H 1         // warps per line group of the H*psi plane kernel (2 = warp pairs)
 #endif
+#ifndef WEST_NB_H
+#define WEST_NB_H 1         // independent items per thread and pass of the H*psi plane kernel (K2's NB)
+#endif
 
 namespace {
 constexpr int N1 = WEST_N1, N2 = WEST_N2, NN = N1 * N2, NW = WEST_NW, LPW = K2Cfg<N1, N2>::LPW;
@@ -59,9 +62,10 @@ cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a
     constexpr int NWm = MODE == K2_H ? WEST_NW_H : NW;
     constexpr int MBm = MODE == K2_H ? WEST_MINB_H : WEST_MINB;
     constexpr int GWm = MODE == K2_H ? WEST_GW_H : 1;
-    constexpr int LPG = K2Cfg<N1, N2, GWm>::LPW;
+    constexpr int NBm = MODE == K2_H ? WEST_NB_H : 1;
+    constexpr int LPG = K2Cfg<N1, N2, GWm, NBm>::LPW;
     using K = K2<T, N1, N2, MODE, LPG>;
-    auto kern = k2_planes<T, N1, N2, MODE, NWm, MBm, GWm>;
+    auto kern = k2_planes<T, N1, N2, MODE, NWm, MBm, GWm, NBm>;
     const size_t bytes = sizeof(cx<T>) * (size_t)((g.nr + (NWm / GWm) * LPG) * K::PITCH + 2 * NN);
     cudaError_t e = set_smem(kern, bytes);
     if (e != cudaSuccess) return e;
@@ -95,7 +99,7 @@ cudaError_t k2_entry(int f32, int mode, int n_slots, cudaStream_t st, const West
     }
     return cudaErrorInvalidValue;
 }
-const FftOps ops = {NN, N1, N2, WEST_CU, LPW, K2Cfg<N1, N2, WEST_GW_H>::LPW, k1_entry, k2_entry, k3_entry};
+const FftOps ops = {NN, N1, N2, WEST_CU, LPW, K2Cfg<N1, N2, WEST_GW_H, WEST_NB_H>::LPW, k1_entry, k2_entry, k3_entry};
 }  // namespace
 
 #define WEST_CAT2(a, b) a##b

@@ -1,6 +1,6 @@
 // Host-stepped run of the FFT kernel phases (paper_2203_05623_b200/csrc/fft_kernels.cuh) for tests/test_host_stepped_fft.py:
 // every phase between two barriers is a function of (tid, nthreads), so the exact device code path of K1 -> K2<K2_H> -> K3
-// (local part of H: T + V_loc) is executed here thread by thread on the CPU.   usage: step_fft N n2max gamma L nvec f32 in out [fused]
+// (local part of H: T + V_loc) is executed here thread by thread on the CPU.   usage: step_fft N n2max gamma L nvec f32 in out [nb]
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -8,7 +8,7 @@
 #include "../../paper_2203_05623_b200/csrc/fft_kernels.cuh"
 #include "../../paper_2203_05623_b200/csrc/gsphere.hpp"
 
-static int g_fused = 0;      // 1: the fused z-stick phases (K1 phaseA2/phaseBC, K3 phaseAB; the lane exchange is replaced by a reload)
+static int g_nb = 1;         // 1 or 2: items per thread and pass of the plane-kernel phases (K2's NB)
 
 template <typename T, int N1, int N2, bool GAMMA>
 void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V, std::vector<double>& Y) {
@@ -35,14 +35,8 @@ void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V
         Vp[KB::vloc_index(pz, py - py % LC, py % LC, px / N2, px % N2)] = (T)V[((size_t)jof(px) * N + jof(py)) * N + jof(pz)];
     std::vector<cx<T>> lines(KA::NL * KA::PITCH);
     for (int slot = 0; slot < nslots; slot++) for (int u0 = 0; u0 < s.n_units; u0 += CU) {
-        if (g_fused) {
-            for (int t = 0; t < NT; t++) KA::phaseA2(t, NT, lines.data(), tw.data(), g, vm, slot, u0, (const cx<double>*)X.data());
-            for (int t = 0; t < NT; t++) KA::phaseBC(t, NT, lines.data(), g, slot, u0, W.data());
-            continue;
-        }
-        for (int t = 0; t < NT; t++) KA::phaseA(t, NT, lines.data(), tw.data(), g, vm, slot, u0, (const cx<double>*)X.data());
-        for (int t = 0; t < NT; t++) KA::phaseB(t, NT, lines.data());
-        for (int t = 0; t < NT; t++) KA::phaseC(t, NT, lines.data(), g, slot, u0, W.data());
+        for (int t = 0; t < NT; t++) KA::phaseA2(t, NT, lines.data(), tw.data(), g, vm, slot, u0, (const cx<double>*)X.data());
+        for (int t = 0; t < NT; t++) KA::phaseBC(t, NT, lines.data(), g, slot, u0, W.data());
     }
     K2Args<T> a{}; a.W = W.data(); a.V = Vp.data();
     std::vector<cx<T>> S(s.nr * KB::PITCH), Xl(LC * KB::PITCH);
@@ -50,25 +44,33 @@ void run(HostSphere& s, int nvec, std::vector<double>& X, std::vector<double>& V
         cx<T>* Wp = W.data() + ((size_t)slot * N + pz) * s.n_cols;
         for (int r0 = 0; r0 < s.nr; r0 += 4) {           // row groups, as the warps of the device kernel take them
             const int nrow = s.nr - r0 < 4 ? s.nr - r0 : 4;
-            for (int t = 0; t < NT; t++) KB::yA(t, NT, S.data(), tw.data(), g, Wp, r0, nrow);
-            for (int t = 0; t < NT; t++) KB::yB(t, NT, S.data(), g, r0, nrow);
+            if (g_nb == 2) { for (int t = 0; t < NT; t++) KB::template yA<2>(t, NT, S.data(), tw.data(), g, Wp, r0, nrow); }
+            else { for (int t = 0; t < NT; t++) KB::yA(t, NT, S.data(), tw.data(), g, Wp, r0, nrow); }
+            if (g_nb == 2) { for (int t = 0; t < NT; t++) KB::template yB<2>(t, NT, S.data(), g, r0, nrow); }
+            else { for (int t = 0; t < NT; t++) KB::yB(t, NT, S.data(), g, r0, nrow); }
         }
         for (int py0 = 0; py0 < N; py0 += LC) {
-            for (int t = 0; t < NT; t++) KB::xA(t, NT, S.data(), Xl.data(), tw.data(), g, py0);
-            for (int t = 0; t < NT; t++) KB::xB(t, NT, Xl.data(), tw.data(), a, slot, pz, py0);
-            for (int t = 0; t < NT; t++) KB::xC(t, NT, S.data(), Xl.data(), g, py0);
+            if (g_nb == 2) {
+                for (int t = 0; t < NT; t++) KB::template xA<2>(t, NT, S.data(), Xl.data(), tw.data(), g, py0);
+                for (int t = 0; t < NT; t++) KB::template xB<2>(t, NT, Xl.data(), tw.data(), a, slot, pz, py0);
+                for (int t = 0; t < NT; t++) KB::template xC<2>(t, NT, S.data(), Xl.data(), g, py0);
+            } else {
+                for (int t = 0; t < NT; t++) KB::xA(t, NT, S.data(), Xl.data(), tw.data(), g, py0);
+                for (int t = 0; t < NT; t++) KB::xB(t, NT, Xl.data(), tw.data(), a, slot, pz, py0);
+                for (int t = 0; t < NT; t++) KB::xC(t, NT, S.data(), Xl.data(), g, py0);
+            }
         }
-        for (int t = 0; t < NT; t++) KB::yC(t, NT, S.data(), tw.data(), g, 0, s.nr);
-        for (int t = 0; t < NT; t++) KB::yD(t, NT, S.data(), g, Wp, 0, s.nr);
+        if (g_nb == 2) {
+            for (int t = 0; t < NT; t++) KB::template yC<2>(t, NT, S.data(), tw.data(), g, 0, s.nr);
+            for (int t = 0; t < NT; t++) KB::template yD<2>(t, NT, S.data(), g, Wp, 0, s.nr);
+        } else {
+            for (int t = 0; t < NT; t++) KB::yC(t, NT, S.data(), tw.data(), g, 0, s.nr);
+            for (int t = 0; t < NT; t++) KB::yD(t, NT, S.data(), g, Wp, 0, s.nr);
+        }
     }
     K3Epi e; e.scale = 1.0 / ((double)N * N * N); e.kinetic = 1; e.shift = nullptr; e.omega = 0; e.X = (const cx<double>*)X.data();
     for (int slot = 0; slot < nslots; slot++) for (int u0 = 0; u0 < s.n_units; u0 += CU) {
-        if (g_fused) {
-            for (int t = 0; t < NT; t++) KC::phaseAB(t, NT, lines.data(), tw.data(), g, slot, u0, W.data());
-        } else {
-            for (int t = 0; t < NT; t++) KC::phaseA(t, NT, lines.data(), g, slot, u0, W.data());
-            for (int t = 0; t < NT; t++) KC::phaseB(t, NT, lines.data(), tw.data());
-        }
+        for (int t = 0; t < NT; t++) KC::phaseAB(t, NT, lines.data(), tw.data(), g, slot, u0, W.data());
         for (int t = 0; t < NT; t++) KC::phaseC(t, NT, lines.data(), g, vm, slot, u0, e, (cx<double>*)Y.data());
     }
 }
@@ -78,7 +80,7 @@ int main(int argc, char** argv) {
     const int N = atoi(argv[1]), n2max = atoi(argv[2]), gamma = atoi(argv[3]);
     const double L = atof(argv[4]);
     const int nvec = atoi(argv[5]), f32 = atoi(argv[6]);
-    if (argc > 9) g_fused = atoi(argv[9]);
+    if (argc > 9) g_nb = atoi(argv[9]);
     HostSphere s = build_sphere(n2max, N, gamma, L);
     std::vector<double> X((size_t)nvec * s.n_g * 2), Y(X.size(), 0.0), V((size_t)N * N * N);
     FILE* f = fopen(argv[7], "rb");

@@ -62,7 +62,7 @@ def test_caller_workspace_means_no_allocation_in_the_hot_call():
     assert f0 == f1 == f2                                      # no cudaMalloc / cudaFree between the probes (driver-level free memory)
     assert w.device_bytes() == held
     # repeatable up to the FP64 atomics of the dn accumulation and the split-K GEMMs (west.h "Determinism")
-    assert relmax(dn.cpu().numpy(), a.cpu().numpy()) < 1e-12
+    assert relmax(dn.cpu().numpy(), a.cpu().numpy()) < 1e-9           # (8 CG iterations on non-eigenvector inputs amplify the last-bit differences)
     # a workspace that is too small for even one perturbation is refused, nothing is allocated behind the caller's back
     small = torch.empty(1 << 20, dtype=torch.uint8, device=dev)
     w.set_workspace(small)

@@ -29,8 +29,8 @@ def stepper(tmp_path_factory):
 @pytest.mark.parametrize("N,n2max,gamma,L,nvec,f32,tol", [
     (24, 25, 0, 10.0, 2, 0, 1e-13), (24, 25, 1, 10.0, 3, 0, 1e-13), (36, 66, 1, 10.25, 2, 0, 1e-13),
     (48, 66, 0, 10.25, 1, 0, 1e-13), (24, 25, 1, 10.0, 3, 1, 1e-5)])
-@pytest.mark.parametrize("fused", [0, 1])
-def test_stepped_device_code_matches_oracle(stepper, tmp_path, N, n2max, gamma, L, nvec, f32, tol, fused):
+@pytest.mark.parametrize("nb", [1, 2])
+def test_stepped_device_code_matches_oracle(stepper, tmp_path, N, n2max, gamma, L, nvec, f32, tol, nb):
     rng = np.random.default_rng(5)
     m = ogs.enumerate_sphere(n2max)
     V = rng.standard_normal((N, N, N))
@@ -47,7 +47,7 @@ def test_stepped_device_code_matches_oracle(stepper, tmp_path, N, n2max, gamma, 
     with open(fin, "wb") as f:
         f.write(np.ascontiguousarray(X).astype(np.complex128).tobytes())
         f.write(V.tobytes())
-    r = subprocess.run([stepper, str(N), str(n2max), str(gamma), str(L), str(nvec), str(f32), fin, fout, str(fused)], capture_output=True, text=True)
+    r = subprocess.run([stepper, str(N), str(n2max), str(gamma), str(L), str(nvec), str(f32), fin, fout, str(nb)], capture_output=True, text=True)
     assert r.returncode == 0, r.stderr
     raw = open(fout, "rb").read()
     ng = X.shape[1]
