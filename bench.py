@@ -339,7 +339,7 @@ def measure_fp64_peak():
     return _FP64_PEAK["v"]
 
 
-def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g, fp64_peak):
+def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g, fp64_peak, shift_updates=0):
     """Roofline entry for the kernel class that took the most time in the profiled step (DESIGN.md section 6 states the per-unit
     figures).  n_h = vectors pushed through H in that step."""
     N = cfg["N"]
@@ -396,8 +396,10 @@ def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g
         # CG vector kernel.  PCG/COCG column-resident or streaming: 4 reads + 3 writes of a column per iteration (p, Ap, x, r | x, r, p).
         # multi-shift: r, p, Ap (3 reads + 2 writes) plus, per live shift, p_s (2 real vectors read + written) and Re x_s (1 read + written)
         if solver == 1:
-            per_col = (5 + 6 * n_freq) * 16 * n_g
-            note = "multi-shift: (5 + 6 n_freq) vector passes of 16 n_g bytes per column and iteration, every shift counted live (an upper bound late in the solve)"
+            # 8 passes for the seed recurrence (p, Ap | r, Ap -> r | r, p -> p) and 6 per live shift (p_s: two real vectors read and written, Re x_s
+            # read and written); the library counts the (column, shift) updates it performed (west_stats.n_shift_updates)
+            per_col = (8 + 6.0 * shift_updates / max(n_h, 1)) * 16 * n_g
+            note = "multi-shift: 8 + 6 x (live shifts per column, measured: %.2f of %d) vector passes of 16 n_g bytes per column and iteration" % (shift_updates / max(n_h, 1), n_freq)
         else:
             per_col = 7 * 16 * n_g
             note = "7 vector passes of 16 n_g bytes per column and iteration"
@@ -514,7 +516,7 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
                    "l2": "inputs per step (vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
         "h_apply_per_s": n_h * world / (ms * 1e-3), "h_apply_per_step": n_h / steps,
         "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": roofline(cfg, top, prof, n_h_prof, n_freq, solver, hbm_peak, peak_src, mixed, w.n_g, fp64_peak),
+        "roofline": roofline(cfg, top, prof, n_h_prof, n_freq, solver, hbm_peak, peak_src, mixed, w.n_g, fp64_peak, pst.get("n_shift_updates", 0)),
         "gemm": {"achieved_tflops": gemm_tf, "peak_tflops": fp64_peak, "frac": (gemm_tf / fp64_peak) if gemm_tf else None,
                  "note": "KB + P_v GEMMs of the CG loop in the profiled step (RHS projection excluded from the flop count)"},
         "kernel_ms_per_step": {k: round(v["ms"], 3) for k, v in prof.items() if v["spans"]},

@@ -128,6 +128,7 @@ typedef struct {            /* host struct, filled when non-NULL (one stream syn
     int32_t n_unconverged;  /* columns above tol at exit */
     double  resid_max;      /* max over columns of ||r|| / ||b|| (recurrence residual) */
     int64_t n_h_apply;      /* vectors pushed through H in this call (real functions in GAMMA mode) */
+    int64_t n_shift_updates;/* multi-shift solver: (column, frequency) vector updates performed (frozen frequencies are skipped) */
     float   ms_rhs, ms_cg, ms_dn;   /* CUDA-event times of the three phases */
 } west_stats;
 

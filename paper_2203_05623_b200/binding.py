@@ -29,7 +29,7 @@ class west_cg_opts(C.Structure):
 
 
 class west_stats(C.Structure):
-    _fields_ = [("iters", C.c_int32), ("iters_min", C.c_int32), ("n_sub_blocks", C.c_int32), ("n_unconverged", C.c_int32), ("resid_max", C.c_double), ("n_h_apply", C.c_int64),
+    _fields_ = [("iters", C.c_int32), ("iters_min", C.c_int32), ("n_sub_blocks", C.c_int32), ("n_unconverged", C.c_int32), ("resid_max", C.c_double), ("n_h_apply", C.c_int64), ("n_shift_updates", C.c_int64),
                 ("ms_rhs", C.c_float), ("ms_cg", C.c_float), ("ms_dn", C.c_float)]
 
 

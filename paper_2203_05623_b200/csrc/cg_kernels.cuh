@@ -413,7 +413,7 @@ struct MsState {
     int*     active;     // [n_col]
     int*     iters;      // [n_col] iterations this column took part in
     int*     sactive;    // [n_shift][n_col]
-    int*     counters;   // [0] live columns
+    int*     counters;   // [0] live columns; [2..3] one 64-bit count of (column, shift) vector updates
 };
 struct MsShifts { int n; double omega[MS_MAX_SHIFTS]; };
 
@@ -533,6 +533,9 @@ __global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts
     if (threadIdx.x == 0) {
         st.a_prev[col] = a; st.b_prev[col] = b; st.rr[col] = rrn;
         st.iters[col] += 1;
+        int n_on = 0;
+        for (int s = 0; s < sh.n; ++s) n_on += s_on[s];
+        atomicAdd(reinterpret_cast<unsigned long long*>(st.counters + 2), (unsigned long long)n_on);     // (column, shift) updates done: the byte model of the bench
         int any = 0;
         for (int s = 0; s < sh.n; ++s) any |= st.sactive[(long long)s * n_col + col];
         if (!any) { st.active[col] = 0; atomicSub(st.counters, 1); }
@@ -633,6 +636,35 @@ __global__ void lowrank_fix(int M, int Nn, long long ldc, double* C, const doubl
         coef = alpha_vec[col % n_occ];
     } else coef = alpha_const;
     C[(long long)m * ldc + n] = coef * c;
+}
+
+// The same step for the tensor path of WEST_MIXED (tc_gemm.cuh): the overlap block arrives TRANSPOSED, Ct[n][ldt] (m contiguous), and
+// leaves as the TF32 hi / lo split of coef(m, n) * fix(Ct[n][m]), [n][ldt] f32 each (rows m >= M are written as zero padding).
+__global__ void lowrank_fix_split(int M, int Nn, long long ldt, const double* Ct, const double* A, long long lda, const double* X, long long ldx,
+                                  const double* dcoef, int n_rows_d, double alpha_const, const double* alpha_vec, const int* colmap, int nvpc,
+                                  int n_occ, int gamma, float* hi, float* lo) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)Nn * ldt) return;
+    const int n = (int)(i / ldt), m = (int)(i - (long long)n * ldt);
+    float h = 0.f, l = 0.f;
+    if (m < M) {
+        double c = Ct[i];
+        if (gamma) c = 2.0 * c - A[(long long)m * lda] * X[(long long)n * ldx];
+        double coef;
+        if (m < n_rows_d) coef = dcoef[m];
+        else if (alpha_vec) {
+            int col = n / nvpc;
+            if (colmap) { col = colmap[col]; if (col < 0) col = 0; }
+            coef = alpha_vec[col % n_occ];
+        } else coef = alpha_const;
+        const float f = (float)(coef * c);
+        unsigned int hb, lb;
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hb) : "f"(f));
+        const float r = f - __uint_as_float(hb);
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lb) : "f"(r));
+        h = __uint_as_float(hb); l = __uint_as_float(lb);
+    }
+    hi[i] = h; lo[i] = l;
 }
 
 }  // namespace wcg

@@ -19,6 +19,8 @@
 #include "gsphere.hpp"
 #include "lanczos_kernels.cuh"
 #include "bcg_kernels.cuh"
+#include "tc_gemm.cuh"
+#include <cudaTypedefs.h>
 
 namespace {
 
@@ -76,6 +78,11 @@ struct west_ctx {
     std::vector<double> h_eps_defl;
     DevBuf A_kb, A_psi;                // [rows][2 n_g] f64 each (kept apart; concatenated lazily into A_all)
     DevBuf A_all;                      // [rows_kb + rows_psi + rows_defl][2 n_g]
+    // WEST_MIXED tensor path (tc_gemm.cuh): the operator matrix pre-split into TF32 hi / lo parts, row-major [rows][Kp] and transposed
+    // [K][rows_p] (both k- resp. row-contiguous "K-major" operands of tcgen05.mma), built on first mixed use after a west_set_* change
+    DevBuf A_hi, A_lo, AT_hi, AT_lo;
+    bool tc_dirty = true;
+    void* tm_encode = nullptr;         // cuTensorMapEncodeTiled (driver entry point; NULL: the mma.sync 3xTF32 kernels are used instead)
     bool A_dirty = true;
     std::vector<double> h_dcoef;       // per stacked KB row
     std::vector<double> h_eps;
@@ -90,7 +97,7 @@ struct west_ctx {
 
     // hot-call workspaces: carved from the arena at the start of every hot call (hot_begin / hot)
     Arena arena;
-    DevBuf W, Cbuf, Rbuf, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk;
+    DevBuf W, Cbuf, Rbuf, Xsplit, Csplit, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk;
     int* h_pinned = nullptr;           // pinned host scratch (64 ints): lagged convergence polls [0], [1]; reports [8..]
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
 
@@ -361,7 +368,7 @@ size_t bytes_W(const west_ctx* c, long long n_slots, int f32) {
     return (size_t)n * c->cell.N * c->hs.n_cols * (f32 ? 8 : 16);
 }
 int ensure_W(west_ctx* c, long long n_slots, int f32) { return hot(c, c->W, bytes_W(c, n_slots, f32)); }
-size_t bytes_C(int rows, long long n_vec) { return (size_t)rows * (size_t)((n_vec + 1) / 2 * 2) * sizeof(double); }
+size_t bytes_C(int rows, long long n_vec) { return (size_t)((rows + 3) / 4 * 4) * (size_t)((n_vec + 1) / 2 * 2) * sizeof(double); }
 
 // opt-in to the GEMM kernels' dynamic shared memory (all four instantiations), once per process
 cudaError_t gemm_attrs() {
@@ -447,10 +454,106 @@ struct LowrankCoef {
     double alpha_const = 0.0; const double* alpha_vec = nullptr; const int* colmap = nullptr; int nvpc = 1, n_occ = 1;
 };
 
+// ---- WEST_MIXED tensor path (tcgen05 kind::tf32, tc_gemm.cuh)
+inline long long pad4(long long n) { return (n + 3) / 4 * 4; }
+bool tc_available(const west_ctx* c) { return c->tm_encode != nullptr; }
+size_t tc_hot_bytes(const west_ctx* c, int rows, long long n_vec) {       // Xsplit + Csplit of one lowrank_apply
+    if (!tc_available(c) || rows <= 0) return 0;
+    const long long Kp = pad4(2 * c->hs.n_g), rp = pad4(rows);
+    return al256(sizeof(float) * 2 * (size_t)n_vec * Kp) + al256(sizeof(float) * 2 * (size_t)n_vec * rp);
+}
+int tc_map(west_ctx* c, CUtensorMap* m, const float* p, long long rows, long long cols, long long ld) {
+    cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    cuuint64_t gstr[1] = {(cuuint64_t)ld * sizeof(float)};
+    cuuint32_t box[2] = {(cuuint32_t)wtc::BK, (cuuint32_t)wtc::BM}, es[2] = {1, 1};
+    const CUresult r = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(c->tm_encode)(
+        m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)p, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(c, WEST_ECUDA, "cuTensorMapEncodeTiled failed (%d) for a %lld x %lld map", (int)r, rows, cols);
+    return WEST_OK;
+}
+// operator data of the tensor path: (re)split the stacked operator matrix after a west_set_* change (not a hot-arena buffer)
+int ensure_tc_operator(west_ctx* c) {
+    if (!c->tc_dirty) return WEST_OK;
+    const long long K = 2 * c->hs.n_g, Kp = pad4(K);
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
+    const long long rp = pad4(rows);
+    int rc;
+    if ((rc = ensure(c, c->A_hi, sizeof(float) * (size_t)rows * Kp))) return rc;
+    if ((rc = ensure(c, c->A_lo, sizeof(float) * (size_t)rows * Kp))) return rc;
+    if ((rc = ensure(c, c->AT_hi, sizeof(float) * (size_t)K * rp))) return rc;
+    if ((rc = ensure(c, c->AT_lo, sizeof(float) * (size_t)K * rp))) return rc;
+    const double* A = (const double*)c->A_all.p;
+    wtc::split_rows<<<blocks_for((long long)rows * Kp, 256), 256, 0, c->st>>>(rows, K, A, K, (float*)c->A_hi.p, (float*)c->A_lo.p, Kp);
+    wtc::split_rows_transposed<<<dim3((unsigned)((K + 31) / 32), (unsigned)((rp + 31) / 32)), dim3(32, 8), 0, c->st>>>(rows, K, A, K, (float*)c->AT_hi.p,
+                                                                                                                   (float*)c->AT_lo.p, rp);
+    CK(cudaGetLastError());
+    c->launches += 2;
+    c->tc_dirty = false;
+    return WEST_OK;
+}
+cudaError_t tc_attrs() {
+    static bool done = false;
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(wtc::tf32x3_gemm<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wtc::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wtc::tf32x3_gemm<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wtc::SMEM_BYTES);
+    done = e == cudaSuccess;
+    return e;
+}
+// rows [0, nr) of the operator matrix on the tensor path:  Y += A^T (coef . fix(A X^T))
+int lowrank_apply_tc(west_ctx* c, int nr, int n_vec, const double* X, double* Y, const LowrankCoef& lc) {
+    const long long K = 2 * c->hs.n_g, Kp = pad4(K), rp = pad4(nr);
+    const int rows_all = c->rows_kb + c->rows_psi + c->rows_defl;
+    const long long rp_all = pad4(rows_all);
+    int rc;
+    CK(tc_attrs());
+    if ((rc = ensure_tc_operator(c))) return rc;
+    if ((rc = hot(c, c->Xsplit, sizeof(float) * 2 * (size_t)n_vec * Kp))) return rc;
+    if ((rc = hot(c, c->Csplit, sizeof(float) * 2 * (size_t)n_vec * rp))) return rc;
+    if ((rc = hot(c, c->Cbuf, bytes_C(nr, n_vec)))) return rc;
+    float* Xh = (float*)c->Xsplit.p; float* Xl = Xh + (size_t)n_vec * Kp;
+    float* Ch = (float*)c->Csplit.p; float* Cl = Ch + (size_t)n_vec * rp;
+    double* Ct = (double*)c->Cbuf.p;                       // [n_vec][rp] (transposed overlap block, rows contiguous)
+    wtc::Maps m1, m2;
+    if ((rc = tc_map(c, &m1.a_hi, (const float*)c->A_hi.p, nr, K, Kp)) || (rc = tc_map(c, &m1.a_lo, (const float*)c->A_lo.p, nr, K, Kp)) ||
+        (rc = tc_map(c, &m1.b_hi, Xh, n_vec, K, Kp)) || (rc = tc_map(c, &m1.b_lo, Xl, n_vec, K, Kp)) ||
+        (rc = tc_map(c, &m2.a_hi, (const float*)c->AT_hi.p, K, nr, rp_all)) || (rc = tc_map(c, &m2.a_lo, (const float*)c->AT_lo.p, K, nr, rp_all)) ||
+        (rc = tc_map(c, &m2.b_hi, Ch, n_vec, nr, rp)) || (rc = tc_map(c, &m2.b_lo, Cl, n_vec, nr, rp)))
+        return rc;
+    {
+        Prof p_(c, PC_GEMM_TN);
+        wtc::split_rows<<<blocks_for((long long)n_vec * Kp, 256), 256, 0, c->st>>>(n_vec, K, X, K, Xh, Xl, Kp);
+        CK(cudaMemsetAsync(Ct, 0, sizeof(double) * (size_t)n_vec * rp, c->st));
+        const int n_kb = (int)((K + wtc::BK - 1) / wtc::BK);
+        const long long tiles = (long long)((nr + 127) / 128) * ((n_vec + 127) / 128);
+        int splits = (int)std::max<long long>(1, std::min<long long>(n_kb / 16, (148 * 2 + tiles - 1) / tiles));
+        int kps = (n_kb + splits - 1) / splits;
+        splits = (n_kb + kps - 1) / kps;
+        wtc::tf32x3_gemm<true><<<dim3((nr + 127) / 128, (n_vec + 127) / 128, splits), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m1, nr, n_vec, n_kb, kps, Ct, rp);
+        CK(cudaGetLastError());
+        c->launches += 2;
+    }
+    wcg::lowrank_fix_split<<<blocks_for((long long)n_vec * rp, 256), 256, 0, c->st>>>(nr, n_vec, rp, Ct, (const double*)c->A_all.p, K, X, K, lc.dcoef, lc.n_rows_d,
+                                                                               lc.alpha_const, lc.alpha_vec, lc.colmap, lc.nvpc, lc.n_occ, is_gamma(c) ? 1 : 0, Ch, Cl);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    {
+        Prof p_(c, PC_GEMM_UP);
+        const int n_kb = (nr + wtc::BK - 1) / wtc::BK;
+        wtc::tf32x3_gemm<false><<<dim3((unsigned)((K + 127) / 128), (n_vec + 127) / 128, 1), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m2, (int)K, n_vec, n_kb, n_kb, Y, K);
+        CK(cudaGetLastError());
+        c->launches += 1;
+    }
+    return WEST_OK;
+}
+
 // Y += sum_{m in [r0, r0+nr)} coef_m A_m <A_m, X>   for n_vec real-function / complex vectors (as 2 n_g reals each).
-// tf32: the WEST_MIXED path of H*psi (3xTF32 tensor-core products, FP32 class) - never the RHS projection or the deflation
+// tf32: the WEST_MIXED path of H*psi (3xTF32 tensor-core products, FP32 class) - never the RHS projection or the deflation.
+// On Blackwell the tf32 products run on tcgen05 (lowrank_apply_tc); the warp-level mma.sync kernels remain as the path taken when the
+// driver offers no tensor-map encoder.
 int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const LowrankCoef& lc, bool tf32 = false) {
     if (nr <= 0 || n_vec <= 0) return WEST_OK;
+    if (tf32 && r0 == 0 && tc_available(c)) return lowrank_apply_tc(c, nr, n_vec, X, Y, lc);
     const long long K = 2 * c->hs.n_g;
     const long long ldc = (n_vec + 1) / 2 * 2;
     int rc = hot(c, c->Cbuf, bytes_C(nr, n_vec));
@@ -499,14 +602,13 @@ size_t plan_lanczos(const west_ctx* c, int n_pert, int n_steps, int f32) {
     const long long slots_h = is_gamma(c) ? ((long long)n_col + 1) / 2 : (long long)n_col, slots_r = (long long)n_pert * c->n_uslots;
     size_t t = 4 * al256(sizeof(cx<double>) * (size_t)c->hs.n_g * n_col) + al256(sizeof(double) * (size_t)n3_of(c) * n_pert) + al256(sizeof(double) * n_col + 64) +
                al256(bytes_W(c, std::max(slots_h, slots_r), 0)) + al256(256);
-    if (c->rows_kb > 0) t += al256(bytes_C(c->rows_kb, (long long)n_col));
+    if (c->rows_kb > 0) t += al256(bytes_C(c->rows_kb, (long long)n_col)) + (f32 ? tc_hot_bytes(c, c->rows_kb, (long long)n_col) : 0);
     if (c->n_occ_user != c->n_occ) t += al256(sizeof(double) * n_col * (2 * (size_t)n_steps + 1));
-    (void)f32;
     return t;
 }
 size_t plan_happly(const west_ctx* c, long long n_vec, int f32) {
     const long long n_slots = is_gamma(c) ? (n_vec + 1) / 2 : n_vec;
-    return al256(bytes_W(c, n_slots, f32)) + (c->rows_kb > 0 ? al256(bytes_C(c->rows_kb, n_vec)) : 0);
+    return al256(bytes_W(c, n_slots, f32)) + (c->rows_kb > 0 ? al256(bytes_C(c->rows_kb, n_vec)) + (f32 ? tc_hot_bytes(c, c->rows_kb, n_vec) : 0) : 0);
 }
 
 }  // namespace
@@ -601,6 +703,12 @@ int west_create(west_ctx** out, const west_cell* cell, void* stream) {
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_poll[0], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_poll[1], cudaEventDisableTiming);
     if (e != cudaSuccess) { fail(c, WEST_ECUDA, "west_create: %s", cudaGetErrorString(e)); return bail(WEST_ECUDA); }
+    {
+        cudaDriverEntryPointQueryResult q;
+        void* fn = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) c->tm_encode = fn;
+        else cudaGetLastError();
+    }
     // twiddle tables of west_fft3d_dense (all three grid sizes, 7 KB): no allocation in the hot call
     for (int n : {64, 128, 256}) {
         std::vector<cx<double>> dtw(n);
@@ -676,7 +784,7 @@ int west_set_kb(west_ctx* c, int32_t n_proj, const void* beta, const double* dco
     const long long n_g = c->hs.n_g;
     c->n_proj = n_proj;
     c->rows_kb = n_proj * (full ? 2 : 1);
-    c->A_dirty = true;
+    c->A_dirty = true; c->tc_dirty = true;
     c->h_dcoef.resize(c->rows_kb);
     for (int k = 0; k < n_proj; ++k) {
         if (full) { c->h_dcoef[2 * k] = dcoef_host[k]; c->h_dcoef[2 * k + 1] = dcoef_host[k]; }
@@ -705,7 +813,7 @@ int west_set_states(west_ctx* c, int32_t n_occ_user, const void* psi, const doub
     c->n_occ = n_occ;
     c->n_occ_user = n_occ_user;
     c->rows_psi = n_occ * (full ? 2 : 1);
-    c->A_dirty = true;
+    c->A_dirty = true; c->tc_dirty = true;
     c->h_eps.assign(eps_host, eps_host + n_occ_user);
     if (n_occ > n_occ_user) c->h_eps.push_back(eps_host[n_occ_user - 1]);
     int rc = ensure(c, c->A_psi, (size_t)c->rows_psi * 2 * n_g * sizeof(double));
@@ -758,7 +866,7 @@ int west_set_deflation(west_ctx* c, int32_t n_defl, const void* psi_c, const dou
     const long long n_g = c->hs.n_g;
     c->n_defl = n_defl;
     c->rows_defl = n_defl * (full ? 2 : 1);
-    c->A_dirty = true;
+    c->A_dirty = true; c->tc_dirty = true;
     if (n_defl == 0) return WEST_OK;
     c->h_eps_defl.assign(eps_host, eps_host + n_defl);
     int rc = ensure(c, c->A_defl, (size_t)c->rows_defl * 2 * n_g * sizeof(double));
@@ -1133,7 +1241,7 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
     const double tol2 = o.tol * o.tol;
     const int every = std::max(1, o.check_every);
     int* colmap = maps; int* newmap = maps + n_col; int* src = maps + 2 * (size_t)n_col;
-    CK(cudaMemsetAsync(st.counters, 0, 2 * sizeof(int), c->st));
+    CK(cudaMemsetAsync(st.counters, 0, 4 * sizeof(int), c->st));
     CK(cudaMemsetAsync(XS, 0, sizeof(cx<double>) * 2 * n_g * n_col * sh.n, c->st));
     wcg::ms_init<<<n_col, wcg::NT, 0, c->st>>>(n_g, n_col, sh, (const double2*)R, (double2*)P, (double2*)PS, st, colmap);
     CK(cudaGetLastError());
@@ -1337,7 +1445,7 @@ struct Chi0Plan {
         return t;
     }
 };
-Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb) {
+Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, int f32 = 0) {
     Chi0Plan p;
     p.solver = solver; p.nvpc = nvpc; p.n_freq = n_freq; p.pb = pb;
     const size_t n_g = (size_t)c->hs.n_g, n3 = (size_t)n3_of(c);
@@ -1354,6 +1462,7 @@ Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb) 
     p.W = bytes_W(c, std::max(slots_h, slots_r), 0);
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     p.C = bytes_C(rows, n_vec);
+    if (f32) p.blk += tc_hot_bytes(c, rows, n_vec);
     p.alpha = sizeof(double) * c->n_occ;
     if (solver == 2) p.blk = bcg_small_bytes(c->n_occ, pb);
     if (solver == 1) {
@@ -1408,7 +1517,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     int pb = n_pert;
     for (int nb = 1;; ++nb) {
         pb = (n_pert + nb - 1) / nb;
-        plan = chi0_plan(c, opts->solver, nvpc_max, n_freq, pb);
+        plan = chi0_plan(c, opts->solver, nvpc_max, n_freq, pb, f32);
         if (plan.total() <= budget || pb == 1) break;
     }
     if (plan.total() > budget)
@@ -1521,7 +1630,9 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             if (stats) CK(cudaEventRecord(ev[3], c->st));
             double* h = (double*)(c->h_pinned + 8);
             CK(cudaMemcpyAsync(h, rep, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+            CK(cudaMemcpyAsync(c->h_pinned + 16, st.counters + 2, sizeof(long long), cudaMemcpyDeviceToHost, c->st));
             CK(cudaStreamSynchronize(c->st));
+            if (stats) stats->n_shift_updates += *reinterpret_cast<long long*>(c->h_pinned + 16);
             if (h[1] > 0) ret = WEST_NOTCONVERGED;
             if (stats) {
                 add_times();
@@ -1600,10 +1711,10 @@ extern "C" size_t west_workspace_bytes(const west_ctx* c, int32_t op, int32_t n_
     switch (op) {
         case WEST_OP_FFT3D: return plan_fft3d(c, n_pert);
         case WEST_OP_H_APPLY: return plan_happly(c, n_pert, f32);
-        case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert).total();
-        case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert).total();
-        case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert).total();
-        case WEST_OP_CHI0_BLOCK: return chi0_plan(c, 2, 1, std::max(1, n_freq), n_pert).total();
+        case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert, f32).total();
+        case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert, f32).total();
+        case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32).total();
+        case WEST_OP_CHI0_BLOCK: return chi0_plan(c, 2, 1, std::max(1, n_freq), n_pert, f32).total();
         case WEST_OP_LANCZOS: return plan_lanczos(c, n_pert, std::max(1, n_freq), f32);
     }
     return 0;
