@@ -331,14 +331,14 @@ struct K2 {
                 const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
 #pragma unroll
                 for (int n1 = 0; n1 < N1; ++n1)
-                    v[b][n1] = (it < nrow * N2 && keep_n1<N1, N2>(n1)) ? load_disc(Wp, g, row, N2 * n1 + n2) : mk<T>(0, 0);
+                    v[b][n1] = ((NB == 1 || it < nrow * N2) && keep_n1<N1, N2>(n1)) ? load_disc(Wp, g, row, N2 * n1 + n2) : mk<T>(0, 0);
             }
 #pragma unroll
             for (int b = 0; b < NB; ++b) Dft<T, N1, +1>::run(v[b]);
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
-                if (it >= nrow * N2) continue;
+                if (NB > 1 && it >= nrow * N2) continue;
                 const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
                 tw_store_strided(v[b], tw[N2 + n2], S + row * PITCH + n2);
             }
@@ -361,7 +361,7 @@ struct K2 {
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
-                if (it >= nrow * N1) continue;
+                if (NB > 1 && it >= nrow * N1) continue;
                 cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) p[j] = v[b][j];
@@ -372,12 +372,13 @@ struct K2 {
     template <int NB = 1>
     static WHD void xA(int tid, int nthr, const cx<T>* S, cx<T>* X, const cx<T>* tw, const WestGeom& g, int py0) {
         for (int it0 = tid; it0 < LC * N2; it0 += NB * nthr) {
+            if (NB == 1 && py0 + it0 / N2 >= N) continue;                 // NB = 1: an item beyond the grid is skipped outright
             cx<T> v[NB][N1];
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const int l = it / N2, n2 = it - l * N2, py = py0 + l;
-                const bool ok = it < LC * N2 && py < N;
+                const bool ok = NB == 1 || (it < LC * N2 && py < N);
 #pragma unroll
                 for (int n1 = 0; n1 < N1; ++n1) {
                     const int nx = wrap_signed(N2 * n1 + n2, N);
@@ -390,7 +391,7 @@ struct K2 {
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const int l = it / N2, n2 = it - l * N2;
-                if (it >= LC * N2 || py0 + l >= N) continue;
+                if (NB > 1 && (it >= LC * N2 || py0 + l >= N)) continue;
                 tw_store_strided(v[b], tw[N2 + n2], X + l * PITCH + n2);
             }
         }
@@ -446,13 +447,14 @@ struct K2 {
     template <int NB = 1>
     static WHD void xB(int tid, int nthr, cx<T>* X, const cx<T>* tw, const K2Args<T>& a, int slot, int pz, int py0) {
         for (int it0 = tid; it0 < LC * N1; it0 += NB * nthr) {
+            if (NB == 1 && py0 + it0 / N1 >= N) continue;
             cx<T> v[NB][N2];
             bool ok[NB], fwd[NB];
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const int l = it / N1, k1 = it - l * N1;
-                ok[b] = it < LC * N1 && py0 + l < N;
+                ok[b] = NB == 1 || (it < LC * N1 && py0 + l < N);
                 if (MODE != K2_FROMR) {
                     const cx<T>* p = X + l * PITCH + N2 * k1;
 #pragma unroll
@@ -484,12 +486,13 @@ struct K2 {
     template <int NB = 1>
     static WHD void xC(int tid, int nthr, cx<T>* S, const cx<T>* X, const WestGeom& g, int py0) {
         for (int it0 = tid; it0 < LC * N2; it0 += NB * nthr) {
+            if (NB == 1 && py0 + it0 / N2 >= N) continue;
             cx<T> v[NB][N1];
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const int l = it / N2, n2 = it - l * N2;
-                const bool ok = it < LC * N2 && py0 + l < N;
+                const bool ok = NB == 1 || (it < LC * N2 && py0 + l < N);
                 const cx<T>* p = X + l * PITCH + n2;
 #pragma unroll
                 for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[N2 * k1] : mk<T>(0, 0);
@@ -500,7 +503,7 @@ struct K2 {
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const int l = it / N2, n2 = it - l * N2, py = py0 + l;
-                if (it >= LC * N2 || py >= N) continue;
+                if (NB > 1 && (it >= LC * N2 || py >= N)) continue;
 #pragma unroll
                 for (int n1 = 0; n1 < N1; ++n1) {
                     if (!keep_n1<N1, N2>(n1)) continue;
@@ -527,7 +530,7 @@ struct K2 {
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
-                if (it >= nrow * N1) continue;
+                if (NB > 1 && it >= nrow * N1) continue;
                 const int k1 = it % N1;
                 tw_store_contig(v[b], tw[N + N1 + k1], S + (row0 + it / N1) * PITCH + N2 * k1);
             }
@@ -550,7 +553,7 @@ struct K2 {
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
-                if (it >= nrow * N2) continue;
+                if (NB > 1 && it >= nrow * N2) continue;
                 const int rl = it / N2, n2 = it - rl * N2, row = row0 + rl;
                 const int c0 = g.row_off[row], ymax = (g.row_off[row + 1] - c0 - 1) >> 1;
 #pragma unroll

@@ -178,13 +178,26 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
         }
         const int r = r0 + warp * 32 + lane;
         if (r < rows_a) {
+            if (ATOMIC) {
 #pragma unroll
-            for (int j = 0; j < BN; ++j) {
-                const int cc = c0 + j;
-                if (cc < rows_b) {
-                    double* o = out + (long long)cc * ldo + r;
-                    if (ATOMIC) atomicAdd(o, (double)acc[j]);
-                    else *o += (double)acc[j];
+                for (int j = 0; j < BN; ++j)
+                    if (c0 + j < rows_b) atomicAdd(out + (long long)(c0 + j) * ldo + r, (double)acc[j]);
+            } else {
+                // read-modify-write in groups of 16 columns: all loads of a group are in flight before the first add (one memory latency per
+                // group instead of one per element)
+#pragma unroll
+                for (int q = 0; q < BN / 16; ++q) {
+                    double old[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const int cc = c0 + q * 16 + j;
+                        old[j] = cc < rows_b ? __ldcg(out + (long long)cc * ldo + r) : 0.0;
+                    }
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const int cc = c0 + q * 16 + j;
+                        if (cc < rows_b) __stcg(out + (long long)cc * ldo + r, old[j] + (double)acc[q * 16 + j]);
+                    }
                 }
             }
         }

@@ -1435,10 +1435,11 @@ int bcg_solve(west_ctx* c, int f32, int s, const west_cg_opts& o, cx<double>* X,
 // ---- workspace plan of west_chi0_apply for a sub-block of pb perturbations
 struct Chi0Plan {
     int solver = 0, nvpc = 1, n_freq = 1, pb = 0;
+    size_t tc = 0;         // WEST_MIXED tensor path: split operands of one low-rank apply (a sum of al256 pieces)
     size_t blk = 0;        // block CG: Gram / coefficient / factor blocks and flags (already a sum of al256 pieces)
     size_t vec = 0, xs = 0, shift = 0, grid = 0, scal = 0, maps = 0, misc = 0, W = 0, C = 0, msst = 0, craw = 0, dcoefd = 0, alpha = 0;
     size_t total() const {
-        size_t t = (solver == 1 ? 3 : (solver == 2 ? 5 : 4)) * al256(vec) + blk + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) +
+        size_t t = (solver == 1 ? 3 : (solver == 2 ? 5 : 4)) * al256(vec) + blk + tc + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) +
                    al256(C) + al256(alpha);
         if (solver == 1) t += 2 * al256(xs) + al256(msst);
         if (craw) t += al256(craw) + al256(dcoefd);
@@ -1462,7 +1463,7 @@ Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, 
     p.W = bytes_W(c, std::max(slots_h, slots_r), 0);
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     p.C = bytes_C(rows, n_vec);
-    if (f32) p.blk += tc_hot_bytes(c, rows, n_vec);
+    if (f32) p.tc = tc_hot_bytes(c, rows, n_vec);
     p.alpha = sizeof(double) * c->n_occ;
     if (solver == 2) p.blk = bcg_small_bytes(c->n_occ, pb);
     if (solver == 1) {
