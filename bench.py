@@ -440,8 +440,11 @@ def make_workspace(w, wb, op, n_pert, n_freq, precision, reserve_bytes):
     return ws, fit
 
 
-def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps, warmup, local, world, barrier, e2e_steps, want_cpu, label):
-    """Times `steps` calls of west_chi0_apply on the block dV_np (after `warmup` untimed ones) and returns the record of that workload."""
+def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps, warmup, local, world, barrier, e2e_steps, want_cpu, label, profile_in_timed=False):
+    """Times `steps` calls of west_chi0_apply on the block dV_np (after `warmup` untimed ones) and returns the record of that workload.
+    want_cpu: 0 nothing from the oracle, 1 parity_sample only, 2 parity_sample + cpu_baseline with its legs.
+    profile_in_timed: take the per-kernel-class times from the timed steps themselves (one CUDA-event pair around every launch) instead of
+    an extra step - only for the long sub-record, where a step takes a hundred seconds and the events cost nothing next to it."""
     import torch
     import torch.distributed as dist
     dev = torch.device("cuda")
@@ -462,6 +465,8 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
     sampler = ClockSampler(local)
     sampler.start()
     launches0 = w.launch_count()
+    if profile_in_timed:
+        w.set_profile(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     n_h = 0
@@ -473,12 +478,20 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
     ms = e0.elapsed_time(e1)
     launches = w.launch_count() - launches0
     clocks = sampler.finish()
-    # ---- per-kernel-class times: one extra, untimed step with the event profiler on
-    w.set_profile(True)
-    _, _, pst = w.chi0_apply(dV, omegas, **kw)
-    prof = w.get_profile()
-    w.set_profile(False)
-    n_h_prof = pst["n_h_apply"]
+    if profile_in_timed:
+        prof = w.get_profile()
+        w.set_profile(False)
+        for v in prof.values():
+            v["ms"] /= steps
+            v["spans"] = max(v["spans"] // steps, 1) if v["spans"] else 0
+        n_h_prof, pst = n_h / steps, stats
+    else:
+        # ---- per-kernel-class times: one extra, untimed step with the event profiler on
+        w.set_profile(True)
+        _, _, pst = w.chi0_apply(dV, omegas, **kw)
+        prof = w.get_profile()
+        w.set_profile(False)
+        n_h_prof = pst["n_h_apply"]
     # ---- end to end: pinned host dV -> device, chi0_apply, dn -> pinned host, all inside the timed region
     e2e_ms = None
     if e2e_steps > 0:
@@ -520,7 +533,7 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
         "gemm": {"achieved_tflops": gemm_tf, "peak_tflops": fp64_peak, "frac": (gemm_tf / fp64_peak) if gemm_tf else None,
                  "note": "KB + P_v GEMMs of the CG loop in the profiled step (RHS projection excluded from the flop count)"},
         "kernel_ms_per_step": {k: round(v["ms"], 3) for k, v in prof.items() if v["spans"]},
-        "kernel_ms_note": "one extra untimed step with CUDA events around every launch; the timed steps run without them",
+        "kernel_ms_note": "CUDA events around every launch of the timed step(s)" if profile_in_timed else "one extra untimed step with CUDA events around every launch; the timed steps run without them",
         "phase_ms_last_step": {"rhs": stats["ms_rhs"], "cg": stats["ms_cg"], "dn": stats["ms_dn"]},
         "device_gb": (w.device_bytes() + (ws.numel() if ws is not None else 0)) / 1e9,
     }
@@ -529,7 +542,7 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
                       "h2d_bytes_per_step": int(dV.numel() * 8), "d2h_bytes_per_step": int(dn.numel() * 8)}
     if want_cpu:
         try:
-            rec.update(parity_and_cpu(a, wb, cfg, w, dV, dV_np, alpha, aux, omegas, kw, n_h / steps))
+            rec.update(parity_and_cpu(a, wb, cfg, w, dV, dV_np, alpha, aux, omegas, kw, n_h / steps, want_cpu))
         except Exception as e:          # the oracle legs never take the GPU numbers down with them
             rec["cpu_baseline_error"] = repr(e)[:300]
     w.set_workspace(None)
@@ -538,7 +551,7 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
     return rec
 
 
-def parity_and_cpu(a, wb, cfg, w, dV, dV_np, alpha, aux, omegas, kw, n_h_step):
+def parity_and_cpu(a, wb, cfg, w, dV, dV_np, alpha, aux, omegas, kw, n_h_step, level):
     """parity_sample: the TIMED configuration (same options, same block) once more with dpsi requested, sampled columns against the
     oracle - its own PCG / COCG solutions where a column is affordable on the host, else the true residual with its H.
     cpu_baseline: the oracle's PCG on a bounded sample of the same workload, plus SURVEY 8(d)'s legs (i) and (ii)."""
@@ -559,10 +572,14 @@ def parity_and_cpu(a, wb, cfg, w, dV, dV_np, alpha, aux, omegas, kw, n_h_step):
         mean_iters = n_h_step / (n_pert * n_occ)                      # one Krylov sequence serves every frequency
     else:
         mean_iters = n_h_step / (n_pert * n_occ * sum(2 if om > 0 else 1 for om in omegas)) * 1.0
-    base, sols = cpu_pcg_leg(cfg, osd, dV_np[0], alpha, aux, budget_s=12.0 if big else 15.0, iters_hint=mean_iters)
-    base["h_apply_leg"] = cpu_h_apply_leg(cfg, osd, 4 if big else 64)
-    base["sum_over_states_leg"] = cpu_sum_over_states_leg()
-    out["cpu_baseline"] = base
+    sols = {}
+    if level >= 2:
+        base, sols = cpu_pcg_leg(cfg, osd, dV_np[0], alpha, aux, budget_s=12.0 if big else 15.0, iters_hint=mean_iters)
+        base["h_apply_leg"] = cpu_h_apply_leg(cfg, osd, 4 if big else 64)
+        base["sum_over_states_leg"] = cpu_sum_over_states_leg()
+        out["cpu_baseline"] = base
+    elif not big and omegas[0] == 0.0:
+        _, sols = cpu_pcg_leg(cfg, osd, dV_np[0], alpha, aux, budget_s=3.0)
 
     def col(wi, i, v):
         if gamma:
@@ -651,7 +668,7 @@ def main():
     big = cfg["N"] >= 144
     e2e_steps = min(a.steps, 2) if big else a.steps
     rec = run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, a.steps, a.warmup, local, world, barrier, e2e_steps,
-                   want_cpu=(world == 1 and rank == 0 and not a.no_cpu_baseline), label=a.workload)
+                   want_cpu=(2 if (world == 1 and rank == 0 and not a.no_cpu_baseline) else 0), label=a.workload)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -670,7 +687,7 @@ def main():
         try:
             om_iw = [x for x in cfg["omegas"] if x > 0]
             r = run_chi0(a, wb, cfg, w, dV_np, alpha, aux, om_iw, 1 if a.solver < 0 else a.solver, precision, 1, 0, local, world, barrier, 0,
-                         want_cpu=not a.no_cpu_baseline, label="cfg5 imaginary frequencies")
+                         want_cpu=0 if a.no_cpu_baseline else 1, label="cfg5 imaginary frequencies", profile_in_timed=True)
             r["note"] = "ONE timed step, no warm-up of its own (the kernels are warm from the headline steps; a step takes about 100 s)"
             subs["cfg5_iw"] = r
         except Exception as e:
@@ -687,7 +704,7 @@ def main():
                     om = omegas_for(a, c, name)
                     prec = wb.WEST_MIXED if c["precision"] == "mixed" else wb.WEST_FP64
                     subs[name] = run_chi0(a, wb, c, w2, dV2[:c["n_pert"]], alpha2, aux2, om, 1 if len(om) > 1 else 0, prec, SUB_STEPS, SUB_WARMUP, local, world,
-                                          barrier, SUB_STEPS if name == "cfg2" else 0, want_cpu=(name == "cfg2" and not a.no_cpu_baseline), label=name)
+                                          barrier, SUB_STEPS if name == "cfg2" else 0, want_cpu=0 if a.no_cpu_baseline else (2 if name == "cfg2" else 1), label=name)
                 except Exception as e:
                     subs[name] = {"error": repr(e)[:300]}
             w2.close()

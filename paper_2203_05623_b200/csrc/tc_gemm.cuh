@@ -10,7 +10,8 @@
 // tcgen05.ld and add it to FP32 registers with round-to-nearest while the next chunk is being multiplied.
 //
 // One kernel, D[r][c] = sum_k A[r][k] B[c][k] for a 128 x 128 tile:
-//   A, B : FP32 hi / lo arrays, row-major [rows][ld], k contiguous ("K-major"), ld a multiple of 4 (16-byte TMA strides);
+//   A, B : FP32 hi / lo arrays, k contiguous ("K-major"), addressed as (k, batch, row) tensors with strides that are multiples of 4 floats
+//          (16-byte TMA strides); a plain [rows][ld] matrix is the case of one batch entry;
 //          rows / k beyond the arrays read as zero (TMA out-of-bounds fill)
 //   out  : FP64, out[c * ldo + r] (r contiguous: lanes of a warp = consecutive r, so stores and atomics coalesce)
 //          ATOMIC: out += D by atomicAdd (split-K partial sums)      else: out += D (each element owned by one CTA)
@@ -51,9 +52,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     }
     __trap();
 }
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-                 ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+// tile of a (k, batch, row) tensor: box {BK, 1, 128}: 128 rows of one batch entry, BK reals along k; lands as a dense [128][BK] tile
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 // shared-memory matrix descriptor of a K-major tile with 128-byte swizzle: rows of 128 bytes, 8-row groups 1024 bytes apart
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
@@ -80,9 +82,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 
 struct Maps { CUtensorMap a_hi, a_lo, b_hi, b_lo; };
 
-// grid: (row tiles of A, row tiles of B, K splits).  kb_per_split: k-blocks (of BK) per split; n_kb: total k-blocks.
+// Persistent kernel: min(n_tiles, #SMs) CTAs walk the tile list (row tiles of A fastest, then row tiles of B, then K splits) so that the
+// TMA ring never drains between tiles and the epilogue of one tile overlaps the multiplications of the next (the two TMEM chunk
+// accumulators double as the hand-over buffers).  k-block, chunk and tile counters run on across tiles; barrier parities follow them.
+// kb_per_split: k-blocks (of BK) per split; n_kb: total k-blocks.
+struct TileGrid { int tiles_a, tiles_b, splits, n_batch; long long out_batch_stride; };      // batch entries: independent products (own slice of both operands and of out)
 template <bool ATOMIC>
-__global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant__ Maps maps, int rows_a, int rows_b, int n_kb, int kb_per_split,
+__global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant__ Maps maps, TileGrid tg, int rows_a, int rows_b, int n_kb, int kb_per_split,
                                                             double* __restrict__ out, long long ldo) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* tiles = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);      // swizzle-128B atoms need 1024-byte alignment
@@ -93,10 +99,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
     uint64_t* acc_empty = acc_full + 2;       // [2]       epilogue -> MMA
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int r0 = blockIdx.x * BM, c0 = blockIdx.y * BN;
-    const int kb0 = blockIdx.z * kb_per_split;
-    const int nkb = min(kb_per_split, n_kb - kb0);
-    const int n_chunks = (nkb + CHUNK_KB - 1) / CHUNK_KB;
+    const int n_tiles = tg.tiles_a * tg.tiles_b * tg.splits * tg.n_batch;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
@@ -111,92 +114,120 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
+    // tile t -> (row tile of A, row tile of B, split), k-block range of the split
+    auto tile_of = [&](int t, int& r0, int& c0, int& kb0, int& nkb, int& bt) {
+        const int ta = t % tg.tiles_a, rest = t / tg.tiles_a;
+        const int tb = rest % tg.tiles_b, rest2 = rest / tg.tiles_b;
+        const int sp = rest2 % tg.splits;
+        bt = rest2 / tg.splits;
+        r0 = ta * BM; c0 = tb * BN; kb0 = sp * kb_per_split;
+        nkb = min(kb_per_split, n_kb - kb0);
+        if (nkb < 0) nkb = 0;
+    };
 
     if (warp == 4) {
         // ===== TMA producer =====
         if (lane == 0) {
-            for (int i = 0; i < nkb; ++i) {
-                const int s = i % STAGES;
-                if (i >= STAGES) mbar_wait(empty + s, ((i / STAGES) - 1) & 1);
-                unsigned char* st = tiles + (size_t)s * STAGE_BYTES;
-                mbar_expect_tx(full + s, STAGE_BYTES);
-                const int k = (kb0 + i) * BK;
-                tma_load_2d(st, &maps.a_hi, full + s, k, r0);
-                tma_load_2d(st + TILE_BYTES, &maps.a_lo, full + s, k, r0);
-                tma_load_2d(st + 2 * TILE_BYTES, &maps.b_hi, full + s, k, c0);
-                tma_load_2d(st + 3 * TILE_BYTES, &maps.b_lo, full + s, k, c0);
+            int it = 0;                                                    // k-blocks issued so far (all tiles)
+            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+                int r0, c0, kb0, nkb, bt;
+                tile_of(t, r0, c0, kb0, nkb, bt);
+                for (int i = 0; i < nkb; ++i, ++it) {
+                    const int s = it % STAGES;
+                    if (it >= STAGES) mbar_wait(empty + s, ((it / STAGES) - 1) & 1);
+                    unsigned char* st = tiles + (size_t)s * STAGE_BYTES;
+                    mbar_expect_tx(full + s, STAGE_BYTES);
+                    const int k = (kb0 + i) * BK;
+                    tma_load_3d(st, &maps.a_hi, full + s, k, bt, r0);
+                    tma_load_3d(st + TILE_BYTES, &maps.a_lo, full + s, k, bt, r0);
+                    tma_load_3d(st + 2 * TILE_BYTES, &maps.b_hi, full + s, k, bt, c0);
+                    tma_load_3d(st + 3 * TILE_BYTES, &maps.b_lo, full + s, k, bt, c0);
+                }
             }
         }
     } else if (warp == 5) {
         // ===== MMA issuer =====
         if (lane == 0) {
-            for (int ch = 0; ch < n_chunks; ++ch) {
-                const int buf = ch & 1;
-                if (ch >= 2) mbar_wait(acc_empty + buf, ((ch >> 1) - 1) & 1);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t d = tmem + (uint32_t)(buf * BN);
-                const int i_end = min(nkb, (ch + 1) * CHUNK_KB);
-                for (int i = ch * CHUNK_KB; i < i_end; ++i) {
-                    const int s = i % STAGES;
-                    mbar_wait(full + s, (i / STAGES) & 1);
+            int it = 0, g = 0;                                             // k-blocks consumed, chunks started (all tiles)
+            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+                int r0, c0, kb0, nkb, bt;
+                tile_of(t, r0, c0, kb0, nkb, bt);
+                const int n_chunks = (nkb + CHUNK_KB - 1) / CHUNK_KB;
+                for (int ch = 0; ch < n_chunks; ++ch, ++g) {
+                    const int buf = g & 1;
+                    if (g >= 2) mbar_wait(acc_empty + buf, ((g >> 1) - 1) & 1);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t sa = smem_u32(tiles + (size_t)s * STAGE_BYTES);
-                    const uint64_t ah = umma_desc(sa), al = umma_desc(sa + TILE_BYTES), bh = umma_desc(sa + 2 * TILE_BYTES), bl = umma_desc(sa + 3 * TILE_BYTES);
+                    const uint32_t d = tmem + (uint32_t)(buf * BN);
+                    const int i_end = min(nkb, (ch + 1) * CHUNK_KB);
+                    for (int i = ch * CHUNK_KB; i < i_end; ++i, ++it) {
+                        const int s = it % STAGES;
+                        mbar_wait(full + s, (it / STAGES) & 1);
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        const uint32_t sa = smem_u32(tiles + (size_t)s * STAGE_BYTES);
+                        const uint64_t ah = umma_desc(sa), al = umma_desc(sa + TILE_BYTES), bh = umma_desc(sa + 2 * TILE_BYTES), bl = umma_desc(sa + 3 * TILE_BYTES);
 #pragma unroll
-                    for (int kk = 0; kk < BK / 8; ++kk) {
-                        const uint64_t o = (uint64_t)(kk * 2);              // 8 fp32 = 32 bytes = 2 sixteen-byte units along k
-                        const uint32_t first = (i == ch * CHUNK_KB && kk == 0) ? 0u : 1u;
-                        umma_tf32(d, al + o, bh + o, first);               // small terms first
-                        umma_tf32(d, ah + o, bl + o, 1u);
-                        umma_tf32(d, ah + o, bh + o, 1u);
+                        for (int kk = 0; kk < BK / 8; ++kk) {
+                            const uint64_t o = (uint64_t)(kk * 2);          // 8 fp32 = 32 bytes = 2 sixteen-byte units along k
+                            const uint32_t first = (i == ch * CHUNK_KB && kk == 0) ? 0u : 1u;
+                            umma_tf32(d, al + o, bh + o, first);           // small terms first
+                            umma_tf32(d, ah + o, bl + o, 1u);
+                            umma_tf32(d, ah + o, bh + o, 1u);
+                        }
+                        umma_commit(empty + s);                            // frees the stage when these MMAs have read it
                     }
-                    umma_commit(empty + s);                                // frees the stage when these MMAs have read it
+                    umma_commit(acc_full + buf);                           // chunk accumulator complete
                 }
-                umma_commit(acc_full + buf);                               // chunk accumulator complete
             }
         }
     } else {
         // ===== epilogue warps 0-3: TMEM lane quarter `warp`, row r = r0 + 32 warp + lane =====
-        float acc[BN];
+        int g = 0;
+        for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+            int r0, c0, kb0, nkb, bt;
+            tile_of(t, r0, c0, kb0, nkb, bt);
+            const int n_chunks = (nkb + CHUNK_KB - 1) / CHUNK_KB;
+            float acc[BN];
 #pragma unroll
-        for (int j = 0; j < BN; ++j) acc[j] = 0.f;
-        for (int ch = 0; ch < n_chunks; ++ch) {
-            const int buf = ch & 1;
-            mbar_wait(acc_full + buf, (ch >> 1) & 1);
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            for (int j = 0; j < BN; ++j) acc[j] = 0.f;
+            for (int ch = 0; ch < n_chunks; ++ch, ++g) {
+                const int buf = g & 1;
+                mbar_wait(acc_full + buf, (g >> 1) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-            for (int q = 0; q < BN / 32; ++q) {
-                uint32_t v[32];
-                tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * BN + q * 32), v);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                for (int q = 0; q < BN / 32; ++q) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * BN + q * 32), v);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-                for (int j = 0; j < 32; ++j) acc[q * 32 + j] += __uint_as_float(v[j]);
+                    for (int j = 0; j < 32; ++j) acc[q * 32 + j] += __uint_as_float(v[j]);
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(acc_empty + buf);
             }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(acc_empty + buf);
-        }
-        const int r = r0 + warp * 32 + lane;
-        if (r < rows_a) {
-            if (ATOMIC) {
+            const int r = r0 + warp * 32 + lane;
+            double* outb = out + (long long)bt * tg.out_batch_stride;
+            if (r < rows_a && n_chunks > 0) {
+                if (ATOMIC) {
 #pragma unroll
-                for (int j = 0; j < BN; ++j)
-                    if (c0 + j < rows_b) atomicAdd(out + (long long)(c0 + j) * ldo + r, (double)acc[j]);
-            } else {
-                // read-modify-write in groups of 16 columns: all loads of a group are in flight before the first add (one memory latency per
-                // group instead of one per element)
+                    for (int j = 0; j < BN; ++j)
+                        if (c0 + j < rows_b) atomicAdd(outb + (long long)(c0 + j) * ldo + r, (double)acc[j]);
+                } else {
+                    // read-modify-write in groups of 16 columns: all loads of a group are in flight before the first add (one memory
+                    // latency per group instead of one per element)
 #pragma unroll
-                for (int q = 0; q < BN / 16; ++q) {
-                    double old[16];
+                    for (int q = 0; q < BN / 16; ++q) {
+                        double old[16];
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const int cc = c0 + q * 16 + j;
-                        old[j] = cc < rows_b ? __ldcg(out + (long long)cc * ldo + r) : 0.0;
-                    }
+                        for (int j = 0; j < 16; ++j) {
+                            const int cc = c0 + q * 16 + j;
+                            old[j] = cc < rows_b ? __ldcg(outb + (long long)cc * ldo + r) : 0.0;
+                        }
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const int cc = c0 + q * 16 + j;
-                        if (cc < rows_b) __stcg(out + (long long)cc * ldo + r, old[j] + (double)acc[q * 16 + j]);
+                        for (int j = 0; j < 16; ++j) {
+                            const int cc = c0 + q * 16 + j;
+                            if (cc < rows_b) __stcg(outb + (long long)cc * ldo + r, old[j] + (double)acc[q * 16 + j]);
+                        }
                     }
                 }
             }

@@ -462,14 +462,16 @@ size_t tc_hot_bytes(const west_ctx* c, int rows, long long n_vec) {       // Xsp
     const long long Kp = pad4(2 * c->hs.n_g), rp = pad4(rows);
     return al256(sizeof(float) * 2 * (size_t)n_vec * Kp) + al256(sizeof(float) * 2 * (size_t)n_vec * rp);
 }
-int tc_map(west_ctx* c, CUtensorMap* m, const float* p, long long rows, long long cols, long long ld) {
-    cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-    cuuint64_t gstr[1] = {(cuuint64_t)ld * sizeof(float)};
-    cuuint32_t box[2] = {(cuuint32_t)wtc::BK, (cuuint32_t)wtc::BM}, es[2] = {1, 1};
+// (k, batch, row) tensor map: element (k, b, r) at p[r * ld + b * ldb + k]; box {BK, 1, 128}, 128-byte swizzle, zero fill out of bounds
+int tc_map(west_ctx* c, CUtensorMap* m, const float* p, long long rows, long long cols, long long ld, long long n_batch = 1, long long ldb = 0) {
+    if (n_batch == 1) ldb = rows * ld;
+    cuuint64_t gdim[3] = {(cuuint64_t)cols, (cuuint64_t)n_batch, (cuuint64_t)rows};
+    cuuint64_t gstr[2] = {(cuuint64_t)ldb * sizeof(float), (cuuint64_t)ld * sizeof(float)};
+    cuuint32_t box[3] = {(cuuint32_t)wtc::BK, 1, (cuuint32_t)wtc::BM}, es[3] = {1, 1, 1};
     const CUresult r = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(c->tm_encode)(
-        m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)p, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+        m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)p, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(c, WEST_ECUDA, "cuTensorMapEncodeTiled failed (%d) for a %lld x %lld map", (int)r, rows, cols);
+    if (r != CUDA_SUCCESS) return fail(c, WEST_ECUDA, "cuTensorMapEncodeTiled failed (%d) for a %lld x %lld x %lld map", (int)r, rows, n_batch, cols);
     return WEST_OK;
 }
 // operator data of the tensor path: (re)split the stacked operator matrix after a west_set_* change (not a hot-arena buffer)
@@ -529,7 +531,9 @@ int lowrank_apply_tc(west_ctx* c, int nr, int n_vec, const double* X, double* Y,
         int splits = (int)std::max<long long>(1, std::min<long long>(n_kb / 16, (148 * 2 + tiles - 1) / tiles));
         int kps = (n_kb + splits - 1) / splits;
         splits = (n_kb + kps - 1) / kps;
-        wtc::tf32x3_gemm<true><<<dim3((nr + 127) / 128, (n_vec + 127) / 128, splits), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m1, nr, n_vec, n_kb, kps, Ct, rp);
+        const wtc::TileGrid tg{(nr + 127) / 128, (n_vec + 127) / 128, splits, 1, 0};
+        const long long nt = (long long)tg.tiles_a * tg.tiles_b * tg.splits;
+        wtc::tf32x3_gemm<true><<<(unsigned)std::min<long long>(nt, 148), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m1, tg, nr, n_vec, n_kb, kps, Ct, rp);
         CK(cudaGetLastError());
         c->launches += 2;
     }
@@ -540,7 +544,9 @@ int lowrank_apply_tc(west_ctx* c, int nr, int n_vec, const double* X, double* Y,
     {
         Prof p_(c, PC_GEMM_UP);
         const int n_kb = (nr + wtc::BK - 1) / wtc::BK;
-        wtc::tf32x3_gemm<false><<<dim3((unsigned)((K + 127) / 128), (n_vec + 127) / 128, 1), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m2, (int)K, n_vec, n_kb, n_kb, Y, K);
+        const wtc::TileGrid tg{(int)((K + 127) / 128), (n_vec + 127) / 128, 1, 1, 0};
+        const long long nt = (long long)tg.tiles_a * tg.tiles_b;
+        wtc::tf32x3_gemm<false><<<(unsigned)std::min<long long>(nt, 148), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m2, tg, (int)K, n_vec, n_kb, n_kb, Y, K);
         CK(cudaGetLastError());
         c->launches += 1;
     }
@@ -604,6 +610,7 @@ size_t plan_lanczos(const west_ctx* c, int n_pert, int n_steps, int f32) {
                al256(bytes_W(c, std::max(slots_h, slots_r), 0)) + al256(256);
     if (c->rows_kb > 0) t += al256(bytes_C(c->rows_kb, (long long)n_col)) + (f32 ? tc_hot_bytes(c, c->rows_kb, (long long)n_col) : 0);
     if (c->n_occ_user != c->n_occ) t += al256(sizeof(double) * n_col * (2 * (size_t)n_steps + 1));
+    if (f32 && tc_available(c)) t += al256(sizeof(float) * 4 * n_col * (size_t)pad4(2 * c->hs.n_g));      // TF32 splits of q^1 and q^l (brakets)
     return t;
 }
 size_t plan_happly(const west_ctx* c, long long n_vec, int f32) {
@@ -1778,6 +1785,17 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
     c->launches += 1;
     if (braket_opt) CK(cudaMemsetAsync(braket_opt, 0, sizeof(double) * (size_t)n_user * n_steps * n_pert * n_pert, c->st));
     const int f32 = precision == WEST_MIXED;
+    const long long Kp = pad4(K);
+    const bool tc_brakets = braket_opt && f32 && tc_available(c);
+    float* Qs = nullptr; float* Q1s = nullptr;
+    if (tc_brakets) {
+        CK(tc_attrs());
+        if ((rc = hot(c, c->xs, sizeof(float) * 4 * (size_t)n_col * Kp))) return rc;
+        Qs = (float*)c->xs.p; Q1s = Qs + 2 * (size_t)n_col * Kp;
+        wtc::split_rows<<<blocks_for((long long)n_col * Kp, 256), 256, 0, c->st>>>(n_col, K, (const double*)Q1, K, Q1s, Q1s + (size_t)n_col * Kp, Kp);
+        CK(cudaGetLastError());
+        c->launches += 1;
+    }
     VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_col, 0};
     const int n_slots = gamma ? (n_col + 1) / 2 : n_col;
     for (int l = 0; l < n_steps; ++l) {
@@ -1785,8 +1803,26 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
             // <q^1_{n i} | q^l_{m i}> for every orbital i: n_occ Gram blocks, rows of one block n_occ vectors apart (Fig. 4)
             double* C = braket_opt + (size_t)l * n_pert * n_pert;
             const long long sC = (long long)n_steps * n_pert * n_pert;
-            if ((rc = launch_gemm_tn(c, n_pert, n_pert, K, (const double*)Q1, (long long)n_occ * K, (const double*)Q, (long long)n_occ * K, C,
-                                     n_pert, n_user, K, K, sC, false)))
+            if (tc_brakets) {
+                // WEST_MIXED: FP32 operands (the FP32 payload of Fig. 5c, as an FP32-operand product): q^l is split into
+                // TF32 hi / lo like q^1 and the n_occ blocks run as ONE batched tcgen05 launch (batch entry = orbital, tc_gemm.cuh)
+                Prof p_(c, PC_GEMM_TN);
+                wtc::split_rows<<<blocks_for((long long)n_col * Kp, 256), 256, 0, c->st>>>(n_col, K, (const double*)Q, K, Qs, Qs + (size_t)n_col * Kp, Kp);
+                wtc::Maps m;
+                if ((rc = tc_map(c, &m.a_hi, Qs, n_pert, K, (long long)n_occ * Kp, n_user, Kp)) ||
+                    (rc = tc_map(c, &m.a_lo, Qs + (size_t)n_col * Kp, n_pert, K, (long long)n_occ * Kp, n_user, Kp)) ||
+                    (rc = tc_map(c, &m.b_hi, Q1s, n_pert, K, (long long)n_occ * Kp, n_user, Kp)) ||
+                    (rc = tc_map(c, &m.b_lo, Q1s + (size_t)n_col * Kp, n_pert, K, (long long)n_occ * Kp, n_user, Kp)))
+                    return rc;
+                const int n_kb = (int)((K + wtc::BK - 1) / wtc::BK), tp = (n_pert + 127) / 128;
+                const wtc::TileGrid tg{tp, tp, 1, n_user, sC};
+                const long long nt = (long long)tp * tp * n_user;
+                // out[c * ldo + r]: r = row of the A operand (q^l_m), c = row of the B operand (q^1_n)  ->  C[i][n][m]
+                wtc::tf32x3_gemm<false><<<(unsigned)std::min<long long>(nt, 148), wtc::NTHREADS, wtc::SMEM_BYTES, c->st>>>(m, tg, n_pert, n_pert, n_kb, n_kb, C, n_pert);
+                CK(cudaGetLastError());
+                c->launches += 2;
+            } else if ((rc = launch_gemm_tn(c, n_pert, n_pert, K, (const double*)Q1, (long long)n_occ * K, (const double*)Q, (long long)n_occ * K, C,
+                                            n_pert, n_user, K, K, sC, false)))
                 return rc;
             wlz::braket_fix<<<blocks_for((long long)n_user * n_pert * n_pert, 256), 256, 0, c->st>>>(n_user, n_pert, sC, C, (const double*)Q1,
                                                                                                   (const double*)Q, (long long)n_occ * K, K);

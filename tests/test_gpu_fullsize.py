@@ -171,3 +171,30 @@ def test_cfg2_block_cg_sampled_columns(states):
     _, _, st2 = w.chi0_apply(dV, [0.0], tol=1e-8, max_iter=300, alpha_pv=0.0, check_every=1, solver=2)
     _, _, st0 = w.chi0_apply(dV, [0.0], tol=1e-8, max_iter=300, alpha_pv=0.0, check_every=1, solver=0)
     assert st2["rc"] == 0 and st0["rc"] == 0 and st2["n_h_apply"] < 0.9 * st0["n_h_apply"]
+
+
+def test_pdep_shell_at_cfg2_size(states):
+    """SURVEY 8(f)-3 at config-2 size: the Davidson shell's Ritz values do not move when the inner CG tolerance is
+    tightened, and the eigen-residual || chi0bar u - lambda u || of one eigenpotential is recomputed with the ORACLE's pieces: the
+    perturbation v^1/2 u built by the oracle's transforms, Eq. 11 evaluated by oracle.chi0.dn_from_dpsi on the GPU's dpsi."""
+    import torch
+    from paper_2203_05623_b200 import pdep as gp
+    from oracle import pdep as opd
+    p, eps, U, alpha, w, dev = (states[k] for k in ("p", "eps", "U", "alpha", "w", "dev"))
+    n_pdep = 8
+    lam1, C1, res1, n1 = gp.pdep(w, n_pdep, p.n_occ, alpha, tol=1e-5, tol_cg=1e-8)
+    lam2, C2, res2, n2 = gp.pdep(w, n_pdep, p.n_occ, alpha, tol=1e-5, tol_cg=1e-11)
+    assert np.max(res1) < 1e-5 and np.max(res2) < 1e-5 and np.all(lam2 < 0)
+    assert np.max(np.abs(lam1 - lam2)) < 1e-6 * abs(lam2[0])
+    u = C2[0].cpu().numpy()                                               # half-sphere coefficients, c(0) = 0, unit norm
+    assert abs(np.linalg.norm(opd.y_from_coeffs(u)) - 1.0) < 1e-10
+    sv = opd.sqrt_coulomb(p.miller, p.L)
+    dV = oham.to_real_space(ogs.expand_half_to_full((u * sv)[None], p.miller), p.fft_idx, p.N)[0]
+    assert np.max(np.abs(dV.imag)) < 1e-10 * np.max(np.abs(dV.real))
+    _, dpsi, st = w.chi0_apply(torch.from_numpy(np.ascontiguousarray(dV.real[None])).to(dev), [0.0], tol=1e-11, max_iter=500, alpha_pv=alpha,
+                               want_dpsi=True)
+    assert st["rc"] == 0
+    dn = ochi0.dn_from_dpsi(U, _full(p, dpsi[0, 0, :, 0].cpu().numpy()), p.miller, p.L, p.N)
+    out = oham.to_g_space(dn[None], p.fft_idx)[0][p.half] * sv
+    r = opd.y_from_coeffs(out) - lam2[0] * opd.y_from_coeffs(u)
+    assert np.linalg.norm(r) < 5e-5 * max(1.0, abs(lam2[0]))

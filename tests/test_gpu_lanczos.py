@@ -143,3 +143,26 @@ def test_tridiagonal_eigensolver_on_real_chains_and_errors():
     d0, U0 = w.lanczos_diag(torch.zeros((0, 30), dtype=torch.float64, device="cuda"), torch.zeros((0, 30), dtype=torch.float64, device="cuda"))
     assert d0.shape == (0, 30) and U0.shape == (0, 30, 30)
     w.close()
+
+
+def test_lanczos_fp32_operand_brakets():
+    """WEST_MIXED: the braket Gram blocks of Eq. 19 / Fig. 4 with FP32 (TF32 hi + lo) operands on the tcgen05 path - the FP32 payload of
+    Fig. 5c as an operand format.  FP32-class agreement with the oracle's FP64 brakets; the chains themselves run the
+    mixed H*psi and agree to its tolerance."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build("mini2")
+    w, sel = make_west(p)
+    n_pert, n_steps = 5, 12
+    phi = np.ascontiguousarray(p.dV[:n_pert])
+    a, b, nrm, br = w.lanczos(torch.from_numpy(phi).cuda(), n_steps, p.n_occ, want_brakets=True, precision=wb.WEST_MIXED)
+    a64, b64, _, br64 = w.lanczos(torch.from_numpy(phi).cuda(), n_steps, p.n_occ, want_brakets=True)
+    q1, _ = olz.start_vectors(p.U[:, :p.n_occ], phi, p.fft_idx, p.N)
+    ar, brf, brak = olz.chains_with_brakets(lambda y: p.H @ y, q1, n_steps)
+    got = br.cpu().numpy()
+    assert np.max(np.abs(br64.cpu().numpy() - brak.real)) < 1e-9
+    # step 0 is the Gram matrix of the start vectors: pure operand-format error (no mixed H*psi yet)
+    assert 1e-12 < np.max(np.abs(got[:, 0] - brak.real[:, 0])) < 5e-6
+    assert np.max(np.abs(got - brak.real)) < 1e-4
+    assert relmax(a.cpu().numpy(), ar) < 1e-4
+    w.close()
