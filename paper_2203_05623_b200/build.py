@@ -21,9 +21,9 @@ LIB = os.path.join(HERE, "libwest.so")
 # ZMINB = resident CTAs per SM the z-stick kernels are compiled for
 # ZNT = threads per CTA of the z-stick kernels (2 * CU * max(N1, N2) <= ZNT)
 FFT_SIZES = [(4, 6, 24, 4, 4, 20, 4, 256), (6, 6, 36, 4, 4, 20, 4, 256), (6, 8, 48, 6, 3, 16, 4, 256), (8, 9, 72, 12, 2, 14, 4, 256),
-             (12, 12, 144, 16, 1, 10, 2, 256)]
+             (12, 12, 144, 12, 1, 10, 2, 256)]
 K2H_SHAPES = {72: tuple(int(x) for x in os.environ.get("WEST_K2H_72", "6,3,2,1").split(",")),
-              144: tuple(int(x) for x in os.environ.get("WEST_K2H_144", "16,1,1,1").split(","))}
+              144: tuple(int(x) for x in os.environ.get("WEST_K2H_144", "12,1,1,1").split(","))}
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 

@@ -290,7 +290,14 @@ struct K2Args {
 // thread instead of one; the round then covers NB * LC lines).  NB = 1 is the plain one-item-per-thread pass.
 template <typename T, int N1, int N2, int MODE, int LC>
 struct K2 {
-    static constexpr int N = N1 * N2, PITCH = N + WEST_PAD;
+    // Shared-memory line layout.  Position p = N2 k1 + k2 of a line sits at element B2 k1 + k2: when N2 is even the N2-blocks are padded
+    // by one element (B2 = N2 + 1), because the contiguous passes put the lanes of a warp B2 elements apart and an even stride maps
+    // them onto half (N2 = 12: a quarter) of the eight 16-byte bank groups (measured at N = 144: 57 % of the shared-memory wavefronts
+    // were conflict replays).  The row pitch is the smallest value >= the line length that is congruent to N2 modulo 8, so that the
+    // strided passes (lanes = (line, n2), consecutive) stay conflict-free as well.
+    static constexpr int N = N1 * N2, B2 = N2 + ((N2 % 2 == 0) ? 1 : 0), NP = N1 * B2;
+    static constexpr int PITCH = NP + ((N2 - NP) % 8 + 8) % 8 + ((NP + ((N2 - NP) % 8 + 8) % 8 == N) ? 8 : 0);
+    static WHD int pos(int p) { return (N2 % 2 == 0) ? p + p / N2 : p; }          // padded element index of position p
     static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + 2 * N); }
 
     // layout of V_loc for the K2_H variant: position (pz, py = py0 + l, px = N2 k1 + k2), py0 a multiple of LC
@@ -310,7 +317,7 @@ struct K2 {
         cx<T> zp[N1];
         tw_powers<T, N1>(z, zp);
 #pragma unroll
-        for (int k1 = 0; k1 < N1; ++k1) dst[N2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
+        for (int k1 = 0; k1 < N1; ++k1) dst[B2 * k1] = k1 == 0 ? v[0] : cmul(v[k1], zp[k1]);
     }
     // contiguous-pass epilogue of the forward direction: v[j] * conj(w^(k1 j)) -> p[j]
     static WHD void tw_store_contig(cx<T> (&v)[N2], cx<T> z, cx<T>* p) {
@@ -352,7 +359,7 @@ struct K2 {
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const bool ok = NB == 1 || it < nrow * N1;            // (the loop bound covers b = 0)
-                const cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
+                const cx<T>* p = S + (row0 + it / N1) * PITCH + B2 * (it % N1);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) v[b][j] = ok ? p[j] : mk<T>(0, 0);
             }
@@ -362,7 +369,7 @@ struct K2 {
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 if (NB > 1 && it >= nrow * N1) continue;
-                cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
+                cx<T>* p = S + (row0 + it / N1) * PITCH + B2 * (it % N1);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) p[j] = v[b][j];
             }
@@ -382,7 +389,7 @@ struct K2 {
 #pragma unroll
                 for (int n1 = 0; n1 < N1; ++n1) {
                     const int nx = wrap_signed(N2 * n1 + n2, N);
-                    v[b][n1] = (ok && keep_n1<N1, N2>(n1) && nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + py] : mk<T>(0, 0);
+                    v[b][n1] = (ok && keep_n1<N1, N2>(n1) && nx <= g.n_max && nx >= -g.n_max) ? S[(nx + g.n_max) * PITCH + pos(py)] : mk<T>(0, 0);
                 }
             }
 #pragma unroll
@@ -456,7 +463,7 @@ struct K2 {
                 const int l = it / N1, k1 = it - l * N1;
                 ok[b] = NB == 1 || (it < LC * N1 && py0 + l < N);
                 if (MODE != K2_FROMR) {
-                    const cx<T>* p = X + l * PITCH + N2 * k1;
+                    const cx<T>* p = X + l * PITCH + B2 * k1;
 #pragma unroll
                     for (int j = 0; j < N2; ++j) v[b][j] = ok[b] ? p[j] : mk<T>(0, 0);
                 }
@@ -477,7 +484,7 @@ struct K2 {
                 for (int b = 0; b < NB; ++b) {
                     const int it = it0 + b * nthr;
                     const int l = it / N1, k1 = it - l * N1;
-                    if (fwd[b]) tw_store_contig(v[b], tw[N + N1 + k1], X + l * PITCH + N2 * k1);
+                    if (fwd[b]) tw_store_contig(v[b], tw[N + N1 + k1], X + l * PITCH + B2 * k1);
                 }
             }
         }
@@ -495,7 +502,7 @@ struct K2 {
                 const bool ok = NB == 1 || (it < LC * N2 && py0 + l < N);
                 const cx<T>* p = X + l * PITCH + n2;
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[N2 * k1] : mk<T>(0, 0);
+                for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[B2 * k1] : mk<T>(0, 0);
             }
 #pragma unroll
             for (int b = 0; b < NB; ++b) Dft<T, N1, -1>::run(v[b]);
@@ -508,7 +515,7 @@ struct K2 {
                 for (int n1 = 0; n1 < N1; ++n1) {
                     if (!keep_n1<N1, N2>(n1)) continue;
                     const int nx = wrap_signed(N2 * n1 + n2, N);
-                    if (nx <= g.n_max && nx >= -g.n_max) S[(nx + g.n_max) * PITCH + py] = v[b][n1];
+                    if (nx <= g.n_max && nx >= -g.n_max) S[(nx + g.n_max) * PITCH + pos(py)] = v[b][n1];
                 }
             }
         }
@@ -521,7 +528,7 @@ struct K2 {
             for (int b = 0; b < NB; ++b) {
                 const int it = it0 + b * nthr;
                 const bool ok = NB == 1 || it < nrow * N1;            // (the loop bound covers b = 0)
-                const cx<T>* p = S + (row0 + it / N1) * PITCH + N2 * (it % N1);
+                const cx<T>* p = S + (row0 + it / N1) * PITCH + B2 * (it % N1);
 #pragma unroll
                 for (int j = 0; j < N2; ++j) v[b][j] = ok ? p[j] : mk<T>(0, 0);
             }
@@ -532,7 +539,7 @@ struct K2 {
                 const int it = it0 + b * nthr;
                 if (NB > 1 && it >= nrow * N1) continue;
                 const int k1 = it % N1;
-                tw_store_contig(v[b], tw[N + N1 + k1], S + (row0 + it / N1) * PITCH + N2 * k1);
+                tw_store_contig(v[b], tw[N + N1 + k1], S + (row0 + it / N1) * PITCH + B2 * k1);
             }
         }
     }
@@ -546,7 +553,7 @@ struct K2 {
                 const bool ok = NB == 1 || it < nrow * N2;
                 const cx<T>* p = S + (row0 + it / N2) * PITCH + it % N2;
 #pragma unroll
-                for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[N2 * k1] : mk<T>(0, 0);
+                for (int k1 = 0; k1 < N1; ++k1) v[b][k1] = ok ? p[B2 * k1] : mk<T>(0, 0);
             }
 #pragma unroll
             for (int b = 0; b < NB; ++b) Dft<T, N1, -1>::run(v[b]);

@@ -100,7 +100,9 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_tn_kernel(int M, int Nn, 
     double* Bs = smem + (size_t)STAGES * BM * PITCH_TN;  // [STAGES][BN][PITCH_TN]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp / WN, wn = warp % WN;            // 2 x WN warps
-    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+    // row tiles of A (m) are the FASTEST grid axis: the CTAs that share one (vector tile, K split) panel of B run together, so B streams
+    // from HBM once and the other row tiles hit L2 (with the vector tiles fastest every row tile re-streamed B: 24x at the cfg-5 shape)
+    const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
     // blockIdx.z = batch * splits + split; the batch strides shift all three matrices
     const int batch = blockIdx.z / splits;
     A += (long long)batch * sA; B += (long long)batch * sB; C += (long long)batch * sC;
@@ -230,8 +232,18 @@ __global__ void __launch_bounds__(NTHREADS, MINB) gemm_update_kernel(int M, int 
     double* As = smem + (size_t)STAGES * BK * PITCH_UPC;      // [STAGES][BK][PITCH_UPA]  (m, k)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp / WN, wn = warp % WN;
-    const int n0 = blockIdx.y * BM;
-    const long long k0 = (long long)blockIdx.x * BN;
+    // Grouped tile order: consecutive CTAs sweep GN vector tiles of the SAME k tile before moving to the next k tile, so one wave works
+    // on GN coefficient panels (C, rows x 128 vectors) and ~30 operator panels (A, rows x 64 reals) that fit the L2 together.  In plain
+    // (k fastest) order every vector tile re-streamed the whole operator matrix from HBM (ncu at the cfg-5 shape: 481 GB read for 42 GB
+    // of algorithmic traffic).
+    constexpr int GN = 16;
+    const long long id = blockIdx.x + (long long)gridDim.x * blockIdx.y;
+    const long long per_group = (long long)GN * gridDim.x;
+    const int grp = (int)(id / per_group);
+    const int gsz = min(GN, (int)gridDim.y - grp * GN);
+    const long long in_g = id - grp * per_group;
+    const int n0 = (grp * GN + (int)(in_g % gsz)) * BM;
+    const long long k0 = (in_g / gsz) * BN;
     const int nm = (M + BK - 1) / BK;
 
     constexpr int NA = TF32 ? 1 : 8;

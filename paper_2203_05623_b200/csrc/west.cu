@@ -405,7 +405,7 @@ int launch_gemm_tn(west_ctx* c, int M, int Nn, long long K, const double* A, lon
     kps = (kps + BK - 1) / BK * BK;
     splits = (K + kps - 1) / kps;
     if (zero_c) CK(cudaMemsetAsync(C, 0, (size_t)M * ldc * sizeof(double), c->st));     // batched callers zero their own output
-    dim3 grid(tn, tm, (unsigned)(splits * n_batch));
+    dim3 grid(tm, tn, (unsigned)(splits * n_batch));        // row tiles fastest (gemm_f64.cuh)
     Prof prof_(c, PC_GEMM_TN);
     if (tf32) gemm_tn_kernel<true><<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1, (int)splits, sA, sB, sC);
     else gemm_tn_kernel<false><<<grid, NTHREADS, SMEM_TN, c->st>>>(M, Nn, K, A, lda, B, ldb, C, ldc, kps, 1, (int)splits, sA, sB, sC);
