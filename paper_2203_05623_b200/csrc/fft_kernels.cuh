@@ -296,7 +296,9 @@ struct K2 {
     // were conflict replays).  The row pitch is the smallest value >= the line length that is congruent to N2 modulo 8, so that the
     // strided passes (lanes = (line, n2), consecutive) stay conflict-free as well.
     static constexpr int N = N1 * N2, B2 = N2 + ((N2 % 2 == 0) ? 1 : 0), NP = N1 * B2;
-    static constexpr int PITCH = NP + ((N2 - NP) % 8 + 8) % 8 + ((NP + ((N2 - NP) % 8 + 8) % 8 == N) ? 8 : 0);
+    // even N2: the row pitch is made ODD as well - the x passes gather / scatter one element per row of S (lanes = consecutive n_x rows)
+    // and an even pitch folds those onto fewer bank groups (pitch 156 at N = 144 still showed 24 % replays)
+    static constexpr int PITCH = (N2 % 2 == 0) ? (NP | 1) : NP + ((N2 - NP) % 8 + 8) % 8 + ((NP + ((N2 - NP) % 8 + 8) % 8 == N) ? 8 : 0);
     static WHD int pos(int p) { return (N2 % 2 == 0) ? p + p / N2 : p; }          // padded element index of position p
     static WHD size_t smem_bytes(int nr) { return sizeof(cx<T>) * (size_t)((nr + LC) * PITCH + 2 * N); }
 
