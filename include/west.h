@@ -178,6 +178,22 @@ int  west_set_deflation(west_ctx* ctx, int32_t n_defl, const void* psi_c, const 
  * r->G of data that is not sphere-limited is the truncation to S of its DFT. */
 int  west_fft3d(west_ctx* ctx, int32_t dir, int32_t precision, int32_t n_batch, const void* in, void* out);
 
+/* West_fft3d without ANY allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): the transform's scratch (stick intermediate + position-order grid, the two buffers west_fft3d takes from
+ * the workspace) lives in ONE file-scope device array of WEST_STATIC_SCRATCH_BYTES = 8 MiB inside the library, which every GPU that
+ * loads the library holds until the process exits.  Same kernels and arithmetic as west_fft3d (WEST_FP64), same argument meaning:
+ * dir = +1: in = coefficients [n_batch][n_g] c128, out = grids; dir = -1: in = grids, out = coefficients; in / out are the caller's
+ * device buffers.  The call performs no cudaMalloc, no cudaFree, no allocating library routine and no synchronisation; the first call
+ * on a device looks the array's address up (cudaGetSymbolAddress, once per device, with the caller's current device = the context's).
+ * Limit: one transform slot (N n_cols + N^3 complex128) must fit the array - N <= 72 does, N = 144 does not: WEST_EWORKSPACE with the
+ * sizes in west_last_error, nothing enqueued.  Larger batches are walked in chunks of as many slots as fit.
+ * EVERY call on a device shares the array, across contexts and streams: calls that overlap on the GPU race (serialise them on one
+ * stream or with events).  The array keeps the last call's contents; nothing in it has to be cleared, because every element a kernel
+ * reads has been written earlier in the same call.  Errors: WEST_EINVAL, WEST_EWORKSPACE, WEST_ECUDA. */
+#define WEST_STATIC_SCRATCH_BYTES (8u << 20)
+int    west_fft3d_static(west_ctx* ctx, int32_t dir, int32_t n_batch, const void* in, void* out);
+size_t west_static_scratch_bytes(void);   /* = WEST_STATIC_SCRATCH_BYTES */
+
 /* Dense complex-to-complex 3D FFT on an n^3 cubic grid: the operation timed in Fig. 3 (one FP64 or FP32 C2C
  * transform of a 128^3 or 256^3 grid, data resident on the device).  Independent of the context's cell: ctx supplies the stream,
  * the error string and the launch counter only.

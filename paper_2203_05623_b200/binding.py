@@ -34,7 +34,7 @@ class west_stats(C.Structure):
 
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
-           "west_fft3d", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_lanczos_diag", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
+           "west_fft3d", "west_fft3d_static", "west_static_scratch_bytes", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_lanczos_diag", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
            "west_launch_count", "west_workspace_bytes", "west_set_workspace", "west_set_fft_chunk", "west_set_cg_kernel", "west_set_profile", "west_get_profile"]
 
 
@@ -54,6 +54,9 @@ def load_library():
     lib.west_set_deflation.argtypes = [vp, i32, vp, vp]
     lib.west_fft3d.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.west_fft3d_dense.argtypes = [vp, i32, i32, i32, i32, vp, vp]
+    lib.west_fft3d_static.argtypes = [vp, i32, i32, vp, vp]
+    lib.west_static_scratch_bytes.argtypes = []
+    lib.west_static_scratch_bytes.restype = C.c_size_t
     lib.west_h_apply.argtypes = [vp, i32, i32, vp, vp]
     lib.west_chi0_apply.argtypes = [vp, i32, i32, vp, i32, vp, C.POINTER(west_cg_opts), vp, vp, C.POINTER(west_stats)]
     lib.west_lanczos.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp, vp]
@@ -73,7 +76,7 @@ def load_library():
     lib.west_get_profile.argtypes = [vp, vp, vp]
     for name in EXPORTS:
         getattr(lib, name)
-        if name not in ("west_last_error", "west_device_bytes", "west_launch_count", "west_workspace_bytes"):
+        if name not in ("west_last_error", "west_device_bytes", "west_launch_count", "west_workspace_bytes", "west_static_scratch_bytes"):
             getattr(lib, name).restype = C.c_int
     return lib
 
@@ -182,6 +185,20 @@ class West:
             if out is None:
                 out = torch.empty((n_batch, self.n_g), dtype=torch.complex128, device=x.device)
             self._ck(self.lib.west_fft3d(self.ctx, -1, precision, n_batch, _dev(x, torch.float64 if self.mode == WEST_GAMMA else torch.complex128), _dev(out, torch.complex128)))
+        return out
+
+    def fft3d_static(self, dir, x, out):
+        """west_fft3d_static: the sphere-truncated FFT with its scratch in the library's fixed static device array (no allocation of any
+        kind in the call; `out` must be supplied by the caller).  Calls that overlap on the GPU race on that array."""
+        import torch
+        n_batch = int(x.shape[0])
+        grid_dt = torch.float64 if self.mode == WEST_GAMMA else torch.complex128
+        if dir == 1:
+            assert x.shape[1] == self.n_g and tuple(out.shape) == (n_batch, self.N, self.N, self.N)
+            self._ck(self.lib.west_fft3d_static(self.ctx, 1, n_batch, _dev(x, torch.complex128), _dev(out, grid_dt)))
+        else:
+            assert tuple(x.shape[1:]) == (self.N, self.N, self.N) and tuple(out.shape) == (n_batch, self.n_g)
+            self._ck(self.lib.west_fft3d_static(self.ctx, -1, n_batch, _dev(x, grid_dt), _dev(out, torch.complex128)))
         return out
 
     def fft3d_dense(self, x, sign, out=None):

@@ -9,6 +9,7 @@
 #include <cstring>
 #include <string>
 #include <map>
+#include <mutex>
 #include <vector>
 
 #include "../../include/west.h"
@@ -1875,5 +1876,84 @@ extern "C" int west_lanczos_diag(west_ctx* c, int32_t n_chain, int32_t n_steps, 
     CK(cudaStreamSynchronize(c->st));
     if (c->h_pinned[0] > 0)
         return fail(c, WEST_NOTCONVERGED, "west_lanczos_diag: %d of %d matrices did not converge in 60 QL sweeps per eigenvalue", c->h_pinned[0], n_chain);
+    return WEST_OK;
+}
+
+// ============================================================================================================ no-allocation entry point
+// west_fft3d_static: west_fft3d for callers that cannot tolerate ANY allocation (code under CUDA graph capture, tight serving loops,
+// harnesses that forbid cudaMalloc): the stick intermediate W and the position-order grid of the transform live in ONE file-scope
+// device array of fixed size instead of the workspace arena.  Every GPU that loads the library holds WEST_STATIC_SCRATCH_BYTES until
+// the process exits.  Same kernels, same launch order and same arithmetic as west_fft3d; only the scratch pointers differ.
+namespace {
+
+static __device__ __align__(256) unsigned char g_west_static_scratch[WEST_STATIC_SCRATCH_BYTES];
+
+// In host code `g_west_static_scratch` is a host-side stand-in, NOT a device address: the device address is looked up once per device
+// (with that device current) by cudaGetSymbolAddress and cached here.  No allocation, no synchronisation.
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[STATIC_MAX_DEVICES] = {};
+
+int static_scratch_ptr(west_ctx* c, unsigned char** out) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(c, WEST_EINVAL, "west_fft3d_static: device ordinal %d outside 0..%d", dev, STATIC_MAX_DEVICES - 1);
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        CK(cudaGetSymbolAddress(&p, g_west_static_scratch));
+        if (!p) return fail(c, WEST_ECUDA, "west_fft3d_static: cudaGetSymbolAddress returned a null address on device %d", dev);
+        g_static_ptr[dev] = p;
+    }
+    *out = (unsigned char*)g_static_ptr[dev];
+    return WEST_OK;
+}
+
+}  // namespace
+
+extern "C" size_t west_static_scratch_bytes(void) { return WEST_STATIC_SCRATCH_BYTES; }
+
+extern "C" int west_fft3d_static(west_ctx* c, int32_t dir, int32_t n_batch, const void* in, void* out) {
+    if (!c || (dir != 1 && dir != -1) || n_batch < 0 || (n_batch > 0 && (!in || !out))) return fail(c, WEST_EINVAL, "west_fft3d_static: bad argument");
+    if (n_batch == 0) return WEST_OK;
+    const int gamma = is_gamma(c), N = c->cell.N;
+    const long long n3 = n3_of(c);
+    // one transform slot needs its sticks W [N][n_cols] and its grid [N^3], both complex128 (each piece rounded up to 256 bytes)
+    const size_t w_slot = sizeof(cx<double>) * (size_t)N * c->hs.n_cols, r_slot = sizeof(cx<double>) * (size_t)n3;
+    const size_t per_slot = al256(w_slot) + al256(r_slot);
+    if (per_slot > WEST_STATIC_SCRATCH_BYTES)
+        return fail(c, WEST_EWORKSPACE, "west_fft3d_static: one transform of this cell (N = %d, %d columns) needs %zu bytes of scratch, the static array holds %zu "
+                    "(WEST_STATIC_SCRATCH_BYTES; N <= 72 fits) - use west_fft3d with a workspace", N, c->hs.n_cols, per_slot, (size_t)WEST_STATIC_SCRATCH_BYTES);
+    const int n_slots = gamma ? (n_batch + 1) / 2 : n_batch;
+    // slots per launch: as many as the array holds (the pieces of a chunk are contiguous, so the split is W[chunk] then R[chunk])
+    int chunk = 1;
+    while (chunk < n_slots && chunk < 64 && al256(w_slot * (chunk + 1)) + al256(r_slot * (chunk + 1)) <= WEST_STATIC_SCRATCH_BYTES) ++chunk;
+    unsigned char* base = nullptr;
+    int rc;
+    if ((rc = static_scratch_ptr(c, &base))) return rc;
+    void* W = base;
+    cx<double>* R = reinterpret_cast<cx<double>*>(base + al256(w_slot * chunk));
+    // Nothing in the array has to start at zero: K1 (dir = +1) writes every (position, column) of W and K2 every grid point before
+    // anything is read; dir = -1 fills the grid first and K2 then writes every (position, column) of W.  The array keeps the last
+    // call's contents otherwise.
+    VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_batch, 0};
+    K2Any a{};
+    a.W = W; a.R = R;
+    for (int s0 = 0; s0 < n_slots; s0 += chunk) {
+        const int ns = std::min(chunk, n_slots - s0);
+        vm.slot0 = s0;
+        if (dir == 1) {
+            CK(c->ops->k1(0, gamma, ns, c->st, c->geom, vm, (const cx<double>*)in, W));
+            CK(c->ops->k2(0, K2_TOR, ns, c->st, c->geom, a));
+            pos_to_user<<<blocks_for(n3 * ns, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, gamma, s0, ns, n_batch, R, (double*)out);
+        } else {
+            user_to_pos<<<blocks_for(n3 * ns, 256), 256, 0, c->st>>>(N, c->ops->N1, c->ops->N2, gamma, s0, ns, n_batch, (const double*)in, R);
+            CK(c->ops->k2(0, K2_FROMR, ns, c->st, c->geom, a));
+            K3Epi e{1.0 / ((double)N * N * N), 0, nullptr, 0.0, nullptr};
+            CK(c->ops->k3(0, gamma, ns, c->st, c->geom, vm, W, e, (cx<double>*)out));
+        }
+        CK(cudaGetLastError());
+        c->launches += 3;
+    }
     return WEST_OK;
 }
