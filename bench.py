@@ -52,7 +52,7 @@ def parse():
     ap.add_argument("--check-every", type=int, default=1, help="CG convergence poll / compaction period")
     ap.add_argument("--precond", type=int, default=1, help="0 none, 1 R4 default, 2 Teter-Payne-Allan")
     ap.add_argument("--solver", type=int, default=-1, help="0 per-frequency PCG/COCG, 1 multi-shift CG, 2 block CG; -1 = 1 when more than one frequency, else 0")
-    ap.add_argument("--op", default="chi0", choices=["chi0", "happly", "gemm", "lanczos", "pdep", "fft", "spin"],
+    ap.add_argument("--op", default="chi0", choices=["chi0", "happly", "gemm", "lanczos", "pdep", "fft", "spin", "pipes"],
                     help="chi0 = the hot path (default); happly = west_h_apply alone (H*psi/s, kernel classes); gemm = the projector GEMM shapes "
                          "against cuBLAS; lanczos = Eq. 15-19 chains; pdep = Davidson shell for chi0bar; fft = the dense C2C FFT of Fig. 3 "
                          "(--workload fft128 | fft256, --precision); spin = N_spin = 2 chi0 (widening rows)")
@@ -63,6 +63,7 @@ def parse():
     ap.add_argument("--alpha-factor", type=float, default=0.0, help="alpha_pv = factor x (eps_Nv - eps_1), reading R3 (the result does not depend on it; "
                                                                          "must exceed 1); 0 = the library's per-orbital default alpha_v = (eps_v - eps_1) + W/2")
     ap.add_argument("--cg-kernel", type=int, default=0, help="west_set_cg_kernel: 0 automatic (column-resident where it fits), 1 streaming, 2 column split over a 2-CTA cluster")
+    ap.add_argument("--ms-history", type=int, default=0, help="west_set_ms_history: 0 automatic Krylov-history ring of the multi-shift solver, -1 per-shift recurrences, 2..128 fixed ring size")
     ap.add_argument("--workspace", type=int, default=1, help="1: the bench allocates west_workspace_bytes and hands it over (no allocation in the timed calls); 0: lazy context-owned block")
     return ap.parse_args()
 
@@ -339,7 +340,7 @@ def measure_fp64_peak():
     return _FP64_PEAK["v"]
 
 
-def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g, fp64_peak, shift_updates=0):
+def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g, fp64_peak, shift_updates=0, hist_passes=0):
     """Roofline entry for the kernel class that took the most time in the profiled step (DESIGN.md section 6 states the per-unit
     figures).  n_h = vectors pushed through H in that step."""
     N = cfg["N"]
@@ -398,8 +399,14 @@ def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g
         if solver == 1:
             # 8 passes for the seed recurrence (p, Ap | r, Ap -> r | r, p -> p) and 6 per live shift (p_s: two real vectors read and written, Re x_s
             # read and written); the library counts the (column, shift) updates it performed (west_stats.n_shift_updates)
-            per_col = (8 + 6.0 * shift_updates / max(n_h, 1)) * 16 * n_g
-            note = "multi-shift: 8 + 6 x (live shifts per column, measured: %.2f of %d) vector passes of 16 n_g bytes per column and iteration" % (shift_updates / max(n_h, 1), n_freq)
+            if hist_passes > 0:
+                # Krylov-history variant: 8 passes for the seed recurrence (p, Ap | r_k, Ap -> r_k+1 | r_k+1, p -> p) and the history contractions,
+                # whose column-vector passes the library counts (west_stats.n_hist_passes); both run in this kernel class
+                per_col = (8 + float(hist_passes) / max(n_h, 1)) * 16 * n_g
+                note = "multi-shift with Krylov history: 8 + %.2f (history contractions, counted by the library) vector passes of 16 n_g bytes per column and iteration" % (hist_passes / max(n_h, 1))
+            else:
+                per_col = (8 + 6.0 * shift_updates / max(n_h, 1)) * 16 * n_g
+                note = "multi-shift: 8 + 6 x (live shifts per column, measured: %.2f of %d) vector passes of 16 n_g bytes per column and iteration" % (shift_updates / max(n_h, 1), n_freq)
         else:
             per_col = 7 * 16 * n_g
             note = "7 vector passes of 16 n_g bytes per column and iteration"
@@ -430,6 +437,15 @@ def make_workspace(w, wb, op, n_pert, n_freq, precision, reserve_bytes):
     import torch
     free = torch.cuda.mem_get_info()[0] - reserve_bytes
     fit = n_pert
+    if op == wb.binding.WEST_OP_CHI0_MULTISHIFT:
+        # multi-shift solver: the library turns every byte beyond the minimum into ring slots of its Krylov history (west_set_ms_history),
+        # so hand it the full-history size if the device has it, else what is free
+        full = w.workspace_bytes(wb.binding.WEST_OP_CHI0_MULTISHIFT_HIST, n_pert, n_freq, precision)
+        need = min(full, free // 256 * 256)
+        if need >= w.workspace_bytes(op, 1, n_freq, precision):
+            ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+            w.set_workspace(ws)
+            return ws, n_pert
     for nb in range(1, n_pert + 1):
         fit = (n_pert + nb - 1) // nb
         need = w.workspace_bytes(op, fit, n_freq, precision)
@@ -456,8 +472,11 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
               precision=precision, dn=dn)
     ws = None
     if a.workspace:
+        # room left for the parity sample's dpsi block (parity_and_cpu: the whole block if it is below 40 GB, else one perturbation)
         dpsi_bytes = 16 * w.n_g * n_pert * cfg["n_occ"] * (2 if cfg["mode"] == "gamma" else 1) * n_freq
-        ws, fit = make_workspace(w, wb, chi0_op(wb, solver, omegas), n_pert, n_freq, precision, reserve_bytes=(3 << 30) + min(dpsi_bytes, 40 << 30))
+        if dpsi_bytes >= (40 << 30):
+            dpsi_bytes //= n_pert
+        ws, fit = make_workspace(w, wb, chi0_op(wb, solver, omegas), n_pert, n_freq, precision, reserve_bytes=(4 << 30) + min(dpsi_bytes, 40 << 30))
     stats = None
     for _ in range(warmup):
         _, _, stats = w.chi0_apply(dV, omegas, **kw)
@@ -523,13 +542,13 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
         "dtype": "f64" if not mixed else "f32 FFT + 3xTF32 GEMMs inside H*psi / f64 vectors, dots, dn",
         "config": {"workload": label, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": n_freq, "omega_ry": [round(x, 6) for x in omegas],
                    "n_proj": cfg["n_proj"], "n_deflated": a.deflate, "alpha_pv": "per-orbital (eps_v - eps_1) + W/2" if alpha <= 0 else alpha, "tol": TOL,
-                   "solver": {0: "PCG/COCG per frequency", 1: "multi-shift CG", 2: "block CG"}[solver], "cg_iters": stats["iters"], "cg_iters_min": stats["iters_min"],
+                   "solver": {0: "PCG/COCG per frequency", 1: "multi-shift CG", 2: "block CG"}[solver], "ms_history_slots": stats.get("ms_history_slots", 0), "cg_iters": stats["iters"], "cg_iters_min": stats["iters_min"],
                    "unconverged": stats["n_unconverged"], "sub_blocks": stats["n_sub_blocks"], "gap_ry": aux["gap"],
                    "workspace": "caller-owned, %.1f GB (west_set_workspace): no allocation in the timed calls" % (ws.numel() / 1e9) if ws is not None else "context-owned (lazy)",
                    "l2": "inputs per step (vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
         "h_apply_per_s": n_h * world / (ms * 1e-3), "h_apply_per_step": n_h / steps,
         "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": roofline(cfg, top, prof, n_h_prof, n_freq, solver, hbm_peak, peak_src, mixed, w.n_g, fp64_peak, pst.get("n_shift_updates", 0)),
+        "roofline": roofline(cfg, top, prof, n_h_prof, n_freq, solver, hbm_peak, peak_src, mixed, w.n_g, fp64_peak, pst.get("n_shift_updates", 0), pst.get("n_hist_passes", 0)),
         "gemm": {"achieved_tflops": gemm_tf, "peak_tflops": fp64_peak, "frac": (gemm_tf / fp64_peak) if gemm_tf else None,
                  "note": "KB + P_v GEMMs of the CG loop in the profiled step (RHS projection excluded from the flop count)"},
         "kernel_ms_per_step": {k: round(v["ms"], 3) for k, v in prof.items() if v["spans"]},
@@ -645,11 +664,28 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if a.op == "pipes":
+        # yardstick: DMMA and DFMA warps alone and together (west_probe_fp64_pipes)
+        c1 = synth.get_config("cfg1")
+        wp = wb.West(c1["L"], c1["n2max"], c1["N"], wb.WEST_FULL)
+        rows = []
+        for nd in (0, 4, 8, 12, 16):
+            for mode in (1, 2, 3):
+                if (nd == 0 and mode & 1) or (nd == 16 and mode & 2):
+                    continue
+                ms, fd, ff = wp.probe_fp64_pipes(mode, nd)
+                rows.append({"dmma_warps": nd, "dfma_warps": 16 - nd, "mode": {1: "DMMA only", 2: "DFMA only", 3: "both"}[mode], "ms": round(ms, 3),
+                             "dmma_tflops": round(fd / ms / 1e9, 2), "dfma_tflops": round(ff / ms / 1e9, 2), "sum_tflops": round((fd + ff) / ms / 1e9, 2)})
+        wp.close()
+        if rank == 0:
+            print(json.dumps({"metric": "FP64 pipe yardstick: DMMA / DFMA warps alone and together", "unit": "TFLOP/s", "n_gpus": 1, "rows": rows}))
+        return
     if a.op in ("happly", "gemm"):
         return bench_kernels(a, wb, cfg, rank, world, barrier)
     # every rank: same cell and orbitals, its own block of perturbations (seeded stream offset by rank)
     w, dV_np, alpha, aux = setup_gpu(cfg, n_pert, a.chunk, verbose=(rank == 0), n_defl=a.deflate, alpha_factor=a.alpha_factor)
     w.set_cg_kernel(a.cg_kernel)
+    w.set_ms_history(a.ms_history)
     if world > 1:
         dV_np = synth.perturbations(cfg, n_pert=n_pert, first=rank * n_pert)
     dev = torch.device("cuda")
@@ -698,6 +734,7 @@ def main():
         try:
             c4 = synth.get_config("cfg4")
             w2, dV2, alpha2, aux2 = setup_gpu(c4, c4["n_pert"], a.chunk, verbose=True, alpha_factor=a.alpha_factor)
+            w2.set_ms_history(a.ms_history)
             for name in ("cfg2", "cfg3", "cfg4"):
                 try:
                     c = synth.get_config(name)
@@ -708,6 +745,23 @@ def main():
                 except Exception as e:
                     subs[name] = {"error": repr(e)[:300]}
             w2.close()
+            del w2, aux2
+            torch.cuda.empty_cache()
+            # cfg3 once more with west_set_deflation: 128 conduction eigenstates (an eigensolver's guard states) handed over as extra inputs.
+            # Exact (DESIGN 6e); it lifts the lower end of the UNPRECONDITIONED multi-shift operator's spectrum, which is what sets its
+            # iteration count.  A separate record: BASELINE's cfg3 is the plain one above.
+            try:
+                c3 = synth.get_config("cfg3")
+                w3, dV3, alpha3, aux3 = setup_gpu(c3, c3["n_pert"], a.chunk, verbose=True, n_defl=128, alpha_factor=a.alpha_factor)
+                w3.set_ms_history(a.ms_history)
+                keep = a.deflate
+                a.deflate = 128
+                subs["cfg3_deflated"] = run_chi0(a, wb, c3, w3, dV3, alpha3, aux3, omegas_for(a, c3, "cfg3"), 1, wb.WEST_FP64, SUB_STEPS, SUB_WARMUP, local, world,
+                                                 barrier, 0, want_cpu=0 if a.no_cpu_baseline else 1, label="cfg3 + 128 deflated conduction states")
+                a.deflate = keep
+                w3.close()
+            except Exception as e:
+                subs["cfg3_deflated"] = {"error": repr(e)[:300]}
         except Exception as e:
             subs["cfg2-4"] = {"error": repr(e)[:300]}
         line["workloads"] = subs

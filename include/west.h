@@ -88,6 +88,9 @@ extern "C" {
 #define WEST_OP_CHI0_MULTISHIFT  4   /* west_chi0_apply, solver 1, n_freq frequencies */
 #define WEST_OP_LANCZOS          5   /* west_lanczos, n_freq = n_steps */
 #define WEST_OP_CHI0_BLOCK       6   /* west_chi0_apply, solver 2, every omega = 0 (block CG: five vector sets) */
+#define WEST_OP_CHI0_MULTISHIFT_HIST 7 /* west_chi0_apply, solver 1 with room for a full 128-slot Krylov history for all n_pert perturbations as one
+                                        block (the fast variant; WEST_OP_CHI0_MULTISHIFT is the smallest comfortable size, and any block in
+                                        between is used for as many ring slots as fit) */
 
 #define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
@@ -111,7 +114,9 @@ typedef struct {
     int32_t check_every;/* host polls convergence every this many iterations (>=1) */
     int32_t solver;     /* 0: one preconditioned PCG (omega = 0) / COCG (omega > 0) solve per frequency (R7);
                            1: multi-shift CG (WEST_GAMMA only, <= 16 frequencies): all frequencies from ONE unpreconditioned Krylov
-                              sequence of the real seed operator H - eps_v + alpha P_v, one H*psi per iteration for every omega;
+                              sequence of the real seed operator H - eps_v + alpha P_v, one H*psi per iteration for every omega.  The
+                              shifted solutions are contracted from the seed residuals, which are kept in a ring of up to 128 vectors
+                              per column when the workspace has room (west_set_ms_history); else per-shift vector recurrences;
                            2: block CG: at omega = 0 the n_pert right-hand sides of one orbital share ONE Krylov space (Gram
                               matrices of the search block, rank-revealing pivoted-Cholesky solves that drop dependent directions, csrc/
                               bcg_kernels.cuh); same dpsi, fewer H*psi.  Blocks of 2 .. 128 perturbations (per sub-block); frequencies
@@ -130,6 +135,8 @@ typedef struct {            /* host struct, filled when non-NULL (one stream syn
     int64_t n_h_apply;      /* vectors pushed through H in this call (real functions in GAMMA mode) */
     int64_t n_shift_updates;/* multi-shift solver: (column, frequency) vector updates performed (frozen frequencies are skipped) */
     float   ms_rhs, ms_cg, ms_dn;   /* CUDA-event times of the three phases */
+    int64_t n_hist_passes;  /* multi-shift solver with the Krylov history: column-vector passes (16 n_g bytes each) of the history contractions */
+    int32_t ms_history_slots; /* multi-shift solver: ring slots of the Krylov history used (0 = per-shift recurrences) */
 } west_stats;
 
 /* Context. cuda_stream: cudaStream_t as void*. */
@@ -276,6 +283,20 @@ int  west_set_fft_chunk(west_ctx* ctx, int32_t n_slots);
  * over a cluster of two CTAs (partial sums through distributed shared memory; same size limit).  Same results up to summation order.
  * Errors: WEST_EINVAL (NULL ctx, which not 0 / 1 / 2). */
 int  west_set_cg_kernel(west_ctx* ctx, int32_t which);
+/* Tuning knob of the multi-shift solver (west_cg_opts.solver = 1).  slots = 0 (default): keep the seed residuals of every column in a
+ * ring of min(max_iter + 1, 128) vectors - fewer if the workspace is smaller, down to 32, below which the perturbation sub-block is
+ * shrunk instead - and contract the shifted solutions x_s from them once per ring revolution (every history vector is read once for all
+ * frequencies; carry vectors bridge the revolutions).  slots = -1: the per-shift vector recurrences (x_s and p_s updated in every
+ * iteration: 6 vector passes per live shift and iteration, but only 3 + 4 n_freq vectors of workspace per column).  slots = 2 .. 128: that
+ * ring size exactly (tests).  Same results up to summation order.  Errors: WEST_EINVAL. */
+int  west_set_ms_history(west_ctx* ctx, int32_t slots);
+
+/* Yardstick for the roofline statements of DESIGN.md section 10: do the FP64 tensor instruction (DMMA, what the projector GEMMs issue) and
+ * the FP64 FMA instruction (what the FFT kernels issue) have separate pipes on this GPU?  One 16-warp CTA per SM (148 CTAs); the first
+ * n_dmma_warps warps run independent DMMA chains, the other warps DFMA chains; mode bit 0 switches the DMMA warps on, bit 1 the DFMA warps.
+ * Times one launch (after a warm-up launch) with CUDA events and synchronises.  ms_host: milliseconds; dmma_flop_host / dfma_flop_host
+ * (may be NULL): floating-point operations each kind of warp executed in the timed launch.  Errors: WEST_EINVAL, WEST_ECUDA. */
+int  west_probe_fp64_pipes(west_ctx* ctx, int32_t mode, int32_t n_dmma_warps, int32_t iters, float* ms_host, double* dmma_flop_host, double* dfma_flop_host);
 
 #ifdef __cplusplus
 }

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(HERE, "libwest.so")
 
 WEST_OK, WEST_NOTCONVERGED = 0, 1
 WEST_EINVAL, WEST_ECUDA, WEST_ESTATE, WEST_ENOMEM, WEST_EWORKSPACE = -1, -2, -3, -4, -5
-WEST_OP_FFT3D, WEST_OP_H_APPLY, WEST_OP_CHI0, WEST_OP_CHI0_IW, WEST_OP_CHI0_MULTISHIFT, WEST_OP_LANCZOS, WEST_OP_CHI0_BLOCK = 0, 1, 2, 3, 4, 5, 6
+WEST_OP_FFT3D, WEST_OP_H_APPLY, WEST_OP_CHI0, WEST_OP_CHI0_IW, WEST_OP_CHI0_MULTISHIFT, WEST_OP_LANCZOS, WEST_OP_CHI0_BLOCK, WEST_OP_CHI0_MULTISHIFT_HIST = 0, 1, 2, 3, 4, 5, 6, 7
 WEST_FULL, WEST_GAMMA = 0, 1
 WEST_FP64, WEST_MIXED, WEST_FP32 = 0, 1, 2
 
@@ -30,12 +30,12 @@ class west_cg_opts(C.Structure):
 
 class west_stats(C.Structure):
     _fields_ = [("iters", C.c_int32), ("iters_min", C.c_int32), ("n_sub_blocks", C.c_int32), ("n_unconverged", C.c_int32), ("resid_max", C.c_double), ("n_h_apply", C.c_int64), ("n_shift_updates", C.c_int64),
-                ("ms_rhs", C.c_float), ("ms_cg", C.c_float), ("ms_dn", C.c_float)]
+                ("ms_rhs", C.c_float), ("ms_cg", C.c_float), ("ms_dn", C.c_float), ("n_hist_passes", C.c_int64), ("ms_history_slots", C.c_int32)]
 
 
 EXPORTS = ["west_create", "west_destroy", "west_last_error", "west_gsphere", "west_set_vloc", "west_set_kb", "west_set_states", "west_set_deflation",
            "west_fft3d", "west_fft3d_static", "west_static_scratch_bytes", "west_fft3d_dense", "west_h_apply", "west_chi0_apply", "west_lanczos", "west_lanczos_diag", "west_gemm_tn", "west_gemm_update", "west_device_bytes",
-           "west_launch_count", "west_workspace_bytes", "west_set_workspace", "west_set_fft_chunk", "west_set_cg_kernel", "west_set_profile", "west_get_profile"]
+           "west_launch_count", "west_workspace_bytes", "west_set_workspace", "west_set_fft_chunk", "west_set_cg_kernel", "west_set_ms_history", "west_probe_fp64_pipes", "west_set_profile", "west_get_profile"]
 
 
 def load_library():
@@ -72,6 +72,8 @@ def load_library():
     lib.west_set_workspace.argtypes = [vp, vp, C.c_size_t]
     lib.west_set_fft_chunk.argtypes = [vp, i32]
     lib.west_set_cg_kernel.argtypes = [vp, i32]
+    lib.west_set_ms_history.argtypes = [vp, i32]
+    lib.west_probe_fp64_pipes.argtypes = [vp, i32, i32, i32, C.POINTER(C.c_float), C.POINTER(dbl), C.POINTER(dbl)]
     lib.west_set_profile.argtypes = [vp, i32]
     lib.west_get_profile.argtypes = [vp, vp, vp]
     for name in EXPORTS:
@@ -328,6 +330,15 @@ class West:
 
     def set_cg_kernel(self, which):
         self._ck(self.lib.west_set_cg_kernel(self.ctx, int(which)))
+
+    def set_ms_history(self, slots):
+        self._ck(self.lib.west_set_ms_history(self.ctx, int(slots)))
+
+    def probe_fp64_pipes(self, mode, n_dmma_warps, iters=20000):
+        """(ms, DMMA flop, DFMA flop) of one launch of the FP64 pipe yardstick (west.h)"""
+        ms, fd, ff = C.c_float(), C.c_double(), C.c_double()
+        self._ck(self.lib.west_probe_fp64_pipes(self.ctx, int(mode), int(n_dmma_warps), int(iters), C.byref(ms), C.byref(fd), C.byref(ff)))
+        return ms.value, fd.value, ff.value
 
     def set_fft_chunk(self, n):
         self._ck(self.lib.west_set_fft_chunk(self.ctx, int(n)))

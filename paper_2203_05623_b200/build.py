@@ -24,6 +24,12 @@ FFT_SIZES = [(4, 6, 24, 4, 4, 20, 4, 256), (6, 6, 36, 4, 4, 20, 4, 256), (6, 8, 
              (12, 12, 144, 12, 1, 10, 2, 256)]
 K2H_SHAPES = {72: tuple(int(x) for x in os.environ.get("WEST_K2H_72", "6,3,2,1").split(",")),
               144: tuple(int(x) for x in os.environ.get("WEST_K2H_144", "12,1,1,1").split(","))}
+# measured alternatives of the z-stick kernels' shape: WEST_Z_<N>="CU,ZMINB,ZNT" overrides the table entry of grid size N
+for _i, _t in enumerate(FFT_SIZES):
+    _v = os.environ.get("WEST_Z_%d" % _t[2])
+    if _v:
+        _cu, _zminb, _znt = (int(x) for x in _v.split(","))
+        FFT_SIZES[_i] = _t[:5] + (_cu, _zminb, _znt)
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 

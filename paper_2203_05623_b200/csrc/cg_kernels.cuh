@@ -433,11 +433,12 @@ __global__ void __launch_bounds__(NT) ms_init(long long n_g, int n_col, MsShifts
         const double2 v = r[g];
         acc[0] += rdot_gamma(v, v, g);
         p[g] = v;
-        for (int s = 0; s < sh.n; ++s) {
-            double2* ps = PS + ((long long)s * n_col + col) * 2 * n_g;
-            ps[g] = v;
-            ps[n_g + g] = make_double2(0.0, 0.0);
-        }
+        if (PS)                                   // PS == nullptr: Krylov-history variant (ms_hist_step), no per-shift search directions
+            for (int s = 0; s < sh.n; ++s) {
+                double2* ps = PS + ((long long)s * n_col + col) * 2 * n_g;
+                ps[g] = v;
+                ps[n_g + g] = make_double2(0.0, 0.0);
+            }
     }
     block_reduce<1>(acc, red);
     if (threadIdx.x == 0) {
@@ -539,6 +540,278 @@ __global__ void __launch_bounds__(NT) ms_step(long long n_g, int n_col, MsShifts
         int any = 0;
         for (int s = 0; s < sh.n; ++s) any |= st.sactive[(long long)s * n_col + col];
         if (!any) { st.active[col] = 0; atomicSub(st.counters, 1); }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- multi-shift CG with a Krylov history
+// The per-shift vector recurrences of ms_step move 6 vector passes per live shift and iteration.  They are linear in the seed
+// residuals: with  p_s,k = zeta_k r_k + Q_k,  Q_{k+1} = b_s,k p_s,k,  x_s += a_s,k p_s,k  (a_s,k, b_s,k, zeta_k as in ms_step) the
+// iterations k = j0 .. n-1 of a segment add
+//     x_s += sum_j zeta_j w_j r_j + w_j0 Q_j0,        w_j = a_s,j + b_s,j w_{j+1},  w_n = 0
+//     Q_n  = sum_j zeta_j B_j r_j + B_j0 Q_j0,         B_j = b_s,j B_{j+1},          B_n = 1
+// so it is enough to KEEP the residuals r_j (they are written anyway: the seed recurrence writes r_{k+1} into the next slot of a ring
+// instead of over r_k), store three complex scalars per (iteration, shift, column), and contract once per segment (ms_hist_combine):
+// every history vector is read once for ALL shifts.  This is the Lanczos form of the shifted solves (PAPER.md:138-157 uses the same
+// idea for its frequency dependence); results equal ms_step's up to summation order.
+// Ring: r_j lives in slot j mod H of HIST [H][n_col][n_g] (original column order), the scalars of iteration k in slot k mod H of
+// HS [H][3][n_shift][n_col] (a_s, b_s, zeta_k; zero once the shift is frozen).  A segment ends (flush) before slot j0 would be overwritten.
+struct MsHist {
+    double2* vec;      // [H][n_col][n_g]
+    double2* scal;     // [H][3][n_shift][n_col]
+    int H;
+};
+
+__global__ void __launch_bounds__(NT) ms_hist_step(long long n_g, int n_col, MsShifts sh, double tol2, int k_iter, MsHist hs, double2* P,
+                                                   const double2* AP, MsState st, const int* colmap) {
+    __shared__ double red[32];
+    const int k = blockIdx.x, col = colmap[k];
+    if (col < 0 || !st.active[col]) return;
+    double2* p = P + (long long)k * n_g; const double2* ap = AP + (long long)k * n_g;
+    const double2* r = hs.vec + ((long long)(k_iter % hs.H) * n_col + col) * n_g;
+    double2* rnew = hs.vec + ((long long)((k_iter + 1) % hs.H) * n_col + col) * n_g;
+    // ---- a_k
+    double acc[1] = {0};
+    for (int g = threadIdx.x; g < n_g; g += NT) acc[0] += rdot_gamma(p[g], ap[g], g);
+    block_reduce<1>(acc, red);
+    const double rr = st.rr[col], a = rr / acc[0];
+    // ---- r_{k+1} (next ring slot), b_k
+    acc[0] = 0;
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        double2 v = r[g]; const double2 q = ap[g];
+        v.x -= a * q.x; v.y -= a * q.y;
+        rnew[g] = v;
+        acc[0] += rdot_gamma(v, v, g);
+    }
+    block_reduce<1>(acc, red);
+    const double rrn = acc[0], b = rrn / rr;
+    // ---- shifted scalars (same recurrences as ms_step), kept for the segment's contraction
+    if (threadIdx.x < sh.n) {
+        const int s = threadIdx.x;
+        const long long i = (long long)s * n_col + col;
+        double2* slot = hs.scal + (long long)(k_iter % hs.H) * 3 * sh.n * n_col;
+        double2 as = make_double2(0.0, 0.0), bs = as, zc = as;
+        if (st.sactive[i]) {
+            const double2 z = st.zeta[i], zp = st.zeta_prev[i];
+            const double ap_ = st.a_prev[col], bp_ = st.b_prev[col];
+            const double2 sigma = make_double2(0.0, -sh.omega[s]);
+            const double2 t1 = make_double2(a * bp_ * (zp.x - z.x), a * bp_ * (zp.y - z.y));
+            const double2 one_sa = make_double2(1.0 + sigma.x * a, sigma.y * a);
+            const double2 t2 = cmul2(make_double2(zp.x * ap_, zp.y * ap_), one_sa);
+            const double2 num = cmul2(z, make_double2(zp.x * ap_, zp.y * ap_));
+            const double2 zn = cdiv(num, make_double2(t1.x + t2.x, t1.y + t2.y));
+            const double2 ratio = cdiv(zn, z);
+            as = make_double2(a * ratio.x, a * ratio.y);
+            const double2 r2 = cmul2(ratio, ratio);
+            bs = make_double2(b * r2.x, b * r2.y);
+            zc = z;
+            st.zeta_prev[i] = z; st.zeta[i] = zn;
+            const double res2 = (zn.x * zn.x + zn.y * zn.y) * rrn / st.b2[col];
+            st.res2[i] = res2;
+            if (!(res2 > tol2)) st.sactive[i] = 0;       // x_s still takes this iteration's update (as is stored), then freezes
+        }
+        slot[i] = as; slot[(long long)sh.n * n_col + i] = bs; slot[2ll * sh.n * n_col + i] = zc;
+    }
+    // ---- p = r_{k+1} + b p
+    for (int g = threadIdx.x; g < n_g; g += NT) {
+        const double2 rn = rnew[g], pp = p[g];
+        p[g] = make_double2(rn.x + b * pp.x, rn.y + b * pp.y);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        st.a_prev[col] = a; st.b_prev[col] = b; st.rr[col] = rrn;
+        st.iters[col] += 1;
+        int any = 0;
+        for (int s = 0; s < sh.n; ++s) any |= st.sactive[(long long)s * n_col + col];
+        if (!any) { st.active[col] = 0; atomicSub(st.counters, 1); }
+    }
+}
+
+// The same iteration with the column resident on one SM (n_g <= NTR * EPT; cfgs 1-4): p parked in shared memory, Ap and then r_{k+1} in
+// registers, so HBM sees 3 reads (p, Ap, r_k) and 2 writes (r_{k+1}, p) of the column instead of the 8 passes of the streaming kernel.
+__device__ __forceinline__ void ms_shift_scalars(const MsShifts& sh, int n_col, int col, int k_iter, const MsHist& hs, MsState& st, double a, double b,
+                                                 double rrn, double tol2) {
+    if (threadIdx.x < sh.n) {
+        const int s = threadIdx.x;
+        const long long i = (long long)s * n_col + col;
+        double2* slot = hs.scal + (long long)(k_iter % hs.H) * 3 * sh.n * n_col;
+        double2 as = make_double2(0.0, 0.0), bs = as, zc = as;
+        if (st.sactive[i]) {
+            const double2 z = st.zeta[i], zp = st.zeta_prev[i];
+            const double ap_ = st.a_prev[col], bp_ = st.b_prev[col];
+            const double2 sigma = make_double2(0.0, -sh.omega[s]);
+            const double2 t1 = make_double2(a * bp_ * (zp.x - z.x), a * bp_ * (zp.y - z.y));
+            const double2 one_sa = make_double2(1.0 + sigma.x * a, sigma.y * a);
+            const double2 t2 = cmul2(make_double2(zp.x * ap_, zp.y * ap_), one_sa);
+            const double2 num = cmul2(z, make_double2(zp.x * ap_, zp.y * ap_));
+            const double2 zn = cdiv(num, make_double2(t1.x + t2.x, t1.y + t2.y));
+            const double2 ratio = cdiv(zn, z);
+            as = make_double2(a * ratio.x, a * ratio.y);
+            const double2 r2 = cmul2(ratio, ratio);
+            bs = make_double2(b * r2.x, b * r2.y);
+            zc = z;
+            st.zeta_prev[i] = z; st.zeta[i] = zn;
+            const double res2 = (zn.x * zn.x + zn.y * zn.y) * rrn / st.b2[col];
+            st.res2[i] = res2;
+            if (!(res2 > tol2)) st.sactive[i] = 0;       // x_s still takes this iteration's update (as is stored), then freezes
+        }
+        slot[i] = as; slot[(long long)sh.n * n_col + i] = bs; slot[2ll * sh.n * n_col + i] = zc;
+    }
+}
+template <int NTR, int EPT>
+__global__ void __launch_bounds__(NTR, 1) ms_hist_step_resident(long long n_g, int n_col, MsShifts sh, double tol2, int k_iter, MsHist hs, double2* P,
+                                                                const double2* AP, MsState st, const int* colmap) {
+    extern __shared__ __align__(16) double2 psh[];            // [EPT][NTR]: thread t owns psh[e * NTR + t]
+    __shared__ double shr[NTR / 32];
+    const int k = blockIdx.x, col = colmap[k], t = threadIdx.x;
+    if (col < 0 || !st.active[col]) return;
+    double2* p = P + (long long)k * n_g; const double2* ap = AP + (long long)k * n_g;
+    const double2* r = hs.vec + ((long long)(k_iter % hs.H) * n_col + col) * n_g;
+    double2* rnew = hs.vec + ((long long)((k_iter + 1) % hs.H) * n_col + col) * n_g;
+    double2 q[EPT];
+    double d1[1] = {0};
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = e * NTR + t;
+        if (g < n_g) {
+            const double2 pp = p[g];
+            q[e] = ap[g];
+            psh[e * NTR + t] = pp;
+            d1[0] += rdot_gamma(pp, q[e], g);
+        }
+    }
+    block_reduce_w<1, NTR / 32>(d1, shr);
+    const double rr = st.rr[col], a = rr / d1[0];
+    double acc[1] = {0};
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = e * NTR + t;
+        if (g < n_g) {
+            double2 v = r[g];
+            v.x -= a * q[e].x; v.y -= a * q[e].y;
+            rnew[g] = v; q[e] = v;
+            acc[0] += rdot_gamma(v, v, g);
+        }
+    }
+    block_reduce_w<1, NTR / 32>(acc, shr);
+    const double rrn = acc[0], b = rrn / rr;
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int g = e * NTR + t;
+        if (g < n_g) {
+            const double2 pp = psh[e * NTR + t];
+            p[g] = make_double2(q[e].x + b * pp.x, q[e].y + b * pp.y);
+        }
+    }
+    ms_shift_scalars(sh, n_col, col, k_iter, hs, st, a, b, rrn, tol2);      // after the vector work: the column's registers are dead by now
+    __syncthreads();
+    if (t == 0) {
+        st.a_prev[col] = a; st.b_prev[col] = b; st.rr[col] = rrn;
+        st.iters[col] += 1;
+        int any = 0;
+        for (int s = 0; s < sh.n; ++s) any |= st.sactive[(long long)s * n_col + col];
+        if (!any) { st.active[col] = 0; atomicSub(st.counters, 1); }
+    }
+}
+
+// Contraction of one segment [j0, n) of the history for column blockIdx.x, elements [blockIdx.y * MSH_CHUNK, +MSH_CHUNK):
+//   XS[s][col] (Re part, and Im part if IMAG) += sum_j cx_j r_j + dx Q_s          QS[s][col] = sum_j cq_j r_j + dq Q_s   (CARRY_OUT)
+// carry_in = 0: Q_s is taken as zero (first segment) and never read.  Columns use only the iterations they took part in
+// (j < iters[col]); a column that left before j0 has nothing to add.  Dynamic shared memory: 2 * n_shift * (n - j0 + 1) double2.
+constexpr int MSH_CHUNK = 2048;
+constexpr int MSH_HMAX = 128;        // most ring slots (bounds the coefficient tables: 2 * 16 shifts * 129 double2 = 66 KB)
+// MSH_G = shifts per register group: every group re-reads the segment's history, so the plain final contraction (Re x_s only) takes 8
+template <bool IMAG, bool CARRY_OUT, int MSH_G>
+__global__ void __launch_bounds__(NT) ms_hist_combine(long long n_g, int n_col, int n_shift, int j0, int n_end, int carry_in, MsHist hs,
+                                                      const int* iters, double2* XS, double2* QS, unsigned long long* pass_counter) {
+    extern __shared__ double2 msh_sm[];
+    const int col = blockIdx.x;
+    const int jend = min(n_end, iters[col]);
+    const int len = jend - j0;
+    if (len <= 0) return;
+    const int L = n_end - j0 + 1;                       // row length of the coefficient tables (last entry: the carry coefficients dx, dq)
+    double2* cx = msh_sm;                               // [n_shift][L]
+    double2* cq = msh_sm + (size_t)n_shift * L;         // [n_shift][L]
+    // stage the segment's scalars: cx <- a_s, cq <- b_s, then the backward recurrences in place (zeta read from global, L2-resident)
+    for (int t = threadIdx.x; t < n_shift * len; t += NT) {
+        const int s = t / len, i = t - s * len;
+        const double2* slot = hs.scal + (long long)((j0 + i) % hs.H) * 3 * n_shift * n_col + (long long)s * n_col + col;
+        cx[s * L + i] = slot[0];
+        cq[s * L + i] = slot[(long long)n_shift * n_col];
+    }
+    __syncthreads();
+    if (threadIdx.x < n_shift) {
+        const int s = threadIdx.x;
+        double2 w = make_double2(0.0, 0.0), bt = make_double2(1.0, 0.0);
+        for (int i = len - 1; i >= 0; --i) {
+            const double2 as = cx[s * L + i], bs = cq[s * L + i];
+            const double2 zc = hs.scal[(long long)((j0 + i) % hs.H) * 3 * n_shift * n_col + 2ll * n_shift * n_col + (long long)s * n_col + col];
+            const double2 bw = cmul2(bs, w);
+            w = make_double2(as.x + bw.x, as.y + bw.y);
+            bt = cmul2(bs, bt);
+            cx[s * L + i] = cmul2(zc, w);
+            cq[s * L + i] = cmul2(zc, bt);
+        }
+        cx[s * L + L - 1] = w;                          // dx
+        cq[s * L + L - 1] = bt;                         // dq
+    }
+    __syncthreads();
+    if (blockIdx.y == 0 && threadIdx.x == 0 && pass_counter) {
+        // column-vector passes (16 n_g bytes each) of this column's contraction: history reads once per shift group, x_s (and carry) traffic
+        const int groups = (n_shift + MSH_G - 1) / MSH_G;
+        unsigned long long passes = (unsigned long long)len * groups + (unsigned long long)n_shift * ((IMAG ? 4 : 2) + (carry_in ? 2 : 0) + (CARRY_OUT ? 2 : 0));
+        atomicAdd(pass_counter, passes);
+    }
+    const long long g_lo = (long long)blockIdx.y * MSH_CHUNK, g_hi = min(n_g, g_lo + MSH_CHUNK);
+    for (int s0 = 0; s0 < n_shift; s0 += MSH_G) {
+        const int ns = min(MSH_G, n_shift - s0);
+        for (long long g = g_lo + threadIdx.x; g < g_hi; g += NT) {
+            double2 xr[MSH_G], xi[MSH_G], qr[MSH_G], qi[MSH_G];
+#pragma unroll
+            for (int q = 0; q < MSH_G; ++q) xr[q] = xi[q] = qr[q] = qi[q] = make_double2(0.0, 0.0);
+            const double2* hv = hs.vec + (long long)col * n_g + g;
+#pragma unroll 4
+            for (int i = 0; i < len; ++i) {
+                const double2 v = hv[(long long)((j0 + i) % hs.H) * n_col * n_g];
+#pragma unroll
+                for (int q = 0; q < MSH_G; ++q) {
+                    if (q < ns) {
+                        const double2 c1 = cx[(s0 + q) * L + i];
+                        xr[q].x += c1.x * v.x; xr[q].y += c1.x * v.y;
+                        if (IMAG) { xi[q].x += c1.y * v.x; xi[q].y += c1.y * v.y; }
+                        if (CARRY_OUT) {
+                            const double2 c2 = cq[(s0 + q) * L + i];
+                            qr[q].x += c2.x * v.x; qr[q].y += c2.x * v.y;
+                            qi[q].x += c2.y * v.x; qi[q].y += c2.y * v.y;
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < MSH_G; ++q) {
+                if (q < ns) {
+                    const long long base = ((long long)(s0 + q) * n_col + col) * 2 * n_g + g;
+                    if (carry_in) {
+                        const double2 Qr = QS[base], Qi = QS[base + n_g];
+                        const double2 dx = cx[(s0 + q) * L + L - 1], dq = cq[(s0 + q) * L + L - 1];
+                        xr[q].x += dx.x * Qr.x - dx.y * Qi.x; xr[q].y += dx.x * Qr.y - dx.y * Qi.y;
+                        if (IMAG) { xi[q].x += dx.x * Qi.x + dx.y * Qr.x; xi[q].y += dx.x * Qi.y + dx.y * Qr.y; }
+                        if (CARRY_OUT) {
+                            qr[q].x += dq.x * Qr.x - dq.y * Qi.x; qr[q].y += dq.x * Qr.y - dq.y * Qi.y;
+                            qi[q].x += dq.x * Qi.x + dq.y * Qr.x; qi[q].y += dq.x * Qi.y + dq.y * Qr.y;
+                        }
+                    }
+                    double2 x0 = XS[base];
+                    x0.x += xr[q].x; x0.y += xr[q].y;
+                    XS[base] = x0;
+                    if (IMAG) {
+                        double2 x1 = XS[base + n_g];
+                        x1.x += xi[q].x; x1.y += xi[q].y;
+                        XS[base + n_g] = x1;
+                    }
+                    if (CARRY_OUT) { QS[base] = qr[q]; QS[base + n_g] = qi[q]; }
+                }
+            }
+        }
     }
 }
 

@@ -57,6 +57,7 @@ struct west_ctx {
     int64_t dev_bytes = 0;
     int fft_chunk = 0;
     int cg_kernel = 0;                 // west_set_cg_kernel: 0 automatic, 1 always streaming
+    int ms_hist = 0;                   // west_set_ms_history: 0 automatic, -1 per-shift recurrences (ms_step), 2 .. 128 fixed ring size
     std::vector<void*> owned;          // every cudaMalloc of this context
 
     // geometry tables
@@ -98,7 +99,7 @@ struct west_ctx {
 
     // hot-call workspaces: carved from the arena at the start of every hot call (hot_begin / hot)
     Arena arena;
-    DevBuf W, Cbuf, Rbuf, Xsplit, Csplit, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk;
+    DevBuf W, Cbuf, Rbuf, Xsplit, Csplit, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk, hist, hist_scal;
     int* h_pinned = nullptr;           // pinned host scratch (64 ints): lagged convergence polls [0], [1]; reports [8..]
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
 
@@ -648,6 +649,11 @@ int west_get_profile(west_ctx* c, double* ms, int64_t* count) {
 int west_set_cg_kernel(west_ctx* c, int32_t which) {
     if (!c || which < 0 || which > 2) return WEST_EINVAL;
     c->cg_kernel = which;
+    return WEST_OK;
+}
+int west_set_ms_history(west_ctx* c, int32_t slots) {
+    if (!c || slots < -1 || slots == 1 || slots > wcg::MSH_HMAX) return fail(c, WEST_EINVAL, "west_set_ms_history: slots must be -1, 0 or 2 .. %d", wcg::MSH_HMAX);
+    c->ms_hist = slots;
     return WEST_OK;
 }
 int west_set_fft_chunk(west_ctx* c, int32_t n) {
@@ -1294,6 +1300,111 @@ int ms_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::
     return WEST_OK;
 }
 
+// multi-shift CG with a Krylov history (cg_kernels.cuh, ms_hist_*): the seed recurrence keeps its residuals r_j in a ring of hs.H slots
+// (slot 0 holds b on entry) and the shifted solutions are contracted from them once per segment, instead of 6 vector passes per live
+// shift and iteration.  QS (carry vectors, [shift][col][2][n_g]) is only touched when the ring wraps (more than H - 1 iterations).
+cudaError_t ms_hist_attrs() {
+    static bool done = false;
+    if (done) return cudaSuccess;
+    const int bytes = (int)(2 * wcg::MS_MAX_SHIFTS * (wcg::MSH_HMAX + 1) * sizeof(double2));
+    cudaError_t e = cudaFuncSetAttribute(wcg::ms_hist_combine<false, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<true, false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<false, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<true, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    done = e == cudaSuccess;
+    return e;
+}
+int ms_hist_combine_launch(west_ctx* c, int n_col, int n_shift, int j0, int n_end, bool carry_in, bool carry_out, bool imag, const wcg::MsHist& hs,
+                           const wcg::MsState& st, cx<double>* XS, cx<double>* QS) {
+    if (n_end <= j0) return WEST_OK;
+    const long long n_g = c->hs.n_g;
+    const size_t sm = 2 * (size_t)n_shift * (size_t)(n_end - j0 + 1) * sizeof(double2);
+    dim3 grid((unsigned)n_col, (unsigned)((n_g + wcg::MSH_CHUNK - 1) / wcg::MSH_CHUNK));
+    unsigned long long* ctr = reinterpret_cast<unsigned long long*>(st.counters + 2);
+    Prof p_(c, PC_CGVEC);
+    if (imag && carry_out) wcg::ms_hist_combine<true, true, 4><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
+    else if (imag) wcg::ms_hist_combine<true, false, 4><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
+    else if (carry_out) wcg::ms_hist_combine<false, true, 4><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
+    else wcg::ms_hist_combine<false, false, 8><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+int ms_hist_solve(west_ctx* c, int f32, int n_col, const west_cg_opts& o, const wcg::MsShifts& sh, const wcg::MsHist& hs, cx<double>*& P, cx<double>*& AP,
+                  cx<double>* XS, cx<double>* QS, int want_imag, double* shift, wcg::MsState st, int* maps, int* iters_out, int64_t* n_h_out) {
+    const long long n_g = c->hs.n_g;
+    const int n_occ = c->n_occ;
+    const double tol2 = o.tol * o.tol;
+    const int every = std::max(1, o.check_every);
+    int* colmap = maps; int* newmap = maps + n_col; int* src = maps + 2 * (size_t)n_col;
+    CK(ms_hist_attrs());
+    CK(cudaMemsetAsync(st.counters, 0, 4 * sizeof(int), c->st));
+    CK(cudaMemsetAsync(XS, 0, sizeof(cx<double>) * 2 * n_g * n_col * sh.n, c->st));
+    wcg::ms_init<<<n_col, wcg::NT, 0, c->st>>>(n_g, n_col, sh, (const double2*)hs.vec, (double2*)P, (double2*)nullptr, st, colmap);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
+    // column-resident vector kernel where a column fits one SM (cfgs 1-4), as in cg_solve
+    const bool resident = n_g <= (long long)RES_EPT * RES_NT && c->cg_kernel == 0;
+    if (resident)
+        CK(cudaFuncSetAttribute(wcg::ms_hist_step_resident<RES_NT, RES_EPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double2) * RES_NT * RES_EPT)));
+    int n_act = n_col, it = 0, j0 = 0;
+    bool carry = false;
+    int64_t n_h = 0;
+    Poller poll;
+    bool done = false;
+    int rc;
+    for (; it < o.max_iter && !done; ++it) {
+        if (it - j0 + 1 == hs.H) {            // iteration `it` would overwrite r_j0: contract the segment [j0, it) first, keep the carry vectors
+            if ((rc = ms_hist_combine_launch(c, n_col, sh.n, j0, it, carry, true, want_imag != 0, hs, st, XS, QS))) return rc;
+            j0 = it; carry = true;
+        }
+        VecMap vm{2, 1, n_act, 0};
+        rc = hloc_apply(c, f32, vm, (n_act + 1) / 2, P, AP, shift, 0.0);
+        if (rc) return rc;
+        LowrankCoef lc;
+        lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb; lc.alpha_vec = (const double*)c->alpha_v.p; lc.colmap = colmap; lc.nvpc = 1; lc.n_occ = n_occ;
+        rc = lowrank_apply(c, 0, rows, n_act, (const double*)P, (double*)AP, lc, f32 != 0);
+        if (rc) return rc;
+        n_h += n_act;
+        {
+            Prof p_(c, PC_CGVEC);
+            if (resident) {
+                const int ept = (int)((n_g + RES_NT - 1) / RES_NT);
+                wcg::ms_hist_step_resident<RES_NT, RES_EPT><<<n_act, RES_NT, sizeof(double2) * RES_NT * ept, c->st>>>(n_g, n_col, sh, tol2, it, hs, (double2*)P,
+                                                                                                                  (const double2*)AP, st, colmap);
+            } else
+                wcg::ms_hist_step<<<n_act, wcg::NT, 0, c->st>>>(n_g, n_col, sh, tol2, it, hs, (double2*)P, (const double2*)AP, st, colmap);
+            CK(cudaGetLastError());
+            c->launches += 1;
+        }
+        if (poll.ready()) {
+            const int live = poll.collect(c);
+            if (live <= 0) done = true;
+            else if (it + 1 < o.max_iter && live <= n_act - std::max(2, n_act / 16)) {
+                // only p is a compacted working vector here (the residuals stay in the ring in original column order)
+                Prof p_(c, PC_CGVEC);
+                wcg::cg_compact_map<<<1, 1024, 0, c->st>>>(n_act, colmap, st.active, newmap, src, live);
+                wcg::cg_gather_cols<<<live, wcg::NT, 0, c->st>>>(n_g, src, (const double2*)P, (double2*)AP);
+                CK(cudaGetLastError());
+                c->launches += 2;
+                std::swap(P, AP);
+                std::swap(colmap, newmap);
+                n_act = live;
+                fill_shift<<<blocks_for(n_act, 256), 256, 0, c->st>>>(n_act, 1, n_occ, c->d_eps, shift, colmap);
+                CK(cudaGetLastError());
+                c->launches += 1;
+            }
+        }
+        if (!done && ((it + 1) % every == 0 || it + 1 == o.max_iter)) CK(poll.post(c, st.counters));
+    }
+    if (poll.ready()) poll.collect(c);
+    if ((rc = ms_hist_combine_launch(c, n_col, sh.n, j0, it, carry, false, want_imag != 0, hs, st, XS, QS))) return rc;
+    *iters_out = it;
+    *n_h_out = n_h;
+    return WEST_OK;
+}
+
 // ---- block CG (solver 2, omega = 0): one Krylov space per orbital shared by its s = np right-hand sides (bcg_kernels.cuh)
 size_t bcg_small_bytes(int n_occ, int s) {
     const size_t ss = (size_t)s * s, no = (size_t)n_occ, nc = no * s;
@@ -1440,23 +1551,29 @@ int bcg_solve(west_ctx* c, int f32, int s, const west_cg_opts& o, cx<double>* X,
     return WEST_OK;
 }
 
+constexpr int MS_HIST_MIN = 32;      // fewest ring slots worth planning a Krylov history for (below that the sub-block shrinks instead)
+
 // ---- workspace plan of west_chi0_apply for a sub-block of pb perturbations
 struct Chi0Plan {
     int solver = 0, nvpc = 1, n_freq = 1, pb = 0;
     size_t tc = 0;         // WEST_MIXED tensor path: split operands of one low-rank apply (a sum of al256 pieces)
     size_t blk = 0;        // block CG: Gram / coefficient / factor blocks and flags (already a sum of al256 pieces)
     size_t vec = 0, xs = 0, shift = 0, grid = 0, scal = 0, maps = 0, misc = 0, W = 0, C = 0, msst = 0, craw = 0, dcoefd = 0, alpha = 0;
-    size_t total() const {
-        size_t t = (solver == 1 ? 3 : (solver == 2 ? 5 : 4)) * al256(vec) + blk + tc + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) +
-                   al256(C) + al256(alpha);
-        if (solver == 1) t += 2 * al256(xs) + al256(msst);
+    int H = 0;             // multi-shift solver: ring slots of the Krylov history (0 = the per-shift recurrences of ms_step)
+    bool carry = false;    // history ring smaller than max_iter + 1: carry vectors Q_s are planned
+    size_t hscal = 0;
+    size_t fixed() const {                     // everything but the history ring
+        size_t t = blk + tc + al256(shift) + 2 * al256(grid) + al256(scal) + al256(maps) + al256(misc) + al256(W) + al256(C) + al256(alpha);
+        if (solver == 1 && H > 0) t += 2 * al256(vec) + al256(xs) + (carry ? al256(xs) : 0) + al256(msst);
+        else t += (solver == 1 ? 3 : (solver == 2 ? 5 : 4)) * al256(vec) + (solver == 1 ? 2 * al256(xs) + al256(msst) : 0);
         if (craw) t += al256(craw) + al256(dcoefd);
         return t;
     }
+    size_t total() const { return fixed() + (solver == 1 && H > 0 ? al256((size_t)H * vec) + al256((size_t)H * hscal) : 0); }
 };
-Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, int f32 = 0) {
+Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, int f32 = 0, int H = 0, bool carry = false) {
     Chi0Plan p;
-    p.solver = solver; p.nvpc = nvpc; p.n_freq = n_freq; p.pb = pb;
+    p.solver = solver; p.nvpc = nvpc; p.n_freq = n_freq; p.pb = pb; p.H = solver == 1 ? H : 0; p.carry = carry;
     const size_t n_g = (size_t)c->hs.n_g, n3 = (size_t)n3_of(c);
     const size_t n_col = (size_t)pb * c->n_occ;
     const int vp = solver == 1 ? 1 : nvpc;                     // vectors per column in the working sets r, p, Ap (, x)
@@ -1478,6 +1595,7 @@ Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, 
         p.xs = sizeof(cx<double>) * n_g * n_col * 2 * n_freq;
         const size_t ncs = n_col * n_freq;
         p.msst = sizeof(double) * 4 * n_col + sizeof(double2) * 2 * ncs + sizeof(double) * ncs + sizeof(int) * (2 * n_col + ncs) + 64;
+        p.hscal = sizeof(double2) * 3 * ncs;                   // per ring slot: a_s, b_s, zeta of every (shift, column)
     }
     if (c->rows_defl > 0) {
         p.craw = sizeof(double) * (size_t)c->rows_defl * (size_t)((n_vec + 1) / 2 * 2);
@@ -1524,7 +1642,31 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     const size_t budget = arena_budget(c);
     Chi0Plan plan;
     int pb = n_pert;
-    for (int nb = 1;; ++nb) {
+    bool planned = false;
+    if (opts->solver == 1 && c->ms_hist >= 0) {
+        // multi-shift with a Krylov history: the largest sub-block that leaves room for a useful ring (at least MS_HIST_MIN slots, or
+        // the whole run when max_iter is smaller); the ring then takes what is left, up to min(max_iter + 1, 128) slots.  In the lazy
+        // mode the ring may use half of the free device memory (the context keeps its arena until it is destroyed).
+        const int h_want = c->ms_hist > 0 ? std::min(c->ms_hist, opts->max_iter + 1) : std::min(opts->max_iter + 1, wcg::MSH_HMAX);
+        const int h_min = c->ms_hist > 0 ? h_want : std::min(h_want, MS_HIST_MIN);
+        const size_t hbudget = c->arena.user ? budget : budget / 2;
+        for (int nb = 1; h_want >= 2; ++nb) {
+            pb = (n_pert + nb - 1) / nb;
+            // a ring that only fits sub-blocks of fewer than ~2000 columns costs more in GEMM efficiency than it saves in vector traffic
+            // (measured at cfg 5, 4 frequencies: 1 024-column sub-blocks ran the projector GEMMs at 0.86 instead of 0.92 of the DGEMM rate)
+            if (c->ms_hist == 0 && nb > 1 && (long long)pb * n_occ < 2048) break;
+            Chi0Plan q = chi0_plan(c, 1, nvpc_max, n_freq, pb, f32, h_want, h_want < opts->max_iter + 1);
+            const size_t fx = q.fixed(), per = al256(q.vec) + al256(q.hscal) + 512;
+            if (fx + (size_t)h_min * per <= hbudget) {
+                const int h = (int)std::min<size_t>((size_t)h_want, (hbudget - fx) / per);
+                plan = chi0_plan(c, 1, nvpc_max, n_freq, pb, f32, h, h < opts->max_iter + 1);
+                planned = plan.total() <= budget;
+                break;
+            }
+            if (pb == 1) break;
+        }
+    }
+    for (int nb = 1; !planned; ++nb) {
         pb = (n_pert + nb - 1) / nb;
         plan = chi0_plan(c, opts->solver, nvpc_max, n_freq, pb, f32);
         if (plan.total() <= budget || pb == 1) break;
@@ -1533,7 +1675,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         return fail(c, c->arena.user ? WEST_EWORKSPACE : WEST_ENOMEM, "west_chi0_apply: one perturbation needs %zu bytes of workspace, %zu available",
                     plan.total(), budget);
     if ((rc = hot_begin(c, plan.total()))) return rc;
-    const int n_vecsets = opts->solver == 1 ? 3 : 4;
+    const int n_vecsets = opts->solver == 1 ? (plan.H > 0 ? 2 : 3) : 4;
     for (int i = 4 - n_vecsets; i < 4; ++i)
         if ((rc = hot(c, c->vecs[i], plan.vec))) return rc;
     if ((rc = hot(c, c->shift, plan.shift))) return rc;
@@ -1551,8 +1693,12 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     }
     if (opts->solver == 1) {
         if ((rc = hot(c, c->xs, plan.xs))) return rc;
-        if ((rc = hot(c, c->ps, plan.xs))) return rc;
+        if (plan.H == 0 || plan.carry) { if ((rc = hot(c, c->ps, plan.xs))) return rc; }      // p_s of ms_step, or the carry vectors of the history ring
         if ((rc = hot(c, c->msst, plan.msst))) return rc;
+        if (plan.H > 0) {
+            if ((rc = hot(c, c->hist, (size_t)plan.H * plan.vec))) return rc;
+            if ((rc = hot(c, c->hist_scal, (size_t)plan.H * plan.hscal))) return rc;
+        }
     }
     if (plan.craw) {
         if ((rc = hot(c, c->craw, plan.craw))) return rc;
@@ -1615,13 +1761,19 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             fill_shift<<<blocks_for(n_col, 256), 256, 0, c->st>>>(n_col, 1, n_occ, c->d_eps, (double*)c->shift.p, nullptr);
             CK(cudaGetLastError());
             if (stats) CK(cudaEventRecord(ev[0], c->st));
-            if ((rc = chi0_rhs(c, np, 1, R))) return rc;
+            // history variant: b goes straight into ring slot 0 (the ring is laid out for THIS sub-block's column count)
+            wcg::MsHist hs{(double2*)c->hist.p, (double2*)c->hist_scal.p, plan.H};
+            if ((rc = chi0_rhs(c, np, 1, plan.H > 0 ? (cx<double>*)c->hist.p : R))) return rc;
             if (stats) CK(cudaEventRecord(ev[1], c->st));
             int iters = 0;
             int64_t n_h = 0;
-            if ((rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, dpsi_opt != nullptr, (double*)c->shift.p, st,
-                               (int*)c->maps.p, &iters, &n_h)))
-                return rc;
+            if (plan.H > 0)
+                rc = ms_hist_solve(c, f32, n_col, *opts, sh, hs, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, dpsi_opt != nullptr, (double*)c->shift.p, st,
+                                   (int*)c->maps.p, &iters, &n_h);
+            else
+                rc = ms_solve(c, f32, n_col, *opts, sh, R, P, AP, (cx<double>*)c->xs.p, (cx<double>*)c->ps.p, dpsi_opt != nullptr, (double*)c->shift.p, st,
+                              (int*)c->maps.p, &iters, &n_h);
+            if (rc) return rc;
             if (stats) CK(cudaEventRecord(ev[2], c->st));
             for (int w = 0; w < n_freq; ++w) {
                 cx<double>* Xw = (cx<double>*)c->xs.p + (size_t)w * per;
@@ -1641,7 +1793,11 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             CK(cudaMemcpyAsync(h, rep, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
             CK(cudaMemcpyAsync(c->h_pinned + 16, st.counters + 2, sizeof(long long), cudaMemcpyDeviceToHost, c->st));
             CK(cudaStreamSynchronize(c->st));
-            if (stats) stats->n_shift_updates += *reinterpret_cast<long long*>(c->h_pinned + 16);
+            if (stats) {
+                if (plan.H > 0) stats->n_hist_passes += *reinterpret_cast<long long*>(c->h_pinned + 16);
+                else stats->n_shift_updates += *reinterpret_cast<long long*>(c->h_pinned + 16);
+                stats->ms_history_slots = plan.H;
+            }
             if (h[1] > 0) ret = WEST_NOTCONVERGED;
             if (stats) {
                 add_times();
@@ -1723,6 +1879,7 @@ extern "C" size_t west_workspace_bytes(const west_ctx* c, int32_t op, int32_t n_
         case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert, f32).total();
         case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert, f32).total();
         case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32).total();
+        case WEST_OP_CHI0_MULTISHIFT_HIST: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32, wcg::MSH_HMAX, true).total();
         case WEST_OP_CHI0_BLOCK: return chi0_plan(c, 2, 1, std::max(1, n_freq), n_pert, f32).total();
         case WEST_OP_LANCZOS: return plan_lanczos(c, n_pert, std::max(1, n_freq), f32);
     }
@@ -1955,5 +2112,60 @@ extern "C" int west_fft3d_static(west_ctx* c, int32_t dir, int32_t n_batch, cons
         CK(cudaGetLastError());
         c->launches += 3;
     }
+    return WEST_OK;
+}
+
+// ============================================================================================================ FP64 pipe yardstick
+// Do DMMA (mma.sync m8n8k4 f64) and DFMA run on separate pipes of an sm_100a SM?  One CTA of 16 warps per SM: the first n_dmma_warps
+// issue dependent-free DMMA chains, the others DFMA chains (mode bit 0: DMMA warps active, bit 1: DFMA warps active).  bench.py --op pipes
+// times the three modes; DESIGN.md section 10 states the result (one shared pipe: the mixed rate never exceeds either alone).
+namespace {
+__global__ void __launch_bounds__(512, 1) fp64_pipe_probe(int mode, int n_dmma_warps, int iters, double* out) {
+    constexpr int NACC = 8;
+    const int warp = threadIdx.x >> 5;
+    const double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+    double acc[NACC][2];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i][0] = acc[i][1] = 0.0;
+    if (warp < n_dmma_warps) {
+        if (mode & 1)
+            for (int it = 0; it < iters; ++it) {
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) wgemm::dmma(acc[i][0], acc[i][1], a, b);
+            }
+    } else if (mode & 2) {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) { acc[i][0] = fma(a, b, acc[i][0]); acc[i][1] = fma(b, a, acc[i][1]); }
+        }
+    }
+    double sum = 0;
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) sum += acc[i][0] + acc[i][1];
+    if (sum == 12345.678) out[0] = sum;          // keeps the chains alive
+}
+}  // namespace
+extern "C" int west_probe_fp64_pipes(west_ctx* c, int32_t mode, int32_t n_dmma_warps, int32_t iters, float* ms_host, double* dmma_flop_host, double* dfma_flop_host) {
+    if (!c || mode < 1 || mode > 3 || n_dmma_warps < 0 || n_dmma_warps > 16 || iters < 1 || !ms_host) return fail(c, WEST_EINVAL, "west_probe_fp64_pipes: bad argument");
+    int rc = hot_begin(c, al256(256));
+    if (rc) return rc;
+    if ((rc = hot(c, c->misc, 256))) return rc;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    fp64_pipe_probe<<<148, 512, 0, c->st>>>(mode, n_dmma_warps, iters, (double*)c->misc.p);       // warm-up
+    cudaEventRecord(e0, c->st);
+    fp64_pipe_probe<<<148, 512, 0, c->st>>>(mode, n_dmma_warps, iters, (double*)c->misc.p);
+    cudaEventRecord(e1, c->st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms_host, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    CK(e);
+    CK(cudaGetLastError());
+    c->launches += 2;
+    // one DMMA m8n8k4 = 512 flop per warp instruction; one DFMA warp instruction = 64 flop; 8 accumulator pairs per iteration (DFMA: x4)
+    if (dmma_flop_host) *dmma_flop_host = (mode & 1) ? 148.0 * n_dmma_warps * (double)iters * 8 * 512.0 : 0.0;
+    if (dfma_flop_host) *dfma_flop_host = (mode & 2) ? 148.0 * (16 - n_dmma_warps) * (double)iters * 8 * 4 * 64.0 : 0.0;
     return WEST_OK;
 }

@@ -11,22 +11,23 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-9
 
 
-def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500, n_defl=0, cg_kernel=0):
+def _run(name, precision=None, tol_cg=1e-12, alpha=None, precond=1, solver=0, omegas=None, max_iter=500, n_defl=0, cg_kernel=0, ms_history=0, want_dpsi=True):
     import torch
     import paper_2203_05623_b200 as wb
     p = oracle_problem.build(name)
     w, sel = make_west(p)
     w.set_cg_kernel(cg_kernel)
+    w.set_ms_history(ms_history)
     if n_defl:
         w.set_deflation(torch.from_numpy(np.ascontiguousarray(p.U[:, p.n_occ:p.n_occ + n_defl].T[:, sel])).cuda(), p.eps[p.n_occ:p.n_occ + n_defl])
     dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
     prec = wb.WEST_FP64 if precision is None else precision
     om = p.omegas if omegas is None else omegas
     dn, dpsi, st = w.chi0_apply(dV, om, tol=tol_cg, max_iter=max_iter, alpha_pv=p.alpha if alpha is None else alpha,
-                                precond=precond, precision=prec, want_dpsi=True, n_occ=p.n_occ, solver=solver)
+                                precond=precond, precision=prec, want_dpsi=want_dpsi, n_occ=p.n_occ, solver=solver)
     ref_dn, ref_dpsi = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, p.dV, om, p.miller, p.L, p.N, return_dpsi=True)
     w.close()
-    return p, sel, dn.cpu().numpy(), dpsi.cpu().numpy(), st, ref_dn, ref_dpsi
+    return p, sel, dn.cpu().numpy(), dpsi.cpu().numpy() if want_dpsi else None, st, ref_dn, ref_dpsi
 
 
 def _check_dpsi(p, sel, dpsi, ref_dpsi, tol):
@@ -96,6 +97,37 @@ def test_chi0_multishift_all_frequencies_from_one_krylov_sequence():
     _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
     # one H*psi per column and iteration serves all four frequencies
     assert st["n_h_apply"] <= st["iters"] * p.n_occ * len(p.dV)
+
+
+@pytest.mark.parametrize("slots", [-1, 2, 3, 7, 32, 128])
+@pytest.mark.parametrize("want_dpsi", [True, False])
+def test_chi0_multishift_krylov_history_and_per_shift_recurrences_agree(slots, want_dpsi):
+    """west_set_ms_history: the shifted solutions contracted from a ring of seed residuals (ring sizes that wrap after every iteration,
+    every second, every sixth, a few times, never) and the per-shift vector recurrences (-1) all reach the sum over states (Eq. 10-11
+    with the i omega shift) within the same 1e-9, with the same iteration count; the carry vectors of a wrapping
+    ring and the Re-only contraction (no dpsi requested) are covered."""
+    omegas = [0.0, 0.05, 0.6947, 5.0]
+    p, sel, dn, dpsi, st, ref_dn, ref_dpsi = _run("mini3", solver=1, omegas=omegas, max_iter=2000, ms_history=slots, want_dpsi=want_dpsi)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    assert st["ms_history_slots"] == (0 if slots < 0 else slots)
+    for w in range(len(omegas)):
+        assert relmax(dn[w], ref_dn[w]) < TOL
+    if want_dpsi:
+        _check_dpsi(p, sel, dpsi, ref_dpsi, TOL)
+    _, _, dn0, _, st0, _, _ = _run("mini3", solver=1, omegas=omegas, max_iter=2000, ms_history=-1, want_dpsi=False)
+    assert st0["iters"] == st["iters"] and st0["n_h_apply"] == st["n_h_apply"]
+    assert relmax(dn, dn0) < 1e-11
+    assert (st["n_hist_passes"] > 0) == (slots >= 0) and (st["n_shift_updates"] > 0) == (slots < 0)
+
+
+def test_chi0_multishift_history_hits_the_iteration_cap_cleanly():
+    """max_iter below convergence: WEST_NOTCONVERGED, partial sums written (finite), the ring sized by max_iter + 1."""
+    import paper_2203_05623_b200 as wb
+    p, sel, dn, _, st, ref_dn, _ = _run("mini3", solver=1, omegas=[0.0, 0.5], max_iter=9, want_dpsi=False)
+    assert st["rc"] == wb.WEST_NOTCONVERGED and st["n_unconverged"] > 0 and st["iters"] == 9 and st["ms_history_slots"] == 10
+    assert np.all(np.isfinite(dn))
+    _, _, dn0, _, st0, _, _ = _run("mini3", solver=1, omegas=[0.0, 0.5], max_iter=9, want_dpsi=False, ms_history=-1)
+    assert relmax(dn, dn0) < 1e-11
 
 
 @pytest.mark.parametrize("name,solver,omegas", [("cfg1", 0, None), ("mini2", 0, None), ("mini3", 0, None), ("mini3", 1, [0.0, 0.05, 5.0])])
