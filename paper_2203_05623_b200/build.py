@@ -20,8 +20,9 @@ LIB = os.path.join(HERE, "libwest.so")
 # CU = stick units per CTA of the z kernels (2 * CU * max(N1, N2) <= 256 threads)
 # ZMINB = resident CTAs per SM the z-stick kernels are compiled for
 # ZNT = threads per CTA of the z-stick kernels (2 * CU * max(N1, N2) <= ZNT)
+# N = 144: four resident CTAs of 9 units instead of two of 10 (K1 3.67 -> 2.60 ms, K3 4.05 -> 3.32 ms per 1024 slots; sweep in profiles/r02_z_kernel_shapes.md)
 FFT_SIZES = [(4, 6, 24, 4, 4, 20, 4, 256), (6, 6, 36, 4, 4, 20, 4, 256), (6, 8, 48, 6, 3, 16, 4, 256), (8, 9, 72, 12, 2, 14, 4, 256),
-             (12, 12, 144, 12, 1, 10, 2, 256)]
+             (12, 12, 144, 12, 1, 9, 4, 224)]
 K2H_SHAPES = {72: tuple(int(x) for x in os.environ.get("WEST_K2H_72", "6,3,2,1").split(",")),
               144: tuple(int(x) for x in os.environ.get("WEST_K2H_144", "12,1,1,1").split(","))}
 # measured alternatives of the z-stick kernels' shape: WEST_Z_<N>="CU,ZMINB,ZNT" overrides the table entry of grid size N
@@ -30,6 +31,8 @@ for _i, _t in enumerate(FFT_SIZES):
     if _v:
         _cu, _zminb, _znt = (int(x) for x in _v.split(","))
         FFT_SIZES[_i] = _t[:5] + (_cu, _zminb, _znt)
+# FP32 variant of the H*psi plane kernel (WEST_MIXED): (warps per CTA, resident CTAs per SM); absent = the FP64 shape
+K2H32_SHAPES = {n: tuple(int(x) for x in os.environ["WEST_K2H32_%d" % n].split(",")) for n in (72, 144) if os.environ.get("WEST_K2H32_%d" % n)}
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
@@ -73,6 +76,9 @@ def build(force=False, verbose=False):
         # other N: the one-way variants' shape.  Measured alternatives: profiles/r02_k2_ilp.md
         k2h = K2H_SHAPES.get(n)
         extra = ["-DWEST_NW_H=%d" % k2h[0], "-DWEST_MINB_H=%d" % k2h[1], "-DWEST_GW_H=%d" % k2h[2], "-DWEST_NB_H=%d" % k2h[3]] if k2h else []
+        k2h32 = K2H32_SHAPES.get(n)
+        if k2h32:
+            extra += ["-DWEST_NW_H32=%d" % k2h32[0], "-DWEST_MINB_H32=%d" % k2h32[1]]
         jobs.append((o, [nvcc] + NVCC_FLAGS + extra + ["-DWEST_N1=%d" % n1, "-DWEST_N2=%d" % n2, "-DWEST_NN=%d" % n, "-DWEST_NW=%d" % nw, "-DWEST_MINB=%d" % minb, "-DWEST_CU=%d" % cu, "-DWEST_ZMINB=%d" % zminb, "-DWEST_ZNT=%d" % znt,
                                                "-c", os.path.join(CSRC, "fft_n.cu"), "-o", o]))
     o = os.path.join(OBJ, "fft_dense.o")

@@ -16,6 +16,10 @@
 #define WEST_NW_H WEST_NW
 #define WEST_MINB_H WEST_MINB
 #endif
+#ifndef WEST_NW_H32         // shape of the FP32 H*psi plane kernel (WEST_MIXED): half the shared memory per CTA, so more CTAs fit
+#define WEST_NW_H32 WEST_NW_H
+#define WEST_MINB_H32 WEST_MINB_H
+#endif
 #ifndef WEST_GW_H
 #define WEST_GW_H 1         // warps per line group of the H*psi plane kernel (2 = warp pairs)
 #endif
@@ -59,8 +63,8 @@ cudaError_t k3_t(int n_slots, cudaStream_t st, const WestGeom& g, VecMap vm, con
 template <typename T, int MODE>
 cudaError_t k2_t(int n_slots, cudaStream_t st, const WestGeom& g, const K2Any& a) {
     // the H*psi variant may use a different CTA shape from the one-way variants (store / dn / load)
-    constexpr int NWm = MODE == K2_H ? WEST_NW_H : NW;
-    constexpr int MBm = MODE == K2_H ? WEST_MINB_H : WEST_MINB;
+    constexpr int NWm = MODE == K2_H ? (sizeof(T) == 4 ? WEST_NW_H32 : WEST_NW_H) : NW;
+    constexpr int MBm = MODE == K2_H ? (sizeof(T) == 4 ? WEST_MINB_H32 : WEST_MINB_H) : WEST_MINB;
     constexpr int GWm = MODE == K2_H ? WEST_GW_H : 1;
     constexpr int NBm = MODE == K2_H ? WEST_NB_H : 1;
     constexpr int LPG = K2Cfg<N1, N2, GWm, NBm>::LPW;

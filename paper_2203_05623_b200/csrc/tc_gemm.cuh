@@ -15,7 +15,9 @@
 //          rows / k beyond the arrays read as zero (TMA out-of-bounds fill)
 //   out  : FP64, out[c * ldo + r] (r contiguous: lanes of a warp = consecutive r, so stores and atomics coalesce)
 //          ATOMIC: out += D by atomicAdd (split-K partial sums)      else: out += D (each element owned by one CTA)
-// Warp roles: warps 0-3 epilogue (TMEM lane quarter = warp id), warp 4 TMA producer (one lane), warp 5 MMA issuer (one lane) + TMEM owner.
+// Warp roles: warps 0-7 epilogue (TMEM lane quarter = warp id mod 4, column half = warp id / 4: eight warps keep twice the global loads of
+// the read-modify-write epilogue in flight and halve the drain time of a chunk), warp 8 TMA producer (one lane), warp 9 MMA issuer (one lane) +
+// TMEM owner.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -25,7 +27,7 @@ namespace wtc {
 
 constexpr int BM = 128, BN = 128, BK = 32;          // BK fp32 = 128 bytes = one swizzle row
 constexpr int STAGES = 3, CHUNK_KB = 4;             // k-blocks per TMEM chunk: 4 x (32 / 8) x 3 = 48 accumulations
-constexpr int NTHREADS = 192;
+constexpr int NTHREADS = 320, EPI_WARPS = 8, EPI_COLS = BN / 2;      // columns per epilogue warp
 constexpr uint32_t TILE_BYTES = BM * BK * 4;        // 16 KB per operand part (BM == BN)
 constexpr uint32_t STAGE_BYTES = 4 * TILE_BYTES;    // A hi, A lo, B hi, B lo
 constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */;
@@ -103,10 +105,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(acc_full + b, 1); mbar_init(acc_empty + b, 4); }
+        for (int b = 0; b < 2; ++b) { mbar_init(acc_full + b, 1); mbar_init(acc_empty + b, EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 5) {                          // TMEM owner: allocate 2 x BN columns, publish the base address
+    if (warp == EPI_WARPS + 1) {              // TMEM owner: allocate 2 x BN columns, publish the base address
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(TMEM_COLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -125,7 +127,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
         if (nkb < 0) nkb = 0;
     };
 
-    if (warp == 4) {
+    if (warp == EPI_WARPS) {
         // ===== TMA producer =====
         if (lane == 0) {
             int it = 0;                                                    // k-blocks issued so far (all tiles)
@@ -145,7 +147,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
                 }
             }
         }
-    } else if (warp == 5) {
+    } else if (warp == EPI_WARPS + 1) {
         // ===== MMA issuer =====
         if (lane == 0) {
             int it = 0, g = 0;                                             // k-blocks consumed, chunks started (all tiles)
@@ -180,23 +182,24 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
             }
         }
     } else {
-        // ===== epilogue warps 0-3: TMEM lane quarter `warp`, row r = r0 + 32 warp + lane =====
+        // ===== epilogue warps 0-7: TMEM lane quarter lq = warp & 3 (row r = r0 + 32 lq + lane), columns [ch0, ch0 + EPI_COLS) =====
+        const int lq = warp & 3, ch0 = (warp >> 2) * EPI_COLS;
         int g = 0;
         for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
             int r0, c0, kb0, nkb, bt;
             tile_of(t, r0, c0, kb0, nkb, bt);
             const int n_chunks = (nkb + CHUNK_KB - 1) / CHUNK_KB;
-            float acc[BN];
+            float acc[EPI_COLS];
 #pragma unroll
-            for (int j = 0; j < BN; ++j) acc[j] = 0.f;
+            for (int j = 0; j < EPI_COLS; ++j) acc[j] = 0.f;
             for (int ch = 0; ch < n_chunks; ++ch, ++g) {
                 const int buf = g & 1;
                 mbar_wait(acc_full + buf, (g >> 1) & 1);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-                for (int q = 0; q < BN / 32; ++q) {
+                for (int q = 0; q < EPI_COLS / 32; ++q) {
                     uint32_t v[32];
-                    tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(buf * BN + q * 32), v);
+                    tmem_ld32(tmem + ((uint32_t)(lq * 32) << 16) + (uint32_t)(buf * BN + ch0 + q * 32), v);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
                     for (int j = 0; j < 32; ++j) acc[q * 32 + j] += __uint_as_float(v[j]);
@@ -205,27 +208,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
                 __syncwarp();
                 if (lane == 0) mbar_arrive(acc_empty + buf);
             }
-            const int r = r0 + warp * 32 + lane;
+            const int r = r0 + lq * 32 + lane;
             double* outb = out + (long long)bt * tg.out_batch_stride;
             if (r < rows_a && n_chunks > 0) {
                 if (ATOMIC) {
 #pragma unroll
-                    for (int j = 0; j < BN; ++j)
-                        if (c0 + j < rows_b) atomicAdd(outb + (long long)(c0 + j) * ldo + r, (double)acc[j]);
+                    for (int j = 0; j < EPI_COLS; ++j)
+                        if (c0 + ch0 + j < rows_b) atomicAdd(outb + (long long)(c0 + ch0 + j) * ldo + r, (double)acc[j]);
                 } else {
                     // read-modify-write in groups of 16 columns: all loads of a group are in flight before the first add (one memory
                     // latency per group instead of one per element)
 #pragma unroll
-                    for (int q = 0; q < BN / 16; ++q) {
+                    for (int q = 0; q < EPI_COLS / 16; ++q) {
                         double old[16];
 #pragma unroll
                         for (int j = 0; j < 16; ++j) {
-                            const int cc = c0 + q * 16 + j;
+                            const int cc = c0 + ch0 + q * 16 + j;
                             old[j] = cc < rows_b ? __ldcg(outb + (long long)cc * ldo + r) : 0.0;
                         }
 #pragma unroll
                         for (int j = 0; j < 16; ++j) {
-                            const int cc = c0 + q * 16 + j;
+                            const int cc = c0 + ch0 + q * 16 + j;
                             if (cc < rows_b) __stcg(outb + (long long)cc * ldo + r, old[j] + (double)acc[q * 16 + j]);
                         }
                     }
@@ -235,7 +238,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) tf32x3_gemm(const __grid_constant
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 5) {
+    if (warp == EPI_WARPS + 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS) : "memory");
     }

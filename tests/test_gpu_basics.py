@@ -146,3 +146,21 @@ def test_full_sphere_mode_on_the_large_grids(name, with_kb):
     ref = oham.apply_h(c, p.miller, p.L, p.N, p.vloc, p.beta if with_kb else None, p.dcoef if with_kb else None)
     assert relmax(y, ref) < TOL
     w.close()
+
+
+def test_fp64_pipe_yardstick_runs_and_shows_one_shared_pipe():
+    """west_probe_fp64_pipes: DMMA-only, DFMA-only and mixed launches all finish, report the flop counts west.h
+    states, and the mixed rate does not exceed the better single-kind rate by more than 10 % - DMMA and DFMA share one pipe on B200."""
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build("cfg1")
+    w = wb.West(p.L, p.n2max, p.N, wb.WEST_FULL)
+    rate = {}
+    for mode, nd in ((1, 16), (2, 0), (3, 8)):
+        ms, fd, ff = w.probe_fp64_pipes(mode, nd, iters=4000)
+        assert ms > 0
+        assert fd == ((148.0 * nd * 4000 * 8 * 512) if mode & 1 else 0.0) and ff == ((148.0 * (16 - nd) * 4000 * 8 * 4 * 64) if mode & 2 else 0.0)
+        rate[mode] = (fd + ff) / ms
+    assert rate[3] < 1.10 * max(rate[1], rate[2])
+    with pytest.raises(wb.WestError):
+        w.probe_fp64_pipes(0, 8)
+    w.close()
