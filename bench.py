@@ -35,6 +35,8 @@ sys.path.insert(0, ROOT)
 TOL = 1e-8          # CG stopping tolerance of the throughput runs (reading R5)
 MAX_ITER = 300
 SUB_STEPS, SUB_WARMUP = 3, 1     # timed / warm-up steps of every sub-record (the kernels are warm from the headline by then)
+T_START = time.time()
+SUB_DEADLINE_S = 1400.0          # a sub-record is skipped (and says so) if the run has already taken this long: the line must still be printed
 
 
 def parse():
@@ -353,7 +355,7 @@ def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g
     fp64_src = "measured in this run: cuBLAS DGEMM 8192^3 FP64 (DMMA and the FP64 FMA pipe have the same nominal rate on B200, 37.2 TFLOP/s)"
     out = {"kernel": top, "avg_launch_ms": prof[top]["ms"] / spans, "launches": spans, "traffic": None}
     table = ncu_traffic_table()
-    tkey = ("cg_vec_ms" if (top == "cg_vec" and solver == 1) else top, N, "mixed" if mixed else "fp64")
+    tkey = ((("cg_vec_msh" if hist_passes > 0 else "cg_vec_ms") if (top == "cg_vec" and solver == 1) else top), N, "mixed" if mixed else "fp64")
     rows = cfg["n_proj"] + cfg["n_occ"]
     if not gamma:
         rows *= 2
@@ -720,7 +722,11 @@ def main():
     # ---- sub-records: the other configs of BASELINE.json on the same driver clock (default workload, one GPU only)
     if a.workload == "cfg5" and a.omegas == "default" and world == 1 and not a.no_sub:
         subs = {}
+        late = lambda: time.time() - T_START > SUB_DEADLINE_S
+        skipped = {"skipped": "time budget of the run (%d s) reached before this sub-record" % SUB_DEADLINE_S}
         try:
+            if late():
+                raise TimeoutError(skipped["skipped"])
             om_iw = [x for x in cfg["omegas"] if x > 0]
             r = run_chi0(a, wb, cfg, w, dV_np, alpha, aux, om_iw, 1 if a.solver < 0 else a.solver, precision, 1, 0, local, world, barrier, 0,
                          want_cpu=0 if a.no_cpu_baseline else 1, label="cfg5 imaginary frequencies", profile_in_timed=True)
@@ -736,6 +742,9 @@ def main():
             w2, dV2, alpha2, aux2 = setup_gpu(c4, c4["n_pert"], a.chunk, verbose=True, alpha_factor=a.alpha_factor)
             w2.set_ms_history(a.ms_history)
             for name in ("cfg2", "cfg3", "cfg4"):
+                if late():
+                    subs[name] = dict(skipped)
+                    continue
                 try:
                     c = synth.get_config(name)
                     om = omegas_for(a, c, name)
@@ -751,6 +760,8 @@ def main():
             # Exact (DESIGN 6e); it lifts the lower end of the UNPRECONDITIONED multi-shift operator's spectrum, which is what sets its
             # iteration count.  A separate record: BASELINE's cfg3 is the plain one above.
             try:
+                if late():
+                    raise TimeoutError(skipped["skipped"])
                 c3 = synth.get_config("cfg3")
                 w3, dV3, alpha3, aux3 = setup_gpu(c3, c3["n_pert"], a.chunk, verbose=True, n_defl=128, alpha_factor=a.alpha_factor)
                 w3.set_ms_history(a.ms_history)

@@ -138,3 +138,35 @@ def test_stats_free_call_reports_non_convergence():
     _, _, st = w.chi0_apply(dV, [0.0], tol=1e-12, max_iter=500, alpha_pv=p.alpha, want_stats=False)
     assert st["rc"] == 0
     w.close()
+
+
+def test_multishift_history_workspace_sizes():
+    """WEST_OP_CHI0_MULTISHIFT_HIST is the size that holds the full 128-slot Krylov ring for the whole block; WEST_OP_CHI0_MULTISHIFT (the
+    minimum) still runs - as sub-blocks or with the per-shift recurrences - and both give the sum over states; no allocation in either."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    B = wb.binding
+    p = oracle_problem.build("mini3")
+    w, sel = make_west(p)
+    omegas = [0.0, 0.05, 5.0]
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
+    n_pert = dV.shape[0]
+    ref = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, p.dV, omegas, p.miller, p.L, p.N)
+    big = w.workspace_bytes(B.WEST_OP_CHI0_MULTISHIFT_HIST, n_pert, len(omegas))
+    small = w.workspace_bytes(B.WEST_OP_CHI0_MULTISHIFT, n_pert, len(omegas))
+    assert big > small > 0
+    dn = torch.empty((len(omegas), n_pert, p.N, p.N, p.N), dtype=torch.float64, device="cuda")
+    for need, slots in ((big, 128), (small, None)):
+        ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        w.set_workspace(ws)
+        kw = dict(tol=1e-12, max_iter=3000, alpha_pv=p.alpha, solver=1, dn=dn)
+        w.chi0_apply(dV, omegas, **kw)
+        held, f0 = w.device_bytes(), _free_bytes()
+        _, _, st = w.chi0_apply(dV, omegas, **kw)
+        assert _free_bytes() == f0 and w.device_bytes() == held
+        assert st["rc"] == 0 and st["n_unconverged"] == 0
+        if slots is not None:
+            assert st["ms_history_slots"] == slots and st["n_sub_blocks"] == 1
+        assert relmax(dn.cpu().numpy(), ref) < 1e-9
+        w.set_workspace(None)
+    w.close()
