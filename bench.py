@@ -58,7 +58,7 @@ def parse():
                     help="chi0 = the hot path (default); happly = west_h_apply alone (H*psi/s, kernel classes); gemm = the projector GEMM shapes "
                          "against cuBLAS; lanczos = Eq. 15-19 chains; pdep = Davidson shell for chi0bar; fft = the dense C2C FFT of Fig. 3 "
                          "(--workload fft128 | fft256, --precision); spin = N_spin = 2 chi0 (widening rows)")
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"], help="--op fft: fp64 | fp32; --op happly / gemm: fp64 | mixed")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed", "i8"], help="--op fft: fp64 | fp32; --op happly / gemm: fp64 | mixed | i8 (FP64 from int8 slices, WEST_FP64_I8); --op chi0: i8 overrides the workload's precision")
     ap.add_argument("--n-vec", type=int, default=0, help="--op happly / gemm: number of vectors (0 = the workload's CG-loop width)")
     ap.add_argument("--deflate", type=int, default=0, help="number of conduction eigenstates handed to west_set_deflation (0 = off)")
     ap.add_argument("--n-pert", type=int, default=0, help="override the perturbation count (0 = the config's)")
@@ -342,7 +342,7 @@ def measure_fp64_peak():
     return _FP64_PEAK["v"]
 
 
-def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g, fp64_peak, shift_updates=0, hist_passes=0):
+def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g, fp64_peak, shift_updates=0, hist_passes=0, i8=False):
     """Roofline entry for the kernel class that took the most time in the profiled step (DESIGN.md section 6 states the per-unit
     figures).  n_h = vectors pushed through H in that step."""
     N = cfg["N"]
@@ -355,7 +355,7 @@ def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g
     fp64_src = "measured in this run: cuBLAS DGEMM 8192^3 FP64 (DMMA and the FP64 FMA pipe have the same nominal rate on B200, 37.2 TFLOP/s)"
     out = {"kernel": top, "avg_launch_ms": prof[top]["ms"] / spans, "launches": spans, "traffic": None}
     table = ncu_traffic_table()
-    tkey = ((("cg_vec_msh" if hist_passes > 0 else "cg_vec_ms") if (top == "cg_vec" and solver == 1) else top), N, "mixed" if mixed else "fp64")
+    tkey = ((("cg_vec_msh" if hist_passes > 0 else "cg_vec_ms") if (top == "cg_vec" and solver == 1) else top), N, "mixed" if mixed else ("i8" if (i8 and top.startswith("gemm")) else "fp64"))
     rows = cfg["n_proj"] + cfg["n_occ"]
     if not gamma:
         rows *= 2
@@ -394,6 +394,16 @@ def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g
                     "algorithmic_flops_per_vector": 2.0 * rows * 2 * n_g,
                     "algorithmic_bytes_per_vector": (1 if top == "gemm_tn" else 2) * 2 * n_g * 8,
                     "note": "FP64 DMMA (mma.sync m8n8k4; tcgen05 has no FP64 kind)" if not mixed else "3xTF32 products, FP64 operands in memory; peak shown is the FP64 one"})
+        if i8:
+            # WEST_FP64_I8: the contraction runs as 36 int8 slice-pair products per FP64 product (8 slices, pairs with i + j <= 7) on the INT8
+            # tensor path; its roofline is the int8 tensor peak = the measured dense bf16 rate x the nominal ratio 2 (B200_PROFILING.md)
+            p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+            bf16 = float(json.load(open(p)).get("bf16_tflops_sustained", 1370.0)) if os.path.exists(p) else 1370.0
+            ops = 36.0 * flops
+            out.update({"bound": "tensor", "achieved": ops / t / 1e12, "peak": 2.0 * bf16, "unit": "TFLOP/s", "frac": ops / t / 1e12 / (2.0 * bf16),
+                        "peak_source": "int8 tensor: 2 x the sustained dense bf16 rate of MEASURED_PEAKS.json (else 2 x 1370)", "fp64_equivalent_tflops": ach,
+                        "note": "tcgen05.mma kind::i8: 36 exact int8 slice-pair products per FP64 product, int32 accumulation in TMEM, FP64 sums; the class time "
+                                "includes the per-call slicing of the vector / coefficient block; `achieved` counts int8 operations"})
         units = n_h
     else:
         # CG vector kernel.  PCG/COCG column-resident or streaming: 4 reads + 3 writes of a column per iteration (p, Ap, x, r | x, r, p).
@@ -541,7 +551,7 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
     gemm_tf = 2 * 2.0 * rows * (2 * w.n_g) * n_h_prof / t_gemm / 1e12 if t_gemm > 0 else None
     rec = {
         "value": units * steps / (ms * 1e-3), "unit": "perturbations/s", "steps": steps, "warmup": warmup, "ms_per_step": ms / steps,
-        "dtype": "f64" if not mixed else "f32 FFT + 3xTF32 GEMMs inside H*psi / f64 vectors, dots, dn",
+        "dtype": ("f64" if precision != wb.WEST_FP64_I8 else "f64 (projector GEMMs inside H*psi: exact int8-slice products on tcgen05 kind::i8, FP64 sums)") if not mixed else "f32 FFT + 3xTF32 GEMMs inside H*psi / f64 vectors, dots, dn",
         "config": {"workload": label, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": n_freq, "omega_ry": [round(x, 6) for x in omegas],
                    "n_proj": cfg["n_proj"], "n_deflated": a.deflate, "alpha_pv": "per-orbital (eps_v - eps_1) + W/2" if alpha <= 0 else alpha, "tol": TOL,
                    "solver": {0: "PCG/COCG per frequency", 1: "multi-shift CG", 2: "block CG"}[solver], "ms_history_slots": stats.get("ms_history_slots", 0), "cg_iters": stats["iters"], "cg_iters_min": stats["iters_min"],
@@ -550,9 +560,10 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
                    "l2": "inputs per step (vector sets, %.1f GB) exceed the 126 MB L2" % (4 * 16 * w.n_g * n_pert * cfg["n_occ"] / 1e9)},
         "h_apply_per_s": n_h * world / (ms * 1e-3), "h_apply_per_step": n_h / steps,
         "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": roofline(cfg, top, prof, n_h_prof, n_freq, solver, hbm_peak, peak_src, mixed, w.n_g, fp64_peak, pst.get("n_shift_updates", 0), pst.get("n_hist_passes", 0)),
+        "roofline": roofline(cfg, top, prof, n_h_prof, n_freq, solver, hbm_peak, peak_src, mixed, w.n_g, fp64_peak, pst.get("n_shift_updates", 0), pst.get("n_hist_passes", 0), precision == wb.WEST_FP64_I8),
         "gemm": {"achieved_tflops": gemm_tf, "peak_tflops": fp64_peak, "frac": (gemm_tf / fp64_peak) if gemm_tf else None,
-                 "note": "KB + P_v GEMMs of the CG loop in the profiled step (RHS projection excluded from the flop count)"},
+                 "note": "KB + P_v GEMMs of the CG loop in the profiled step (RHS projection excluded from the flop count)" +
+                         ("; FP64-EQUIVALENT rate of the int8-slice products against the FP64 peak (may exceed 1)" if precision == wb.WEST_FP64_I8 else "")},
         "kernel_ms_per_step": {k: round(v["ms"], 3) for k, v in prof.items() if v["spans"]},
         "kernel_ms_note": "CUDA events around every launch of the timed step(s)" if profile_in_timed else "one extra untimed step with CUDA events around every launch; the timed steps run without them",
         "phase_ms_last_step": {"rhs": stats["ms_rhs"], "cg": stats["ms_cg"], "dn": stats["ms_dn"]},
@@ -660,6 +671,8 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import paper_2203_05623_b200 as wb
     precision = wb.WEST_MIXED if cfg["precision"] == "mixed" else wb.WEST_FP64
+    if a.precision == "i8" and precision == wb.WEST_FP64:
+        precision = wb.WEST_FP64_I8
 
     def barrier():
         if world > 1:
@@ -724,6 +737,16 @@ def main():
         subs = {}
         late = lambda: time.time() - T_START > SUB_DEADLINE_S
         skipped = {"skipped": "time budget of the run (%d s) reached before this sub-record" % SUB_DEADLINE_S}
+        if precision == wb.WEST_FP64:
+            # the headline workload once more with WEST_FP64_I8: the projector GEMMs as exact int8-slice products on tcgen05 kind::i8
+            # (DESIGN.md section 6j).  Same inputs, same tolerance, same parity sample; a separate record because its dtype statement differs.
+            try:
+                if late():
+                    raise TimeoutError(skipped["skipped"])
+                subs["cfg5_i8"] = run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, wb.WEST_FP64_I8, SUB_STEPS, SUB_WARMUP, local, world, barrier, 0,
+                                           want_cpu=0 if a.no_cpu_baseline else 1, label="cfg5, projector GEMMs from int8 slices (WEST_FP64_I8)")
+            except Exception as e:
+                subs["cfg5_i8"] = {"error": repr(e)[:300]}
         try:
             if late():
                 raise TimeoutError(skipped["skipped"])
@@ -796,7 +819,7 @@ def bench_kernels(a, wb, cfg, rank, world, barrier):
     n_vec = a.n_vec or cfg.get("pert_batch", cfg["n_pert"]) * cfg["n_occ"]
     rows = (cfg["n_proj"] + cfg["n_occ"]) * (1 if mode == wb.WEST_GAMMA else 2)
     K = 2 * w.n_g
-    prec = wb.WEST_MIXED if a.precision == "mixed" else wb.WEST_FP64
+    prec = wb.WEST_MIXED if a.precision == "mixed" else (wb.WEST_FP64_I8 if a.precision == "i8" else wb.WEST_FP64)
     hbm_peak, peak_src = peaks()
     if a.op == "gemm":
         A = torch.randn(rows, K, dtype=torch.float64, device="cuda", generator=g)
@@ -861,7 +884,7 @@ def bench_kernels(a, wb, cfg, rank, world, barrier):
     fft_bytes = (4 * cfg["N"] * n_cols * csz + 3 * (2 if mode == wb.WEST_GAMMA else 1) * w.n_g * 16) * slots
     print(json.dumps({"metric": "H*psi applications/s (west_h_apply, KB projectors included)", "value": n_vec * world / (ms * 1e-3), "unit": "vectors/s", "n_gpus": world,
                       "steps": a.steps, "warmup": a.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                      "dtype": "f64" if prec == wb.WEST_FP64 else "f32 FFT + 3xTF32 GEMMs", "data": "synthetic (normal random vectors)",
+                      "dtype": {wb.WEST_FP64: "f64", wb.WEST_MIXED: "f32 FFT + 3xTF32 GEMMs", wb.WEST_FP64_I8: "f64 (projector GEMMs: exact int8-slice products on tcgen05 kind::i8, FP64 sums)"}[prec], "data": "synthetic (normal random vectors)",
                       "config": {"workload": a.workload, "op": "happly", "n_vec": n_vec, "N": cfg["N"], "n_g": w.n_g, "n_proj": cfg["n_proj"]},
                       "gpu_launches": int(launches), "kernel_ms_per_step": {k: round(v["ms"], 3) for k, v in prof.items() if v["spans"]},
                       "fft_path": {"ms": t_fft * 1e3, "algorithmic_gbs": fft_bytes / t_fft / 1e9, "frac_of_hbm": fft_bytes / t_fft / 1e9 / hbm_peak, "peak_source": peak_src,

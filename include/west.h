@@ -92,6 +92,12 @@ extern "C" {
                                         block (the fast variant; WEST_OP_CHI0_MULTISHIFT is the smallest comfortable size, and any block in
                                         between is used for as many ring slots as fit) */
 
+#define WEST_FP64_I8 3  /* west_h_apply / west_chi0_apply: everything in FP64 as WEST_FP64, except that the KB / P_v projector GEMMs inside H*psi form
+                           their FP64 products from error-free int8 slices on the INT8 tensor path (tcgen05 kind::i8, int32 accumulation in
+                           tensor memory; csrc/i8_gemm.cuh): every operand row is cut into 8 signed 7-bit slices below
+                           its own power-of-two scale (2^-56 of the row's largest element is dropped), slice pairs contract exactly in
+                           int32, the weight classes are summed in FP64.  Same parity bar as WEST_FP64 (1e-9); the RHS projection and the
+                           deflation update stay on DMMA.  Falls back to WEST_FP64 when the driver offers no tensor-map encoder. */
 #define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
 typedef struct west_ctx west_ctx;

@@ -16,7 +16,7 @@ WEST_OK, WEST_NOTCONVERGED = 0, 1
 WEST_EINVAL, WEST_ECUDA, WEST_ESTATE, WEST_ENOMEM, WEST_EWORKSPACE = -1, -2, -3, -4, -5
 WEST_OP_FFT3D, WEST_OP_H_APPLY, WEST_OP_CHI0, WEST_OP_CHI0_IW, WEST_OP_CHI0_MULTISHIFT, WEST_OP_LANCZOS, WEST_OP_CHI0_BLOCK, WEST_OP_CHI0_MULTISHIFT_HIST = 0, 1, 2, 3, 4, 5, 6, 7
 WEST_FULL, WEST_GAMMA = 0, 1
-WEST_FP64, WEST_MIXED, WEST_FP32 = 0, 1, 2
+WEST_FP64, WEST_MIXED, WEST_FP32, WEST_FP64_I8 = 0, 1, 2, 3
 
 
 class west_cell(C.Structure):

@@ -716,14 +716,20 @@ __global__ void __launch_bounds__(NTR, 1) ms_hist_step_resident(long long n_g, i
 // Contraction of one segment [j0, n) of the history for column blockIdx.x, elements [blockIdx.y * MSH_CHUNK, +MSH_CHUNK):
 //   XS[s][col] (Re part, and Im part if IMAG) += sum_j cx_j r_j + dx Q_s          QS[s][col] = sum_j cq_j r_j + dq Q_s   (CARRY_OUT)
 // carry_in = 0: Q_s is taken as zero (first segment) and never read.  Columns use only the iterations they took part in
-// (j < iters[col]); a column that left before j0 has nothing to add.  Dynamic shared memory: 2 * n_shift * (n - j0 + 1) double2.
+// (j < iters[col]); a column that left before j0 has nothing to add.  Carry vectors are formed only for the shifts that are still
+// live at the end of the segment (B_j0 != 0: a shift that froze inside it never reads its Q again), so a flush needs the x accumulators of
+// XG shifts and the carry accumulators of at most MSH_QG live shifts per pass over the history: one pass for up to 8 frequencies unless
+// more than four of a column's shifts are still live (then further carry-only passes).  Q of a dead shift is never written NOR read.
+// Dynamic shared memory: 2 * n_shift * (n - j0 + 1) double2.
 constexpr int MSH_CHUNK = 2048;
 constexpr int MSH_HMAX = 128;        // most ring slots (bounds the coefficient tables: 2 * 16 shifts * 129 double2 = 66 KB)
-// MSH_G = shifts per register group: every group re-reads the segment's history, so the plain final contraction (Re x_s only) takes 8
-template <bool IMAG, bool CARRY_OUT, int MSH_G>
+constexpr int MSH_QG = 4;            // carry accumulators (live shifts) per pass
+// XG = shifts whose x accumulators a pass holds: 8 for Re x_s only, 4 when Im x_s is wanted too (dpsi requested)
+template <bool IMAG, bool CARRY_OUT, int XG>
 __global__ void __launch_bounds__(NT) ms_hist_combine(long long n_g, int n_col, int n_shift, int j0, int n_end, int carry_in, MsHist hs,
                                                       const int* iters, double2* XS, double2* QS, unsigned long long* pass_counter) {
     extern __shared__ double2 msh_sm[];
+    __shared__ int s_qlist[MS_MAX_SHIFTS], s_nq, s_xin[MS_MAX_SHIFTS];
     const int col = blockIdx.x;
     const int jend = min(n_end, iters[col]);
     const int len = jend - j0;
@@ -753,33 +759,57 @@ __global__ void __launch_bounds__(NT) ms_hist_combine(long long n_g, int n_col, 
         }
         cx[s * L + L - 1] = w;                          // dx
         cq[s * L + L - 1] = bt;                         // dq
+        s_xin[s] = carry_in && (w.x != 0.0 || w.y != 0.0);                                        // x_s takes a contribution of the old carry
+        s_qlist[s] = (CARRY_OUT && jend == n_end && (bt.x != 0.0 || bt.y != 0.0)) ? 1 : 0;        // live at the end of the segment (flag, compacted below)
     }
     __syncthreads();
-    if (blockIdx.y == 0 && threadIdx.x == 0 && pass_counter) {
-        // column-vector passes (16 n_g bytes each) of this column's contraction: history reads once per shift group, x_s (and carry) traffic
-        const int groups = (n_shift + MSH_G - 1) / MSH_G;
-        unsigned long long passes = (unsigned long long)len * groups + (unsigned long long)n_shift * ((IMAG ? 4 : 2) + (carry_in ? 2 : 0) + (CARRY_OUT ? 2 : 0));
-        atomicAdd(pass_counter, passes);
+    if (threadIdx.x == 0) {
+        int nq = 0, nxin = 0;
+        for (int s = 0; s < n_shift; ++s) { const int live = s_qlist[s]; nxin += s_xin[s] || (live && carry_in); if (live) s_qlist[nq++] = s; }
+        s_nq = nq;
+        if (blockIdx.y == 0 && pass_counter) {
+            // column-vector passes (16 n_g bytes each) of this column's contraction: one history read per pass, x_s traffic, carry reads / writes
+            const int nxp = (n_shift + XG - 1) / XG, nqp = (nq + MSH_QG - 1) / MSH_QG;
+            const int P = nxp - 1 + max(1, nqp);
+            atomicAdd(pass_counter, (unsigned long long)len * P + (unsigned long long)n_shift * (IMAG ? 4 : 2) + 2ull * nxin + 2ull * nq);
+        }
     }
+    __syncthreads();
+    const int nq = s_nq;
+    const int nxp = (n_shift + XG - 1) / XG, nqp = (nq + MSH_QG - 1) / MSH_QG;
+    const int n_pass = nxp - 1 + max(1, nqp);           // the last x pass also takes the first carry group
     const long long g_lo = (long long)blockIdx.y * MSH_CHUNK, g_hi = min(n_g, g_lo + MSH_CHUNK);
-    for (int s0 = 0; s0 < n_shift; s0 += MSH_G) {
-        const int ns = min(MSH_G, n_shift - s0);
-        for (long long g = g_lo + threadIdx.x; g < g_hi; g += NT) {
-            double2 xr[MSH_G], xi[MSH_G], qr[MSH_G], qi[MSH_G];
+    for (int pass = 0; pass < n_pass; ++pass) {
+        const int s0 = pass * XG, nx = pass < nxp ? min(XG, n_shift - s0) : 0;
+        const int qg = pass - (nxp - 1), q0 = qg * MSH_QG, nqs = (CARRY_OUT && qg >= 0) ? max(0, min(MSH_QG, nq - q0)) : 0;
+        int qoff[MSH_QG];                                // coefficient rows of this pass's live shifts
 #pragma unroll
-            for (int q = 0; q < MSH_G; ++q) xr[q] = xi[q] = qr[q] = qi[q] = make_double2(0.0, 0.0);
+        for (int q = 0; q < MSH_QG; ++q) qoff[q] = (CARRY_OUT && q < nqs) ? s_qlist[q0 + q] : 0;
+        for (long long g = g_lo + threadIdx.x; g < g_hi; g += NT) {
+            double2 xr[XG], xi[IMAG ? XG : 1], qr[CARRY_OUT ? MSH_QG : 1], qi[CARRY_OUT ? MSH_QG : 1];
+#pragma unroll
+            for (int q = 0; q < XG; ++q) { xr[q] = make_double2(0.0, 0.0); if (IMAG) xi[q] = make_double2(0.0, 0.0); }
+            if (CARRY_OUT) {
+#pragma unroll
+                for (int q = 0; q < MSH_QG; ++q) qr[q] = qi[q] = make_double2(0.0, 0.0);
+            }
             const double2* hv = hs.vec + (long long)col * n_g + g;
 #pragma unroll 4
             for (int i = 0; i < len; ++i) {
                 const double2 v = hv[(long long)((j0 + i) % hs.H) * n_col * n_g];
 #pragma unroll
-                for (int q = 0; q < MSH_G; ++q) {
-                    if (q < ns) {
+                for (int q = 0; q < XG; ++q) {
+                    if (q < nx) {
                         const double2 c1 = cx[(s0 + q) * L + i];
                         xr[q].x += c1.x * v.x; xr[q].y += c1.x * v.y;
                         if (IMAG) { xi[q].x += c1.y * v.x; xi[q].y += c1.y * v.y; }
-                        if (CARRY_OUT) {
-                            const double2 c2 = cq[(s0 + q) * L + i];
+                    }
+                }
+                if (CARRY_OUT) {
+#pragma unroll
+                    for (int q = 0; q < MSH_QG; ++q) {
+                        if (q < nqs) {
+                            const double2 c2 = cq[qoff[q] * L + i];
                             qr[q].x += c2.x * v.x; qr[q].y += c2.x * v.y;
                             qi[q].x += c2.y * v.x; qi[q].y += c2.y * v.y;
                         }
@@ -787,18 +817,15 @@ __global__ void __launch_bounds__(NT) ms_hist_combine(long long n_g, int n_col, 
                 }
             }
 #pragma unroll
-            for (int q = 0; q < MSH_G; ++q) {
-                if (q < ns) {
-                    const long long base = ((long long)(s0 + q) * n_col + col) * 2 * n_g + g;
-                    if (carry_in) {
+            for (int q = 0; q < XG; ++q) {
+                if (q < nx) {
+                    const int s = s0 + q;
+                    const long long base = ((long long)s * n_col + col) * 2 * n_g + g;
+                    if (s_xin[s]) {
                         const double2 Qr = QS[base], Qi = QS[base + n_g];
-                        const double2 dx = cx[(s0 + q) * L + L - 1], dq = cq[(s0 + q) * L + L - 1];
+                        const double2 dx = cx[s * L + L - 1];
                         xr[q].x += dx.x * Qr.x - dx.y * Qi.x; xr[q].y += dx.x * Qr.y - dx.y * Qi.y;
                         if (IMAG) { xi[q].x += dx.x * Qi.x + dx.y * Qr.x; xi[q].y += dx.x * Qi.y + dx.y * Qr.y; }
-                        if (CARRY_OUT) {
-                            qr[q].x += dq.x * Qr.x - dq.y * Qi.x; qr[q].y += dq.x * Qr.y - dq.y * Qi.y;
-                            qi[q].x += dq.x * Qi.x + dq.y * Qr.x; qi[q].y += dq.x * Qi.y + dq.y * Qr.y;
-                        }
                     }
                     double2 x0 = XS[base];
                     x0.x += xr[q].x; x0.y += xr[q].y;
@@ -808,7 +835,24 @@ __global__ void __launch_bounds__(NT) ms_hist_combine(long long n_g, int n_col, 
                         x1.x += xi[q].x; x1.y += xi[q].y;
                         XS[base + n_g] = x1;
                     }
-                    if (CARRY_OUT) { QS[base] = qr[q]; QS[base + n_g] = qi[q]; }
+                }
+            }
+            if (CARRY_OUT) {
+                // (the x update of a live shift read its old carry above, in this pass or an earlier one: carry groups never run before the
+                // x pass of their shifts)
+#pragma unroll
+                for (int q = 0; q < MSH_QG; ++q) {
+                    if (q < nqs) {
+                        const int s = qoff[q];
+                        const long long base = ((long long)s * n_col + col) * 2 * n_g + g;
+                        if (carry_in) {
+                            const double2 Qr = QS[base], Qi = QS[base + n_g];
+                            const double2 dq = cq[s * L + L - 1];
+                            qr[q].x += dq.x * Qr.x - dq.y * Qi.x; qr[q].y += dq.x * Qr.y - dq.y * Qi.y;
+                            qi[q].x += dq.x * Qi.x + dq.y * Qr.x; qi[q].y += dq.x * Qi.y + dq.y * Qr.y;
+                        }
+                        QS[base] = qr[q]; QS[base + n_g] = qi[q];
+                    }
                 }
             }
         }
@@ -938,6 +982,30 @@ __global__ void lowrank_fix_split(int M, int Nn, long long ldt, const double* Ct
         h = __uint_as_float(hb); l = __uint_as_float(lb);
     }
     hi[i] = h; lo[i] = l;
+}
+
+// The same fix for the int8-slice path (i8_gemm.cuh): the overlap block arrives TRANSPOSED, Ct[n][ldt] (m contiguous), and is overwritten in
+// place by coef(m, n) * fix(Ct[n][m]) in FP64 (the slicing kernel reads it next); entries m >= M are set to zero.
+__global__ void lowrank_fix_t(int M, int Nn, long long ldt, double* Ct, const double* A, long long lda, const double* X, long long ldx,
+                              const double* dcoef, int n_rows_d, double alpha_const, const double* alpha_vec, const int* colmap, int nvpc,
+                              int n_occ, int gamma) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)Nn * ldt) return;
+    const int n = (int)(i / ldt), m = (int)(i - (long long)n * ldt);
+    double v = 0.0;
+    if (m < M) {
+        double c = Ct[i];
+        if (gamma) c = 2.0 * c - A[(long long)m * lda] * X[(long long)n * ldx];
+        double coef;
+        if (m < n_rows_d) coef = dcoef[m];
+        else if (alpha_vec) {
+            int col = n / nvpc;
+            if (colmap) { col = colmap[col]; if (col < 0) col = 0; }
+            coef = alpha_vec[col % n_occ];
+        } else coef = alpha_const;
+        v = coef * c;
+    }
+    Ct[i] = v;
 }
 
 }  // namespace wcg

@@ -21,6 +21,7 @@
 #include "lanczos_kernels.cuh"
 #include "bcg_kernels.cuh"
 #include "tc_gemm.cuh"
+#include "i8_gemm.cuh"
 #include <cudaTypedefs.h>
 
 namespace {
@@ -84,6 +85,11 @@ struct west_ctx {
     // [K][rows_p] (both k- resp. row-contiguous "K-major" operands of tcgen05.mma), built on first mixed use after a west_set_* change
     DevBuf A_hi, A_lo, AT_hi, AT_lo;
     bool tc_dirty = true;
+    // WEST_FP64_I8 path (i8_gemm.cuh): the operator matrix as int8 slices, row-major [S][rows][Kp] with one power-of-two scale per row and
+    // transposed [S][K][Mp] with one scale per plane-wave component k; built on first use after a west_set_* change
+    DevBuf A_i8, AT_i8, A_i8_scale, AT_i8_scale;
+    bool i8_dirty = true;
+    bool gemm_i8 = false;              // set by every hot call from its precision argument
     void* tm_encode = nullptr;         // cuTensorMapEncodeTiled (driver entry point; NULL: the mma.sync 3xTF32 kernels are used instead)
     bool A_dirty = true;
     std::vector<double> h_dcoef;       // per stacked KB row
@@ -99,7 +105,7 @@ struct west_ctx {
 
     // hot-call workspaces: carved from the arena at the start of every hot call (hot_begin / hot)
     Arena arena;
-    DevBuf W, Cbuf, Rbuf, Xsplit, Csplit, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk, hist, hist_scal;
+    DevBuf W, Cbuf, Rbuf, Xsplit, Csplit, Xi8, Ci8, Xi8_scale, Ci8_scale, vecs[4], vec5, shift, dVpos, dnpos, scal, misc, maps, xs, ps, msst, alpha_v, blk, hist, hist_scal;
     int* h_pinned = nullptr;           // pinned host scratch (64 ints): lagged convergence polls [0], [1]; reports [8..]
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
 
@@ -555,6 +561,123 @@ int lowrank_apply_tc(west_ctx* c, int nr, int n_vec, const double* X, double* Y,
     return WEST_OK;
 }
 
+// ---- WEST_FP64_I8 tensor path (tcgen05 kind::i8, i8_gemm.cuh): FP64-accurate products from error-free int8 slices
+constexpr int I8S = 8;                                       // slices per operand: 56 bits below every row's largest element
+inline long long pad64(long long n) { return (n + 63) / 64 * 64; }
+size_t i8_hot_bytes(const west_ctx* c, int rows, long long n_vec) {       // X slices + scales, C slices + scales of one low-rank apply
+    if (!tc_available(c) || rows <= 0) return 0;
+    const long long Kp = pad64(2 * c->hs.n_g), Mp = pad64(rows);
+    return al256((size_t)I8S * n_vec * Kp) + al256((size_t)I8S * n_vec * Mp) + 2 * al256(sizeof(double) * (size_t)n_vec);
+}
+// (k byte, slice, row) tensor map over slices [S][rows_alloc][ld]: the first k_extent bytes of the first `rows` rows; box {64, 1, 128},
+// 64-byte swizzle, zero fill out of bounds (so a contraction over the first k_extent entries of longer rows is exact)
+int i8_map(west_ctx* c, CUtensorMap* m, const signed char* p, long long rows, long long rows_alloc, long long k_extent, long long ld) {
+    const long long Kp = k_extent;
+    cuuint64_t gdim[3] = {(cuuint64_t)k_extent, (cuuint64_t)I8S, (cuuint64_t)rows};
+    cuuint64_t gstr[2] = {(cuuint64_t)(rows_alloc * ld), (cuuint64_t)ld};
+    cuuint32_t box[3] = {(cuuint32_t)wi8::BKB, 1, (cuuint32_t)wi8::BM}, es[3] = {1, 1, 1};
+    const CUresult r = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(c->tm_encode)(
+        m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void*)p, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(c, WEST_ECUDA, "cuTensorMapEncodeTiled failed (%d) for an int8 slice map of %lld x %lld", (int)r, rows, Kp);
+    return WEST_OK;
+}
+cudaError_t i8_attrs() {
+    static bool done = false;
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(wi8::i8_slice_gemm<I8S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wi8::Sched<I8S>::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wi8::i8_slice_gemm<I8S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wi8::Sched<I8S>::SMEM_BYTES);
+    done = e == cudaSuccess;
+    return e;
+}
+// out[c * ldo + r] += sum_k A[r][k] B[c][k] from slice arrays (both [S][rows_alloc][Kp], scales per row).  atomic: split along k (the
+// caller zeroes out); else every element is owned by one CTA (read-modify-write).
+int launch_i8_gemm(west_ctx* c, bool atomic, int rows_a, long long alloc_a, long long ld_a, const signed char* A, const double* sa, int rows_b, long long alloc_b,
+                   long long ld_b, const signed char* B, const double* sb, long long Kp /* contraction length */, double* out, long long ldo, int prof_class) {
+    if (rows_a <= 0 || rows_b <= 0) return WEST_OK;
+    int rc;
+    CK(i8_attrs());
+    wi8::Maps m;
+    if ((rc = i8_map(c, &m.a, A, rows_a, alloc_a, std::min(Kp, ld_a), ld_a)) || (rc = i8_map(c, &m.b, B, rows_b, alloc_b, std::min(Kp, ld_b), ld_b))) return rc;
+    const int n_kb = (int)((Kp + wi8::BKB - 1) / wi8::BKB);
+    const long long tiles = (long long)((rows_a + 127) / 128) * ((rows_b + 127) / 128);
+    int splits = 1;
+    if (atomic) {
+        // exactness of the int32 sums bounds a split's k range; beyond that, splits only to give every SM a tile
+        const int need = (int)((Kp + wi8::MAX_K_PER_SPLIT - 1) / wi8::MAX_K_PER_SPLIT);
+        splits = (int)std::max<long long>(need, std::min<long long>(n_kb / 32, (148 + tiles - 1) / tiles));
+        splits = std::max(1, splits);
+    } else if (Kp > wi8::MAX_K_PER_SPLIT) {
+        return fail(c, WEST_EINVAL, "int8 slice GEMM: contraction length %lld exceeds the exact int32 range of an unsplit product", Kp);
+    }
+    int kps = (n_kb + splits - 1) / splits;
+    splits = (n_kb + kps - 1) / kps;
+    const wi8::TileGrid tg{(rows_a + 127) / 128, (rows_b + 127) / 128, splits};
+    const long long nt = tiles * splits;
+    Prof p_(c, prof_class);
+    if (atomic) wi8::i8_slice_gemm<I8S, true><<<(unsigned)std::min<long long>(nt, 148), wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+    else wi8::i8_slice_gemm<I8S, false><<<(unsigned)std::min<long long>(nt, 148), wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    return WEST_OK;
+}
+// operator data of the int8 path: (re)slice the stacked operator matrix after a west_set_* change (not a hot-arena buffer)
+int ensure_i8_operator(west_ctx* c) {
+    if (!c->i8_dirty) return WEST_OK;
+    const long long K = 2 * c->hs.n_g, Kp = pad64(K);
+    const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
+    const long long Mp = pad64(rows);
+    int rc;
+    if ((rc = ensure(c, c->A_i8, (size_t)I8S * rows * Kp))) return rc;
+    if ((rc = ensure(c, c->AT_i8, (size_t)I8S * K * Mp))) return rc;
+    if ((rc = ensure(c, c->A_i8_scale, sizeof(double) * (size_t)rows))) return rc;
+    if ((rc = ensure(c, c->AT_i8_scale, sizeof(double) * (size_t)K))) return rc;
+    const double* A = (const double*)c->A_all.p;
+    wi8::slice_rows<I8S><<<rows, 256, 0, c->st>>>(K, A, K, (signed char*)c->A_i8.p, rows, Kp, (double*)c->A_i8_scale.p);
+    wi8::col_absmax<<<blocks_for(K, 256), 256, 0, c->st>>>(rows, K, A, K, (double*)c->AT_i8_scale.p);
+    wi8::slice_rows_transposed<I8S><<<dim3((unsigned)((K + 31) / 32), (unsigned)((Mp + 31) / 32)), dim3(32, 8), 0, c->st>>>(rows, K, A, K, (const double*)c->AT_i8_scale.p,
+                                                                                                                    (signed char*)c->AT_i8.p, Mp);
+    CK(cudaGetLastError());
+    c->launches += 3;
+    c->i8_dirty = false;
+    return WEST_OK;
+}
+// rows [0, nr) of the operator matrix on the int8 path:  Y += A^T (coef . fix(A X^T))
+int lowrank_apply_i8(west_ctx* c, int nr, int n_vec, const double* X, double* Y, const LowrankCoef& lc) {
+    const long long K = 2 * c->hs.n_g, Kp = pad64(K), Mp = pad64(nr);
+    const int rows_all = c->rows_kb + c->rows_psi + c->rows_defl;
+    const long long Mp_all = pad64(rows_all), rp = pad4(nr);
+    int rc;
+    if ((rc = ensure_i8_operator(c))) return rc;
+    if ((rc = hot(c, c->Xi8, (size_t)I8S * n_vec * Kp))) return rc;
+    if ((rc = hot(c, c->Ci8, (size_t)I8S * n_vec * Mp))) return rc;
+    if ((rc = hot(c, c->Xi8_scale, sizeof(double) * (size_t)n_vec))) return rc;
+    if ((rc = hot(c, c->Ci8_scale, sizeof(double) * (size_t)n_vec))) return rc;
+    if ((rc = hot(c, c->Cbuf, bytes_C(nr, n_vec)))) return rc;
+    double* Ct = (double*)c->Cbuf.p;                       // [n_vec][rp] (transposed overlap block, rows contiguous)
+    {
+        Prof p_(c, PC_GEMM_TN);
+        wi8::slice_rows<I8S><<<n_vec, 256, 0, c->st>>>(K, X, K, (signed char*)c->Xi8.p, n_vec, Kp, (double*)c->Xi8_scale.p);
+        CK(cudaMemsetAsync(Ct, 0, sizeof(double) * (size_t)n_vec * rp, c->st));
+        CK(cudaGetLastError());
+        c->launches += 1;
+    }
+    if ((rc = launch_i8_gemm(c, true, nr, rows_all, Kp, (const signed char*)c->A_i8.p, (const double*)c->A_i8_scale.p, n_vec, n_vec, Kp, (const signed char*)c->Xi8.p,
+                             (const double*)c->Xi8_scale.p, K, Ct, rp, PC_GEMM_TN)))
+        return rc;
+    {
+        Prof p_(c, PC_GEMM_UP);
+        wcg::lowrank_fix_t<<<blocks_for((long long)n_vec * rp, 256), 256, 0, c->st>>>(nr, n_vec, rp, Ct, (const double*)c->A_all.p, K, X, K, lc.dcoef, lc.n_rows_d,
+                                                                                 lc.alpha_const, lc.alpha_vec, lc.colmap, lc.nvpc, lc.n_occ, is_gamma(c) ? 1 : 0);
+        wi8::slice_rows<I8S><<<n_vec, 256, 0, c->st>>>(nr, Ct, rp, (signed char*)c->Ci8.p, n_vec, Mp, (double*)c->Ci8_scale.p);
+        CK(cudaGetLastError());
+        c->launches += 2;
+    }
+    // Y[n][k] += sum_m C[m][n] A[m][k]: k on the TMEM lanes (operator transposed, scale per k), vectors on the columns
+    return launch_i8_gemm(c, false, (int)K, K, Mp_all, (const signed char*)c->AT_i8.p, (const double*)c->AT_i8_scale.p, n_vec, n_vec, Mp, (const signed char*)c->Ci8.p,
+                          (const double*)c->Ci8_scale.p, nr, Y, K, PC_GEMM_UP);
+}
+
 // Y += sum_{m in [r0, r0+nr)} coef_m A_m <A_m, X>   for n_vec real-function / complex vectors (as 2 n_g reals each).
 // tf32: the WEST_MIXED path of H*psi (3xTF32 tensor-core products, FP32 class) - never the RHS projection or the deflation.
 // On Blackwell the tf32 products run on tcgen05 (lowrank_apply_tc); the warp-level mma.sync kernels remain as the path taken when the
@@ -562,6 +685,7 @@ int lowrank_apply_tc(west_ctx* c, int nr, int n_vec, const double* X, double* Y,
 int lowrank_apply(west_ctx* c, int r0, int nr, int n_vec, const double* X, double* Y, const LowrankCoef& lc, bool tf32 = false) {
     if (nr <= 0 || n_vec <= 0) return WEST_OK;
     if (tf32 && r0 == 0 && tc_available(c)) return lowrank_apply_tc(c, nr, n_vec, X, Y, lc);
+    if (c->gemm_i8 && !tf32 && r0 == 0 && tc_available(c)) return lowrank_apply_i8(c, nr, n_vec, X, Y, lc);
     const long long K = 2 * c->hs.n_g;
     const long long ldc = (n_vec + 1) / 2 * 2;
     int rc = hot(c, c->Cbuf, bytes_C(nr, n_vec));
@@ -615,9 +739,10 @@ size_t plan_lanczos(const west_ctx* c, int n_pert, int n_steps, int f32) {
     if (f32 && tc_available(c)) t += al256(sizeof(float) * 4 * n_col * (size_t)pad4(2 * c->hs.n_g));      // TF32 splits of q^1 and q^l (brakets)
     return t;
 }
-size_t plan_happly(const west_ctx* c, long long n_vec, int f32) {
+size_t plan_happly(const west_ctx* c, long long n_vec, int f32, int i8 = 0) {
     const long long n_slots = is_gamma(c) ? (n_vec + 1) / 2 : n_vec;
-    return al256(bytes_W(c, n_slots, f32)) + (c->rows_kb > 0 ? al256(bytes_C(c->rows_kb, n_vec)) + (f32 ? tc_hot_bytes(c, c->rows_kb, n_vec) : 0) : 0);
+    return al256(bytes_W(c, n_slots, f32)) +
+           (c->rows_kb > 0 ? al256(bytes_C(c->rows_kb, n_vec)) + (f32 ? tc_hot_bytes(c, c->rows_kb, n_vec) : (i8 ? i8_hot_bytes(c, c->rows_kb, n_vec) : 0)) : 0);
 }
 
 }  // namespace
@@ -798,7 +923,7 @@ int west_set_kb(west_ctx* c, int32_t n_proj, const void* beta, const double* dco
     const long long n_g = c->hs.n_g;
     c->n_proj = n_proj;
     c->rows_kb = n_proj * (full ? 2 : 1);
-    c->A_dirty = true; c->tc_dirty = true;
+    c->A_dirty = true; c->tc_dirty = true; c->i8_dirty = true;
     c->h_dcoef.resize(c->rows_kb);
     for (int k = 0; k < n_proj; ++k) {
         if (full) { c->h_dcoef[2 * k] = dcoef_host[k]; c->h_dcoef[2 * k + 1] = dcoef_host[k]; }
@@ -827,7 +952,7 @@ int west_set_states(west_ctx* c, int32_t n_occ_user, const void* psi, const doub
     c->n_occ = n_occ;
     c->n_occ_user = n_occ_user;
     c->rows_psi = n_occ * (full ? 2 : 1);
-    c->A_dirty = true; c->tc_dirty = true;
+    c->A_dirty = true; c->tc_dirty = true; c->i8_dirty = true;
     c->h_eps.assign(eps_host, eps_host + n_occ_user);
     if (n_occ > n_occ_user) c->h_eps.push_back(eps_host[n_occ_user - 1]);
     int rc = ensure(c, c->A_psi, (size_t)c->rows_psi * 2 * n_g * sizeof(double));
@@ -880,7 +1005,7 @@ int west_set_deflation(west_ctx* c, int32_t n_defl, const void* psi_c, const dou
     const long long n_g = c->hs.n_g;
     c->n_defl = n_defl;
     c->rows_defl = n_defl * (full ? 2 : 1);
-    c->A_dirty = true; c->tc_dirty = true;
+    c->A_dirty = true; c->tc_dirty = true; c->i8_dirty = true;
     if (n_defl == 0) return WEST_OK;
     c->h_eps_defl.assign(eps_host, eps_host + n_defl);
     int rc = ensure(c, c->A_defl, (size_t)c->rows_defl * 2 * n_g * sizeof(double));
@@ -943,15 +1068,16 @@ int west_fft3d_dense(west_ctx* c, int32_t n, int32_t sign, int32_t precision, in
 
 int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, void* y) {
     if (!c || n_vec < 0 || (n_vec > 0 && (!x || !y))) return fail(c, WEST_EINVAL, "west_h_apply: bad argument");
-    if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_h_apply: bad precision %d", precision);
+    if (precision != WEST_FP64 && precision != WEST_MIXED && precision != WEST_FP64_I8) return fail(c, WEST_EINVAL, "west_h_apply: bad precision %d", precision);
     if (!c->have_vloc) return fail(c, WEST_ESTATE, "west_h_apply: west_set_vloc has not been called");
+    c->gemm_i8 = precision == WEST_FP64_I8 && tc_available(c);
     if (n_vec == 0) return WEST_OK;
     const int gamma = is_gamma(c);
     const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
     VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
     int rc;
     if ((rc = ensure_opmatrix(c))) return rc;
-    if ((rc = hot_begin(c, plan_happly(c, n_vec, precision == WEST_MIXED)))) return rc;
+    if ((rc = hot_begin(c, plan_happly(c, n_vec, precision == WEST_MIXED, c->gemm_i8)))) return rc;
     if ((rc = hloc_apply(c, precision == WEST_MIXED, vm, n_slots, (const cx<double>*)x, (cx<double>*)y, nullptr, 0.0))) return rc;
     if (c->rows_kb > 0) {
         LowrankCoef lc; lc.dcoef = c->d_dcoef; lc.n_rows_d = c->rows_kb;
@@ -1309,7 +1435,7 @@ cudaError_t ms_hist_attrs() {
     const int bytes = (int)(2 * wcg::MS_MAX_SHIFTS * (wcg::MSH_HMAX + 1) * sizeof(double2));
     cudaError_t e = cudaFuncSetAttribute(wcg::ms_hist_combine<false, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<true, false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<false, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<false, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(wcg::ms_hist_combine<true, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     done = e == cudaSuccess;
     return e;
@@ -1324,7 +1450,7 @@ int ms_hist_combine_launch(west_ctx* c, int n_col, int n_shift, int j0, int n_en
     Prof p_(c, PC_CGVEC);
     if (imag && carry_out) wcg::ms_hist_combine<true, true, 4><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
     else if (imag) wcg::ms_hist_combine<true, false, 4><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
-    else if (carry_out) wcg::ms_hist_combine<false, true, 4><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
+    else if (carry_out) wcg::ms_hist_combine<false, true, 8><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
     else wcg::ms_hist_combine<false, false, 8><<<grid, wcg::NT, sm, c->st>>>(n_g, n_col, n_shift, j0, n_end, carry_in, hs, st.iters, (double2*)XS, (double2*)QS, ctr);
     CK(cudaGetLastError());
     c->launches += 1;
@@ -1571,7 +1697,7 @@ struct Chi0Plan {
     }
     size_t total() const { return fixed() + (solver == 1 && H > 0 ? al256((size_t)H * vec) + al256((size_t)H * hscal) : 0); }
 };
-Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, int f32 = 0, int H = 0, bool carry = false) {
+Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, int f32 = 0, int H = 0, bool carry = false, int i8 = 0) {
     Chi0Plan p;
     p.solver = solver; p.nvpc = nvpc; p.n_freq = n_freq; p.pb = pb; p.H = solver == 1 ? H : 0; p.carry = carry;
     const size_t n_g = (size_t)c->hs.n_g, n3 = (size_t)n3_of(c);
@@ -1589,6 +1715,7 @@ Chi0Plan chi0_plan(const west_ctx* c, int solver, int nvpc, int n_freq, int pb, 
     const int rows = c->rows_kb + c->rows_psi + c->rows_defl;
     p.C = bytes_C(rows, n_vec);
     if (f32) p.tc = tc_hot_bytes(c, rows, n_vec);
+    else if (i8) p.tc = i8_hot_bytes(c, rows, n_vec);
     p.alpha = sizeof(double) * c->n_occ;
     if (solver == 2) p.blk = bcg_small_bytes(c->n_occ, pb);
     if (solver == 1) {
@@ -1610,7 +1737,8 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
                                const double* omega_host, const west_cg_opts* opts, double* dn, void* dpsi_opt, west_stats* stats) {
     if (!c || n_pert < 0 || n_freq < 0 || !opts || (n_freq > 0 && !omega_host) || (n_pert > 0 && n_freq > 0 && (!dV || !dn)))
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
-    if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
+    if (precision != WEST_FP64 && precision != WEST_MIXED && precision != WEST_FP64_I8) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
+    c->gemm_i8 = precision == WEST_FP64_I8 && tc_available(c);
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
     if (opts->max_iter < 1 || !(opts->tol > 0) || opts->solver < 0 || opts->solver > 2 || opts->occupation < 0 || opts->occupation > 2 ||
         (opts->dn_accumulate != 0 && opts->dn_accumulate != 1))
@@ -1655,20 +1783,23 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
             // a ring that only fits sub-blocks of fewer than ~2000 columns costs more in GEMM efficiency than it saves in vector traffic
             // (measured at cfg 5, 4 frequencies: 1 024-column sub-blocks ran the projector GEMMs at 0.86 instead of 0.92 of the DGEMM rate)
             if (c->ms_hist == 0 && nb > 1 && (long long)pb * n_occ < 2048) break;
-            Chi0Plan q = chi0_plan(c, 1, nvpc_max, n_freq, pb, f32, h_want, h_want < opts->max_iter + 1);
+            Chi0Plan q = chi0_plan(c, 1, nvpc_max, n_freq, pb, f32, h_want, h_want < opts->max_iter + 1, c->gemm_i8);
             const size_t fx = q.fixed(), per = al256(q.vec) + al256(q.hscal) + 512;
             if (fx + (size_t)h_min * per <= hbudget) {
-                const int h = (int)std::min<size_t>((size_t)h_want, (hbudget - fx) / per);
-                plan = chi0_plan(c, 1, nvpc_max, n_freq, pb, f32, h, h < opts->max_iter + 1);
-                planned = plan.total() <= budget;
-                break;
+                int h = (int)std::min<size_t>((size_t)h_want, (hbudget - fx) / per + 2);      // (per over-estimates a slot: refine against the exact total)
+                for (; h >= h_min; --h) {
+                    plan = chi0_plan(c, 1, nvpc_max, n_freq, pb, f32, h, h < opts->max_iter + 1, c->gemm_i8);
+                    if (plan.total() <= hbudget) break;
+                }
+                planned = h >= h_min && plan.total() <= budget;
+                if (planned) break;
             }
             if (pb == 1) break;
         }
     }
     for (int nb = 1; !planned; ++nb) {
         pb = (n_pert + nb - 1) / nb;
-        plan = chi0_plan(c, opts->solver, nvpc_max, n_freq, pb, f32);
+        plan = chi0_plan(c, opts->solver, nvpc_max, n_freq, pb, f32, 0, false, c->gemm_i8);
         if (plan.total() <= budget || pb == 1) break;
     }
     if (plan.total() > budget)
@@ -1872,15 +2003,15 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
 
 extern "C" size_t west_workspace_bytes(const west_ctx* c, int32_t op, int32_t n_pert, int32_t n_freq, int32_t precision) {
     if (!c || n_pert <= 0) return 0;
-    const int f32 = precision == WEST_MIXED;
+    const int f32 = precision == WEST_MIXED, i8 = precision == WEST_FP64_I8 && tc_available(c);
     switch (op) {
         case WEST_OP_FFT3D: return plan_fft3d(c, n_pert);
-        case WEST_OP_H_APPLY: return plan_happly(c, n_pert, f32);
-        case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert, f32).total();
-        case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert, f32).total();
-        case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32).total();
-        case WEST_OP_CHI0_MULTISHIFT_HIST: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32, wcg::MSH_HMAX, true).total();
-        case WEST_OP_CHI0_BLOCK: return chi0_plan(c, 2, 1, std::max(1, n_freq), n_pert, f32).total();
+        case WEST_OP_H_APPLY: return plan_happly(c, n_pert, f32, i8);
+        case WEST_OP_CHI0: return chi0_plan(c, 0, 1, std::max(1, n_freq), n_pert, f32, 0, false, i8).total();
+        case WEST_OP_CHI0_IW: return chi0_plan(c, 0, is_gamma(c) ? 2 : 1, std::max(1, n_freq), n_pert, f32, 0, false, i8).total();
+        case WEST_OP_CHI0_MULTISHIFT: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32, 0, false, i8).total();
+        case WEST_OP_CHI0_MULTISHIFT_HIST: return chi0_plan(c, 1, 1, std::max(1, n_freq), n_pert, f32, wcg::MSH_HMAX, true, i8).total();
+        case WEST_OP_CHI0_BLOCK: return chi0_plan(c, 2, 1, std::max(1, n_freq), n_pert, f32, 0, false, i8).total();
         case WEST_OP_LANCZOS: return plan_lanczos(c, n_pert, std::max(1, n_freq), f32);
     }
     return 0;
@@ -1904,6 +2035,7 @@ extern "C" int west_lanczos(west_ctx* c, int32_t precision, int32_t n_pert, cons
                             double* norm, double* braket_opt) {
     if (!c || n_pert < 0 || n_steps < 1 || (n_pert > 0 && (!phi || !alpha || !beta || !norm))) return fail(c, WEST_EINVAL, "west_lanczos: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED) return fail(c, WEST_EINVAL, "west_lanczos: bad precision %d", precision);
+    c->gemm_i8 = false;
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_lanczos: west_set_vloc and west_set_states are required");
     const int gamma = is_gamma(c), N = c->cell.N, n_occ = c->n_occ;
     if (braket_opt && !gamma) return fail(c, WEST_EINVAL, "west_lanczos: brakets are implemented for WEST_GAMMA only");

@@ -134,3 +134,33 @@ def test_cfg5_bench_configuration_batch_16(cell):
     M = ochi0.response_matrix(p.dV[:n_pert], dn[0], p.L)
     assert np.max(np.abs(M - M.T)) < 1e-6 * np.max(np.abs(M))          # symmetric to the solver tolerance
     assert np.max(np.linalg.eigvalsh(0.5 * (M + M.T))) < 0.0
+
+
+def test_cfg5_int8_slice_gemms(cell):
+    """WEST_FP64_I8 at config-5 size (2048 projectors + 1024 orbitals = 3072 operator rows, contraction length 145 406: the int32 sums
+    need their K split): H*psi against the DMMA path on 64 random vectors and against the oracle's matrix-free H on two of them; chi0*dV for
+    two perturbations - true residual of sampled columns with the oracle's H, and the same dn as the FP64 run of the chain-of-trust test."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p, w, dev, alpha = (cell[k] for k in ("p", "w", "dev", "alpha"))
+    rng = np.random.Generator(np.random.PCG64(5099))
+    c = rng.standard_normal((64, w.n_g)) + 1j * rng.standard_normal((64, w.n_g))
+    c[:, 0] = c[:, 0].real
+    x = torch.from_numpy(c).to(dev)
+    y64 = w.h_apply(x, precision=wb.WEST_FP64).cpu().numpy()
+    y8 = w.h_apply(x, precision=wb.WEST_FP64_I8).cpu().numpy()
+    assert relmax(y8, y64) < 1e-13
+    for v in (0, 63):
+        ref = cell["apply_H"](ogs.expand_half_to_full(c[v], p.miller))[p.half]
+        assert relmax(y8[v], ref) < 1e-12
+    n_pert = 2
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV[:n_pert])).to(dev)
+    dn, dpsi, st = w.chi0_apply(dV, [0.0], tol=1e-10, max_iter=500, alpha_pv=alpha, want_dpsi=True, precision=wb.WEST_FP64_I8)
+    assert st["rc"] == 0 and st["n_unconverged"] == 0
+    for i, v in ((0, 0), (1, 700)):
+        xr = ogs.expand_half_to_full(dpsi[0, i, v, 0].cpu().numpy(), p.miller)
+        assert _true_residual(cell, i, v, xr + 0j, 0.0, alpha) < 1e-8
+    del dpsi
+    torch.cuda.empty_cache()
+    if 0.0 in cell["small"]:
+        assert relmax(dn[0].cpu().numpy(), cell["small"][0.0][0]) < 1e-8
