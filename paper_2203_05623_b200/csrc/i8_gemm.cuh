@@ -17,8 +17,13 @@
 //   phase 0:  i, j <  S/2, i + j <= S/2 - 1          weight classes 0 .. S/2 - 1      A slices 0 .. S/2-1,  B slices 0 .. S/2-1
 //   phase 1:  j <  S/2, S/2 - j <= i <= S - 1 - j    weight classes S/2 .. S - 1      A slices 1 .. S-1,    B slices 0 .. S/2-1
 //   phase 2:  j >= S/2, i <= S - 1 - j               weight classes S/2 .. S - 1      A slices 0 .. S/2-1,  B slices S/2 .. S-1
-// Warp roles as in tc_gemm.cuh: warps 0-7 epilogue (TMEM lane quarter = warp mod 4, column half = warp / 4), warp 8 TMA producer, warp 9
-// MMA issuer + TMEM owner.  The epilogue warps keep the FP64 sums of a tile in registers across its three phases and write once:
+// Measured alternatives of this staging (cfg-5 H*psi batch of 16 384 vectors, overlap / update product in ms; this version 153 / 189):
+// 32-byte rows with a 5-stage ring 182 / 216; 64-byte rows, four sub-phases of <= 8 tiles, 3 stages 182 / 213; 128-byte rows, six sub-phases
+// of <= 7 tiles, two drains per tile 161 / 196.  Time follows the slice-tile BYTES loaded (27 tiles of 8 KB per 64-byte k-block here), not the
+// ring depth or the row length: the kernel is bound by the L2 -> shared-memory fill at ~7-8 TB/s with an L2 hit rate of 51 % (ncu), i.e. by
+// how well concurrently running CTAs share operand tiles in L2.
+// Warp roles as in tc_gemm.cuh: EPI_WARPS epilogue warps (TMEM lane quarter = warp mod 4, column block = warp / 4), then the TMA producer
+// warp and the MMA issuer warp (+ TMEM owner).  The epilogue warps keep the FP64 sums of a tile in registers across its three phases and write once:
 //   ATOMIC  out[c * ldo + r] += value by atomicAdd (overlap block, split along K)       else  out[c * ldo + r] += value (update).
 #pragma once
 #include <cuda.h>
@@ -38,9 +43,12 @@ using wtc::tmem_ld32;
 using wtc::umma_commit;
 
 constexpr int BM = 128, BN = 128, BKB = 64;          // BKB int8 = 64 bytes = one swizzle row
-constexpr int STAGES = 2, NTHREADS = 320, EPI_WARPS = 8, EPI_COLS = BN / 2;
+#ifndef WEST_I8_EPI_WARPS
+#define WEST_I8_EPI_WARPS 16       // 8 measured slower on the update product of small cells (1.90 against 1.75 ms at cfg-2 size), equal at cfg 5
+#endif
+constexpr int STAGES = 2, EPI_WARPS = WEST_I8_EPI_WARPS, NTHREADS = (EPI_WARPS + 2) * 32, EPI_COLS = BN / (EPI_WARPS / 4);
 constexpr uint32_t TILE_BYTES = BM * BKB;            // 8 KB per slice tile
-constexpr int MAX_K_PER_SPLIT = 1 << 17;             // int32 exactness: 4 pairs x 2^17 x 2^12 = 2^31
+constexpr int MAX_K_PER_SPLIT = 1 << 16;             // int32 exactness: at most 4 pairs per accumulator and phase: 4 x 2^16 x 2^12 = 2^30 (a factor 2 to spare)
 
 template <int S> struct Sched {
     static constexpr int H = S / 2;
@@ -67,7 +75,9 @@ __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_
 }
 
 struct Maps { CUtensorMap a, b; };                   // (k byte, slice, row) tensors, box {64, 1, 128}
-struct TileGrid { int tiles_a, tiles_b, splits; };
+// tile order: B tiles in groups of gb; inside a group the gb B tiles run fastest, then the A tiles; then the next group; K splits slowest.
+// Concurrently running CTAs then cover ~148 / gb A tiles x gb B tiles, so both operands are shared in L2 (gb = 1: A tiles fastest).
+struct TileGrid { int tiles_a, tiles_b, splits, gb; };
 
 template <int S, bool ATOMIC>
 __global__ void __launch_bounds__(NTHREADS, 1) i8_slice_gemm(const __grid_constant__ Maps maps, TileGrid tg, int rows_a, int rows_b, int n_kb, int kb_per_split,
@@ -100,8 +110,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) i8_slice_gemm(const __grid_consta
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
     auto tile_of = [&](int t, int& r0, int& c0, int& kb0, int& nkb) {
-        const int ta = t % tg.tiles_a, rest = t / tg.tiles_a;
-        const int tb = rest % tg.tiles_b, sp = rest / tg.tiles_b;
+        const int per_split = tg.tiles_a * tg.tiles_b;
+        const int sp = t / per_split, u = t - sp * per_split;
+        const int tbg = u / (tg.gb * tg.tiles_a), r = u - tbg * tg.gb * tg.tiles_a;
+        const int gsize = min(tg.gb, tg.tiles_b - tbg * tg.gb);
+        const int ta = r / gsize, tb = tbg * tg.gb + (r - ta * gsize);
         r0 = ta * BM; c0 = tb * BN; kb0 = sp * kb_per_split;
         nkb = min(kb_per_split, n_kb - kb0);
     };

@@ -605,14 +605,20 @@ int launch_i8_gemm(west_ctx* c, bool atomic, int rows_a, long long alloc_a, long
     if (atomic) {
         // exactness of the int32 sums bounds a split's k range; beyond that, splits only to give every SM a tile
         const int need = (int)((Kp + wi8::MAX_K_PER_SPLIT - 1) / wi8::MAX_K_PER_SPLIT);
-        splits = (int)std::max<long long>(need, std::min<long long>(n_kb / 32, (148 + tiles - 1) / tiles));
+        // and k chunks of ~8 KB per slice row: the operator chunk all tiles of a split share then stays closer to the L2 (measured at the cfg-5
+        // shape: 153.5 ms with 3 splits, 134-136 ms with 12-40)
+        splits = (int)std::max<long long>(need, std::min<long long>(n_kb / 32, std::max<long long>((Kp + 8191) / 8192, (148 + tiles - 1) / tiles)));
         splits = std::max(1, splits);
     } else if (Kp > wi8::MAX_K_PER_SPLIT) {
         return fail(c, WEST_EINVAL, "int8 slice GEMM: contraction length %lld exceeds the exact int32 range of an unsplit product", Kp);
     }
     int kps = (n_kb + splits - 1) / splits;
     splits = (n_kb + kps - 1) / kps;
-    const wi8::TileGrid tg{(rows_a + 127) / 128, (rows_b + 127) / 128, splits};
+    // update product (rows_a = 2 n_g rows of the transposed operator): vector tiles in groups, else every CTA streams its own operator tile
+    // from DRAM once per vector tile; overlap product: few operator tiles, small groups
+    // (measured at the cfg-5 shape: update product 190 ms with the operator tiles fastest, 142-148 ms with groups of 4-16 vector tiles)
+    const int gb = atomic ? 4 : 6;
+    const wi8::TileGrid tg{(rows_a + 127) / 128, (rows_b + 127) / 128, splits, gb};
     const long long nt = tiles * splits;
     Prof p_(c, prof_class);
     if (atomic) wi8::i8_slice_gemm<I8S, true><<<(unsigned)std::min<long long>(nt, 148), wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
