@@ -757,6 +757,17 @@ def main():
             subs["cfg5_iw"] = r
         except Exception as e:
             subs["cfg5_iw"] = {"error": repr(e)[:300]}
+        if precision == wb.WEST_FP64:
+            # the same four frequencies with the int8-slice GEMMs - only while the run is early enough to leave the named configs their time
+            try:
+                if time.time() - T_START > 1150.0:
+                    raise TimeoutError("skipped: the run had taken more than 1150 s before this optional sub-record")
+                r = run_chi0(a, wb, cfg, w, dV_np, alpha, aux, om_iw, 1 if a.solver < 0 else a.solver, wb.WEST_FP64_I8, 1, 0, local, world, barrier, 0,
+                             want_cpu=0 if a.no_cpu_baseline else 1, label="cfg5 imaginary frequencies, projector GEMMs from int8 slices (WEST_FP64_I8)", profile_in_timed=True)
+                r["note"] = "ONE timed step, no warm-up of its own"
+                subs["cfg5_iw_i8"] = r
+            except Exception as e:
+                subs["cfg5_iw_i8"] = {"error": repr(e)[:300]}
         w.close()
         del w, aux
         torch.cuda.empty_cache()

@@ -90,6 +90,7 @@ struct west_ctx {
     DevBuf A_i8, AT_i8, A_i8_scale, AT_i8_scale;
     bool i8_dirty = true;
     bool gemm_i8 = false;              // set by every hot call from its precision argument
+    bool arena_release_ok = false;     // true only while a hot call builds operator data BEFORE carving its workspace (ensure() may then free the lazy arena)
     void* tm_encode = nullptr;         // cuTensorMapEncodeTiled (driver entry point; NULL: the mma.sync 3xTF32 kernels are used instead)
     bool A_dirty = true;
     std::vector<double> h_dcoef;       // per stacked KB row
@@ -157,6 +158,16 @@ int ensure(west_ctx* c, DevBuf& b, size_t bytes) {
         b.p = nullptr; b.bytes = 0;
     }
     int rc = dev_alloc(c, &b.p, bytes);
+    if (rc == WEST_ENOMEM && c->arena_release_ok && c->arena.base && !c->arena.user) {
+        // operator data does not fit next to the context's own (lazy, grow-only) workspace of an earlier, larger call: give that block back
+        // and try again - the next hot call regrows it to what it needs (never done with a caller-owned workspace)
+        cudaStreamSynchronize(c->st);
+        cudaFree(c->arena.base);
+        c->dev_bytes -= (int64_t)c->arena.cap;
+        c->arena.base = nullptr; c->arena.cap = 0; c->arena.off = 0;
+        c->arena.epoch += 1;
+        rc = dev_alloc(c, &b.p, bytes);
+    }
     if (rc == WEST_OK) b.bytes = bytes;
     return rc;
 }
@@ -1083,6 +1094,12 @@ int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, v
     VecMap vm{gamma ? 2 : 1, gamma ? 1 : 0, n_vec, 0};
     int rc;
     if ((rc = ensure_opmatrix(c))) return rc;
+    // operator data of the tensor paths is (re)built BEFORE the workspace is carved: ensure() may give the lazy workspace back to make room
+    c->arena_release_ok = true;
+    if (c->gemm_i8 && c->rows_kb > 0) rc = ensure_i8_operator(c);
+    if (!rc && precision == WEST_MIXED && tc_available(c) && c->rows_kb > 0) rc = ensure_tc_operator(c);
+    c->arena_release_ok = false;
+    if (rc) return rc;
     if ((rc = hot_begin(c, plan_happly(c, n_vec, precision == WEST_MIXED, c->gemm_i8)))) return rc;
     if ((rc = hloc_apply(c, precision == WEST_MIXED, vm, n_slots, (const cx<double>*)x, (cx<double>*)y, nullptr, 0.0))) return rc;
     if (c->rows_kb > 0) {
@@ -1771,6 +1788,12 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
     const int nvpc_max = any_omega ? 2 : 1;
     int rc;
     if ((rc = ensure_opmatrix(c))) return rc;
+    // operator data of the tensor paths is (re)built BEFORE the workspace is planned and carved: ensure() may give the lazy workspace back
+    c->arena_release_ok = true;
+    if (c->gemm_i8) rc = ensure_i8_operator(c);
+    if (!rc && f32 && tc_available(c)) rc = ensure_tc_operator(c);
+    c->arena_release_ok = false;
+    if (rc) return rc;
 
     // ---- workspace: the largest perturbation sub-block whose buffers fit the arena (the caller's, or what the device has free)
     const size_t budget = arena_budget(c);
