@@ -395,14 +395,16 @@ def roofline(cfg, top, prof, n_h, n_freq, solver, hbm_peak, peak_src, mixed, n_g
                     "algorithmic_bytes_per_vector": (1 if top == "gemm_tn" else 2) * 2 * n_g * 8,
                     "note": "FP64 DMMA (mma.sync m8n8k4; tcgen05 has no FP64 kind)" if not mixed else "3xTF32 products, FP64 operands in memory; peak shown is the FP64 one"})
         if i8:
-            # WEST_FP64_I8: the contraction runs as 36 int8 slice-pair products per FP64 product (8 slices, pairs with i + j <= 7) on the INT8
+            # WEST_FP64_I8: the contraction runs as 21 or 36 int8 slice-pair products per FP64 product (6 or 8 slices, pairs with i + j < S) on the INT8
             # tensor path; its roofline is the int8 tensor peak = the measured dense bf16 rate x the nominal ratio 2 (B200_PROFILING.md)
             p = os.path.join(ROOT, "MEASURED_PEAKS.json")
             bf16 = float(json.load(open(p)).get("bf16_tflops_sustained", 1370.0)) if os.path.exists(p) else 1370.0
-            ops = 36.0 * flops
+            n_prod = 21.0 if TOL >= 1e-9 else 36.0     # west.h: 6 slices (21 pair products) when the CG tolerance is 1e-9 or looser, else 8 (36)
+            ops = n_prod * flops
             out.update({"bound": "tensor", "achieved": ops / t / 1e12, "peak": 2.0 * bf16, "unit": "TFLOP/s", "frac": ops / t / 1e12 / (2.0 * bf16),
                         "peak_source": "int8 tensor: 2 x the sustained dense bf16 rate of MEASURED_PEAKS.json (else 2 x 1370)", "fp64_equivalent_tflops": ach,
-                        "note": "tcgen05.mma kind::i8: 36 exact int8 slice-pair products per FP64 product, int32 accumulation in TMEM, FP64 sums; the class time "
+                        "int8_products_per_fp64_product": n_prod,
+                        "note": "tcgen05.mma kind::i8: exact int8 slice-pair products (6 slices = 21 products at this tolerance), int32 accumulation in TMEM, FP64 sums; the class time "
                                 "includes the per-call slicing of the vector / coefficient block; `achieved` counts int8 operations"})
         units = n_h
     else:
@@ -551,7 +553,7 @@ def run_chi0(a, wb, cfg, w, dV_np, alpha, aux, omegas, solver, precision, steps,
     gemm_tf = 2 * 2.0 * rows * (2 * w.n_g) * n_h_prof / t_gemm / 1e12 if t_gemm > 0 else None
     rec = {
         "value": units * steps / (ms * 1e-3), "unit": "perturbations/s", "steps": steps, "warmup": warmup, "ms_per_step": ms / steps,
-        "dtype": ("f64" if precision != wb.WEST_FP64_I8 else "f64 (projector GEMMs inside H*psi: exact int8-slice products on tcgen05 kind::i8, FP64 sums)") if not mixed else "f32 FFT + 3xTF32 GEMMs inside H*psi / f64 vectors, dots, dn",
+        "dtype": ("f64" if precision != wb.WEST_FP64_I8 else "f64 (projector GEMMs inside H*psi: exact int8-slice products on tcgen05 kind::i8 - 6 slices of 7 bits per operand row at this tolerance - FP64 sums)") if not mixed else "f32 FFT + 3xTF32 GEMMs inside H*psi / f64 vectors, dots, dn",
         "config": {"workload": label, "N": N, "n_g": w.n_g, "n_occ": cfg["n_occ"], "n_pert_per_gpu": n_pert, "n_freq": n_freq, "omega_ry": [round(x, 6) for x in omegas],
                    "n_proj": cfg["n_proj"], "n_deflated": a.deflate, "alpha_pv": "per-orbital (eps_v - eps_1) + W/2" if alpha <= 0 else alpha, "tol": TOL,
                    "solver": {0: "PCG/COCG per frequency", 1: "multi-shift CG", 2: "block CG"}[solver], "ms_history_slots": stats.get("ms_history_slots", 0), "cg_iters": stats["iters"], "cg_iters_min": stats["iters_min"],

@@ -97,7 +97,9 @@ extern "C" {
                            tensor memory; csrc/i8_gemm.cuh): every operand row is cut into 8 signed 7-bit slices below
                            its own power-of-two scale (2^-56 of the row's largest element is dropped), slice pairs contract exactly in
                            int32, the weight classes are summed in FP64.  Same parity bar as WEST_FP64 (1e-9); the RHS projection and the
-                           deflation update stay on DMMA.  Falls back to WEST_FP64 when the driver offers no tensor-map encoder. */
+                           deflation update stay on DMMA.  west_chi0_apply with opts->tol >= 1e-9 uses 6 slices (2^-42 of the row maxima,
+                           four orders below such a tolerance; 21 instead of 36 slice-pair products); tighter tolerances and west_h_apply
+                           use 8.  Falls back to WEST_FP64 when the driver offers no tensor-map encoder. */
 #define WEST_FP32   2   /* west_fft3d_dense only: complex64 data and arithmetic (the FP32 curves of Fig. 3) */
 
 typedef struct west_ctx west_ctx;

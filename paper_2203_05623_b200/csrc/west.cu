@@ -90,6 +90,8 @@ struct west_ctx {
     DevBuf A_i8, AT_i8, A_i8_scale, AT_i8_scale;
     bool i8_dirty = true;
     bool gemm_i8 = false;              // set by every hot call from its precision argument
+    int i8_slices = 8;                 // slices per operand the int8 GEMMs of the current hot call use: 8 (2^-56 of the row maxima), or 6 (2^-42) when
+                                       // the CG tolerance of the call is 1e-9 or looser (west.h, WEST_FP64_I8)
     bool arena_release_ok = false;     // true only while a hot call builds operator data BEFORE carving its workspace (ensure() may then free the lazy arena)
     void* tm_encode = nullptr;         // cuTensorMapEncodeTiled (driver entry point; NULL: the mma.sync 3xTF32 kernels are used instead)
     bool A_dirty = true;
@@ -598,6 +600,8 @@ cudaError_t i8_attrs() {
     if (done) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(wi8::i8_slice_gemm<I8S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wi8::Sched<I8S>::SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(wi8::i8_slice_gemm<I8S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wi8::Sched<I8S>::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wi8::i8_slice_gemm<6, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wi8::Sched<6>::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(wi8::i8_slice_gemm<6, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wi8::Sched<6>::SMEM_BYTES);
     done = e == cudaSuccess;
     return e;
 }
@@ -632,8 +636,14 @@ int launch_i8_gemm(west_ctx* c, bool atomic, int rows_a, long long alloc_a, long
     const wi8::TileGrid tg{(rows_a + 127) / 128, (rows_b + 127) / 128, splits, gb};
     const long long nt = tiles * splits;
     Prof p_(c, prof_class);
-    if (atomic) wi8::i8_slice_gemm<I8S, true><<<(unsigned)std::min<long long>(nt, 148), wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
-    else wi8::i8_slice_gemm<I8S, false><<<(unsigned)std::min<long long>(nt, 148), wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+    const unsigned grid = (unsigned)std::min<long long>(nt, 148);
+    if (c->i8_slices == 6) {           // the slice arrays always hold 8 planes; the 6-slice schedule touches the first six
+        if (atomic) wi8::i8_slice_gemm<6, true><<<grid, wi8::NTHREADS, wi8::Sched<6>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+        else wi8::i8_slice_gemm<6, false><<<grid, wi8::NTHREADS, wi8::Sched<6>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+    } else {
+        if (atomic) wi8::i8_slice_gemm<I8S, true><<<grid, wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+        else wi8::i8_slice_gemm<I8S, false><<<grid, wi8::NTHREADS, wi8::Sched<I8S>::SMEM_BYTES, c->st>>>(m, tg, rows_a, rows_b, n_kb, kps, sa, sb, out, ldo);
+    }
     CK(cudaGetLastError());
     c->launches += 1;
     return WEST_OK;
@@ -674,7 +684,8 @@ int lowrank_apply_i8(west_ctx* c, int nr, int n_vec, const double* X, double* Y,
     double* Ct = (double*)c->Cbuf.p;                       // [n_vec][rp] (transposed overlap block, rows contiguous)
     {
         Prof p_(c, PC_GEMM_TN);
-        wi8::slice_rows<I8S><<<n_vec, 256, 0, c->st>>>(K, X, K, (signed char*)c->Xi8.p, n_vec, Kp, (double*)c->Xi8_scale.p);
+        if (c->i8_slices == 6) wi8::slice_rows<6><<<n_vec, 256, 0, c->st>>>(K, X, K, (signed char*)c->Xi8.p, n_vec, Kp, (double*)c->Xi8_scale.p);
+        else wi8::slice_rows<I8S><<<n_vec, 256, 0, c->st>>>(K, X, K, (signed char*)c->Xi8.p, n_vec, Kp, (double*)c->Xi8_scale.p);
         CK(cudaMemsetAsync(Ct, 0, sizeof(double) * (size_t)n_vec * rp, c->st));
         CK(cudaGetLastError());
         c->launches += 1;
@@ -686,7 +697,8 @@ int lowrank_apply_i8(west_ctx* c, int nr, int n_vec, const double* X, double* Y,
         Prof p_(c, PC_GEMM_UP);
         wcg::lowrank_fix_t<<<blocks_for((long long)n_vec * rp, 256), 256, 0, c->st>>>(nr, n_vec, rp, Ct, (const double*)c->A_all.p, K, X, K, lc.dcoef, lc.n_rows_d,
                                                                                  lc.alpha_const, lc.alpha_vec, lc.colmap, lc.nvpc, lc.n_occ, is_gamma(c) ? 1 : 0);
-        wi8::slice_rows<I8S><<<n_vec, 256, 0, c->st>>>(nr, Ct, rp, (signed char*)c->Ci8.p, n_vec, Mp, (double*)c->Ci8_scale.p);
+        if (c->i8_slices == 6) wi8::slice_rows<6><<<n_vec, 256, 0, c->st>>>(nr, Ct, rp, (signed char*)c->Ci8.p, n_vec, Mp, (double*)c->Ci8_scale.p);
+        else wi8::slice_rows<I8S><<<n_vec, 256, 0, c->st>>>(nr, Ct, rp, (signed char*)c->Ci8.p, n_vec, Mp, (double*)c->Ci8_scale.p);
         CK(cudaGetLastError());
         c->launches += 2;
     }
@@ -1088,6 +1100,7 @@ int west_h_apply(west_ctx* c, int32_t precision, int32_t n_vec, const void* x, v
     if (precision != WEST_FP64 && precision != WEST_MIXED && precision != WEST_FP64_I8) return fail(c, WEST_EINVAL, "west_h_apply: bad precision %d", precision);
     if (!c->have_vloc) return fail(c, WEST_ESTATE, "west_h_apply: west_set_vloc has not been called");
     c->gemm_i8 = precision == WEST_FP64_I8 && tc_available(c);
+    c->i8_slices = 8;
     if (n_vec == 0) return WEST_OK;
     const int gamma = is_gamma(c);
     const int n_slots = gamma ? (n_vec + 1) / 2 : n_vec;
@@ -1762,6 +1775,7 @@ extern "C" int west_chi0_apply(west_ctx* c, int32_t precision, int32_t n_pert, c
         return fail(c, WEST_EINVAL, "west_chi0_apply: bad argument");
     if (precision != WEST_FP64 && precision != WEST_MIXED && precision != WEST_FP64_I8) return fail(c, WEST_EINVAL, "west_chi0_apply: bad precision %d", precision);
     c->gemm_i8 = precision == WEST_FP64_I8 && tc_available(c);
+    c->i8_slices = opts->tol >= 1e-9 ? 6 : 8;      // products accurate to 2^-42 of the row maxima are four orders below such a tolerance
     if (!c->have_vloc || c->n_occ == 0) return fail(c, WEST_ESTATE, "west_chi0_apply: west_set_vloc and west_set_states are required");
     if (opts->max_iter < 1 || !(opts->tol > 0) || opts->solver < 0 || opts->solver > 2 || opts->occupation < 0 || opts->occupation > 2 ||
         (opts->dn_accumulate != 0 && opts->dn_accumulate != 1))

@@ -66,3 +66,23 @@ def test_h_apply_i8_cfg2_size():
         ref = oham.apply_h(c_full[v], p.miller, p.L, p.N, p.vloc, p.beta, p.dcoef)[p.half]
         assert relmax(y8[v], ref) < 1e-12
     w.close()
+
+
+@pytest.mark.parametrize("name", ["mini2", "mini48"])
+def test_chi0_i8_six_slices_at_a_loose_tolerance(name):
+    """west.h: with tol >= 1e-9 the int8 path cuts every operand row into 6 slices (2^-42 of the row maxima).  The solve must behave as
+    the DMMA solve at the same tolerance: same iteration count (+-1), both within the tolerance's reach of the sum over states, and close
+    to each other far below it."""
+    import torch
+    import paper_2203_05623_b200 as wb
+    p = oracle_problem.build(name)
+    w, sel = make_west(p)
+    dV = torch.from_numpy(np.ascontiguousarray(p.dV)).cuda()
+    ref = ochi0.chi0_sum_over_states(p.eps, p.U, p.n_occ, p.dV, [0.0], p.miller, p.L, p.N)
+    dn8, _, st8 = w.chi0_apply(dV, [0.0], tol=1e-8, max_iter=500, alpha_pv=p.alpha, precision=wb.WEST_FP64_I8, check_every=1)
+    dn64, _, st64 = w.chi0_apply(dV, [0.0], tol=1e-8, max_iter=500, alpha_pv=p.alpha, check_every=1)
+    assert st8["rc"] == 0 and st64["rc"] == 0 and abs(st8["iters"] - st64["iters"]) <= 1
+    e8, e64 = relmax(dn8.cpu().numpy(), ref), relmax(dn64.cpu().numpy(), ref)
+    assert e8 < 1e-6 and e64 < 1e-6
+    assert relmax(dn8.cpu().numpy(), dn64.cpu().numpy()) < 1e-7
+    w.close()
