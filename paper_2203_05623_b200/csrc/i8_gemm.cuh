@@ -19,9 +19,11 @@
 //   phase 2:  j >= S/2, i <= S - 1 - j               weight classes S/2 .. S - 1      A slices 0 .. S/2-1,  B slices S/2 .. S-1
 // Measured alternatives of this staging (cfg-5 H*psi batch of 16 384 vectors, overlap / update product in ms; this version 153 / 189):
 // 32-byte rows with a 5-stage ring 182 / 216; 64-byte rows, four sub-phases of <= 8 tiles, 3 stages 182 / 213; 128-byte rows, six sub-phases
-// of <= 7 tiles, two drains per tile 161 / 196.  Time follows the slice-tile BYTES loaded (27 tiles of 8 KB per 64-byte k-block here), not the
-// ring depth or the row length: the kernel is bound by the L2 -> shared-memory fill at ~7-8 TB/s with an L2 hit rate of 51 % (ncu), i.e. by
-// how well concurrently running CTAs share operand tiles in L2.
+// of <= 7 tiles, two drains per tile 161 / 196; 2-CTA clusters multicasting the A tiles, and CTA pairs with tcgen05.mma.cta_group::2 on
+// 256 x 128 tiles: same time as this version.  The source-level ncu capture says why (profiles/r02_i8_gemm.md): the MMA issuer finds its
+// stage ready at the first poll for every k-block, the producer waits on the `empty` barriers - the kernel is bound by MMA execution at the
+// rate the tensor pipe sustains under the box's power cap, so staging changes nothing and only moving fewer bytes (tile order in
+// launch_i8_gemm: K chunks of ~8 KB, vector tiles in groups; fewer slices) helps.
 // Warp roles as in tc_gemm.cuh: EPI_WARPS epilogue warps (TMEM lane quarter = warp mod 4, column block = warp / 4), then the TMA producer
 // warp and the MMA issuer warp (+ TMEM owner).  The epilogue warps keep the FP64 sums of a tile in registers across its three phases and write once:
 //   ATOMIC  out[c * ldo + r] += value by atomicAdd (overlap block, split along K)       else  out[c * ldo + r] += value (update).
